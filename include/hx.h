@@ -1,0 +1,196 @@
+/* hx.h — C ABI of libhx: the decode-phase KV-cache path of disaggregated LLM serving
+ * (HexGen-2, arxiv 2502.07903), hand-written CUDA for sm_100a (B200).
+ *
+ * The path (§2, L92 §3.3, L110 §4): a prefill replica produces the KV cache,
+ * sharded over its tensor-parallel (TP) group; it is handed, layer by layer, to the decode
+ * replica, whose TP degree may differ (Table 2: TP in {1,2,4} on either
+ * side); the decode replica keeps it in a paged cache (PagedAttention) and reads
+ * all of it once per generated token ("HBM memory I/O-bound").
+ *
+ * Conventions (all entry points)
+ *  - Payload is IEEE fp16 (B_type = 2).  fp32 accumulation inside attention.
+ *  - DEVICE pointers are marked "device"; everything else is host memory.  The caller owns all
+ *    device memory, including the workspace.  The library allocates no device memory and keeps
+ *    no device state.  hx_page_pool is the only heap object (host).
+ *  - hx_kv_ingest / hx_kv_gather / hx_decode_attention only ENQUEUE work on `stream`
+ *    (a cudaStream_t passed as void*, NULL = legacy default stream) and return.  They never
+ *    synchronise and never read device memory from the host; this is why sizes that only
+ *    shape the launch are also passed as host scalars.
+ *  - Return value: an hx_status.  Nothing is launched unless every host-side check passes.
+ *    hx_last_error() gives a thread-local detail string for the last non-OK return.
+ *  - Device-side contract (not checkable from the host; undefined behaviour if violated):
+ *    page ids in [0, num_pages); row i of the block table holds ceil(n_i/page_size) valid
+ *    entries; cu_seqlens is the exclusive prefix sum of seq_lens; ingest destinations are
+ *    pairwise distinct.  Attention may read a page shared by several requests.
+ *  - Determinism: same inputs -> same bits, run to run (no floating-point atomics; partial
+ *    results are merged in a fixed order).
+ *
+ * Layouts (readings S4, S7, S8, S9)
+ *  - Source shard r of a prefill TP group of degree S:  fp16 [layers][total_tokens][heads/S][head_dim]
+ *    for K and, separately, for V.  Prompts are packed back to back on the token axis; prompt i
+ *    owns rows [cu_seqlens[i], cu_seqlens[i+1]).  Shard r owns the contiguous global kv-head
+ *    range [r*heads/S, (r+1)*heads/S)   (column-wise weight split).
+ *  - Paged cache of ONE decode TP rank q of degree R:  fp16 [layers][num_pages][heads/R][page_size][head_dim]
+ *    for K and, separately, for V.  Rank q owns global kv heads [q*heads/R, (q+1)*heads/R).
+ *    A (page, head) tile is one contiguous page_size*head_dim*2-byte run (4 KiB at 16 x 128).
+ *  - Block table: int32 [batch][block_table_stride]; entry j of row i is the physical page of
+ *    tokens [j*page_size, (j+1)*page_size) of request i; the same table serves every layer,
+ *    K and V, and every decode rank.  Entries at or past ceil(n_i/page_size) are never read.
+ */
+#ifndef HX_H_
+#define HX_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define HX_VERSION 100 /* 0.1.0 */
+
+typedef enum {
+  HX_OK = 0,
+  HX_ERR_INVALID_ARG = 1, /* NULL / misaligned pointer, negative size, indivisible heads, bad rank/layer/stride */
+  HX_ERR_UNSUPPORTED = 2, /* head_dim not in {64,128}; page_size != 16; group size not in {1,2,4,8,16}; tp > heads */
+  HX_ERR_WORKSPACE = 3,   /* workspace NULL or smaller than hx_decode_attention_workspace_bytes() */
+  HX_ERR_CUDA = 4,        /* a CUDA call failed; text in hx_last_error() */
+  HX_ERR_NO_PAGES = 5     /* hx_pool_alloc: not enough free pages; nothing was taken */
+} hx_status;
+
+int hx_version(void);
+const char* hx_status_string(int status); /* static string, never NULL */
+const char* hx_last_error(void);          /* thread-local, never NULL */
+
+/* One decode-TP-rank's paged KV cache (caller-owned device memory). */
+typedef struct {
+  void* k;            /* device, fp16 [layers][num_pages][kv_heads][page_size][head_dim], 16-byte aligned */
+  void* v;            /* device, same shape */
+  int32_t layers;
+  int32_t num_pages;
+  int32_t kv_heads;   /* LOCAL kv heads = global heads / dst_tp */
+  int32_t page_size;  /* 16 */
+  int32_t head_dim;   /* 64 or 128 */
+} hx_paged_cache;
+
+/* Bytes of ONE tensor (k or v) of a paged cache; 0 on overflow / non-positive arguments. */
+size_t hx_paged_cache_bytes(int32_t layers, int32_t num_pages, int32_t kv_heads,
+                            int32_t page_size, int32_t head_dim);
+
+/* ---- (a) KV handoff ingest -------------------------------------------------------------
+ * PAPER.md:L92 (§3.3): "each GPU containing the j-th layer within phi_i should transmit its KV
+ * cache to the matching GPU housing the j-th layer within delta_i"; PAPER.md:L110 (§4): KV
+ * moved by asynchronous SendRecv/cudaMemcpy so that it overlaps compute.  This call is the
+ * LANDING of that handoff on decode rank `dst_rank`: for every layer l < layers, request
+ * i < batch, token t < seq_lens[i], owned global kv head h, tensor X in {K, V}:
+ *
+ *   dst->X[l][ block_table[i][t / ps] ][ h % hd ][ t % ps ][:] = src_X[h / hs][l][ cu_seqlens[i] + t ][ h % hs ][:]
+ *
+ * with hs = heads/src_tp, hd = heads/dst_tp, h in [dst_rank*hd, (dst_rank+1)*hd).  A bit copy:
+ * no arithmetic touches the payload.  Nothing else in dst changes (tail slots of last pages,
+ * unowned pages and other layers beyond `layers` keep their contents).
+ *
+ * src_k, src_v : HOST arrays of src_tp DEVICE pointers (16-byte aligned).  Entries for shards
+ *                that hold none of dst_rank's heads may be NULL.
+ * layers       : layers present in the source buffers; they land at layers [0, layers) of dst
+ *                (a pipeline stage = one call; dst->layers >= layers).
+ * heads        : GLOBAL kv heads; must be divisible by src_tp and dst_tp; dst->kv_heads == heads/dst_tp.
+ * block_table  : device int32 [batch][block_table_stride]; stride >= ceil(max_seq_len/ps).
+ * cu_seqlens   : device int32 [batch+1].   seq_lens: device int32 [batch].
+ * batch, total_tokens, max_seq_len : host copies, used for launch sizing and checks only.
+ * Returns HX_OK without launching when batch == 0 or total_tokens == 0 or layers == 0.      */
+int hx_kv_ingest(const void* const* src_k, const void* const* src_v,
+                 int32_t layers, int32_t heads, int32_t head_dim,
+                 int32_t src_tp, int32_t dst_tp, int32_t dst_rank,
+                 const hx_paged_cache* dst,
+                 const int32_t* block_table, int32_t block_table_stride,
+                 const int32_t* cu_seqlens, const int32_t* seq_lens,
+                 int32_t batch, int32_t total_tokens, int32_t max_seq_len,
+                 void* stream);
+
+/* Exact inverse of hx_kv_ingest (the same equation read right to left): writes dst_rank's
+ * heads of every valid token back into the shard buffers.  src_k/src_v entries are written. */
+int hx_kv_gather(void* const* src_k, void* const* src_v,
+                 int32_t layers, int32_t heads, int32_t head_dim,
+                 int32_t src_tp, int32_t dst_tp, int32_t dst_rank,
+                 const hx_paged_cache* dst,
+                 const int32_t* block_table, int32_t block_table_stride,
+                 const int32_t* cu_seqlens, const int32_t* seq_lens,
+                 int32_t batch, int32_t total_tokens, int32_t max_seq_len,
+                 void* stream);
+
+/* ---- (b) paged decode attention ---------------------------------------------------------
+ * PAPER.md:L110 (§4) integrates PagedAttention / FlashAttention and gives no formula; the
+ * definition is the textbook one (reading S1).  For request i with n = seq_lens[i]
+ * cached tokens (the current token included, already in the cache: reading S12), local query
+ * head h, kv head g = h / (q_heads / cache->kv_heads):
+ *
+ *   s_t = sm_scale * <q[i][h], K[layer][bt[i][t/ps]][g][t%ps]>,   t = 0..n-1
+ *   out[i][h] = sum_t softmax(s)_t * V[layer][bt[i][t/ps]][g][t%ps]
+ *
+ * fp16 in, fp32 accumulate, fp16 out.  n == 0 -> out row = zeros.  Tail slots and unowned
+ * pages are never read into the result.
+ *
+ * out, q      : device fp16 [batch][q_heads][head_dim], 16-byte aligned.
+ * sm_scale    : <= 0 means 1/sqrt(head_dim) rounded to fp32.
+ * workspace   : device, 16-byte aligned, >= hx_decode_attention_workspace_bytes(...) bytes;
+ *               contents need not be initialised and are not preserved.                     */
+size_t hx_decode_attention_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads,
+                                           int32_t head_dim, int32_t max_seq_len, int32_t page_size);
+
+int hx_decode_attention(void* out, const void* q,
+                        const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
+                        const int32_t* block_table, int32_t block_table_stride,
+                        const int32_t* seq_lens,
+                        int32_t batch, int32_t max_seq_len, float sm_scale,
+                        void* workspace, size_t workspace_bytes,
+                        void* stream);
+
+/* ---- host page allocator (paging by citation PAPER.md:L110, OOM
+ * remark PAPER.md:L136).  A free list of page ids; alloc is all-or-nothing.  Not thread-safe. */
+typedef struct hx_page_pool hx_page_pool;
+int     hx_pool_create(hx_page_pool** out, int32_t num_pages);
+int     hx_pool_shuffle(hx_page_pool* pool, uint64_t seed);  /* randomise free-list order (deterministic in seed) */
+int     hx_pool_alloc(hx_page_pool* pool, int32_t n, int32_t* out_page_ids /* host [n] */);
+int     hx_pool_free(hx_page_pool* pool, const int32_t* page_ids /* host [n] */, int32_t n); /* double free / bad id -> INVALID_ARG, nothing freed */
+int32_t hx_pool_num_free(const hx_page_pool* pool);
+int32_t hx_pool_num_pages(const hx_page_pool* pool);
+/* Allocate ceil(seq_lens[i]/page_size) pages for each of `batch` requests and write their rows
+ * into a HOST block table [batch][stride] (unused entries = -1).  All or nothing. */
+int     hx_pool_alloc_table(hx_page_pool* pool, const int32_t* seq_lens, int32_t batch,
+                            int32_t page_size, int32_t* block_table, int32_t stride);
+void    hx_pool_destroy(hx_page_pool* pool);
+
+/* ---- whole decode step with HOST inputs (bench.py "e2e") --------
+ * Copies q, the new prompts' block-table rows / lengths and the source shards from (pinned)
+ * host memory to caller-provided device staging buffers, runs hx_kv_ingest for the new
+ * prompts then hx_decode_attention over the active batch on `stream`, and copies `out` back to
+ * host.  Asynchronous like the rest; the caller synchronises `stream` before reading out_host.
+ * See hx_step_host_args for the buffers. */
+typedef struct {
+  /* attention over the active batch */
+  const void* q_host;            /* host fp16 [batch][q_heads][head_dim] */
+  void*       out_host;          /* host fp16 [batch][q_heads][head_dim] */
+  void*       q_dev;             /* device staging, same size */
+  void*       out_dev;           /* device staging, same size */
+  const hx_paged_cache* cache;
+  int32_t layer, q_heads;
+  const int32_t* block_table_dev; int32_t block_table_stride;   /* device, active batch */
+  const int32_t* seq_lens_dev;    int32_t batch, max_seq_len;
+  float sm_scale;
+  void* workspace; size_t workspace_bytes;
+  /* ingest of the step's new prompts (ing_batch == 0 -> skipped) */
+  const void* const* src_k_host; const void* const* src_v_host; /* host arrays of src_tp HOST shard pointers */
+  void* const* src_k_dev;        void* const* src_v_dev;        /* host arrays of src_tp DEVICE staging pointers */
+  int32_t ing_layers, heads, src_tp, dst_tp, dst_rank;
+  const int32_t* ing_block_table_host; int32_t ing_block_table_stride; /* host [ing_batch][stride] */
+  const int32_t* ing_cu_seqlens_host;  const int32_t* ing_seq_lens_host;
+  int32_t* ing_block_table_dev; int32_t* ing_cu_seqlens_dev; int32_t* ing_seq_lens_dev; /* device staging */
+  int32_t ing_batch, ing_total_tokens, ing_max_seq_len;
+} hx_step_host_args;
+int hx_decode_step_host(const hx_step_host_args* args, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HX_H_ */

@@ -1,0 +1,227 @@
+// libhx C ABI: argument validation and dispatch.  Every step of the path runs in the CUDA
+// kernels of ingest.cu / attention.cu; nothing here touches payload data.
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+
+#include "hx_internal.h"
+
+namespace hx {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+void clear_error() { g_err[0] = 0; }
+
+int device_info(DeviceInfo* out) {
+  static std::mutex mu;
+  static DeviceInfo cache[64];
+  int dev = 0;
+  HX_CUDA_OK(cudaGetDevice(&dev));
+  std::lock_guard<std::mutex> lock(mu);
+  if (dev < 0 || dev >= 64) HX_FAIL(HX_ERR_CUDA, "device id %d out of range", dev);
+  if (cache[dev].device != dev) {
+    DeviceInfo d;
+    d.device = dev;
+    HX_CUDA_OK(cudaDeviceGetAttribute(&d.sm_count, cudaDevAttrMultiProcessorCount, dev));
+    HX_CUDA_OK(cudaDeviceGetAttribute(&d.max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    cache[dev] = d;
+  }
+  *out = cache[dev];
+  return HX_OK;
+}
+
+static int check_cache(const hx_paged_cache* c, const char* who) {
+  if (!c) HX_FAIL(HX_ERR_INVALID_ARG, "%s: cache is NULL", who);
+  if (!c->k || !c->v) HX_FAIL(HX_ERR_INVALID_ARG, "%s: cache k/v pointer is NULL", who);
+  if (!aligned16(c->k) || !aligned16(c->v)) HX_FAIL(HX_ERR_INVALID_ARG, "%s: cache pointers must be 16-byte aligned", who);
+  if (c->layers <= 0 || c->num_pages <= 0 || c->kv_heads <= 0 || c->page_size <= 0 || c->head_dim <= 0)
+    HX_FAIL(HX_ERR_INVALID_ARG, "%s: cache dims must be positive (layers=%d pages=%d kv_heads=%d ps=%d D=%d)", who,
+            c->layers, c->num_pages, c->kv_heads, c->page_size, c->head_dim);
+  if (c->head_dim != 64 && c->head_dim != 128) HX_FAIL(HX_ERR_UNSUPPORTED, "%s: head_dim %d not in {64,128}", who, c->head_dim);
+  if (c->page_size != 16) HX_FAIL(HX_ERR_UNSUPPORTED, "%s: page_size %d != 16", who, c->page_size);
+  return HX_OK;
+}
+
+static int ingest_common(const void* const* src_k, const void* const* src_v, int32_t layers, int32_t heads,
+                         int32_t head_dim, int32_t src_tp, int32_t dst_tp, int32_t dst_rank,
+                         const hx_paged_cache* dst, const int32_t* block_table, int32_t stride,
+                         const int32_t* cu_seqlens, const int32_t* seq_lens, int32_t batch,
+                         int32_t total_tokens, int32_t max_seq_len, void* stream, bool gather) {
+  const char* who = gather ? "hx_kv_gather" : "hx_kv_ingest";
+  clear_error();
+  if (layers < 0 || batch < 0 || total_tokens < 0 || max_seq_len < 0)
+    HX_FAIL(HX_ERR_INVALID_ARG, "%s: negative size (layers=%d batch=%d total_tokens=%d max_seq_len=%d)", who, layers, batch, total_tokens, max_seq_len);
+  if (heads <= 0 || src_tp <= 0 || dst_tp <= 0) HX_FAIL(HX_ERR_INVALID_ARG, "%s: heads/src_tp/dst_tp must be positive", who);
+  if (src_tp > heads || dst_tp > heads) HX_FAIL(HX_ERR_UNSUPPORTED, "%s: TP degree above kv heads (replicated KV) is not supported (heads=%d src_tp=%d dst_tp=%d)", who, heads, src_tp, dst_tp);
+  if (heads % src_tp || heads % dst_tp) HX_FAIL(HX_ERR_INVALID_ARG, "%s: heads=%d not divisible by src_tp=%d / dst_tp=%d", who, heads, src_tp, dst_tp);
+  if (src_tp > 16) HX_FAIL(HX_ERR_UNSUPPORTED, "%s: src_tp %d > 16", who, src_tp);
+  if (dst_rank < 0 || dst_rank >= dst_tp) HX_FAIL(HX_ERR_INVALID_ARG, "%s: dst_rank %d not in [0,%d)", who, dst_rank, dst_tp);
+  int rc = check_cache(dst, who);
+  if (rc) return rc;
+  if (dst->head_dim != head_dim) HX_FAIL(HX_ERR_INVALID_ARG, "%s: head_dim %d != cache head_dim %d", who, head_dim, dst->head_dim);
+  if (dst->kv_heads != heads / dst_tp) HX_FAIL(HX_ERR_INVALID_ARG, "%s: cache kv_heads %d != heads/dst_tp = %d", who, dst->kv_heads, heads / dst_tp);
+  if (layers > dst->layers) HX_FAIL(HX_ERR_INVALID_ARG, "%s: layers %d > cache layers %d", who, layers, dst->layers);
+  if (batch == 0 || total_tokens == 0 || layers == 0) return HX_OK;
+  if (!src_k || !src_v) HX_FAIL(HX_ERR_INVALID_ARG, "%s: src_k/src_v array is NULL", who);
+  if (!block_table || !cu_seqlens || !seq_lens) HX_FAIL(HX_ERR_INVALID_ARG, "%s: block_table/cu_seqlens/seq_lens is NULL", who);
+  if (max_seq_len > total_tokens) HX_FAIL(HX_ERR_INVALID_ARG, "%s: max_seq_len %d > total_tokens %d", who, max_seq_len, total_tokens);
+  const int32_t ps = dst->page_size;
+  if ((int64_t)stride * ps < (int64_t)max_seq_len) HX_FAIL(HX_ERR_INVALID_ARG, "%s: block_table_stride %d < ceil(max_seq_len %d / %d)", who, stride, max_seq_len, ps);
+  if ((int64_t)layers * total_tokens * (heads / src_tp) * head_dim >= (int64_t)1 << 40) HX_FAIL(HX_ERR_UNSUPPORTED, "%s: shard too large", who);
+
+  IngestParams p;
+  memset(&p, 0, sizeof(p));
+  p.hs = heads / src_tp; p.hd = heads / dst_tp; p.head0 = dst_rank * p.hd;
+  const int r_lo = p.head0 / p.hs, r_hi = (p.head0 + p.hd - 1) / p.hs;
+  for (int r = r_lo; r <= r_hi; ++r) {
+    if (!src_k[r] || !src_v[r]) HX_FAIL(HX_ERR_INVALID_ARG, "%s: shard %d is needed by dst_rank %d but its pointer is NULL", who, r, dst_rank);
+    if (!aligned16(src_k[r]) || !aligned16(src_v[r])) HX_FAIL(HX_ERR_INVALID_ARG, "%s: shard %d pointer not 16-byte aligned", who, r);
+    p.src_k[r] = src_k[r]; p.src_v[r] = src_v[r];
+  }
+  p.dst_k = dst->k; p.dst_v = dst->v;
+  p.block_table = block_table; p.cu_seqlens = cu_seqlens; p.seq_lens = seq_lens;
+  p.layers = layers; p.total_tokens = total_tokens; p.batch = batch;
+  p.head_dim = head_dim; p.page_size = ps; p.num_pages = dst->num_pages; p.bt_stride = stride;
+  return launch_ingest(p, gather, static_cast<cudaStream_t>(stream));
+}
+
+}  // namespace hx
+
+extern "C" {
+
+int hx_version(void) { return HX_VERSION; }
+
+const char* hx_status_string(int s) {
+  switch (s) {
+    case HX_OK: return "HX_OK";
+    case HX_ERR_INVALID_ARG: return "HX_ERR_INVALID_ARG";
+    case HX_ERR_UNSUPPORTED: return "HX_ERR_UNSUPPORTED";
+    case HX_ERR_WORKSPACE: return "HX_ERR_WORKSPACE";
+    case HX_ERR_CUDA: return "HX_ERR_CUDA";
+    case HX_ERR_NO_PAGES: return "HX_ERR_NO_PAGES";
+    default: return "HX_ERR_UNKNOWN";
+  }
+}
+
+const char* hx_last_error(void) { return hx::g_err; }
+
+size_t hx_paged_cache_bytes(int32_t layers, int32_t num_pages, int32_t kv_heads, int32_t page_size, int32_t head_dim) {
+  if (layers <= 0 || num_pages <= 0 || kv_heads <= 0 || page_size <= 0 || head_dim <= 0) return 0;
+  unsigned __int128 b = (unsigned __int128)layers * num_pages;
+  b = b * kv_heads * page_size * head_dim * 2;
+  if (b >> 62) return 0;
+  return (size_t)b;
+}
+
+int hx_kv_ingest(const void* const* src_k, const void* const* src_v, int32_t layers, int32_t heads, int32_t head_dim,
+                 int32_t src_tp, int32_t dst_tp, int32_t dst_rank, const hx_paged_cache* dst,
+                 const int32_t* block_table, int32_t block_table_stride, const int32_t* cu_seqlens,
+                 const int32_t* seq_lens, int32_t batch, int32_t total_tokens, int32_t max_seq_len, void* stream) {
+  return hx::ingest_common(src_k, src_v, layers, heads, head_dim, src_tp, dst_tp, dst_rank, dst, block_table,
+                           block_table_stride, cu_seqlens, seq_lens, batch, total_tokens, max_seq_len, stream, false);
+}
+
+int hx_kv_gather(void* const* src_k, void* const* src_v, int32_t layers, int32_t heads, int32_t head_dim,
+                 int32_t src_tp, int32_t dst_tp, int32_t dst_rank, const hx_paged_cache* dst,
+                 const int32_t* block_table, int32_t block_table_stride, const int32_t* cu_seqlens,
+                 const int32_t* seq_lens, int32_t batch, int32_t total_tokens, int32_t max_seq_len, void* stream) {
+  return hx::ingest_common(const_cast<const void* const*>(src_k), const_cast<const void* const*>(src_v), layers, heads,
+                           head_dim, src_tp, dst_tp, dst_rank, dst, block_table, block_table_stride, cu_seqlens,
+                           seq_lens, batch, total_tokens, max_seq_len, stream, true);
+}
+
+size_t hx_decode_attention_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, int32_t head_dim,
+                                           int32_t max_seq_len, int32_t page_size) {
+  if (batch < 0 || q_heads <= 0 || kv_heads <= 0 || head_dim <= 0 || max_seq_len < 0 || page_size <= 0) return 0;
+  return hx::attn_workspace_bytes(batch, q_heads, kv_heads, head_dim, max_seq_len, page_size);
+}
+
+int hx_decode_attention(void* out, const void* q, const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
+                        const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
+                        int32_t batch, int32_t max_seq_len, float sm_scale, void* workspace,
+                        size_t workspace_bytes, void* stream) {
+  using namespace hx;
+  const char* who = "hx_decode_attention";
+  clear_error();
+  if (batch < 0 || max_seq_len < 0) HX_FAIL(HX_ERR_INVALID_ARG, "%s: negative size (batch=%d max_seq_len=%d)", who, batch, max_seq_len);
+  int rc = check_cache(cache, who);
+  if (rc) return rc;
+  if (layer < 0 || layer >= cache->layers) HX_FAIL(HX_ERR_INVALID_ARG, "%s: layer %d not in [0,%d)", who, layer, cache->layers);
+  if (q_heads <= 0 || q_heads % cache->kv_heads) HX_FAIL(HX_ERR_INVALID_ARG, "%s: q_heads %d not a positive multiple of kv_heads %d", who, q_heads, cache->kv_heads);
+  const int G = q_heads / cache->kv_heads;
+  if (G != 1 && G != 2 && G != 4 && G != 8 && G != 16) HX_FAIL(HX_ERR_UNSUPPORTED, "%s: group size %d not in {1,2,4,8,16}", who, G);
+  if (!(sm_scale == sm_scale) || sm_scale > 1e30f) HX_FAIL(HX_ERR_INVALID_ARG, "%s: sm_scale is NaN or too large", who);
+  if (batch == 0) return HX_OK;
+  if (!out || !q) HX_FAIL(HX_ERR_INVALID_ARG, "%s: out/q is NULL", who);
+  if (!aligned16(out) || !aligned16(q)) HX_FAIL(HX_ERR_INVALID_ARG, "%s: out/q must be 16-byte aligned", who);
+  if (!block_table || !seq_lens) HX_FAIL(HX_ERR_INVALID_ARG, "%s: block_table/seq_lens is NULL", who);
+  if ((int64_t)block_table_stride * cache->page_size < (int64_t)max_seq_len)
+    HX_FAIL(HX_ERR_INVALID_ARG, "%s: block_table_stride %d < ceil(max_seq_len %d / %d)", who, block_table_stride, max_seq_len, cache->page_size);
+  const size_t need = attn_workspace_bytes(batch, q_heads, cache->kv_heads, cache->head_dim, max_seq_len, cache->page_size);
+  if (need > 0 && (!workspace || workspace_bytes < need)) HX_FAIL(HX_ERR_WORKSPACE, "%s: workspace %zu bytes < required %zu (or NULL)", who, workspace_bytes, need);
+  if (need > 0 && !aligned16(workspace)) HX_FAIL(HX_ERR_INVALID_ARG, "%s: workspace must be 16-byte aligned", who);
+  if (sm_scale <= 0.f) sm_scale = 1.0f / sqrtf((float)cache->head_dim);
+
+  AttnParams p;
+  memset(&p, 0, sizeof(p));
+  const size_t layer_elems = (size_t)cache->num_pages * cache->kv_heads * cache->page_size * cache->head_dim;
+  p.out = out; p.q = q;
+  p.k = static_cast<const char*>(cache->k) + (size_t)layer * layer_elems * 2;
+  p.v = static_cast<const char*>(cache->v) + (size_t)layer * layer_elems * 2;
+  p.block_table = block_table; p.seq_lens = seq_lens;
+  p.workspace = workspace; p.workspace_bytes = workspace_bytes;
+  p.batch = batch; p.q_heads = q_heads; p.kv_heads = cache->kv_heads; p.head_dim = cache->head_dim;
+  p.page_size = cache->page_size; p.num_pages = cache->num_pages; p.bt_stride = block_table_stride;
+  p.max_seq_len = max_seq_len; p.sm_scale = sm_scale;
+  return launch_attention(p, static_cast<cudaStream_t>(stream));
+}
+
+int hx_decode_step_host(const hx_step_host_args* a, void* stream_) {
+  using namespace hx;
+  clear_error();
+  if (!a) HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_host: args is NULL");
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (!a->cache) HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_host: cache is NULL");
+  const size_t qbytes = (size_t)a->batch * a->q_heads * a->cache->head_dim * 2;
+  if (a->ing_batch > 0) {
+    if (!a->src_k_host || !a->src_v_host || !a->src_k_dev || !a->src_v_dev || !a->ing_block_table_host ||
+        !a->ing_cu_seqlens_host || !a->ing_seq_lens_host || !a->ing_block_table_dev || !a->ing_cu_seqlens_dev ||
+        !a->ing_seq_lens_dev)
+      HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_host: ingest buffers missing");
+    if (a->src_tp <= 0 || a->src_tp > 16 || a->heads <= 0 || a->heads % a->src_tp)
+      HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_host: bad heads/src_tp");
+    const size_t shard = (size_t)a->ing_layers * a->ing_total_tokens * (a->heads / a->src_tp) * a->cache->head_dim * 2;
+    for (int r = 0; r < a->src_tp; ++r) {
+      if (!a->src_k_host[r] || !a->src_k_dev[r]) continue;   // shard not needed by this rank
+      HX_CUDA_OK(cudaMemcpyAsync(a->src_k_dev[r], a->src_k_host[r], shard, cudaMemcpyHostToDevice, stream));
+      HX_CUDA_OK(cudaMemcpyAsync(a->src_v_dev[r], a->src_v_host[r], shard, cudaMemcpyHostToDevice, stream));
+    }
+    HX_CUDA_OK(cudaMemcpyAsync(a->ing_block_table_dev, a->ing_block_table_host,
+                               (size_t)a->ing_batch * a->ing_block_table_stride * 4, cudaMemcpyHostToDevice, stream));
+    HX_CUDA_OK(cudaMemcpyAsync(a->ing_cu_seqlens_dev, a->ing_cu_seqlens_host, (size_t)(a->ing_batch + 1) * 4, cudaMemcpyHostToDevice, stream));
+    HX_CUDA_OK(cudaMemcpyAsync(a->ing_seq_lens_dev, a->ing_seq_lens_host, (size_t)a->ing_batch * 4, cudaMemcpyHostToDevice, stream));
+    int rc = hx_kv_ingest(const_cast<const void* const*>(a->src_k_dev), const_cast<const void* const*>(a->src_v_dev),
+                          a->ing_layers, a->heads, a->cache->head_dim, a->src_tp, a->dst_tp, a->dst_rank, a->cache,
+                          a->ing_block_table_dev, a->ing_block_table_stride, a->ing_cu_seqlens_dev,
+                          a->ing_seq_lens_dev, a->ing_batch, a->ing_total_tokens, a->ing_max_seq_len, stream_);
+    if (rc) return rc;
+  }
+  if (a->batch > 0) {
+    if (!a->q_host || !a->out_host || !a->q_dev || !a->out_dev) HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_host: q/out buffers missing");
+    HX_CUDA_OK(cudaMemcpyAsync(a->q_dev, a->q_host, qbytes, cudaMemcpyHostToDevice, stream));
+    int rc = hx_decode_attention(a->out_dev, a->q_dev, a->cache, a->layer, a->q_heads, a->block_table_dev,
+                                 a->block_table_stride, a->seq_lens_dev, a->batch, a->max_seq_len, a->sm_scale,
+                                 a->workspace, a->workspace_bytes, stream_);
+    if (rc) return rc;
+    HX_CUDA_OK(cudaMemcpyAsync(a->out_host, a->out_dev, qbytes, cudaMemcpyDeviceToHost, stream));
+  }
+  return HX_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,69 @@
+// Internal helpers shared by the libhx translation units (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdarg>
+#include <cstdint>
+#include <cstdio>
+
+#include "hx.h"
+
+namespace hx {
+
+// Thread-local error text behind hx_last_error().
+void set_error(const char* fmt, ...);
+void clear_error();
+
+#define HX_FAIL(status, ...)        \
+  do {                              \
+    ::hx::set_error(__VA_ARGS__);   \
+    return (status);                \
+  } while (0)
+
+#define HX_CUDA_OK(expr)                                                              \
+  do {                                                                                \
+    cudaError_t e_ = (expr);                                                          \
+    if (e_ != cudaSuccess) HX_FAIL(HX_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e_)); \
+  } while (0)
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+struct DeviceInfo {
+  int device = -1;
+  int sm_count = 0;
+  int max_smem_optin = 0;
+};
+// Properties of the current device (cached per device id).
+int device_info(DeviceInfo* out);
+
+// ---- launchers implemented in ingest.cu / attention.cu (arguments already validated) ----
+struct IngestParams {
+  const void* src_k[16];
+  const void* src_v[16];
+  void* dst_k;
+  void* dst_v;
+  const int32_t* block_table;
+  const int32_t* cu_seqlens;
+  const int32_t* seq_lens;
+  int32_t layers, total_tokens, batch;
+  int32_t hs, hd, head0;          // heads per source shard, per dest rank, first owned global head
+  int32_t head_dim, page_size, num_pages, bt_stride;
+};
+int launch_ingest(const IngestParams& p, bool gather, cudaStream_t stream);
+
+struct AttnParams {
+  void* out;
+  const void* q;
+  const void* k;                  // layer base already applied
+  const void* v;
+  const int32_t* block_table;
+  const int32_t* seq_lens;
+  void* workspace;
+  size_t workspace_bytes;
+  int32_t batch, q_heads, kv_heads, head_dim, page_size, num_pages, bt_stride, max_seq_len;
+  float sm_scale;
+};
+size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, int32_t head_dim,
+                            int32_t max_seq_len, int32_t page_size);
+int launch_attention(const AttnParams& p, cudaStream_t stream);
+
+}  // namespace hx

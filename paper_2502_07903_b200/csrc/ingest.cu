@@ -1,0 +1,116 @@
+// hx_kv_ingest / hx_kv_gather kernels (SURVEY.md §8(a) rows A2 + A3).
+//
+// A bit copy with index math: every 16-byte chunk of every valid (layer, token, owned head,
+// K|V) row moves once from its source shard to its slot in the paged cache (or back, gather).
+// HBM-bound: algorithmic traffic = 2 x payload (read once, write once), zero flops.
+//
+// Kernel "rows": one thread owns one 16-byte column of one packed token for the whole call.
+// It resolves (request, page, slot) ONCE (binary search over cu_seqlens + one block-table
+// load), then streams every (layer, tensor, head) item of that token: up to 8 independent
+// 16-byte loads are issued before the 8 stores (128 B in flight per thread).  A half-warp
+// (D=128) covers one 256-byte row: reads and writes are both full 32-byte-sector runs, and
+// the 16 tokens of a CTA tile that share a page write one contiguous 4 KiB (page, head) run.
+#include <cuda_fp16.h>
+
+#include "hx_internal.h"
+
+namespace hx {
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kBatch = 8;     // independent 16-byte loads in flight per thread
+
+__device__ __forceinline__ int4 ld_stream(const int4* p) {
+  int4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.L2::128B.v4.s32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_stream(int4* p, const int4& v) {
+  asm volatile("st.global.L1::no_allocate.v4.s32 [%0], {%1,%2,%3,%4};"
+               :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+template <int D, bool GATHER>
+__global__ void __launch_bounds__(kThreads) ingest_rows_kernel(const __grid_constant__ IngestParams p, int layer_splits) {
+  constexpr int CH = D / 8;                 // 16-byte chunks per row
+  constexpr int TOK = kThreads / CH;        // packed tokens per CTA tile
+  const int dc = threadIdx.x % CH;
+  const int tk = blockIdx.x * TOK + threadIdx.x / CH;
+  if (tk >= p.total_tokens) return;
+
+  // request i with cu[i] <= tk < cu[i+1] (largest i whose start is <= tk; empty requests skipped)
+  int lo = 0, hi = p.batch;                 // invariant: cu[lo] <= tk < cu[hi]
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (__ldg(p.cu_seqlens + mid) <= tk) lo = mid; else hi = mid;
+  }
+  const int t = tk - __ldg(p.cu_seqlens + lo);
+  if (t >= __ldg(p.seq_lens + lo)) return;  // inconsistent cu/seq_lens: move nothing for this row
+  const int ps = p.page_size;
+  const int page = __ldg(p.block_table + (size_t)lo * p.bt_stride + t / ps);
+  const int slot = t % ps;
+
+  const int nitems = 2 * p.hd;              // (K|V) x owned heads
+  const size_t src_layer = (size_t)p.total_tokens * p.hs * D;          // elements
+  const size_t dst_layer = (size_t)p.num_pages * p.hd * ps * D;
+  const size_t src_tok = ((size_t)tk * p.hs) * D + dc * 8;
+  const size_t dst_tok = ((size_t)page * p.hd * ps + slot) * D + dc * 8;
+
+  for (int l = blockIdx.y; l < p.layers; l += layer_splits) {
+    for (int base = 0; base < nitems; base += kBatch) {
+      int4 val[kBatch];
+      int4* wr[kBatch];
+#pragma unroll
+      for (int u = 0; u < kBatch; ++u) {
+        const int it = base + u;
+        if (it < nitems) {
+          const int x = it >= p.hd;
+          const int j = it - x * p.hd;
+          const int h = p.head0 + j;
+          const int r = h / p.hs;
+          const __half* sbase = static_cast<const __half*>(x ? p.src_v[r] : p.src_k[r]);
+          const __half* dbase = static_cast<const __half*>(x ? p.dst_v : p.dst_k);
+          const __half* s = sbase + l * src_layer + src_tok + (size_t)(h - r * p.hs) * D;
+          const __half* d = dbase + l * dst_layer + dst_tok + (size_t)j * ps * D;
+          const __half* from = GATHER ? d : s;
+          const __half* to = GATHER ? s : d;
+          val[u] = ld_stream(reinterpret_cast<const int4*>(from));
+          wr[u] = reinterpret_cast<int4*>(const_cast<__half*>(to));
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < kBatch; ++u)
+        if (base + u < nitems) st_stream(wr[u], val[u]);
+    }
+  }
+}
+
+}  // namespace
+
+int launch_ingest(const IngestParams& p, bool gather, cudaStream_t stream) {
+  DeviceInfo di;
+  int rc = device_info(&di);
+  if (rc) return rc;
+  const int ch = p.head_dim / 8;
+  const int tok = kThreads / ch;
+  const int tiles = (p.total_tokens + tok - 1) / tok;
+  // enough CTAs for >= ~8 waves of 8 resident CTAs per SM, but never more layer splits than layers
+  const long long target = (long long)di.sm_count * 64;
+  int splits = (int)((target + tiles - 1) / tiles);
+  if (splits < 1) splits = 1;
+  if (splits > p.layers) splits = p.layers;
+  if (splits > 65535) splits = 65535;
+  dim3 grid(tiles, splits);
+  if (p.head_dim == 128) {
+    if (gather) ingest_rows_kernel<128, true><<<grid, kThreads, 0, stream>>>(p, splits);
+    else        ingest_rows_kernel<128, false><<<grid, kThreads, 0, stream>>>(p, splits);
+  } else {
+    if (gather) ingest_rows_kernel<64, true><<<grid, kThreads, 0, stream>>>(p, splits);
+    else        ingest_rows_kernel<64, false><<<grid, kThreads, 0, stream>>>(p, splits);
+  }
+  HX_CUDA_OK(cudaGetLastError());
+  return HX_OK;
+}
+
+}  // namespace hx

@@ -1,0 +1,154 @@
+"""CPU-only checks of the C-ABI library: it loads, exports every symbol include/hx.h declares,
+the host page allocator behaves, and every invalid-argument class is rejected BEFORE any CUDA
+call (so these run without a GPU; no compute call is made)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2502_07903_b200 as hx
+from paper_2502_07903_b200 import binding as B
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    header = open(os.path.join(ROOT, "include", "hx.h")).read()
+    declared = set(re.findall(r"\b(hx_[a-z_0-9]+)\s*\(", header))
+    declared -= {"hx_page_pool"}
+    assert declared == set(B.EXPORTS), declared ^ set(B.EXPORTS)
+    L = hx.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+    assert hx.version() == 100
+    assert hx.status_string(0) == "HX_OK" and hx.status_string(5) == "HX_ERR_NO_PAGES"
+    assert hx.status_string(77) == "HX_ERR_UNKNOWN"
+
+
+def test_paged_cache_bytes():
+    assert hx.paged_cache_bytes(80, 100, 4, 16, 128) == 80 * 100 * 4 * 16 * 128 * 2
+    assert hx.paged_cache_bytes(0, 100, 4, 16, 128) == 0
+    assert hx.paged_cache_bytes(2**31 - 1, 2**31 - 1, 2**31 - 1, 16, 128) == 0   # overflow
+
+
+def test_pool_alloc_free_invariants():
+    pool = hx.PagePool(64, shuffle_seed=7)
+    pool2 = hx.PagePool(64, shuffle_seed=7)
+    a = pool.alloc(10)
+    assert np.array_equal(a, pool2.alloc(10))            # deterministic in the seed
+    assert len(set(a.tolist())) == 10 and a.min() >= 0 and a.max() < 64
+    assert pool.num_free == 54 and pool.num_pages == 64
+    b = pool.alloc(54)
+    assert set(a.tolist()) | set(b.tolist()) == set(range(64))
+    with pytest.raises(hx.HxError) as e:
+        pool.alloc(1)
+    assert e.value.status == B.HX_ERR_NO_PAGES and pool.num_free == 0
+    pool.free(a)
+    assert pool.num_free == 10
+    for bad in ([a[0]], [64], [-1], [b[0], b[0]]):       # double free, range, duplicate
+        with pytest.raises(hx.HxError) as e:
+            pool.free(bad)
+        assert e.value.status == B.HX_ERR_INVALID_ARG and pool.num_free == 10
+    pool.free(b)
+    assert pool.num_free == 64
+    assert hx.PagePool(0).num_free == 0
+
+
+def test_pool_alloc_table_all_or_nothing():
+    pool = hx.PagePool(10, shuffle_seed=1)
+    bt = pool.alloc_table([17, 1, 0, 33], stride=4)
+    assert (bt >= 0).sum(axis=1).tolist() == [2, 1, 0, 3] and pool.num_free == 4
+    used = bt[bt >= 0]
+    assert len(set(used.tolist())) == 6
+    assert (bt[0, 2:] == -1).all() and (bt[2] == -1).all()
+    with pytest.raises(hx.HxError) as e:
+        pool.alloc_table([16 * 5], stride=8)
+    assert e.value.status == B.HX_ERR_NO_PAGES and pool.num_free == 4
+    with pytest.raises(hx.HxError) as e:
+        pool.alloc_table([16 * 3], stride=2)             # row does not fit the stride
+    assert e.value.status == B.HX_ERR_INVALID_ARG and pool.num_free == 4
+
+
+class FakeCache:
+    def __init__(self, layers=2, pages=8, heads=2, ps=16, D=128, k=0x1000, v=0x2000):
+        self.c = B._CCache(k, v, layers, pages, heads, ps, D)
+
+    @property
+    def ref(self):
+        return C.byref(self.c)
+
+
+def _attn(cache=None, **over):
+    kw = dict(layer=0, q_heads=4, block_table=0x3000, block_table_stride=4, seq_lens=0x4000, batch=2,
+              max_seq_len=64, sm_scale=0.0, workspace=0x5000, workspace_bytes=1 << 30, stream=0)
+    kw.update(over)
+    out = kw.pop("out", 0x6000)
+    q = kw.pop("q", 0x7000)
+    hx.decode_attention(out, q, cache or FakeCache(), **kw)
+
+
+@pytest.mark.parametrize("over,status", [
+    (dict(out=0), B.HX_ERR_INVALID_ARG), (dict(q=0x7001), B.HX_ERR_INVALID_ARG),
+    (dict(layer=2), B.HX_ERR_INVALID_ARG), (dict(layer=-1), B.HX_ERR_INVALID_ARG),
+    (dict(q_heads=3), B.HX_ERR_INVALID_ARG), (dict(q_heads=6), B.HX_ERR_UNSUPPORTED),
+    (dict(batch=-1), B.HX_ERR_INVALID_ARG), (dict(block_table_stride=3), B.HX_ERR_INVALID_ARG),
+    (dict(block_table=0), B.HX_ERR_INVALID_ARG), (dict(seq_lens=0), B.HX_ERR_INVALID_ARG),
+    (dict(sm_scale=float("nan")), B.HX_ERR_INVALID_ARG),
+    (dict(cache=FakeCache(D=96)), B.HX_ERR_UNSUPPORTED), (dict(cache=FakeCache(ps=32)), B.HX_ERR_UNSUPPORTED),
+    (dict(cache=FakeCache(k=0)), B.HX_ERR_INVALID_ARG), (dict(cache=FakeCache(v=0x2008)), B.HX_ERR_INVALID_ARG),
+    (dict(cache=FakeCache(pages=0)), B.HX_ERR_INVALID_ARG),
+])
+def test_attention_rejects_invalid_arguments_without_launching(over, status):
+    with pytest.raises(hx.HxError) as e:
+        _attn(**over)
+    assert e.value.status == status, str(e.value)
+    assert hx.last_error()
+
+
+def test_attention_workspace_check_and_empty_batch():
+    need = hx.decode_attention_workspace_bytes(256, 64, 8, 128, 8192)
+    assert need > 0 and need % 16 == 0
+    with pytest.raises(hx.HxError) as e:
+        _attn(cache=FakeCache(heads=8), q_heads=64, batch=256, max_seq_len=8192, block_table_stride=512,
+              workspace_bytes=need - 1)
+    assert e.value.status == B.HX_ERR_WORKSPACE
+    with pytest.raises(hx.HxError) as e:
+        _attn(cache=FakeCache(heads=8), q_heads=64, batch=256, max_seq_len=8192, block_table_stride=512,
+              workspace=0, workspace_bytes=need)
+    assert e.value.status == B.HX_ERR_WORKSPACE
+    _attn(batch=0, out=0, q=0, block_table=0, seq_lens=0)          # HX_OK, nothing launched
+
+
+def _ingest(fn=None, cache=None, src=None, **over):
+    kw = dict(layers=2, heads=4, head_dim=128, src_tp=2, dst_tp=2, dst_rank=0, block_table=0x3000,
+              block_table_stride=4, cu_seqlens=0x4000, seq_lens=0x5000, batch=2, total_tokens=100,
+              max_seq_len=64, stream=0)
+    kw.update(over)
+    s = src if src is not None else [0x10000 * (r + 1) for r in range(kw["src_tp"])]
+    (fn or hx.kv_ingest)(s, list(s), dst=cache or FakeCache(), **kw)
+
+
+@pytest.mark.parametrize("over,status", [
+    (dict(heads=5), B.HX_ERR_INVALID_ARG), (dict(heads=6, dst_tp=4), B.HX_ERR_INVALID_ARG),
+    (dict(src_tp=8, src=[0x100] * 8), B.HX_ERR_UNSUPPORTED), (dict(dst_tp=8), B.HX_ERR_UNSUPPORTED),
+    (dict(dst_rank=2), B.HX_ERR_INVALID_ARG), (dict(dst_rank=-1), B.HX_ERR_INVALID_ARG),
+    (dict(layers=3), B.HX_ERR_INVALID_ARG), (dict(layers=-1), B.HX_ERR_INVALID_ARG),
+    (dict(head_dim=64), B.HX_ERR_INVALID_ARG), (dict(cache=FakeCache(heads=4)), B.HX_ERR_INVALID_ARG),
+    (dict(block_table_stride=3), B.HX_ERR_INVALID_ARG), (dict(max_seq_len=200), B.HX_ERR_INVALID_ARG),
+    (dict(cu_seqlens=0), B.HX_ERR_INVALID_ARG), (dict(src=[0, 0x20000]), B.HX_ERR_INVALID_ARG),
+    (dict(src=[0x10004, 0x20000]), B.HX_ERR_INVALID_ARG), (dict(cache=FakeCache(D=96), head_dim=96), B.HX_ERR_UNSUPPORTED),
+])
+@pytest.mark.parametrize("fn", ["kv_ingest", "kv_gather"])
+def test_ingest_rejects_invalid_arguments_without_launching(fn, over, status):
+    with pytest.raises(hx.HxError) as e:
+        _ingest(fn=getattr(hx, fn), **over)
+    assert e.value.status == status, str(e.value)
+
+
+def test_ingest_unneeded_shard_may_be_null_and_empty_is_ok():
+    # dst_rank 1 of dst_tp 2 with src_tp 2 needs only shard 1; batch == 0 returns OK before launch
+    _ingest(src=[0, 0x20000], dst_rank=1, batch=0)
+    _ingest(total_tokens=0, max_seq_len=0)
+    _ingest(layers=0)

@@ -1,0 +1,188 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the oracle, element by element,
+on the same seeded inputs.  Ingest: bit-exact.  Attention: max-abs <= 2e-3 and relative-L2 <= 1e-3
+(north_star; fp16 in, fp32 accumulate).  Run on the B200 box with `pytest -m gpu`."""
+import numpy as np
+import pytest
+
+import workloads as W
+from helpers import (MAX_ABS_TOL, REL_L2_TOL, attn_errors, oracle_ingest, run_gpu_attention,
+                     run_gpu_ingest, to_dev)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device (no CPU fallback exists)")
+    import paper_2502_07903_b200 as hx
+    import oracle
+    oracle.build()
+    return hx, torch, oracle
+
+
+def check_attn(env, w, label="", **kw):
+    hx, torch, oracle = env
+    got = run_gpu_attention(hx, torch, w, **kw)
+    ref = oracle.decode_attention(w["q"] if "q" not in kw else kw["q"], w["k"], w["v"], w["block_table"],
+                                  w["seq_lens"], layer=kw.get("layer", 0), sm_scale=kw.get("sm_scale"))
+    assert np.isfinite(got.astype(np.float32)).all(), label
+    max_abs, rel_l2 = attn_errors(got, ref)
+    assert max_abs <= MAX_ABS_TOL and rel_l2 <= REL_L2_TOL, (label, max_abs, rel_l2)
+    return got, ref
+
+
+# ------------------------------------------------------------------ ingest (bit-exact)
+def test_ingest_tiny_config_bit_exact(env):
+    hx, torch, oracle = env
+    w = W.make_ingest_inputs(W.CONFIGS["tiny_ingest"], bits=True)     # all 16-bit patterns
+    dk, dv, gk, gv = run_gpu_ingest(hx, torch, w, 0, gather_back=True)
+    ok, ov = oracle_ingest(oracle, w, 0)
+    assert np.array_equal(dk, ok) and np.array_equal(dv, ov)
+    for r in range(2):
+        assert np.array_equal(gk[r], w["src_k"][r]) and np.array_equal(gv[r], w["src_v"][r])
+
+
+@pytest.mark.parametrize("S", [1, 2, 4, 8])
+@pytest.mark.parametrize("R", [1, 2, 4, 8])
+@pytest.mark.parametrize("D", [64, 128])
+def test_ingest_sweep_tp_pairs(env, S, R, D):
+    hx, torch, oracle = env
+    lens = np.array([1, 15, 16, 17, 31, 32, 33, 255, 256, 257, 0, 5], dtype=np.int32)
+    c = W.IngestConfig(80, "sweep", 3, 8, D, S, R, len(lens), "x")
+    w = W.make_ingest_inputs(c, lens=lens, bits=True, seed_extra=S * 100 + R * 10 + D)
+    for q in range(R):
+        dk, dv, gk, gv = run_gpu_ingest(hx, torch, w, q, gather_back=True)
+        ok, ov = oracle_ingest(oracle, w, q)
+        assert np.array_equal(dk, ok), (S, R, D, q)
+        assert np.array_equal(dv, ov), (S, R, D, q)
+        # gather rebuilds exactly the heads rank q owns; other positions keep the fill
+        hs, hd = 8 // S, 8 // R
+        for r in range(S):
+            for j in range(hs):
+                h = r * hs + j
+                if q * hd <= h < (q + 1) * hd:
+                    assert np.array_equal(gk[r][:, :, j], w["src_k"][r][:, :, j])
+                    assert np.array_equal(gv[r][:, :, j], w["src_v"][r][:, :, j])
+                else:
+                    assert (gk[r][:, :, j] == 0x0BAD).all() and (gv[r][:, :, j] == 0x0BAD).all()
+
+
+def test_ingest_odd_head_counts(env):
+    hx, torch, oracle = env
+    for heads, S, R in [(14, 2, 7), (56, 4, 4), (6, 3, 2), (12, 4, 3)]:
+        lens = np.array([40, 3, 129], dtype=np.int32)
+        c = W.IngestConfig(81, "odd", 2, heads, 128, S, R, 3, "x")
+        w = W.make_ingest_inputs(c, lens=lens, bits=True, seed_extra=heads)
+        for q in (0, R - 1):
+            dk, dv = run_gpu_ingest(hx, torch, w, q)
+            ok, ov = oracle_ingest(oracle, w, q)
+            assert np.array_equal(dk, ok) and np.array_equal(dv, ov), (heads, S, R, q)
+
+
+def test_ingest_empty_inputs(env):
+    hx, torch, oracle = env
+    c = W.IngestConfig(82, "empty", 1, 4, 128, 2, 1, 2, "x")
+    w = W.make_ingest_inputs(c, lens=np.array([0, 0], dtype=np.int32), bits=True)
+    dk, dv = run_gpu_ingest(hx, torch, w, 0)
+    assert (dk == 0xDEAD).all() and (dv == 0xDEAD).all()
+
+
+# ------------------------------------------------------------------ attention
+def test_attention_tiny_config(env):
+    w = W.make_attention_inputs(W.CONFIGS["tiny"])
+    check_attn(env, w, "tiny")
+
+
+@pytest.mark.parametrize("G,Hkv", [(1, 4), (2, 2), (4, 2), (8, 2), (16, 1), (1, 14), (8, 4)])
+@pytest.mark.parametrize("D", [64, 128])
+def test_attention_sweep_page_boundaries(env, G, Hkv, D):
+    lens = np.array([1, 15, 16, 17, 31, 32, 33, 255, 256, 257, 1000, 2], dtype=np.int32)
+    c = W.AttnConfig(70, "sweep", len(lens), G * Hkv, Hkv, D, 64, "x")
+    w = W.make_attention_inputs(c, lens=lens, layers=2, seed_extra=G * 1000 + Hkv * 10 + D)
+    check_attn(env, w, f"G={G} Hkv={Hkv} D={D}", layer=1)
+
+
+def test_attention_custom_scale_and_empty_request(env):
+    lens = np.array([0, 40, 0, 700], dtype=np.int32)
+    c = W.AttnConfig(71, "scale", 4, 8, 1, 128, 64, "x")
+    w = W.make_attention_inputs(c, lens=lens)
+    got, _ = check_attn(env, w, "scale", sm_scale=0.05)
+    assert (got[0] == 0).all() and (got[2] == 0).all()            # reading S11: zeros
+
+
+def test_attention_single_token_is_bit_exact_v(env):
+    hx, torch, _ = env
+    lens = np.ones(5, dtype=np.int32)
+    c = W.AttnConfig(72, "n1", 5, 8, 2, 128, 4, "x")
+    w = W.make_attention_inputs(c, lens=lens)
+    got = run_gpu_attention(hx, torch, w)
+    for i in range(5):
+        for h in range(8):
+            assert np.array_equal(got[i, h].view(np.uint16), w["v"][0, w["block_table"][i, 0], h // 4, 0].view(np.uint16))
+
+
+def test_attention_constant_v_and_zero_q(env):
+    hx, torch, oracle = env
+    c = W.AttnConfig(73, "cv", 3, 8, 1, 128, 64, "x")
+    w = W.make_attention_inputs(c, lens=np.array([17, 300, 1000], dtype=np.int32))
+    vec = W.draw_fp16_normal((128,), 73, 99)
+    w["v"][:] = vec
+    got = run_gpu_attention(hx, torch, w)
+    assert np.abs(got.astype(np.float64) - vec.astype(np.float64)).max() <= 1e-3   # weights sum to 1
+    w = W.make_attention_inputs(c, lens=np.array([17, 300, 1000], dtype=np.int32))
+    check_attn(env, w, "q=0", q=np.zeros_like(w["q"]))
+
+
+def test_attention_page_permutation_bit_identical(env):
+    hx, torch, _ = env
+    c = W.AttnConfig(74, "perm", 6, 16, 2, 128, 256, "x")
+    w = W.make_attention_inputs(c, lens=np.array([17, 64, 100, 255, 2000, 4000], dtype=np.int32))
+    base = run_gpu_attention(hx, torch, w)
+    P = w["num_pages"]
+    perm = W.rng(74, 50).permutation(P)
+    w2 = dict(w)
+    w2["k"], w2["v"] = np.empty_like(w["k"]), np.empty_like(w["v"])
+    w2["k"][:, perm], w2["v"][:, perm] = w["k"], w["v"]
+    w2["block_table"] = np.where(w["block_table"] >= 0, perm[np.clip(w["block_table"], 0, None)], -1).astype(np.int32)
+    again = run_gpu_attention(hx, torch, w2)
+    assert np.array_equal(base.view(np.uint16), again.view(np.uint16))
+    assert np.array_equal(base.view(np.uint16), run_gpu_attention(hx, torch, w).view(np.uint16))   # run-to-run
+
+
+def test_attention_nan_poison_is_harmless(env):
+    hx, torch, _ = env
+    c = W.AttnConfig(75, "poison", 5, 16, 2, 128, 64, "x")
+    w = W.make_attention_inputs(c, lens=np.array([17, 64, 100, 255, 1], dtype=np.int32))
+    base = run_gpu_attention(hx, torch, w)
+    owned = np.zeros((w["num_pages"], 16), dtype=bool)
+    for i, n in enumerate(w["seq_lens"]):
+        for t in range(n):
+            owned[w["block_table"][i, t // 16], t % 16] = True
+    kb, vb = w["k"].view(np.uint16).copy(), w["v"].view(np.uint16).copy()
+    kb[0].transpose(0, 2, 1, 3)[~owned] = 0x7E01      # NaN
+    vb[0].transpose(0, 2, 1, 3)[~owned] = 0xFC00      # -inf
+    w2 = dict(w, k=kb.view(np.float16), v=vb.view(np.float16))
+    got = run_gpu_attention(hx, torch, w2)
+    assert np.array_equal(got.view(np.uint16), base.view(np.uint16))
+
+
+def test_attention_large_logits_stable(env):
+    c = W.AttnConfig(76, "hot", 4, 8, 1, 128, 64, "x")
+    w = W.make_attention_inputs(c, lens=np.array([100, 255, 777, 16], dtype=np.int32))
+    q8 = (w["q"].astype(np.float32) * 8).astype(np.float16)
+    check_attn(env, w, "8x logits", q=q8)
+
+
+def test_ingest_then_attention_end_to_end_tiny(env):
+    """configs[0] whole path: shards -> hx_kv_ingest -> hx_decode_attention vs oracle on the oracle's cache."""
+    hx, torch, oracle = env
+    w = W.make_ingest_inputs(W.CONFIGS["tiny_ingest"])
+    dk, dv = run_gpu_ingest(hx, torch, w, 0, sentinel=0x7E01)
+    ok, ov = oracle_ingest(oracle, w, 0, sentinel=0x7E01)
+    assert np.array_equal(dk, ok) and np.array_equal(dv, ov)
+    q = W.draw_fp16_normal((4, 4, 64), 1, W.configs.S_Q)
+    wa = dict(q=q, k=dk.view(np.float16), v=dv.view(np.float16), block_table=w["block_table"],
+              seq_lens=w["seq_lens"], num_pages=w["num_pages"])
+    check_attn(env, wa, "tiny e2e")
