@@ -1,91 +1,712 @@
-// hx_decode_attention kernels.
+// hx_decode_attention kernels (PAPER.md:L110 cites PagedAttention /
+// FlashAttention and gives no kernel: the design below is ours, for sm_100a).
+//
+// Roofline: HBM.  Algorithmic bytes = sum_i n_i * kv_heads * head_dim * 2 tensors * 2 B; G flops
+// per byte (G = q heads per kv head), so the job is to keep ~50 KB of loads in flight per SM and
+// to spend as few issue slots as possible per 8 KiB (page, kv-head) K+V tile.
+//
+// attn_stream_kernel — "stream-K over page tiles":
+//  * The work is the linear sequence of (request, kv head, page) tiles.  Every warp of a
+//    persistent grid (one CTA per SM, 8 warps) owns an equal contiguous range of that sequence
+//    (row A4: the cut depends only on seq_lens and the grid size, never on page placement, so the
+//    result is bit-identical under page permutation and from run to run).
+//  * Each warp runs its own 3-stage ring: lane 0 issues one TMA tensor-tile load per K tile and
+//    per V tile (cp.async.bulk.tensor, 128-byte swizzle, mbarrier complete_tx); block-table
+//    entries are fetched 32-64 tiles ahead, one per lane.  No CTA-wide barrier after setup.
+//  * Scores (row A5) and PV (row A7) run on mma.sync.m16n8k16 with the page as M (16 tokens) and
+//    the GQA group as N (8 heads): S^T = K Q^T and O^T += V^T P^T, so one K/V tile serves all G
+//    query heads from shared memory and nothing is padded along tokens.  Online softmax (row A6)
+//    in fp32 on the accumulator fragments; P^T is re-laid for the second MMA with movmatrix.
+//  * A range that covers a whole (request, kv head) writes fp16 output directly; a range that
+//    starts or ends inside one writes an (m, l, acc) partial; attn_merge_kernel (row A8) combines
+//    a pair's partials in worker order (= token order), normalises, and zero-fills n == 0 rows.
+//
+// attn_simple_kernel — one CTA per (request, q head) on CUDA cores; bring-up/debug only
+// (HX_ATTN_IMPL=simple).
+#include <cuda.h>
 #include <cuda_fp16.h>
 
 #include <cstdlib>
+#include <cstring>
+#include <mutex>
 
 #include "hx_internal.h"
 
 namespace hx {
 namespace {
 
+constexpr int kWarps = 8;          // warps (= independent workers) per CTA
+constexpr int kBMax = 2048;        // requests per launch (prefix sums live in shared memory)
+constexpr int kMaxWorkers = 2048;  // workspace is sized for this many workers (>= SMs * kWarps)
+constexpr float kLog2e = 1.4426950408889634f;
+
+template <int D, int NT>
+struct Cfg {
+  static constexpr int kStages = (NT == 1) ? 3 : 2;
+  static constexpr int kTile = 16 * D * 2;           // bytes of one (page, head) K or V tile
+  static constexpr int kStage = 2 * kTile;           // K + V
+  static constexpr int kQBytes = NT * 8 * D * 2;     // Q slot: NT*8 heads
+  static constexpr int kKS = D / 16;                 // k-steps of QK^T
+  static constexpr int kMT = D / 16;                 // m-tiles of PV
+  static constexpr int kSlotFloats = NT * (kMT * 128 + 16);   // partial: acc[NT][MT][32][4], m[NT][8], l[NT][8]
+  static constexpr int kSmem = kWarps * kStages * kStage + kWarps * kQBytes + kWarps * (kStages + 1) * 8 +
+                               (kBMax + 1) * 4 + kBMax * 4;
+};
+
+struct StreamParams {
+  const __half* q;
+  __half* out;
+  const int32_t* bt;
+  const int32_t* lens;
+  float* partials;        // [2 * W][kSlotFloats]
+  int32_t* cum_out;       // [B + 1] page prefix sums, written by CTA 0 for the merge kernel
+  int32_t B, Hq, Hkv, G, bt_stride;
+  uint32_t layer_row0;    // first tensor-map row of the layer
+  float scale_log2;
+  int32_t W;              // total workers = gridDim.x * kWarps
+};
+
+// ---------------------------------------------------------------------------- PTX helpers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+__device__ __forceinline__ void tma_tile_3d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+      ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t (&r)[4]) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void ldsm_x4_t(uint32_t addr, uint32_t (&r)[4]) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void mma16816(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+               : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+               : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ uint32_t movmatrix_t(uint32_t a) {
+  uint32_t d;
+  asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(d) : "r"(a));
+  return d;
+}
+__device__ __forceinline__ float ex2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+struct Loc { int i, g, j, np; };
+
+// tile index k -> (request, kv head, page-in-request).  Tiles are ordered request-major, then kv
+// head, then page: request i owns [Hkv*cum[i], Hkv*cum[i+1]).
+__device__ __forceinline__ Loc locate(long long k, const int* cum, int B, int Hkv) {
+  int lo = 0, hi = B;     // invariant: Hkv*cum[lo] <= k < Hkv*cum[hi]
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if ((long long)Hkv * cum[mid] <= k) lo = mid; else hi = mid;
+  }
+  Loc r;
+  r.i = lo;
+  r.np = cum[lo + 1] - cum[lo];
+  const int rem = (int)(k - (long long)Hkv * cum[lo]);
+  r.g = rem / r.np;
+  r.j = rem - r.g * r.np;
+  return r;
+}
+
+// ------------------------------------------------------------------------------------------
+template <int D, int NT>
+__global__ void __launch_bounds__(kWarps * 32, 1)
+attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
+                   const StreamParams p) {
+  using C = Cfg<D, NT>;
+  constexpr int kStages = C::kStages, kTile = C::kTile, kKS = C::kKS, kMT = C::kMT;
+  constexpr uint32_t FULL = 0xffffffffu;
+  extern __shared__ __align__(1024) uint8_t smem[];
+  uint8_t* q_base = smem + kWarps * kStages * C::kStage;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(q_base + kWarps * C::kQBytes);
+  int* cum = reinterpret_cast<int*>(bars + kWarps * (kStages + 1));
+  int* slen = cum + (kBMax + 1);
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int B = p.B, Hkv = p.Hkv, G = p.G;
+
+  // ---- setup: page-count prefix sums (row A4) and barrier init; the only CTA-wide syncs
+  {
+    constexpr int PER = kBMax / (kWarps * 32);
+    __shared__ int warp_tot[kWarps];
+    int np[PER], sum = 0;
+#pragma unroll
+    for (int e = 0; e < PER; ++e) {
+      const int i = tid * PER + e;
+      const int n = (i < B) ? max(__ldg(p.lens + i), 0) : 0;
+      if (i < B) slen[i] = n;
+      np[e] = (n + 15) >> 4;
+      sum += np[e];
+    }
+    int incl = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int t = __shfl_up_sync(FULL, incl, o);
+      if (lane >= o) incl += t;
+    }
+    if (lane == 31) warp_tot[warp] = incl;
+    if (lane == 0) {
+      const uint32_t b0 = smem_u32(bars + warp * (kStages + 1));
+      for (int s = 0; s <= kStages; ++s) mbar_init(b0 + 8 * s, 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    int off = incl - sum;
+    for (int w = 0; w < warp; ++w) off += warp_tot[w];
+    if (tid == 0) cum[0] = 0;
+#pragma unroll
+    for (int e = 0; e < PER; ++e) {
+      const int i = tid * PER + e;
+      off += np[e];
+      if (i < B) cum[i + 1] = off;
+    }
+    __syncthreads();
+    if (blockIdx.x == 0)
+      for (int i = tid; i <= B; i += kWarps * 32) p.cum_out[i] = cum[i];
+  }
+
+  const long long N = (long long)Hkv * cum[B];
+  const int w = blockIdx.x * kWarps + warp;
+  const long long k0 = (long long)w * N / p.W, k1 = (long long)(w + 1) * N / p.W;
+  if (k0 >= k1) return;
+
+  uint8_t* my_stage = smem + warp * kStages * C::kStage;
+  const uint32_t stage_u32 = smem_u32(my_stage);
+  uint8_t* my_q = q_base + warp * C::kQBytes;
+  const uint32_t q_u32 = smem_u32(my_q);
+  const uint32_t bar_u32 = smem_u32(bars + warp * (kStages + 1));
+  const uint32_t qbar = bar_u32 + 8 * kStages;
+
+  // ---- per-lane lookahead: lane L of round r describes tile k0 + 32 r + L
+  int page_cur = 0, gpart_cur = 0, meta_cur = 0, page_nxt = 0, gpart_nxt = 0, meta_nxt = 0;
+  auto load_round = [&](int r, int& page, int& gpart, int& meta) {
+    const long long k = k0 + 32ll * r + lane;
+    page = 0; gpart = 0; meta = 0;
+    if (k < k1) {
+      const Loc t = locate(k, cum, B, Hkv);
+      page = __ldg(p.bt + (size_t)t.i * p.bt_stride + t.j);
+      gpart = t.g * 16;
+      meta = ((t.i * p.Hq + t.g * G) << 1) | (t.j == 0 ? 1 : 0);
+    }
+  };
+  load_round(0, page_cur, gpart_cur, meta_cur);
+  load_round(1, page_nxt, gpart_nxt, meta_nxt);
+  int cur_round = 0;
+
+  // ---- consumer cursor (warp-uniform)
+  Loc c = locate(k0, cum, B, Hkv);
+  int cn = slen[c.i];
+  int seg_j0 = 0, segs_started = 0;
+  bool q_busy = false;
+
+  // fragment-address constants
+  const int a_row = (lane & 7) + ((lane >> 3) & 1) * 8;   // K (A, non-trans): token row
+  const int a_csel = lane >> 4;                           //   chunk select within the k-step
+  const int v_row = (lane & 7) + (lane >> 4) * 8;         // V (A, trans): token row
+  const int v_csel = (lane >> 3) & 1;
+  const int tok0 = lane >> 2;
+
+  uint32_t qb[NT][kKS][2];
+  float o[NT][kMT][4];
+  float m_run[NT][2], l_run[NT][2];
+
+  long long pk = k0, ck = k0;
+  while (ck < k1) {
+    // ------------------------------------------------ produce: keep kStages tiles in flight
+    while (pk < k1 && pk - ck < kStages) {
+      const int idx = (int)(pk - k0);
+      if ((idx >> 5) != cur_round) {
+        page_cur = page_nxt; gpart_cur = gpart_nxt; meta_cur = meta_nxt;
+        ++cur_round;
+        load_round(cur_round + 1, page_nxt, gpart_nxt, meta_nxt);
+      }
+      const int src = idx & 31;
+      const int meta = __shfl_sync(FULL, meta_cur, src);
+      const bool segstart = (idx == 0) || (meta & 1);
+      if (segstart && q_busy) break;
+      const int page = __shfl_sync(FULL, page_cur, src);
+      const int gpart = __shfl_sync(FULL, gpart_cur, src);
+      const int stage = idx % kStages;
+      if (lane == 0) {
+        if (segstart) {
+          mbar_expect_tx(qbar, (uint32_t)(G * D * 2));
+          bulk_load(q_u32, p.q + (size_t)(meta >> 1) * D, (uint32_t)(G * D * 2), qbar);
+        }
+        const uint32_t full = bar_u32 + 8 * stage;
+        const uint32_t dst = stage_u32 + stage * C::kStage;
+        const int row = (int)(p.layer_row0 + (uint32_t)page * (uint32_t)(Hkv * 16) + (uint32_t)gpart);
+        mbar_expect_tx(full, 2 * kTile);
+        tma_tile_3d(dst, &tmK, 0, row, 0, full);
+        tma_tile_3d(dst + kTile, &tmV, 0, row, 0, full);
+      }
+      if (segstart) q_busy = true;
+      ++pk;
+    }
+
+    // ------------------------------------------------ consume tile ck
+    const int idx = (int)(ck - k0);
+    const int stage = idx % kStages;
+    if (c.j == 0 || idx == 0) {                      // segment start: fetch Q fragments, reset state
+      mbar_wait(qbar, segs_started & 1);
+      ++segs_started;
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt) {
+        const int head = nt * 8 + (lane >> 2);
+        const uint8_t* qrow = my_q + head * (D * 2) + (lane & 3) * 4;
+#pragma unroll
+        for (int ks = 0; ks < kKS; ++ks) {
+          uint32_t b0 = *reinterpret_cast<const uint32_t*>(qrow + ks * 32);
+          uint32_t b1 = *reinterpret_cast<const uint32_t*>(qrow + ks * 32 + 16);
+          qb[nt][ks][0] = head < G ? b0 : 0u;
+          qb[nt][ks][1] = head < G ? b1 : 0u;
+        }
+#pragma unroll
+        for (int mt = 0; mt < kMT; ++mt) o[nt][mt][0] = o[nt][mt][1] = o[nt][mt][2] = o[nt][mt][3] = 0.f;
+        m_run[nt][0] = m_run[nt][1] = -INFINITY;
+        l_run[nt][0] = l_run[nt][1] = 0.f;
+      }
+      __syncwarp();
+      q_busy = false;
+      seg_j0 = c.j;
+    }
+    mbar_wait(bar_u32 + 8 * stage, (idx / kStages) & 1);
+
+    const uint32_t kb = stage_u32 + stage * C::kStage, vb = kb + kTile;
+    const bool last_page = (c.j == c.np - 1);
+    const int valid = last_page ? cn - 16 * (c.np - 1) : 16;
+    if (valid < 16) {
+      // tail slots may hold anything (NaN/Inf): P is 0 there, but 0 * Inf = NaN in the PV MMA,
+      // so the V rows past the context end are zeroed in shared memory (reading S10).
+      for (int e = lane; e < (16 - valid) * (D / 8); e += 32) {
+        const int r = valid + e / (D / 8), ch = e % (D / 8);
+        *reinterpret_cast<int4*>(my_stage + stage * C::kStage + kTile + (ch >> 3) * 2048 + r * 128 + (ch & 7) * 16) =
+            make_int4(0, 0, 0, 0);
+      }
+      __syncwarp();
+    }
+
+    // ---- S^T[16 tok x 8 heads] = K[16 x D] Q^T   (row A5)
+    float sacc[NT][2][4];
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+      for (int h = 0; h < 2; ++h) sacc[nt][h][0] = sacc[nt][h][1] = sacc[nt][h][2] = sacc[nt][h][3] = 0.f;
+#pragma unroll
+    for (int ks = 0; ks < kKS; ++ks) {
+      const int cidx = 2 * ks + a_csel;
+      uint32_t a[4];
+      ldsm_x4(kb + (cidx >> 3) * 2048 + a_row * 128 + (((cidx & 7) ^ (a_row & 7)) << 4), a);
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt) mma16816(sacc[nt][ks & 1], a, qb[nt][ks][0], qb[nt][ks][1]);
+    }
+
+    // ---- online softmax on the accumulator fragments (row A6)
+    uint32_t pb[NT][2];
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) {
+      float s[4];
+#pragma unroll
+      for (int r = 0; r < 4; ++r) s[r] = (sacc[nt][0][r] + sacc[nt][1][r]) * p.scale_log2;
+      if (tok0 >= valid) s[0] = s[1] = -INFINITY;
+      if (tok0 + 8 >= valid) s[2] = s[3] = -INFINITY;
+      float pr[4], corr[2];
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        float mx = fmaxf(s[e], s[e + 2]);
+        mx = fmaxf(mx, __shfl_xor_sync(FULL, mx, 4));
+        mx = fmaxf(mx, __shfl_xor_sync(FULL, mx, 8));
+        mx = fmaxf(mx, __shfl_xor_sync(FULL, mx, 16));
+        const float m_new = fmaxf(m_run[nt][e], mx);        // finite: every tile has >= 1 valid token
+        corr[e] = ex2(m_run[nt][e] - m_new);                // -inf -> 0 on the first tile
+        m_run[nt][e] = m_new;
+        pr[e] = ex2(s[e] - m_new);
+        pr[e + 2] = ex2(s[e + 2] - m_new);
+      }
+      const __half2 p01 = __floats2half2_rn(pr[0], pr[1]);
+      const __half2 p23 = __floats2half2_rn(pr[2], pr[3]);
+      // l sums the ROUNDED weights so that numerator and denominator use the same weights
+      l_run[nt][0] = l_run[nt][0] * corr[0] + __low2float(p01) + __low2float(p23);
+      l_run[nt][1] = l_run[nt][1] * corr[1] + __high2float(p01) + __high2float(p23);
+      pb[nt][0] = movmatrix_t(*reinterpret_cast<const uint32_t*>(&p01));   // P^T B-fragment, tokens 0-7
+      pb[nt][1] = movmatrix_t(*reinterpret_cast<const uint32_t*>(&p23));   //                tokens 8-15
+      if (__any_sync(FULL, corr[0] != 1.f || corr[1] != 1.f)) {
+#pragma unroll
+        for (int mt = 0; mt < kMT; ++mt) {
+          o[nt][mt][0] *= corr[0]; o[nt][mt][1] *= corr[1];
+          o[nt][mt][2] *= corr[0]; o[nt][mt][3] *= corr[1];
+        }
+      }
+    }
+
+    // ---- O^T[D x 8 heads] += V^T[D x 16 tok] P^T   (row A7)
+#pragma unroll
+    for (int mt = 0; mt < kMT; ++mt) {
+      const int cidx = 2 * mt + v_csel;
+      uint32_t a[4];
+      ldsm_x4_t(vb + (cidx >> 3) * 2048 + v_row * 128 + (((cidx & 7) ^ (v_row & 7)) << 4), a);
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt) mma16816(o[nt][mt], a, pb[nt][0], pb[nt][1]);
+    }
+    __syncwarp();                                    // every lane is done reading this stage
+
+    // ------------------------------------------------ segment end: output or partial (row A8)
+    const bool seg_end = last_page || (ck == k1 - 1);
+    bool wrote_smem = valid < 16;
+    if (seg_end) {
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          float l = l_run[nt][e];
+          l += __shfl_xor_sync(FULL, l, 4);
+          l += __shfl_xor_sync(FULL, l, 8);
+          l += __shfl_xor_sync(FULL, l, 16);
+          l_run[nt][e] = l;
+        }
+      if (seg_j0 == 0 && last_page) {
+        // whole (request, kv head) in this range: normalise, transpose through the freed K tile
+        __half* scratch = reinterpret_cast<__half*>(my_stage + stage * C::kStage);
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+          const float inv0 = 1.f / l_run[nt][0], inv1 = 1.f / l_run[nt][1];
+          const int h0 = nt * 8 + 2 * (lane & 3);
+#pragma unroll
+          for (int mt = 0; mt < kMT; ++mt) {
+            const int d0 = 16 * mt + tok0;
+            scratch[h0 * D + d0] = __float2half_rn(o[nt][mt][0] * inv0);
+            scratch[(h0 + 1) * D + d0] = __float2half_rn(o[nt][mt][1] * inv1);
+            scratch[h0 * D + d0 + 8] = __float2half_rn(o[nt][mt][2] * inv0);
+            scratch[(h0 + 1) * D + d0 + 8] = __float2half_rn(o[nt][mt][3] * inv1);
+          }
+        }
+        __syncwarp();
+        int4* dst = reinterpret_cast<int4*>(p.out + ((size_t)c.i * p.Hq + (size_t)c.g * G) * D);
+        const int4* srcv = reinterpret_cast<const int4*>(scratch);
+        for (int e = lane; e < G * D / 8; e += 32) dst[e] = srcv[e];
+        __syncwarp();
+        wrote_smem = true;
+      } else {
+        // first segment of this worker -> slot 2w, any later partial segment is its last -> 2w+1
+        const bool first_seg = (segs_started == 1);
+        float* dstp = p.partials + (size_t)(2 * w + (first_seg ? 0 : 1)) * C::kSlotFloats;
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+#pragma unroll
+          for (int mt = 0; mt < kMT; ++mt)
+            reinterpret_cast<float4*>(dstp)[(nt * kMT + mt) * 32 + lane] =
+                make_float4(o[nt][mt][0], o[nt][mt][1], o[nt][mt][2], o[nt][mt][3]);
+          if (lane < 4) {
+            float* ml = dstp + NT * kMT * 128 + nt * 8 + 2 * lane;
+            ml[0] = m_run[nt][0]; ml[1] = m_run[nt][1];
+            ml[NT * 8] = l_run[nt][0]; ml[NT * 8 + 1] = l_run[nt][1];
+          }
+        }
+      }
+    }
+    if (wrote_smem) { fence_proxy_async(); __syncwarp(); }   // generic writes before the TMA refill
+
+    // ------------------------------------------------ advance the cursor
+    ++ck;
+    if (++c.j == c.np) {
+      c.j = 0;
+      if (++c.g == Hkv) {
+        c.g = 0;
+        do { ++c.i; } while (c.i < B && cum[c.i + 1] == cum[c.i]);
+        if (c.i < B) { c.np = cum[c.i + 1] - cum[c.i]; cn = slen[c.i]; }
+      }
+    }
+  }
+}
+
+// Row A8: merge a (request, kv head) pair's partials in worker order; zero-fill n == 0 rows.
+template <int D, int NT>
+__global__ void __launch_bounds__(128) attn_merge_kernel(const StreamParams p) {
+  using C = Cfg<D, NT>;
+  constexpr int kMT = C::kMT;
+  const int pair = blockIdx.x;
+  const int i = pair / p.Hkv, g = pair - i * p.Hkv;
+  const int G = p.G;
+  const int np = p.cum_out[i + 1] - p.cum_out[i];
+  __half* orow = p.out + ((size_t)i * p.Hq + (size_t)g * G) * D;
+  if (np == 0) {                                             // reading S11: empty context -> zeros
+    for (int e = threadIdx.x; e < G * D; e += blockDim.x) orow[e] = __float2half_rn(0.f);
+    return;
+  }
+  const long long N = (long long)p.Hkv * p.cum_out[p.B];
+  const long long a = (long long)p.Hkv * p.cum_out[i] + (long long)g * np, b = a + np;
+  const int W = p.W;
+  const int wa = (int)(((a + 1) * W - 1) / N), wb = (int)((b * W - 1) / N);   // workers holding tiles a, b-1
+  if (wa == wb) return;                                      // written directly by the stream kernel
+  const bool wa_first = ((long long)wa * N / W) == a;        // pair starts exactly at wa's range start
+  auto slot_of = [&](int w) -> const float* {
+    const int s = (w == wa && !wa_first) ? 2 * w + 1 : 2 * w;
+    return p.partials + (size_t)s * C::kSlotFloats;
+  };
+  // workers with an empty range (N < W) own no tile and wrote nothing: step from owner to owner
+  auto next_owner = [&](int w) -> int {
+    const long long k_next = (long long)(w + 1) * N / W;     // first tile after w's range
+    return k_next >= b ? wb + 1 : (int)(((k_next + 1) * W - 1) / N);
+  };
+  for (int u = threadIdx.x; u < NT * kMT * 32; u += blockDim.x) {
+    const int lane = u & 31, mt = (u >> 5) % kMT, nt = u / (32 * kMT);
+    const int hb = nt * 8 + 2 * (lane & 3);
+    if (hb >= G) continue;
+    float m[2] = {-INFINITY, -INFINITY};
+    for (int w = wa; w <= wb; w = next_owner(w)) {
+      const float* ml = slot_of(w) + NT * kMT * 128 + hb;
+      m[0] = fmaxf(m[0], ml[0]); m[1] = fmaxf(m[1], ml[1]);
+    }
+    float l[2] = {0.f, 0.f}, acc[4] = {0.f, 0.f, 0.f, 0.f};
+    for (int w = wa; w <= wb; w = next_owner(w)) {           // fixed (token) order: deterministic
+      const float* sl = slot_of(w);
+      const float* ml = sl + NT * kMT * 128 + hb;
+      const float c0 = ex2(ml[0] - m[0]), c1 = ex2(ml[1] - m[1]);
+      l[0] += ml[NT * 8] * c0; l[1] += ml[NT * 8 + 1] * c1;
+      const float4 v = reinterpret_cast<const float4*>(sl)[u];
+      acc[0] += v.x * c0; acc[1] += v.y * c1; acc[2] += v.z * c0; acc[3] += v.w * c1;
+    }
+    const int d0 = 16 * mt + (lane >> 2);
+    orow[hb * D + d0] = __float2half_rn(acc[0] / l[0]);
+    orow[hb * D + d0 + 8] = __float2half_rn(acc[2] / l[0]);
+    if (hb + 1 < G) {
+      orow[(hb + 1) * D + d0] = __float2half_rn(acc[1] / l[1]);
+      orow[(hb + 1) * D + d0 + 8] = __float2half_rn(acc[3] / l[1]);
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------
 // Kernel "simple": one CTA per (request, query head), CUDA-core dot products, no split.
-// Bring-up / fallback path for shapes the streaming kernel does not cover (head_dim 64).
 // ------------------------------------------------------------------------------------------
+struct SimpleParams {
+  const __half* q; __half* out; const __half* k; const __half* v;
+  const int32_t* bt; const int32_t* lens;
+  int32_t q_heads, kv_heads, bt_stride;
+  float scale_log2;
+};
+
 template <int D>
-__global__ void __launch_bounds__(128) attn_simple_kernel(const AttnParams p) {
-  constexpr int E = D / 32;                       // elements per lane
+__global__ void __launch_bounds__(128) attn_simple_kernel(const SimpleParams p) {
+  constexpr int E = D / 32;
   const int h = blockIdx.x, i = blockIdx.y;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int n = p.seq_lens[i];
-  const int G = p.q_heads / p.kv_heads;
-  const int g = h / G;
-  const int ps = p.page_size;
-  const __half* K = static_cast<const __half*>(p.k);
-  const __half* V = static_cast<const __half*>(p.v);
-  const __half* qrow = static_cast<const __half*>(p.q) + ((size_t)i * p.q_heads + h) * D;
-  __half* orow = static_cast<__half*>(p.out) + ((size_t)i * p.q_heads + h) * D;
-
+  const int n = p.lens[i];
+  const int g = h / (p.q_heads / p.kv_heads);
+  const __half* qrow = p.q + ((size_t)i * p.q_heads + h) * D;
+  __half* orow = p.out + ((size_t)i * p.q_heads + h) * D;
   float qf[E], acc[E];
 #pragma unroll
   for (int e = 0; e < E; ++e) { qf[e] = __half2float(qrow[lane * E + e]); acc[e] = 0.f; }
   float m = -INFINITY, l = 0.f;
-  const float scale_log2 = p.sm_scale * 1.4426950408889634f;
-
   for (int t = warp; t < n; t += 4) {
-    const int page = p.block_table[(size_t)i * p.bt_stride + t / ps];
-    const size_t off = (((size_t)page * p.kv_heads + g) * ps + (t % ps)) * D + lane * E;
+    const int page = p.bt[(size_t)i * p.bt_stride + (t >> 4)];
+    const size_t off = (((size_t)page * p.kv_heads + g) * 16 + (t & 15)) * D + lane * E;
     float dot = 0.f;
 #pragma unroll
-    for (int e = 0; e < E; ++e) dot += qf[e] * __half2float(K[off + e]);
+    for (int e = 0; e < E; ++e) dot += qf[e] * __half2float(p.k[off + e]);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) dot += __shfl_xor_sync(0xffffffffu, dot, o);
-    const float s = dot * scale_log2;
+    const float s = dot * p.scale_log2;
     const float m_new = fmaxf(m, s);
-    const float corr = exp2f(m - m_new);          // m = -inf on first token -> 0
-    const float w = exp2f(s - m_new);
-    l = l * corr + w;
+    const float corr = exp2f(m - m_new), wgt = exp2f(s - m_new);
+    l = l * corr + wgt;
 #pragma unroll
-    for (int e = 0; e < E; ++e) acc[e] = acc[e] * corr + w * __half2float(V[off + e]);
+    for (int e = 0; e < E; ++e) acc[e] = acc[e] * corr + wgt * __half2float(p.v[off + e]);
     m = m_new;
   }
-
   __shared__ float sm_m[4], sm_l[4], sm_acc[4][D];
   if (lane == 0) { sm_m[warp] = m; sm_l[warp] = l; }
 #pragma unroll
   for (int e = 0; e < E; ++e) sm_acc[warp][lane * E + e] = acc[e];
   __syncthreads();
   if (warp == 0) {
-    float mm = fmaxf(fmaxf(sm_m[0], sm_m[1]), fmaxf(sm_m[2], sm_m[3]));
+    const float mm = fmaxf(fmaxf(sm_m[0], sm_m[1]), fmaxf(sm_m[2], sm_m[3]));
     float ll = 0.f, o[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) o[e] = 0.f;
-    for (int w = 0; w < 4; ++w) {                 // fixed order: deterministic
+    for (int w = 0; w < 4; ++w) {
       const float c = (sm_m[w] == -INFINITY) ? 0.f : exp2f(sm_m[w] - mm);
       ll += sm_l[w] * c;
 #pragma unroll
       for (int e = 0; e < E; ++e) o[e] += sm_acc[w][lane * E + e] * c;
     }
-    const float inv = (n > 0) ? 1.f / ll : 0.f;
 #pragma unroll
-    for (int e = 0; e < E; ++e) orow[lane * E + e] = __float2half_rn(n > 0 ? o[e] * inv : 0.f);
+    for (int e = 0; e < E; ++e) orow[lane * E + e] = __float2half_rn(n > 0 ? o[e] / ll : 0.f);
   }
+}
+
+// ---------------------------------------------------------------------------- host side
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int get_encode_fn(EncodeTiledFn* out) {
+  static EncodeTiledFn fn = nullptr;
+  static std::mutex mu;
+  std::lock_guard<std::mutex> lock(mu);
+  if (!fn) {
+    void* ptr = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    HX_CUDA_OK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres));
+    if (qres != cudaDriverEntryPointSuccess || !ptr) HX_FAIL(HX_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
+    fn = reinterpret_cast<EncodeTiledFn>(ptr);
+  }
+  *out = fn;
+  return HX_OK;
+}
+
+// Tensor map over a whole K or V cache viewed as [D/64 halves][rows][64] with rows = layers*P*Hkv*16:
+// box {64, 16, D/64} = one (page, head) tile, landing in shared memory as [half][16 tok][128 B] with
+// the 128-byte swizzle (conflict-free ldmatrix).
+int make_tile_map(CUtensorMap* tm, const void* base, uint64_t rows, int D) {
+  EncodeTiledFn enc;
+  int rc = get_encode_fn(&enc);
+  if (rc) return rc;
+  cuuint64_t dims[3] = {64, rows, (cuuint64_t)(D / 64)};
+  cuuint64_t strides[2] = {(cuuint64_t)D * 2, 128};
+  cuuint32_t box[3] = {64, 16, (cuuint32_t)(D / 64)};
+  cuuint32_t es[3] = {1, 1, 1};
+  CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, const_cast<void*>(base), dims, strides, box, es,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) HX_FAIL(HX_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d) for base=%p rows=%llu D=%d", (int)r, base,
+                                 (unsigned long long)rows, D);
+  return HX_OK;
+}
+
+struct MapCacheEntry { const void* k; const void* v; uint64_t rows; int D; CUtensorMap tk, tv; };
+
+int get_tile_maps(const void* k, const void* v, uint64_t rows, int D, CUtensorMap* tk, CUtensorMap* tv) {
+  static std::mutex mu;
+  static MapCacheEntry cache[16];
+  static int n = 0, next = 0;
+  std::lock_guard<std::mutex> lock(mu);
+  for (int e = 0; e < n; ++e)
+    if (cache[e].k == k && cache[e].v == v && cache[e].rows == rows && cache[e].D == D) {
+      *tk = cache[e].tk; *tv = cache[e].tv;
+      return HX_OK;
+    }
+  MapCacheEntry ent;
+  ent.k = k; ent.v = v; ent.rows = rows; ent.D = D;
+  int rc = make_tile_map(&ent.tk, k, rows, D);
+  if (rc) return rc;
+  rc = make_tile_map(&ent.tv, v, rows, D);
+  if (rc) return rc;
+  cache[next] = ent;
+  next = (next + 1) % 16;
+  if (n < 16) ++n;
+  *tk = ent.tk; *tv = ent.tv;
+  return HX_OK;
+}
+
+template <int D, int NT>
+int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream) {
+  using C = Cfg<D, NT>;
+  static bool attr_set[64] = {false};
+  if (!attr_set[di.device]) {
+    if (C::kSmem > di.max_smem_optin) HX_FAIL(HX_ERR_UNSUPPORTED, "device offers %d B shared memory per CTA, kernel needs %d", di.max_smem_optin, C::kSmem);
+    HX_CUDA_OK(cudaFuncSetAttribute(attn_stream_kernel<D, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmem));
+    attr_set[di.device] = true;
+  }
+  const uint64_t rows_per_layer = (uint64_t)a.num_pages * a.kv_heads * 16;
+  const uint64_t rows = rows_per_layer * a.layers;
+  if (rows >= (1ull << 31)) HX_FAIL(HX_ERR_UNSUPPORTED, "cache too large for one tensor map (%llu rows)", (unsigned long long)rows);
+  CUtensorMap tk, tv;
+  int rc = get_tile_maps(a.k_base, a.v_base, rows, D, &tk, &tv);
+  if (rc) return rc;
+
+  int grid = di.sm_count;
+  if (grid * kWarps > kMaxWorkers) grid = kMaxWorkers / kWarps;
+  char* ws = static_cast<char*>(a.workspace);
+  const size_t partial_bytes = (size_t)2 * kMaxWorkers * C::kSlotFloats * sizeof(float);
+  for (int b0 = 0; b0 < a.batch; b0 += kBMax) {
+    StreamParams p;
+    p.B = (a.batch - b0 < kBMax) ? a.batch - b0 : kBMax;
+    p.q = static_cast<const __half*>(a.q) + (size_t)b0 * a.q_heads * D;
+    p.out = static_cast<__half*>(a.out) + (size_t)b0 * a.q_heads * D;
+    p.bt = a.block_table + (size_t)b0 * a.bt_stride;
+    p.lens = a.seq_lens + b0;
+    p.partials = reinterpret_cast<float*>(ws);
+    p.cum_out = reinterpret_cast<int32_t*>(ws + partial_bytes);
+    p.Hq = a.q_heads; p.Hkv = a.kv_heads; p.G = a.q_heads / a.kv_heads; p.bt_stride = a.bt_stride;
+    p.layer_row0 = (uint32_t)(rows_per_layer * a.layer);
+    p.scale_log2 = a.sm_scale * kLog2e;
+    p.W = grid * kWarps;
+    attn_stream_kernel<D, NT><<<grid, kWarps * 32, C::kSmem, stream>>>(tk, tv, p);
+    HX_CUDA_OK(cudaGetLastError());
+    attn_merge_kernel<D, NT><<<p.B * p.Hkv, 128, 0, stream>>>(p);
+    HX_CUDA_OK(cudaGetLastError());
+  }
+  return HX_OK;
+}
+
+template <int D>
+int launch_simple(const AttnParams& a, cudaStream_t stream) {
+  SimpleParams p;
+  const size_t layer_elems = (size_t)a.num_pages * a.kv_heads * 16 * D;
+  p.q = static_cast<const __half*>(a.q); p.out = static_cast<__half*>(a.out);
+  p.k = static_cast<const __half*>(a.k_base) + layer_elems * a.layer;
+  p.v = static_cast<const __half*>(a.v_base) + layer_elems * a.layer;
+  p.bt = a.block_table; p.lens = a.seq_lens;
+  p.q_heads = a.q_heads; p.kv_heads = a.kv_heads; p.bt_stride = a.bt_stride;
+  p.scale_log2 = a.sm_scale * kLog2e;
+  attn_simple_kernel<D><<<dim3(a.q_heads, a.batch), 128, 0, stream>>>(p);
+  HX_CUDA_OK(cudaGetLastError());
+  return HX_OK;
 }
 
 }  // namespace
 
 size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, int32_t head_dim,
                             int32_t max_seq_len, int32_t page_size) {
-  (void)batch; (void)q_heads; (void)kv_heads; (void)head_dim; (void)max_seq_len; (void)page_size;
-  return 0;
+  (void)batch; (void)max_seq_len; (void)page_size;
+  const int G = q_heads / kv_heads;
+  const int nt = G > 8 ? 2 : 1;
+  const size_t slot = (size_t)nt * ((head_dim / 16) * 128 + 16) * sizeof(float);
+  const size_t bytes = 2 * (size_t)kMaxWorkers * slot + (size_t)(kBMax + 1) * sizeof(int32_t);
+  return (bytes + 15) & ~(size_t)15;
 }
 
-int launch_attention(const AttnParams& p, cudaStream_t stream) {
-  dim3 grid(p.q_heads, p.batch);
-  if (p.head_dim == 128) attn_simple_kernel<128><<<grid, 128, 0, stream>>>(p);
-  else                   attn_simple_kernel<64><<<grid, 128, 0, stream>>>(p);
-  HX_CUDA_OK(cudaGetLastError());
-  return HX_OK;
+int launch_attention(const AttnParams& a, cudaStream_t stream) {
+  DeviceInfo di;
+  int rc = device_info(&di);
+  if (rc) return rc;
+  static const bool simple = [] { const char* e = getenv("HX_ATTN_IMPL"); return e && !strcmp(e, "simple"); }();
+  if (simple) return a.head_dim == 128 ? launch_simple<128>(a, stream) : launch_simple<64>(a, stream);
+  const int G = a.q_heads / a.kv_heads;
+  if (a.head_dim == 128) return G > 8 ? launch_stream<128, 2>(a, di, stream) : launch_stream<128, 1>(a, di, stream);
+  return G > 8 ? launch_stream<64, 2>(a, di, stream) : launch_stream<64, 1>(a, di, stream);
 }
 
 }  // namespace hx

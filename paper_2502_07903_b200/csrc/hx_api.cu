@@ -170,10 +170,8 @@ int hx_decode_attention(void* out, const void* q, const hx_paged_cache* cache, i
 
   AttnParams p;
   memset(&p, 0, sizeof(p));
-  const size_t layer_elems = (size_t)cache->num_pages * cache->kv_heads * cache->page_size * cache->head_dim;
   p.out = out; p.q = q;
-  p.k = static_cast<const char*>(cache->k) + (size_t)layer * layer_elems * 2;
-  p.v = static_cast<const char*>(cache->v) + (size_t)layer * layer_elems * 2;
+  p.k_base = cache->k; p.v_base = cache->v; p.layer = layer; p.layers = cache->layers;
   p.block_table = block_table; p.seq_lens = seq_lens;
   p.workspace = workspace; p.workspace_bytes = workspace_bytes;
   p.batch = batch; p.q_heads = q_heads; p.kv_heads = cache->kv_heads; p.head_dim = cache->head_dim;

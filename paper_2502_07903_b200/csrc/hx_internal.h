@@ -53,13 +53,14 @@ int launch_ingest(const IngestParams& p, bool gather, cudaStream_t stream);
 struct AttnParams {
   void* out;
   const void* q;
-  const void* k;                  // layer base already applied
-  const void* v;
+  const void* k_base;             // whole cache (all layers)
+  const void* v_base;
   const int32_t* block_table;
   const int32_t* seq_lens;
   void* workspace;
   size_t workspace_bytes;
   int32_t batch, q_heads, kv_heads, head_dim, page_size, num_pages, bt_stride, max_seq_len;
+  int32_t layer, layers;
   float sm_scale;
 };
 size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, int32_t head_dim,
