@@ -18,8 +18,9 @@
 //    query heads from shared memory and nothing is padded along tokens.  Online softmax (row A6)
 //    in fp32 on the accumulator fragments; P^T is re-laid for the second MMA with movmatrix.
 //  * A range that covers a whole (request, kv head) writes fp16 output directly; a range that
-//    starts or ends inside one writes an (m, l, acc) partial; attn_merge_kernel (row A8) combines
-//    a pair's partials in worker order (= token order), normalises, and zero-fills n == 0 rows.
+//    starts or ends inside one writes an (m, l, acc) partial and bumps the pair's arrival counter;
+//    the last arriver merges the pair's partials in worker order (= token order, so the result
+//    does not depend on who arrives last), normalises and writes (row A8).  No second launch.
 //
 // attn_simple_kernel — one CTA per (request, q head) on CUDA cores; bring-up/debug only
 // (HX_ATTN_IMPL=simple).
@@ -59,7 +60,7 @@ struct StreamParams {
   const int32_t* bt;
   const int32_t* lens;
   float* partials;        // [2 * W][kSlotFloats]
-  int32_t* cum_out;       // [B + 1] page prefix sums, written by CTA 0 for the merge kernel
+  int32_t* counters;      // [B * Hkv] arrival counters of split pairs; zero between calls
   int32_t B, Hq, Hkv, G, bt_stride;
   uint32_t layer_row0;    // first tensor-map row of the layer
   float scale_log2;
@@ -192,8 +193,12 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
       if (i < B) cum[i + 1] = off;
     }
     __syncthreads();
-    if (blockIdx.x == 0)
-      for (int i = tid; i <= B; i += kWarps * 32) p.cum_out[i] = cum[i];
+    // reading S11: an empty context gives a zero output row (no tile ever touches it)
+    for (int i = blockIdx.x * (kWarps * 32) + tid; i < B; i += gridDim.x * (kWarps * 32))
+      if (slen[i] == 0) {
+        int4* row = reinterpret_cast<int4*>(p.out + (size_t)i * p.Hq * D);
+        for (int e = 0; e < p.Hq * D / 8; ++e) row[e] = make_int4(0, 0, 0, 0);
+      }
   }
 
   const long long N = (long long)Hkv * cum[B];
@@ -394,8 +399,76 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
           l += __shfl_xor_sync(FULL, l, 16);
           l_run[nt][e] = l;
         }
-      if (seg_j0 == 0 && last_page) {
-        // whole (request, kv head) in this range: normalise, transpose through the freed K tile
+      bool emit = (seg_j0 == 0 && last_page);         // whole (request, kv head) inside this range
+      if (!emit) {
+        // ---- partial: first segment of this worker -> slot 2w, any later partial is its last -> 2w+1
+        const bool first_seg = (segs_started == 1);
+        float* dstp = p.partials + (size_t)(2 * w + (first_seg ? 0 : 1)) * C::kSlotFloats;
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+#pragma unroll
+          for (int mt = 0; mt < kMT; ++mt)
+            __stcg(reinterpret_cast<float4*>(dstp) + (nt * kMT + mt) * 32 + lane,
+                   make_float4(o[nt][mt][0], o[nt][mt][1], o[nt][mt][2], o[nt][mt][3]));
+          if (lane < 4) {
+            float* ml = dstp + NT * kMT * 128 + nt * 8 + 2 * lane;
+            __stcg(reinterpret_cast<float2*>(ml), make_float2(m_run[nt][0], m_run[nt][1]));
+            __stcg(reinterpret_cast<float2*>(ml + NT * 8), make_float2(l_run[nt][0], l_run[nt][1]));
+          }
+        }
+        // ---- last arriver merges (row A8).  Owners of this pair's tiles [a, b): workers wa..wb.
+        const long long a = (long long)Hkv * cum[c.i] + (long long)c.g * c.np, b = a + c.np;
+        const int W = p.W;
+        const int wa = (int)(((a + 1) * W - 1) / N), wb = (int)((b * W - 1) / N);
+        const int nseg = (N >= W) ? wb - wa + 1 : c.np;          // N < W: one tile per non-empty worker
+        int* counter = p.counters + c.i * Hkv + c.g;
+        __threadfence();
+        __syncwarp();
+        int old = 0;
+        if (lane == 0) old = atomicAdd(counter, 1);
+        old = __shfl_sync(FULL, old, 0);
+        if (old == nseg - 1) {
+          if (lane == 0) *counter = 0;                           // leave the workspace clean for the next call
+          __threadfence();
+          const bool wa_first = ((long long)wa * N / W) == a;
+          auto slot_of = [&](int ww) -> const float* {
+            return p.partials + (size_t)((ww == wa && !wa_first) ? 2 * ww + 1 : 2 * ww) * C::kSlotFloats;
+          };
+          auto next_owner = [&](int ww) -> int {                 // skips workers with an empty range
+            const long long kn = (long long)(ww + 1) * N / W;
+            return kn >= b ? wb + 1 : (int)(((kn + 1) * W - 1) / N);
+          };
+          const int hb = 2 * (lane & 3);
+#pragma unroll
+          for (int nt = 0; nt < NT; ++nt) {
+            float mm0 = -INFINITY, mm1 = -INFINITY;
+            for (int ww = wa; ww <= wb; ww = next_owner(ww)) {
+              const float2 mv = __ldcg(reinterpret_cast<const float2*>(slot_of(ww) + NT * kMT * 128 + nt * 8 + hb));
+              mm0 = fmaxf(mm0, mv.x); mm1 = fmaxf(mm1, mv.y);
+            }
+            float l0 = 0.f, l1 = 0.f;
+#pragma unroll
+            for (int mt = 0; mt < kMT; ++mt) o[nt][mt][0] = o[nt][mt][1] = o[nt][mt][2] = o[nt][mt][3] = 0.f;
+            for (int ww = wa; ww <= wb; ww = next_owner(ww)) {     // fixed (token) order: deterministic
+              const float* sl = slot_of(ww);
+              const float2 mv = __ldcg(reinterpret_cast<const float2*>(sl + NT * kMT * 128 + nt * 8 + hb));
+              const float2 lv = __ldcg(reinterpret_cast<const float2*>(sl + NT * kMT * 128 + NT * 8 + nt * 8 + hb));
+              const float c0 = ex2(mv.x - mm0), c1 = ex2(mv.y - mm1);
+              l0 += lv.x * c0; l1 += lv.y * c1;
+#pragma unroll
+              for (int mt = 0; mt < kMT; ++mt) {
+                const float4 v = __ldcg(reinterpret_cast<const float4*>(sl) + (nt * kMT + mt) * 32 + lane);
+                o[nt][mt][0] += v.x * c0; o[nt][mt][1] += v.y * c1;
+                o[nt][mt][2] += v.z * c0; o[nt][mt][3] += v.w * c1;
+              }
+            }
+            l_run[nt][0] = l0; l_run[nt][1] = l1;
+          }
+          emit = true;
+        }
+      }
+      if (emit) {
+        // normalise, transpose through the just-consumed K tile, 16-byte coalesced stores
         __half* scratch = reinterpret_cast<__half*>(my_stage + stage * C::kStage);
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt) {
@@ -416,22 +489,6 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         for (int e = lane; e < G * D / 8; e += 32) dst[e] = srcv[e];
         __syncwarp();
         wrote_smem = true;
-      } else {
-        // first segment of this worker -> slot 2w, any later partial segment is its last -> 2w+1
-        const bool first_seg = (segs_started == 1);
-        float* dstp = p.partials + (size_t)(2 * w + (first_seg ? 0 : 1)) * C::kSlotFloats;
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) {
-#pragma unroll
-          for (int mt = 0; mt < kMT; ++mt)
-            reinterpret_cast<float4*>(dstp)[(nt * kMT + mt) * 32 + lane] =
-                make_float4(o[nt][mt][0], o[nt][mt][1], o[nt][mt][2], o[nt][mt][3]);
-          if (lane < 4) {
-            float* ml = dstp + NT * kMT * 128 + nt * 8 + 2 * lane;
-            ml[0] = m_run[nt][0]; ml[1] = m_run[nt][1];
-            ml[NT * 8] = l_run[nt][0]; ml[NT * 8 + 1] = l_run[nt][1];
-          }
-        }
       }
     }
     if (wrote_smem) { fence_proxy_async(); __syncwarp(); }   // generic writes before the TMA refill
@@ -445,63 +502,6 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         do { ++c.i; } while (c.i < B && cum[c.i + 1] == cum[c.i]);
         if (c.i < B) { c.np = cum[c.i + 1] - cum[c.i]; cn = slen[c.i]; }
       }
-    }
-  }
-}
-
-// Row A8: merge a (request, kv head) pair's partials in worker order; zero-fill n == 0 rows.
-template <int D, int NT>
-__global__ void __launch_bounds__(128) attn_merge_kernel(const StreamParams p) {
-  using C = Cfg<D, NT>;
-  constexpr int kMT = C::kMT;
-  const int pair = blockIdx.x;
-  const int i = pair / p.Hkv, g = pair - i * p.Hkv;
-  const int G = p.G;
-  const int np = p.cum_out[i + 1] - p.cum_out[i];
-  __half* orow = p.out + ((size_t)i * p.Hq + (size_t)g * G) * D;
-  if (np == 0) {                                             // reading S11: empty context -> zeros
-    for (int e = threadIdx.x; e < G * D; e += blockDim.x) orow[e] = __float2half_rn(0.f);
-    return;
-  }
-  const long long N = (long long)p.Hkv * p.cum_out[p.B];
-  const long long a = (long long)p.Hkv * p.cum_out[i] + (long long)g * np, b = a + np;
-  const int W = p.W;
-  const int wa = (int)(((a + 1) * W - 1) / N), wb = (int)((b * W - 1) / N);   // workers holding tiles a, b-1
-  if (wa == wb) return;                                      // written directly by the stream kernel
-  const bool wa_first = ((long long)wa * N / W) == a;        // pair starts exactly at wa's range start
-  auto slot_of = [&](int w) -> const float* {
-    const int s = (w == wa && !wa_first) ? 2 * w + 1 : 2 * w;
-    return p.partials + (size_t)s * C::kSlotFloats;
-  };
-  // workers with an empty range (N < W) own no tile and wrote nothing: step from owner to owner
-  auto next_owner = [&](int w) -> int {
-    const long long k_next = (long long)(w + 1) * N / W;     // first tile after w's range
-    return k_next >= b ? wb + 1 : (int)(((k_next + 1) * W - 1) / N);
-  };
-  for (int u = threadIdx.x; u < NT * kMT * 32; u += blockDim.x) {
-    const int lane = u & 31, mt = (u >> 5) % kMT, nt = u / (32 * kMT);
-    const int hb = nt * 8 + 2 * (lane & 3);
-    if (hb >= G) continue;
-    float m[2] = {-INFINITY, -INFINITY};
-    for (int w = wa; w <= wb; w = next_owner(w)) {
-      const float* ml = slot_of(w) + NT * kMT * 128 + hb;
-      m[0] = fmaxf(m[0], ml[0]); m[1] = fmaxf(m[1], ml[1]);
-    }
-    float l[2] = {0.f, 0.f}, acc[4] = {0.f, 0.f, 0.f, 0.f};
-    for (int w = wa; w <= wb; w = next_owner(w)) {           // fixed (token) order: deterministic
-      const float* sl = slot_of(w);
-      const float* ml = sl + NT * kMT * 128 + hb;
-      const float c0 = ex2(ml[0] - m[0]), c1 = ex2(ml[1] - m[1]);
-      l[0] += ml[NT * 8] * c0; l[1] += ml[NT * 8 + 1] * c1;
-      const float4 v = reinterpret_cast<const float4*>(sl)[u];
-      acc[0] += v.x * c0; acc[1] += v.y * c1; acc[2] += v.z * c0; acc[3] += v.w * c1;
-    }
-    const int d0 = 16 * mt + (lane >> 2);
-    orow[hb * D + d0] = __float2half_rn(acc[0] / l[0]);
-    orow[hb * D + d0 + 8] = __float2half_rn(acc[2] / l[0]);
-    if (hb + 1 < G) {
-      orow[(hb + 1) * D + d0] = __float2half_rn(acc[1] / l[1]);
-      orow[(hb + 1) * D + d0 + 8] = __float2half_rn(acc[3] / l[1]);
     }
   }
 }
@@ -658,14 +658,12 @@ int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream
     p.bt = a.block_table + (size_t)b0 * a.bt_stride;
     p.lens = a.seq_lens + b0;
     p.partials = reinterpret_cast<float*>(ws);
-    p.cum_out = reinterpret_cast<int32_t*>(ws + partial_bytes);
+    p.counters = reinterpret_cast<int32_t*>(ws + partial_bytes);
     p.Hq = a.q_heads; p.Hkv = a.kv_heads; p.G = a.q_heads / a.kv_heads; p.bt_stride = a.bt_stride;
     p.layer_row0 = (uint32_t)(rows_per_layer * a.layer);
     p.scale_log2 = a.sm_scale * kLog2e;
     p.W = grid * kWarps;
     attn_stream_kernel<D, NT><<<grid, kWarps * 32, C::kSmem, stream>>>(tk, tv, p);
-    HX_CUDA_OK(cudaGetLastError());
-    attn_merge_kernel<D, NT><<<p.B * p.Hkv, 128, 0, stream>>>(p);
     HX_CUDA_OK(cudaGetLastError());
   }
   return HX_OK;
@@ -694,7 +692,7 @@ size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, in
   const int G = q_heads / kv_heads;
   const int nt = G > 8 ? 2 : 1;
   const size_t slot = (size_t)nt * ((head_dim / 16) * 128 + 16) * sizeof(float);
-  const size_t bytes = 2 * (size_t)kMaxWorkers * slot + (size_t)(kBMax + 1) * sizeof(int32_t);
+  const size_t bytes = 2 * (size_t)kMaxWorkers * slot + (size_t)kBMax * kv_heads * sizeof(int32_t);
   return (bytes + 15) & ~(size_t)15;
 }
 

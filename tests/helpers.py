@@ -27,7 +27,7 @@ def run_gpu_attention(hx, torch, w, *, layer=0, sm_scale=0.0, q=None):
     max_len = int(w["seq_lens"].max(initial=0))
     Hkv = k.shape[2]
     ws_bytes = hx.decode_attention_workspace_bytes(B, Hq, Hkv, D, max_len, k.shape[3])
-    ws = torch.empty(max(ws_bytes, 16), dtype=torch.uint8, device="cuda")
+    ws = torch.zeros(max(ws_bytes, 16), dtype=torch.uint8, device="cuda")
     hx.decode_attention(out, qd, cache, layer=layer, q_heads=Hq, block_table=bt,
                         block_table_stride=bt.shape[1], seq_lens=sl, batch=B, max_seq_len=max_len,
                         sm_scale=sm_scale, workspace=ws, workspace_bytes=ws_bytes)
