@@ -6,7 +6,7 @@ import os
 from typing import Optional, Sequence
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "libhx.so")
+_SO = os.environ.get("HX_LIB") or os.path.join(_HERE, "libhx.so")   # HX_LIB: load another build (A/B timing)
 
 HX_OK, HX_ERR_INVALID_ARG, HX_ERR_UNSUPPORTED, HX_ERR_WORKSPACE, HX_ERR_CUDA, HX_ERR_NO_PAGES = range(6)
 

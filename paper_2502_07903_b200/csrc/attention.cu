@@ -36,11 +36,9 @@
 namespace hx {
 namespace {
 
-constexpr int kWarps = 8;          // consumer warps per CTA; tile t of a chunk belongs to warp t % 8
-constexpr int kBMax = 1024;        // requests per launch (prefix sums live in shared memory)
-constexpr int kMaxChunks = 4608;   // bound on chunk ids: nCTA * (levels + 2), nCTA <= 256, levels <= 16
-constexpr int kChunkRing = 32;     // per-CTA ring of claimed chunks
-constexpr int kRS = 4;             // own tiles described per lookahead round (lanes 0..kRS-1)
+constexpr int kWarps = 8;          // warps (= independent workers) per CTA
+constexpr int kBMax = 2048;        // requests per launch (prefix sums live in shared memory)
+constexpr int kMaxWorkers = 2048;  // workspace is sized for this many workers (>= SMs * kWarps)
 constexpr float kLog2e = 1.4426950408889634f;
 
 template <int D, int NT>
@@ -48,15 +46,12 @@ struct Cfg {
   static constexpr int kStages = (NT == 1) ? 3 : 2;
   static constexpr int kTile = 16 * D * 2;           // bytes of one (page, head) K or V tile
   static constexpr int kStage = 2 * kTile;           // K + V
-  static constexpr int kQBytes = NT * 8 * D * 2;     // per-warp Q slot: NT*8 heads
+  static constexpr int kQBytes = NT * 8 * D * 2;     // Q slot: NT*8 heads
   static constexpr int kKS = D / 16;                 // k-steps of QK^T
   static constexpr int kMT = D / 16;                 // m-tiles of PV
-  static constexpr int kSlices = NT * kMT;           // 16-row slices of O^T, one float4 per lane each
-  static constexpr int kSlotFloats = kSlices * 128 + NT * 16;   // partial: acc[slices][32][4], m[NT][8], l[NT][8]
-  static constexpr int kCtl = 4 * kChunkRing * 4 + 64 + kWarps * (NT * 16 + 1) * 4 + (6 + 3 * 40) * 4 + 16;
+  static constexpr int kSlotFloats = NT * (kMT * 128 + 16);   // partial: acc[NT][MT][32][4], m[NT][8], l[NT][8]
   static constexpr int kSmem = kWarps * kStages * kStage + kWarps * kQBytes + kWarps * (kStages + 1) * 8 +
-                               (kBMax + 1) * 4 + kBMax * 4 + kCtl;
-  static_assert(kStage >= kSlices * 512, "a consumed stage must hold one warp's O^T as merge scratch");
+                               (kBMax + 1) * 4 + kBMax * 4;
 };
 
 struct StreamParams {
@@ -64,12 +59,12 @@ struct StreamParams {
   __half* out;
   const int32_t* bt;
   const int32_t* lens;
-  int32_t* ctrl;          // [0] next chunk id, [1] finished CTAs; zero between calls
-  int32_t* counters;      // [B * Hkv] arrival counters of pairs split across chunks; zero between calls
-  float* partials;        // [2 * kMaxChunks][kSlotFloats]
+  float* partials;        // [2 * W][kSlotFloats]
+  int32_t* counters;      // [B * Hkv] arrival counters of split pairs; zero between calls
   int32_t B, Hq, Hkv, G, bt_stride;
   uint32_t layer_row0;    // first tensor-map row of the layer
   float scale_log2;
+  int32_t W;              // total workers = gridDim.x * kWarps
 };
 
 // ---------------------------------------------------------------------------- PTX helpers
@@ -146,90 +141,32 @@ __device__ __forceinline__ Loc locate(long long k, const int* cum, int B, int Hk
 }
 
 // ------------------------------------------------------------------------------------------
-// Guided chunk schedule over the tile sequence [0, N): a deterministic function of (N, nC, M).
-// Level l holds nC chunks of s_l = roundup8(R_l / (2 nC)) tiles (R_l = tiles left at the level's
-// start), until s_l <= M; the rest goes out in chunks of M.  Chunk sizes are multiples of 8 (only
-// the very last may be short), so tile t of a chunk always belongs to warp t % 8.
-constexpr int kMaxLv = 40;
-struct ChunkSched {        // level table, built once per CTA in shared memory
-  int N, nC, M, n_lv;
-  int tail_first, tail_base;
-  int lv_first[kMaxLv], lv_base[kMaxLv], lv_size[kMaxLv];
-};
-
-__device__ void build_sched(ChunkSched* cs, int N, int nC) {
-  int m = (N / (nC * 4)) & ~7;                               // ~4 minimum-size chunks per CTA
-  cs->N = N; cs->nC = nC; cs->M = m < 8 ? 8 : (m > 32 ? 32 : m);
-  int base = 0, R = N, first = 0, l = 0;
-  while (l < kMaxLv) {
-    const int s = (R / (2 * nC) + 7) & ~7;
-    if (s <= cs->M) break;
-    cs->lv_first[l] = first; cs->lv_base[l] = base; cs->lv_size[l] = s;
-    base += nC * s; R -= nC * s; first += nC; ++l;
-  }
-  cs->n_lv = l; cs->tail_first = first; cs->tail_base = base;
-}
-__device__ __forceinline__ void chunk_range(const ChunkSched* cs, int id, int& start, int& size) {
-  for (int l = 0; l < cs->n_lv; ++l)
-    if (id < cs->lv_first[l] + cs->nC) {
-      start = cs->lv_base[l] + (id - cs->lv_first[l]) * cs->lv_size[l];
-      size = cs->lv_size[l];
-      return;
-    }
-  const long long st = (long long)cs->tail_base + (long long)(id - cs->tail_first) * cs->M;
-  start = st >= cs->N ? cs->N : (int)st;
-  size = st >= cs->N ? 0 : min(cs->M, cs->N - (int)st);
-}
-__device__ __forceinline__ int chunk_of_tile(const ChunkSched* cs, int k) {
-  for (int l = 0; l < cs->n_lv; ++l)
-    if (k < cs->lv_base[l] + cs->nC * cs->lv_size[l]) return cs->lv_first[l] + (k - cs->lv_base[l]) / cs->lv_size[l];
-  return cs->tail_first + (k - cs->tail_base) / cs->M;
-}
-
-constexpr int kEvRing = 16;        // split-pair events queued for the service warp
-struct Ctl {
-  int ch_start[kChunkRing], ch_size[kChunkRing], ch_id[kChunkRing], ev[2 * kEvRing];
-  int n_chunks, exhausted, lock, ev_head, ev_tail, cons_done, pad2[10];
-};
-
 template <int D, int NT>
-__global__ void __launch_bounds__(kWarps * 32 + 32, 1)
+__global__ void __launch_bounds__(kWarps * 32, 1)
 attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
                    const StreamParams p) {
   using C = Cfg<D, NT>;
-  constexpr int kStages = C::kStages, kTile = C::kTile, kKS = C::kKS, kMT = C::kMT, kSlices = C::kSlices;
+  constexpr int kStages = C::kStages, kTile = C::kTile, kKS = C::kKS, kMT = C::kMT;
   constexpr uint32_t FULL = 0xffffffffu;
   extern __shared__ __align__(1024) uint8_t smem[];
   uint8_t* q_base = smem + kWarps * kStages * C::kStage;
   uint64_t* bars = reinterpret_cast<uint64_t*>(q_base + kWarps * C::kQBytes);
   int* cum = reinterpret_cast<int*>(bars + kWarps * (kStages + 1));
   int* slen = cum + (kBMax + 1);
-  Ctl* ctl = reinterpret_cast<Ctl*>(slen + kBMax);
-  float* ml = reinterpret_cast<float*>(ctl + 1);            // [kWarps][NT*16]: m[8], l[8] per nt
-  int* sc_off = reinterpret_cast<int*>(ml + kWarps * NT * 16);
-  ChunkSched* sched = reinterpret_cast<ChunkSched*>(sc_off + kWarps);
-  static_assert(sizeof(Ctl) == 4 * kChunkRing * 4 + 64 && 2 * kEvRing == kChunkRing, "Ctl size");
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int B = p.B, Hkv = p.Hkv, G = p.G;
-#ifdef HX_TRACE
-  unsigned long long tr[5] = {0, 0, 0, 0, 0};
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tr[0]));
-#define HX_STAMP(x) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tr[x]))
-#else
-#define HX_STAMP(x)
-#endif
 
-  // ---- setup: page-count prefix sums (row A4), control block, barrier init
+  // ---- setup: page-count prefix sums (row A4) and barrier init; the only CTA-wide syncs
   {
     constexpr int PER = kBMax / (kWarps * 32);
     __shared__ int warp_tot[kWarps];
     int np[PER], sum = 0;
 #pragma unroll
     for (int e = 0; e < PER; ++e) {
-      const int i = tid * PER + e;                          // the service warp (tid >= 256) holds none
-      const int n = (i < B && tid < kWarps * 32) ? max(__ldg(p.lens + i), 0) : 0;
-      if (i < B && tid < kWarps * 32) slen[i] = n;
+      const int i = tid * PER + e;
+      const int n = (i < B) ? max(__ldg(p.lens + i), 0) : 0;
+      if (i < B) slen[i] = n;
       np[e] = (n + 15) >> 4;
       sum += np[e];
     }
@@ -239,187 +176,35 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
       const int t = __shfl_up_sync(FULL, incl, o);
       if (lane >= o) incl += t;
     }
-    if (lane == 31 && warp < kWarps) warp_tot[warp] = incl;
-    if (lane == 0 && warp < kWarps) {
+    if (lane == 31) warp_tot[warp] = incl;
+    if (lane == 0) {
       const uint32_t b0 = smem_u32(bars + warp * (kStages + 1));
       for (int s = 0; s <= kStages; ++s) mbar_init(b0 + 8 * s, 1);
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (tid == 0) { ctl->n_chunks = 0; ctl->exhausted = 0; ctl->lock = 0; ctl->ev_head = 0; ctl->ev_tail = 0; ctl->cons_done = 0; cum[0] = 0; }
     __syncthreads();
     int off = incl - sum;
-    for (int w = 0; w < warp && w < kWarps; ++w) off += warp_tot[w];
+    for (int w = 0; w < warp; ++w) off += warp_tot[w];
+    if (tid == 0) cum[0] = 0;
 #pragma unroll
     for (int e = 0; e < PER; ++e) {
       const int i = tid * PER + e;
       off += np[e];
-      if (i < B && tid < kWarps * 32) cum[i + 1] = off;
+      if (i < B) cum[i + 1] = off;
     }
     __syncthreads();
     // reading S11: an empty context gives a zero output row (no tile ever touches it)
-    for (int i = blockIdx.x * (kWarps * 32) + tid; i < B && tid < kWarps * 32; i += gridDim.x * (kWarps * 32))
+    for (int i = blockIdx.x * (kWarps * 32) + tid; i < B; i += gridDim.x * (kWarps * 32))
       if (slen[i] == 0) {
         int4* row = reinterpret_cast<int4*>(p.out + (size_t)i * p.Hq * D);
         for (int e = 0; e < p.Hq * D / 8; ++e) row[e] = make_int4(0, 0, 0, 0);
       }
   }
-  HX_STAMP(1);
 
-  if (tid == 0) build_sched(sched, Hkv * cum[B], (int)gridDim.x);
-  __syncthreads();
-
-  // ---- service warp: finishes pairs that were split across chunks, off the consumers' path.  For
-  // every queued event (request, kv head) it publishes this CTA's partial (fence + arrival counter)
-  // and, when it is the last arriver, merges the pair's partials in chunk order (= token order, so
-  // the result does not depend on who arrives last), normalises and writes the output (row A8).
-  if (warp == kWarps) {
-    const int tok0 = lane >> 2, hb = 2 * (lane & 3);
-    int tail = 0;
-    while (true) {
-      int head = *(volatile int*)&ctl->ev_head;
-      if (head == tail) {
-        if (*(volatile int*)&ctl->cons_done == kWarps) {
-          head = *(volatile int*)&ctl->ev_head;            // re-read: an event may precede the last exit
-          if (head == tail) break;
-        } else {
-          __nanosleep(256);
-          continue;
-        }
-      }
-      __threadfence_block();
-      const int i = ctl->ev[2 * (tail % kEvRing)], g = ctl->ev[2 * (tail % kEvRing) + 1];
-      const int np = cum[i + 1] - cum[i];
-      const int a = Hkv * cum[i] + g * np, b = a + np;      // the pair's tiles [a, b)
-      const int id_a = chunk_of_tile(sched, a), id_b = chunk_of_tile(sched, b - 1);
-      const int nseg = id_b - id_a + 1;                      // chunks that hold a part of the pair
-      int last = 0;
-      if (lane == 0) {
-        int* counter = p.counters + i * Hkv + g;
-        __threadfence();                                    // the CTA's partial slices, cumulatively
-        const int old = atomicAdd(counter, 1);
-        if (old == nseg - 1) { *counter = 0; last = 1; }    // leave the workspace clean for the next call
-        __threadfence();
-      }
-      last = __shfl_sync(FULL, last, 0);
-      if (last) {
-        __half* orow = p.out + ((size_t)i * p.Hq + (size_t)g * G) * D;
-        // slot of owner chunk id: its last segment if the pair starts inside it, else its first
-        int st_a, sz_a;
-        chunk_range(sched, id_a, st_a, sz_a);
-        const int first_slot = st_a < a ? 2 * id_a + 1 : 2 * id_a;
-        auto slot_ptr = [&](int e) -> const float* {
-          return p.partials + (size_t)(e == 0 ? first_slot : 2 * (id_a + e)) * C::kSlotFloats;
-        };
-        // pass 1: running max per head over the owners (independent loads, 4 in flight)
-        float mm[NT][2];
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) mm[nt][0] = mm[nt][1] = -INFINITY;
-        for (int e0 = 0; e0 < nseg; e0 += 4) {
-          float2 mv[4][NT];
-#pragma unroll
-          for (int u = 0; u < 4; ++u)
-#pragma unroll
-            for (int nt = 0; nt < NT; ++nt)
-              mv[u][nt] = (e0 + u < nseg) ? __ldcg(reinterpret_cast<const float2*>(slot_ptr(e0 + u) + kSlices * 128 + nt * 16 + hb))
-                                          : make_float2(-INFINITY, -INFINITY);
-#pragma unroll
-          for (int u = 0; u < 4; ++u)
-#pragma unroll
-            for (int nt = 0; nt < NT; ++nt) { mm[nt][0] = fmaxf(mm[nt][0], mv[u][nt].x); mm[nt][1] = fmaxf(mm[nt][1], mv[u][nt].y); }
-        }
-        // pass 2: owners in chunk order (= token order: deterministic); all slices of one owner in flight
-        float ll[NT][2], acc[kSlices][4];
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) ll[nt][0] = ll[nt][1] = 0.f;
-#pragma unroll
-        for (int sl = 0; sl < kSlices; ++sl) acc[sl][0] = acc[sl][1] = acc[sl][2] = acc[sl][3] = 0.f;
-        for (int e = 0; e < nseg; ++e) {
-          const float* gs = slot_ptr(e);
-          float4 v[kSlices];
-          float2 mv[NT], lv[NT];
-#pragma unroll
-          for (int sl = 0; sl < kSlices; ++sl) v[sl] = __ldcg(reinterpret_cast<const float4*>(gs) + sl * 32 + lane);
-#pragma unroll
-          for (int nt = 0; nt < NT; ++nt) {
-            mv[nt] = __ldcg(reinterpret_cast<const float2*>(gs + kSlices * 128 + nt * 16 + hb));
-            lv[nt] = __ldcg(reinterpret_cast<const float2*>(gs + kSlices * 128 + nt * 16 + 8 + hb));
-          }
-#pragma unroll
-          for (int nt = 0; nt < NT; ++nt) {
-            const float c0 = ex2(mv[nt].x - mm[nt][0]), c1 = ex2(mv[nt].y - mm[nt][1]);
-            ll[nt][0] += lv[nt].x * c0; ll[nt][1] += lv[nt].y * c1;
-#pragma unroll
-            for (int mt = 0; mt < kMT; ++mt) {
-              const int sl = nt * kMT + mt;
-              acc[sl][0] += v[sl].x * c0; acc[sl][1] += v[sl].y * c1;
-              acc[sl][2] += v[sl].z * c0; acc[sl][3] += v[sl].w * c1;
-            }
-          }
-        }
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) {
-          const float i0 = 1.f / ll[nt][0], i1 = 1.f / ll[nt][1];
-          const int h0 = nt * 8 + hb;
-#pragma unroll
-          for (int mt = 0; mt < kMT; ++mt) {
-            const int sl = nt * kMT + mt, d0 = 16 * mt + tok0;
-            if (h0 < G) {
-              orow[h0 * D + d0] = __float2half_rn(acc[sl][0] * i0);
-              orow[h0 * D + d0 + 8] = __float2half_rn(acc[sl][2] * i0);
-            }
-            if (h0 + 1 < G) {
-              orow[(h0 + 1) * D + d0] = __float2half_rn(acc[sl][1] * i1);
-              orow[(h0 + 1) * D + d0 + 8] = __float2half_rn(acc[sl][3] * i1);
-            }
-          }
-        }
-      }
-      ++tail;
-      if (lane == 0) *(volatile int*)&ctl->ev_tail = tail;
-    }
-#ifdef HX_TRACE
-    HX_STAMP(4);
-    if (lane == 0) {
-      unsigned long long* t = reinterpret_cast<unsigned long long*>(p.partials + (size_t)2 * kMaxChunks * C::kSlotFloats) + (size_t)(gridDim.x * kWarps + blockIdx.x) * 8;
-      for (int e = 0; e < 5; ++e) t[e] = tr[e];
-      t[5] = (unsigned long long)tail;
-    }
-#endif
-    // leave the scheduler state clean: the last CTA of the grid zeroes the control words
-    if (lane == 0) {
-      const int old = atomicAdd(p.ctrl + 1, 1);
-      if (old == (int)gridDim.x - 1) { p.ctrl[0] = 0; p.ctrl[1] = 0; }
-    }
-    return;
-  }
-
-  // chunk index n of this CTA's claim list: claimed on demand by whichever warp needs it first
-  auto ensure = [&](int n) -> bool {
-    while (true) {
-      if (*(volatile int*)&ctl->n_chunks > n) return true;
-      if (*(volatile int*)&ctl->exhausted) return false;
-      if (lane == 0 && atomicCAS(&ctl->lock, 0, 1) == 0) {
-        const int nc = *(volatile int*)&ctl->n_chunks;
-        if (nc <= n && !*(volatile int*)&ctl->exhausted) {
-          const int id = atomicAdd(p.ctrl, 1);
-          int st, sz;
-          chunk_range(sched, id, st, sz);
-          if (sz == 0) {
-            *(volatile int*)&ctl->exhausted = 1;
-          } else {
-            const int s = nc % kChunkRing;
-            ctl->ch_start[s] = st; ctl->ch_size[s] = sz; ctl->ch_id[s] = id;
-            __threadfence_block();
-            *(volatile int*)&ctl->n_chunks = nc + 1;
-          }
-        }
-        __threadfence_block();
-        atomicExch(&ctl->lock, 0);
-      }
-      __syncwarp();
-    }
-  };
-  auto own_count = [&](int size) -> int { return size > warp ? ((size - warp - 1) >> 3) + 1 : 0; };
+  const long long N = (long long)Hkv * cum[B];
+  const int w = blockIdx.x * kWarps + warp;
+  const long long k0 = (long long)w * N / p.W, k1 = (long long)(w + 1) * N / p.W;
+  if (k0 >= k1) return;
 
   uint8_t* my_stage = smem + warp * kStages * C::kStage;
   const uint32_t stage_u32 = smem_u32(my_stage);
@@ -428,52 +213,27 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
   const uint32_t bar_u32 = smem_u32(bars + warp * (kStages + 1));
   const uint32_t qbar = bar_u32 + 8 * kStages;
 
-  // ---- lookahead over this warp's own tiles (tile o of a chunk with o % 8 == warp): lane L < kRS of
-  // round r describes own tile kRS*r + L: page id (global load), head part, Q row, "first own tile of
-  // its segment".  Rounds r and r+1 are resident, so block-table loads run 4-8 own tiles ahead.
-  int la_n = 0, la_u = 0;          // (chunk index, own offset) of own tile kRS * (cur_round + 2)
-  auto load_round = [&](int& page, int& gpart, int& meta) {
-    {  // warp-uniform: claim chunks until own tile la_u + kRS - 1 from chunk la_n exists (or none is left)
-      int n = la_n, u = la_u + kRS - 1;
-      while (ensure(n)) {
-        const int cnt = own_count(*(volatile int*)&ctl->ch_size[n % kChunkRing]);
-        if (u < cnt) break;
-        u -= cnt; ++n;
-      }
+  // ---- per-lane lookahead: lane L of round r describes tile k0 + 32 r + L
+  int page_cur = 0, gpart_cur = 0, meta_cur = 0, page_nxt = 0, gpart_nxt = 0, meta_nxt = 0;
+  auto load_round = [&](int r, int& page, int& gpart, int& meta) {
+    const long long k = k0 + 32ll * r + lane;
+    page = 0; gpart = 0; meta = 0;
+    if (k < k1) {
+      const Loc t = locate(k, cum, B, Hkv);
+      page = __ldg(p.bt + (size_t)t.i * p.bt_stride + t.j);
+      gpart = t.g * 16;
+      meta = ((t.i * p.Hq + t.g * G) << 1) | (t.j == 0 ? 1 : 0);
     }
-    const int nc = *(volatile int*)&ctl->n_chunks;
-    page = 0; gpart = 0; meta = -1;
-    int n = la_n, u = la_u + lane;
-    if (lane < kRS) {
-      while (n < nc) {
-        const int size = ctl->ch_size[n % kChunkRing];
-        const int cnt = own_count(size);
-        if (u < cnt) {
-          const int o = warp + 8 * u;
-          const Loc t = locate(ctl->ch_start[n % kChunkRing] + o, cum, B, Hkv);
-          page = __ldg(p.bt + (size_t)t.i * p.bt_stride + t.j);
-          gpart = t.g * 16;
-          const int o_seg0 = o - min(t.j, o);                 // segment's first tile in this chunk
-          const int fo = o_seg0 + ((warp - o_seg0) & 7);      // this warp's first own tile in it
-          meta = ((t.i * p.Hq + t.g * G) << 1) | (o == fo ? 1 : 0);
-          break;
-        }
-        u -= cnt; ++n;
-      }
-    }
-    // advance the round base by kRS own tiles (warp-uniform)
-    n = la_n; u = la_u + kRS;
-    while (n < nc) {
-      const int cnt = own_count(ctl->ch_size[n % kChunkRing]);
-      if (u < cnt) break;
-      u -= cnt; ++n;
-    }
-    la_n = n; la_u = u;
   };
-  int page_cur, gpart_cur, meta_cur, page_nxt, gpart_nxt, meta_nxt;
-  load_round(page_cur, gpart_cur, meta_cur);
-  load_round(page_nxt, gpart_nxt, meta_nxt);
+  load_round(0, page_cur, gpart_cur, meta_cur);
+  load_round(1, page_nxt, gpart_nxt, meta_nxt);
   int cur_round = 0;
+
+  // ---- consumer cursor (warp-uniform)
+  Loc c = locate(k0, cum, B, Hkv);
+  int cn = slen[c.i];
+  int seg_j0 = 0, segs_started = 0;
+  bool q_busy = false;
 
   // fragment-address constants
   const int a_row = (lane & 7) + ((lane >> 3) & 1) * 8;   // K (A, non-trans): token row
@@ -481,277 +241,269 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
   const int v_row = (lane & 7) + (lane >> 4) * 8;         // V (A, trans): token row
   const int v_csel = (lane >> 3) & 1;
   const int tok0 = lane >> 2;
-  const int hb = 2 * (lane & 3);
 
   uint32_t qb[NT][kKS][2];
   float o[NT][kMT][4];
   float m_run[NT][2], l_run[NT][2];
-  int pm = 0, cm = 0, q_issued = 0, q_taken = 0;          // own tiles produced / consumed; Q loads
 
-  for (int cidx = 0; ensure(cidx); ++cidx) {
-    const int cslot = cidx % kChunkRing;
-    const int cstart = ctl->ch_start[cslot], csize = ctl->ch_size[cslot], cid = ctl->ch_id[cslot];
-    Loc c = locate(cstart, cum, B, Hkv);
-    int cn = slen[c.i];
-    int oseg = 0;                                          // chunk offset of the current segment
-    while (oseg < csize) {
-      const int seg_len = min(c.np - c.j, csize - oseg);
-      const int fo = oseg + ((warp - oseg) & 7);
-      const bool has_state = fo < oseg + seg_len;
-      int last_stage = 0;
-      bool wrote_smem = false;
-      for (int oo = fo; oo < oseg + seg_len; oo += 8) {
-        // ------------------------------------------ produce: keep kStages own tiles in flight
-        while (pm < cm + kStages) {
-          if (pm / kRS != cur_round) {
-            page_cur = page_nxt; gpart_cur = gpart_nxt; meta_cur = meta_nxt;
-            ++cur_round;
-            load_round(page_nxt, gpart_nxt, meta_nxt);
-          }
-          const int src = pm % kRS;
-          const int meta = __shfl_sync(FULL, meta_cur, src);
-          if (meta < 0) break;                             // no tile left for this warp
-          const bool segstart = meta & 1;
-          if (segstart && q_issued != q_taken) break;      // Q slot still holds the running segment's Q
-          const int page = __shfl_sync(FULL, page_cur, src);
-          const int gpart = __shfl_sync(FULL, gpart_cur, src);
-          const int stage = pm % kStages;
-          if (lane == 0) {
-            if (segstart) {
-              mbar_expect_tx(qbar, (uint32_t)(G * D * 2));
-              bulk_load(q_u32, p.q + (size_t)(meta >> 1) * D, (uint32_t)(G * D * 2), qbar);
-            }
-            const uint32_t full = bar_u32 + 8 * stage;
-            const uint32_t dst = stage_u32 + stage * C::kStage;
-            const int row = (int)(p.layer_row0 + (uint32_t)page * (uint32_t)(Hkv * 16) + (uint32_t)gpart);
-            mbar_expect_tx(full, 2 * kTile);
-            tma_tile_3d(dst, &tmK, 0, row, 0, full);
-            tma_tile_3d(dst + kTile, &tmV, 0, row, 0, full);
-          }
-          if (segstart) ++q_issued;
-          ++pm;
+  long long pk = k0, ck = k0;
+  while (ck < k1) {
+    // ------------------------------------------------ produce: keep kStages tiles in flight
+    while (pk < k1 && pk - ck < kStages) {
+      const int idx = (int)(pk - k0);
+      if ((idx >> 5) != cur_round) {
+        page_cur = page_nxt; gpart_cur = gpart_nxt; meta_cur = meta_nxt;
+        ++cur_round;
+        load_round(cur_round + 1, page_nxt, gpart_nxt, meta_nxt);
+      }
+      const int src = idx & 31;
+      const int meta = __shfl_sync(FULL, meta_cur, src);
+      const bool segstart = (idx == 0) || (meta & 1);
+      if (segstart && q_busy) break;
+      const int page = __shfl_sync(FULL, page_cur, src);
+      const int gpart = __shfl_sync(FULL, gpart_cur, src);
+      const int stage = idx % kStages;
+      if (lane == 0) {
+        if (segstart) {
+          mbar_expect_tx(qbar, (uint32_t)(G * D * 2));
+          bulk_load(q_u32, p.q + (size_t)(meta >> 1) * D, (uint32_t)(G * D * 2), qbar);
         }
+        const uint32_t full = bar_u32 + 8 * stage;
+        const uint32_t dst = stage_u32 + stage * C::kStage;
+        const int row = (int)(p.layer_row0 + (uint32_t)page * (uint32_t)(Hkv * 16) + (uint32_t)gpart);
+        mbar_expect_tx(full, 2 * kTile);
+        tma_tile_3d(dst, &tmK, 0, row, 0, full);
+        tma_tile_3d(dst + kTile, &tmV, 0, row, 0, full);
+      }
+      if (segstart) q_busy = true;
+      ++pk;
+    }
 
-        // ------------------------------------------ consume own tile cm = (chunk, offset oo)
-        const int stage = cm % kStages;
-        const int j = c.j + (oo - oseg);
-        if (oo == fo) {                                    // first own tile of the segment
-          mbar_wait(qbar, q_taken & 1);
+    // ------------------------------------------------ consume tile ck
+    const int idx = (int)(ck - k0);
+    const int stage = idx % kStages;
+    if (c.j == 0 || idx == 0) {                      // segment start: fetch Q fragments, reset state
+      mbar_wait(qbar, segs_started & 1);
+      ++segs_started;
 #pragma unroll
-          for (int nt = 0; nt < NT; ++nt) {
-            const int head = nt * 8 + (lane >> 2);
-            const uint8_t* qrow = my_q + head * (D * 2) + (lane & 3) * 4;
-#pragma unroll
-            for (int ks = 0; ks < kKS; ++ks) {
-              const uint32_t b0 = *reinterpret_cast<const uint32_t*>(qrow + ks * 32);
-              const uint32_t b1 = *reinterpret_cast<const uint32_t*>(qrow + ks * 32 + 16);
-              qb[nt][ks][0] = head < G ? b0 : 0u;
-              qb[nt][ks][1] = head < G ? b1 : 0u;
-            }
-#pragma unroll
-            for (int mt = 0; mt < kMT; ++mt) o[nt][mt][0] = o[nt][mt][1] = o[nt][mt][2] = o[nt][mt][3] = 0.f;
-            m_run[nt][0] = m_run[nt][1] = -INFINITY;
-            l_run[nt][0] = l_run[nt][1] = 0.f;
-          }
-          __syncwarp();
-          ++q_taken;
-        }
-        mbar_wait(bar_u32 + 8 * stage, (cm / kStages) & 1);
-#ifdef HX_TRACE
-        if (cm == 0) HX_STAMP(2);
-        HX_STAMP(3);
-#endif
-        const uint32_t kb = stage_u32 + stage * C::kStage, vb = kb + kTile;
-        const int valid = (j == c.np - 1) ? cn - 16 * (c.np - 1) : 16;
-        if (valid < 16) {
-          // tail slots may hold anything (NaN/Inf): P is 0 there, but 0 * Inf = NaN in the PV MMA,
-          // so the V rows past the context end are zeroed in shared memory (reading S10).
-          for (int e = lane; e < (16 - valid) * (D / 8); e += 32) {
-            const int r = valid + e / (D / 8), ch = e % (D / 8);
-            *reinterpret_cast<int4*>(my_stage + stage * C::kStage + kTile + (ch >> 3) * 2048 + r * 128 + (ch & 7) * 16) =
-                make_int4(0, 0, 0, 0);
-          }
-          __syncwarp();
-          wrote_smem = true;
-        }
-
-        // ---- S^T[16 tok x 8 heads] = K[16 x D] Q^T   (row A5)
-        float sacc[NT][2][4];
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt)
-#pragma unroll
-          for (int h = 0; h < 2; ++h) sacc[nt][h][0] = sacc[nt][h][1] = sacc[nt][h][2] = sacc[nt][h][3] = 0.f;
+      for (int nt = 0; nt < NT; ++nt) {
+        const int head = nt * 8 + (lane >> 2);
+        const uint8_t* qrow = my_q + head * (D * 2) + (lane & 3) * 4;
 #pragma unroll
         for (int ks = 0; ks < kKS; ++ks) {
-          const int cix = 2 * ks + a_csel;
-          uint32_t a[4];
-          ldsm_x4(kb + (cix >> 3) * 2048 + a_row * 128 + (((cix & 7) ^ (a_row & 7)) << 4), a);
-#pragma unroll
-          for (int nt = 0; nt < NT; ++nt) mma16816(sacc[nt][ks & 1], a, qb[nt][ks][0], qb[nt][ks][1]);
+          uint32_t b0 = *reinterpret_cast<const uint32_t*>(qrow + ks * 32);
+          uint32_t b1 = *reinterpret_cast<const uint32_t*>(qrow + ks * 32 + 16);
+          qb[nt][ks][0] = head < G ? b0 : 0u;
+          qb[nt][ks][1] = head < G ? b1 : 0u;
         }
+#pragma unroll
+        for (int mt = 0; mt < kMT; ++mt) o[nt][mt][0] = o[nt][mt][1] = o[nt][mt][2] = o[nt][mt][3] = 0.f;
+        m_run[nt][0] = m_run[nt][1] = -INFINITY;
+        l_run[nt][0] = l_run[nt][1] = 0.f;
+      }
+      __syncwarp();
+      q_busy = false;
+      seg_j0 = c.j;
+    }
+    mbar_wait(bar_u32 + 8 * stage, (idx / kStages) & 1);
 
-        // ---- online softmax on the accumulator fragments (row A6)
-        uint32_t pb[NT][2];
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) {
-          float s[4];
-#pragma unroll
-          for (int r = 0; r < 4; ++r) s[r] = (sacc[nt][0][r] + sacc[nt][1][r]) * p.scale_log2;
-          if (tok0 >= valid) s[0] = s[1] = -INFINITY;
-          if (tok0 + 8 >= valid) s[2] = s[3] = -INFINITY;
-          float pr[4], corr[2];
-#pragma unroll
-          for (int e = 0; e < 2; ++e) {
-            float mx = fmaxf(s[e], s[e + 2]);
-            mx = fmaxf(mx, __shfl_xor_sync(FULL, mx, 4));
-            mx = fmaxf(mx, __shfl_xor_sync(FULL, mx, 8));
-            mx = fmaxf(mx, __shfl_xor_sync(FULL, mx, 16));
-            const float m_new = fmaxf(m_run[nt][e], mx);      // finite: every tile has >= 1 valid token
-            corr[e] = ex2(m_run[nt][e] - m_new);              // -inf -> 0 on the first tile
-            m_run[nt][e] = m_new;
-            pr[e] = ex2(s[e] - m_new);
-            pr[e + 2] = ex2(s[e + 2] - m_new);
-          }
-          const __half2 p01 = __floats2half2_rn(pr[0], pr[1]);
-          const __half2 p23 = __floats2half2_rn(pr[2], pr[3]);
-          // l sums the ROUNDED weights so that numerator and denominator use the same weights
-          l_run[nt][0] = l_run[nt][0] * corr[0] + __low2float(p01) + __low2float(p23);
-          l_run[nt][1] = l_run[nt][1] * corr[1] + __high2float(p01) + __high2float(p23);
-          pb[nt][0] = movmatrix_t(*reinterpret_cast<const uint32_t*>(&p01));   // P^T B-fragment, tokens 0-7
-          pb[nt][1] = movmatrix_t(*reinterpret_cast<const uint32_t*>(&p23));   //                tokens 8-15
-          if (__any_sync(FULL, corr[0] != 1.f || corr[1] != 1.f)) {
-#pragma unroll
-            for (int mt = 0; mt < kMT; ++mt) {
-              o[nt][mt][0] *= corr[0]; o[nt][mt][1] *= corr[1];
-              o[nt][mt][2] *= corr[0]; o[nt][mt][3] *= corr[1];
-            }
-          }
-        }
+    const uint32_t kb = stage_u32 + stage * C::kStage, vb = kb + kTile;
+    const bool last_page = (c.j == c.np - 1);
+    const int valid = last_page ? cn - 16 * (c.np - 1) : 16;
+    if (valid < 16) {
+      // tail slots may hold anything (NaN/Inf): P is 0 there, but 0 * Inf = NaN in the PV MMA,
+      // so the V rows past the context end are zeroed in shared memory (reading S10).
+      for (int e = lane; e < (16 - valid) * (D / 8); e += 32) {
+        const int r = valid + e / (D / 8), ch = e % (D / 8);
+        *reinterpret_cast<int4*>(my_stage + stage * C::kStage + kTile + (ch >> 3) * 2048 + r * 128 + (ch & 7) * 16) =
+            make_int4(0, 0, 0, 0);
+      }
+      __syncwarp();
+    }
 
-        // ---- O^T[D x 8 heads] += V^T[D x 16 tok] P^T   (row A7)
+    // ---- S^T[16 tok x 8 heads] = K[16 x D] Q^T   (row A5)
+    float sacc[NT][2][4];
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+      for (int h = 0; h < 2; ++h) sacc[nt][h][0] = sacc[nt][h][1] = sacc[nt][h][2] = sacc[nt][h][3] = 0.f;
+#pragma unroll
+    for (int ks = 0; ks < kKS; ++ks) {
+      const int cidx = 2 * ks + a_csel;
+      uint32_t a[4];
+      ldsm_x4(kb + (cidx >> 3) * 2048 + a_row * 128 + (((cidx & 7) ^ (a_row & 7)) << 4), a);
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt) mma16816(sacc[nt][ks & 1], a, qb[nt][ks][0], qb[nt][ks][1]);
+    }
+
+    // ---- online softmax on the accumulator fragments (row A6)
+    uint32_t pb[NT][2];
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) {
+      float s[4];
+#pragma unroll
+      for (int r = 0; r < 4; ++r) s[r] = (sacc[nt][0][r] + sacc[nt][1][r]) * p.scale_log2;
+      if (tok0 >= valid) s[0] = s[1] = -INFINITY;
+      if (tok0 + 8 >= valid) s[2] = s[3] = -INFINITY;
+      float pr[4], corr[2];
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        float mx = fmaxf(s[e], s[e + 2]);
+        mx = fmaxf(mx, __shfl_xor_sync(FULL, mx, 4));
+        mx = fmaxf(mx, __shfl_xor_sync(FULL, mx, 8));
+        mx = fmaxf(mx, __shfl_xor_sync(FULL, mx, 16));
+        const float m_new = fmaxf(m_run[nt][e], mx);        // finite: every tile has >= 1 valid token
+        corr[e] = ex2(m_run[nt][e] - m_new);                // -inf -> 0 on the first tile
+        m_run[nt][e] = m_new;
+        pr[e] = ex2(s[e] - m_new);
+        pr[e + 2] = ex2(s[e + 2] - m_new);
+      }
+      const __half2 p01 = __floats2half2_rn(pr[0], pr[1]);
+      const __half2 p23 = __floats2half2_rn(pr[2], pr[3]);
+      // l sums the ROUNDED weights so that numerator and denominator use the same weights
+      l_run[nt][0] = l_run[nt][0] * corr[0] + __low2float(p01) + __low2float(p23);
+      l_run[nt][1] = l_run[nt][1] * corr[1] + __high2float(p01) + __high2float(p23);
+      pb[nt][0] = movmatrix_t(*reinterpret_cast<const uint32_t*>(&p01));   // P^T B-fragment, tokens 0-7
+      pb[nt][1] = movmatrix_t(*reinterpret_cast<const uint32_t*>(&p23));   //                tokens 8-15
+      if (__any_sync(FULL, corr[0] != 1.f || corr[1] != 1.f)) {
 #pragma unroll
         for (int mt = 0; mt < kMT; ++mt) {
-          const int cix = 2 * mt + v_csel;
-          uint32_t a[4];
-          ldsm_x4_t(vb + (cix >> 3) * 2048 + v_row * 128 + (((cix & 7) ^ (v_row & 7)) << 4), a);
-#pragma unroll
-          for (int nt = 0; nt < NT; ++nt) mma16816(o[nt][mt], a, pb[nt][0], pb[nt][1]);
-        }
-        __syncwarp();                                      // every lane is done reading this stage
-        last_stage = stage;
-        ++cm;
-        if (wrote_smem && oo + 8 < oseg + seg_len) { fence_proxy_async(); __syncwarp(); wrote_smem = false; }
-      }
-
-      // -------------------------------------------- segment end: the 8 warps combine (row A8)
-      const bool complete = (c.j == 0) && (seg_len == c.np);   // whole (request, kv head) in this chunk
-      if (has_state) {
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) {
-#pragma unroll
-          for (int e = 0; e < 2; ++e) {
-            float l = l_run[nt][e];
-            l += __shfl_xor_sync(FULL, l, 4);
-            l += __shfl_xor_sync(FULL, l, 8);
-            l += __shfl_xor_sync(FULL, l, 16);
-            l_run[nt][e] = l;
-          }
-          if (lane < 4) {
-            float* w_ml = ml + warp * (NT * 16) + nt * 16;
-            w_ml[hb] = m_run[nt][0]; w_ml[hb + 1] = m_run[nt][1];
-            w_ml[8 + hb] = l_run[nt][0]; w_ml[8 + hb + 1] = l_run[nt][1];
-          }
-        }
-        float4* sc = reinterpret_cast<float4*>(my_stage + last_stage * C::kStage);   // just-consumed stage
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt)
-#pragma unroll
-          for (int mt = 0; mt < kMT; ++mt)
-            sc[(nt * kMT + mt) * 32 + lane] = make_float4(o[nt][mt][0], o[nt][mt][1], o[nt][mt][2], o[nt][mt][3]);
-        if (lane == 0) sc_off[warp] = (warp * kStages + last_stage) * C::kStage;
-        wrote_smem = true;
-      } else if (lane < NT * 16) {
-        ml[warp * (NT * 16) + lane] = ((lane & 8) == 0) ? -INFINITY : 0.f;            // m = -inf: no state
-      }
-      asm volatile("bar.sync 1, 256;" ::: "memory");
-
-      float* gslot = nullptr;
-      if (!complete) gslot = p.partials + (size_t)(2 * cid + (oseg == 0 ? 0 : 1)) * C::kSlotFloats;
-      __half* orow = p.out + ((size_t)c.i * p.Hq + (size_t)c.g * G) * D;
-      for (int sl = warp; sl < kSlices; sl += kWarps) {
-        const int nt = sl / kMT, mt = sl - nt * kMT;
-        float mm0 = -INFINITY, mm1 = -INFINITY;
-#pragma unroll
-        for (int w = 0; w < kWarps; ++w) {
-          mm0 = fmaxf(mm0, ml[w * (NT * 16) + nt * 16 + hb]);
-          mm1 = fmaxf(mm1, ml[w * (NT * 16) + nt * 16 + hb + 1]);
-        }
-        float l0 = 0.f, l1 = 0.f, acc[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-        for (int w = 0; w < kWarps; ++w) {                  // fixed warp order: deterministic
-          const float* w_ml = ml + w * (NT * 16) + nt * 16;
-          if (w_ml[0] == -INFINITY) continue;               // warp w had no tile in this segment
-          const float c0 = ex2(w_ml[hb] - mm0), c1 = ex2(w_ml[hb + 1] - mm1);
-          l0 += w_ml[8 + hb] * c0; l1 += w_ml[8 + hb + 1] * c1;
-          const float4 v = reinterpret_cast<const float4*>(smem + sc_off[w])[sl * 32 + lane];
-          acc[0] += v.x * c0; acc[1] += v.y * c1; acc[2] += v.z * c0; acc[3] += v.w * c1;
-        }
-        if (complete) {
-          const int d0 = 16 * mt + tok0, h0 = nt * 8 + hb;
-          if (h0 < G) {
-            orow[h0 * D + d0] = __float2half_rn(acc[0] / l0);
-            orow[h0 * D + d0 + 8] = __float2half_rn(acc[2] / l0);
-          }
-          if (h0 + 1 < G) {
-            orow[(h0 + 1) * D + d0] = __float2half_rn(acc[1] / l1);
-            orow[(h0 + 1) * D + d0 + 8] = __float2half_rn(acc[3] / l1);
-          }
-        } else {
-          __stcg(reinterpret_cast<float4*>(gslot) + sl * 32 + lane, make_float4(acc[0], acc[1], acc[2], acc[3]));
-          if (mt == 0 && lane < 4) {
-            float* g_ml = gslot + kSlices * 128 + nt * 16;
-            __stcg(reinterpret_cast<float2*>(g_ml + hb), make_float2(mm0, mm1));
-            __stcg(reinterpret_cast<float2*>(g_ml + 8 + hb), make_float2(l0, l1));
-          }
-        }
-      }
-      asm volatile("bar.sync 1, 256;" ::: "memory");       // scratch stages free; partial slices stored
-      if (!complete && tid == 0) {
-        // the pair continues in other chunks: queue it for the service warp
-        const int head = ctl->ev_head;
-        while (head - *(volatile int*)&ctl->ev_tail >= kEvRing) __nanosleep(64);
-        ctl->ev[2 * (head % kEvRing)] = c.i;
-        ctl->ev[2 * (head % kEvRing) + 1] = c.g;
-        __threadfence_block();
-        *(volatile int*)&ctl->ev_head = head + 1;
-      }
-      if (wrote_smem) { fence_proxy_async(); __syncwarp(); }   // generic writes before the TMA refill
-
-      // -------------------------------------------- next segment
-      oseg += seg_len;
-      c.j += seg_len;
-      if (c.j == c.np) {
-        c.j = 0;
-        if (++c.g == Hkv) {
-          c.g = 0;
-          do { ++c.i; } while (c.i < B && cum[c.i + 1] == cum[c.i]);
-          if (c.i < B) { c.np = cum[c.i + 1] - cum[c.i]; cn = slen[c.i]; }
+          o[nt][mt][0] *= corr[0]; o[nt][mt][1] *= corr[1];
+          o[nt][mt][2] *= corr[0]; o[nt][mt][3] *= corr[1];
         }
       }
     }
-  }
 
-  __syncwarp();
-  if (lane == 0) { __threadfence_block(); atomicAdd(&ctl->cons_done, 1); }
-#ifdef HX_TRACE
-  HX_STAMP(4);
-  if (lane == 0) {
-    unsigned long long* t = reinterpret_cast<unsigned long long*>(p.partials + (size_t)2 * kMaxChunks * C::kSlotFloats) + (size_t)(blockIdx.x * kWarps + warp) * 8;
-    for (int e = 0; e < 5; ++e) t[e] = tr[e];
-    t[5] = (unsigned long long)cm;
-    unsigned smid; asm volatile("mov.u32 %0, %%smid;" : "=r"(smid)); t[6] = smid;
+    // ---- O^T[D x 8 heads] += V^T[D x 16 tok] P^T   (row A7)
+#pragma unroll
+    for (int mt = 0; mt < kMT; ++mt) {
+      const int cidx = 2 * mt + v_csel;
+      uint32_t a[4];
+      ldsm_x4_t(vb + (cidx >> 3) * 2048 + v_row * 128 + (((cidx & 7) ^ (v_row & 7)) << 4), a);
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt) mma16816(o[nt][mt], a, pb[nt][0], pb[nt][1]);
+    }
+    __syncwarp();                                    // every lane is done reading this stage
+
+    // ------------------------------------------------ segment end: output or partial (row A8)
+    const bool seg_end = last_page || (ck == k1 - 1);
+    bool wrote_smem = valid < 16;
+    if (seg_end) {
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          float l = l_run[nt][e];
+          l += __shfl_xor_sync(FULL, l, 4);
+          l += __shfl_xor_sync(FULL, l, 8);
+          l += __shfl_xor_sync(FULL, l, 16);
+          l_run[nt][e] = l;
+        }
+      bool emit = (seg_j0 == 0 && last_page);         // whole (request, kv head) inside this range
+      if (!emit) {
+        // ---- partial: first segment of this worker -> slot 2w, any later partial is its last -> 2w+1
+        const bool first_seg = (segs_started == 1);
+        float* dstp = p.partials + (size_t)(2 * w + (first_seg ? 0 : 1)) * C::kSlotFloats;
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+#pragma unroll
+          for (int mt = 0; mt < kMT; ++mt)
+            __stcg(reinterpret_cast<float4*>(dstp) + (nt * kMT + mt) * 32 + lane,
+                   make_float4(o[nt][mt][0], o[nt][mt][1], o[nt][mt][2], o[nt][mt][3]));
+          if (lane < 4) {
+            float* ml = dstp + NT * kMT * 128 + nt * 8 + 2 * lane;
+            __stcg(reinterpret_cast<float2*>(ml), make_float2(m_run[nt][0], m_run[nt][1]));
+            __stcg(reinterpret_cast<float2*>(ml + NT * 8), make_float2(l_run[nt][0], l_run[nt][1]));
+          }
+        }
+        // ---- last arriver merges (row A8).  Owners of this pair's tiles [a, b): workers wa..wb.
+        const long long a = (long long)Hkv * cum[c.i] + (long long)c.g * c.np, b = a + c.np;
+        const int W = p.W;
+        const int wa = (int)(((a + 1) * W - 1) / N), wb = (int)((b * W - 1) / N);
+        const int nseg = (N >= W) ? wb - wa + 1 : c.np;          // N < W: one tile per non-empty worker
+        int* counter = p.counters + c.i * Hkv + c.g;
+        __threadfence();
+        __syncwarp();
+        int old = 0;
+        if (lane == 0) old = atomicAdd(counter, 1);
+        old = __shfl_sync(FULL, old, 0);
+        if (old == nseg - 1) {
+          if (lane == 0) *counter = 0;                           // leave the workspace clean for the next call
+          __threadfence();
+          const bool wa_first = ((long long)wa * N / W) == a;
+          auto slot_of = [&](int ww) -> const float* {
+            return p.partials + (size_t)((ww == wa && !wa_first) ? 2 * ww + 1 : 2 * ww) * C::kSlotFloats;
+          };
+          auto next_owner = [&](int ww) -> int {                 // skips workers with an empty range
+            const long long kn = (long long)(ww + 1) * N / W;
+            return kn >= b ? wb + 1 : (int)(((kn + 1) * W - 1) / N);
+          };
+          const int hb = 2 * (lane & 3);
+#pragma unroll
+          for (int nt = 0; nt < NT; ++nt) {
+            float mm0 = -INFINITY, mm1 = -INFINITY;
+            for (int ww = wa; ww <= wb; ww = next_owner(ww)) {
+              const float2 mv = __ldcg(reinterpret_cast<const float2*>(slot_of(ww) + NT * kMT * 128 + nt * 8 + hb));
+              mm0 = fmaxf(mm0, mv.x); mm1 = fmaxf(mm1, mv.y);
+            }
+            float l0 = 0.f, l1 = 0.f;
+#pragma unroll
+            for (int mt = 0; mt < kMT; ++mt) o[nt][mt][0] = o[nt][mt][1] = o[nt][mt][2] = o[nt][mt][3] = 0.f;
+            for (int ww = wa; ww <= wb; ww = next_owner(ww)) {     // fixed (token) order: deterministic
+              const float* sl = slot_of(ww);
+              const float2 mv = __ldcg(reinterpret_cast<const float2*>(sl + NT * kMT * 128 + nt * 8 + hb));
+              const float2 lv = __ldcg(reinterpret_cast<const float2*>(sl + NT * kMT * 128 + NT * 8 + nt * 8 + hb));
+              const float c0 = ex2(mv.x - mm0), c1 = ex2(mv.y - mm1);
+              l0 += lv.x * c0; l1 += lv.y * c1;
+#pragma unroll
+              for (int mt = 0; mt < kMT; ++mt) {
+                const float4 v = __ldcg(reinterpret_cast<const float4*>(sl) + (nt * kMT + mt) * 32 + lane);
+                o[nt][mt][0] += v.x * c0; o[nt][mt][1] += v.y * c1;
+                o[nt][mt][2] += v.z * c0; o[nt][mt][3] += v.w * c1;
+              }
+            }
+            l_run[nt][0] = l0; l_run[nt][1] = l1;
+          }
+          emit = true;
+        }
+      }
+      if (emit) {
+        // normalise, transpose through the just-consumed K tile, 16-byte coalesced stores
+        __half* scratch = reinterpret_cast<__half*>(my_stage + stage * C::kStage);
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+          const float inv0 = 1.f / l_run[nt][0], inv1 = 1.f / l_run[nt][1];
+          const int h0 = nt * 8 + 2 * (lane & 3);
+#pragma unroll
+          for (int mt = 0; mt < kMT; ++mt) {
+            const int d0 = 16 * mt + tok0;
+            scratch[h0 * D + d0] = __float2half_rn(o[nt][mt][0] * inv0);
+            scratch[(h0 + 1) * D + d0] = __float2half_rn(o[nt][mt][1] * inv1);
+            scratch[h0 * D + d0 + 8] = __float2half_rn(o[nt][mt][2] * inv0);
+            scratch[(h0 + 1) * D + d0 + 8] = __float2half_rn(o[nt][mt][3] * inv1);
+          }
+        }
+        __syncwarp();
+        int4* dst = reinterpret_cast<int4*>(p.out + ((size_t)c.i * p.Hq + (size_t)c.g * G) * D);
+        const int4* srcv = reinterpret_cast<const int4*>(scratch);
+        for (int e = lane; e < G * D / 8; e += 32) dst[e] = srcv[e];
+        __syncwarp();
+        wrote_smem = true;
+      }
+    }
+    if (wrote_smem) { fence_proxy_async(); __syncwarp(); }   // generic writes before the TMA refill
+
+    // ------------------------------------------------ advance the cursor
+    ++ck;
+    if (++c.j == c.np) {
+      c.j = 0;
+      if (++c.g == Hkv) {
+        c.g = 0;
+        do { ++c.i; } while (c.i < B && cum[c.i + 1] == cum[c.i]);
+        if (c.i < B) { c.np = cum[c.i + 1] - cum[c.i]; cn = slen[c.i]; }
+      }
+    }
   }
-#endif
 }
 
 // ------------------------------------------------------------------------------------------
@@ -894,10 +646,10 @@ int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream
   int rc = get_tile_maps(a.k_base, a.v_base, rows, D, &tk, &tv);
   if (rc) return rc;
 
-  int grid = di.sm_count < 256 ? di.sm_count : 256;       // one persistent CTA per SM
+  int grid = di.sm_count;
+  if (grid * kWarps > kMaxWorkers) grid = kMaxWorkers / kWarps;
   char* ws = static_cast<char*>(a.workspace);
-  const size_t ctrl_bytes = 64;
-  const size_t counter_bytes = ((size_t)kBMax * a.kv_heads * sizeof(int32_t) + 15) & ~(size_t)15;
+  const size_t partial_bytes = (size_t)2 * kMaxWorkers * C::kSlotFloats * sizeof(float);
   for (int b0 = 0; b0 < a.batch; b0 += kBMax) {
     StreamParams p;
     p.B = (a.batch - b0 < kBMax) ? a.batch - b0 : kBMax;
@@ -905,13 +657,13 @@ int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream
     p.out = static_cast<__half*>(a.out) + (size_t)b0 * a.q_heads * D;
     p.bt = a.block_table + (size_t)b0 * a.bt_stride;
     p.lens = a.seq_lens + b0;
-    p.ctrl = reinterpret_cast<int32_t*>(ws);
-    p.counters = reinterpret_cast<int32_t*>(ws + ctrl_bytes);
-    p.partials = reinterpret_cast<float*>(ws + ctrl_bytes + counter_bytes);
+    p.partials = reinterpret_cast<float*>(ws);
+    p.counters = reinterpret_cast<int32_t*>(ws + partial_bytes);
     p.Hq = a.q_heads; p.Hkv = a.kv_heads; p.G = a.q_heads / a.kv_heads; p.bt_stride = a.bt_stride;
     p.layer_row0 = (uint32_t)(rows_per_layer * a.layer);
     p.scale_log2 = a.sm_scale * kLog2e;
-    attn_stream_kernel<D, NT><<<grid, kWarps * 32 + 32, C::kSmem, stream>>>(tk, tv, p);
+    p.W = grid * kWarps;
+    attn_stream_kernel<D, NT><<<grid, kWarps * 32, C::kSmem, stream>>>(tk, tv, p);
     HX_CUDA_OK(cudaGetLastError());
   }
   return HX_OK;
@@ -940,8 +692,8 @@ size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, in
   const int G = q_heads / kv_heads;
   const int nt = G > 8 ? 2 : 1;
   const size_t slot = (size_t)nt * ((head_dim / 16) * 128 + 16) * sizeof(float);
-  const size_t counter_bytes = ((size_t)kBMax * kv_heads * sizeof(int32_t) + 15) & ~(size_t)15;
-  return 64 + counter_bytes + 2 * (size_t)kMaxChunks * slot;
+  const size_t bytes = 2 * (size_t)kMaxWorkers * slot + (size_t)kBMax * kv_heads * sizeof(int32_t);
+  return (bytes + 15) & ~(size_t)15;
 }
 
 int launch_attention(const AttnParams& a, cudaStream_t stream) {
