@@ -10,8 +10,9 @@
  * Conventions (all entry points)
  *  - Payload is IEEE fp16 (B_type = 2).  fp32 accumulation inside attention.
  *  - DEVICE pointers are marked "device"; everything else is host memory.  The caller owns all
- *    device memory, including the workspace.  The library allocates no device memory and keeps
- *    no device state.  hx_page_pool is the only heap object (host).
+ *    device memory, including the workspace.  The library allocates no device memory; its only
+ *    device state is the optional SM rate table of hx_tune_sm_rates (a static __device__ array).
+ *    hx_page_pool is the only heap object (host).
  *  - hx_kv_ingest / hx_kv_gather / hx_decode_attention only ENQUEUE work on `stream`
  *    (a cudaStream_t passed as void*, NULL = legacy default stream) and return.  They never
  *    synchronise and never read device memory from the host; this is why sizes that only
@@ -147,6 +148,15 @@ int hx_decode_attention(void* out, const void* q,
                         int32_t batch, int32_t max_seq_len, float sm_scale,
                         void* workspace, size_t workspace_bytes,
                         void* stream);
+
+/* Optional, once per process and device: measure how fast each SM streams from HBM when all SMs
+ * load at once, and size hx_decode_attention's per-SM ranges accordingly.  On B200 the SMs fall into
+ * stable rate classes (about 1.19 / 1.00 / 0.88 of the mean), so equal ranges leave the fast SMs
+ * idle at the end of the kernel.  `scratch` is any device buffer of >= 256 MiB
+ * (e.g. the KV cache itself); it is only read.  Enqueues ~0.3 ms of probe kernels on `stream`.
+ * The table is library state in device memory; scratch == NULL resets it to equal ranges.
+ * Results stay deterministic for a given table: same inputs -> same bits until the next tune. */
+int hx_tune_sm_rates(const void* scratch, size_t scratch_bytes, void* stream);
 
 /* ---- host page allocator (paging by citation PAPER.md:L110, OOM
  * remark PAPER.md:L136).  A free list of page ids; alloc is all-or-nothing.  Not thread-safe. */

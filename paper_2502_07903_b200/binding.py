@@ -15,7 +15,7 @@ EXPORTS = [
     "hx_version", "hx_status_string", "hx_last_error", "hx_paged_cache_bytes", "hx_kv_ingest",
     "hx_kv_gather", "hx_decode_attention_workspace_bytes", "hx_decode_attention", "hx_pool_create",
     "hx_pool_shuffle", "hx_pool_alloc", "hx_pool_free", "hx_pool_num_free", "hx_pool_num_pages",
-    "hx_pool_alloc_table", "hx_pool_destroy", "hx_decode_step_host",
+    "hx_pool_alloc_table", "hx_pool_destroy", "hx_decode_step_host", "hx_tune_sm_rates",
 ]
 
 
@@ -94,6 +94,9 @@ def lib() -> C.CDLL:
         L.hx_pool_alloc_table.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32]
         L.hx_pool_destroy.restype = None
         L.hx_pool_destroy.argtypes = [C.c_void_p]
+        if not os.environ.get("HX_LIB") or hasattr(L, "hx_tune_sm_rates"):   # older A/B builds lack it
+            L.hx_tune_sm_rates.restype = C.c_int
+            L.hx_tune_sm_rates.argtypes = [C.c_void_p, C.c_size_t, C.c_void_p]
         L.hx_decode_step_host.restype = C.c_int
         L.hx_decode_step_host.argtypes = [C.POINTER(_CStepArgs), C.c_void_p]
         _lib = L
@@ -204,6 +207,16 @@ def decode_attention(out, q, cache: PagedCache, *, layer, q_heads, block_table, 
     _check(lib().hx_decode_attention(_ptr(out), _ptr(q), cache.ref, layer, q_heads, _ptr(block_table),
                                      block_table_stride, _ptr(seq_lens), batch, max_seq_len,
                                      C.c_float(sm_scale), _ptr(workspace), workspace_bytes, _stream_ptr(stream)))
+
+
+def tune_sm_rates(scratch=None, scratch_bytes=None, stream=None):
+    """hx_tune_sm_rates: scratch is a device tensor of >= 256 MiB (only read); None resets."""
+    if scratch is None:
+        _check(lib().hx_tune_sm_rates(None, 0, _stream_ptr(stream)))
+        return
+    if scratch_bytes is None:
+        scratch_bytes = scratch.numel() * scratch.element_size()
+    _check(lib().hx_tune_sm_rates(_ptr(scratch), scratch_bytes, _stream_ptr(stream)))
 
 
 def decode_step_host(**kw):

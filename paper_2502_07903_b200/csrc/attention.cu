@@ -39,6 +39,7 @@ namespace {
 constexpr int kWarps = 8;          // warps (= independent workers) per CTA
 constexpr int kBMax = 2048;        // requests per launch (prefix sums live in shared memory)
 constexpr int kMaxWorkers = 2048;  // workspace is sized for this many workers (>= SMs * kWarps)
+constexpr int kMaxSm = 256;        // CTAs (= SMs) per launch
 constexpr float kLog2e = 1.4426950408889634f;
 
 template <int D, int NT>
@@ -51,7 +52,7 @@ struct Cfg {
   static constexpr int kMT = D / 16;                 // m-tiles of PV
   static constexpr int kSlotFloats = NT * (kMT * 128 + 16);   // partial: acc[NT][MT][32][4], m[NT][8], l[NT][8]
   static constexpr int kSmem = kWarps * kStages * kStage + kWarps * kQBytes + kWarps * (kStages + 1) * 8 +
-                               (kBMax + 1) * 4 + kBMax * 4;
+                               (kBMax + 1) * 4 + kBMax * 4 + (kMaxSm + 1) * 4 + 16;
 };
 
 struct StreamParams {
@@ -61,10 +62,10 @@ struct StreamParams {
   const int32_t* lens;
   float* partials;        // [2 * W][kSlotFloats]
   int32_t* counters;      // [B * Hkv] arrival counters of split pairs; zero between calls
+  int32_t* claim;         // [kMaxSm] range-claim flags + [kMaxSm] finished-CTA counter; zero between calls
   int32_t B, Hq, Hkv, G, bt_stride;
   uint32_t layer_row0;    // first tensor-map row of the layer
   float scale_log2;
-  int32_t W;              // total workers = gridDim.x * kWarps
 };
 
 // ---------------------------------------------------------------------------- PTX helpers
@@ -141,6 +142,101 @@ __device__ __forceinline__ Loc locate(long long k, const int* cum, int B, int Hk
 }
 
 // ------------------------------------------------------------------------------------------
+// SM streaming-rate table (hx_tune_sm_rates).  On B200 the SMs do not stream from HBM at the same
+// rate when all of them load at once: they fall into stable classes (about 1.19 / 1.00 / 0.88 of
+// the mean; TPC pairs alike), a property of the chip's fabric.  With equal ranges the kernel waits
+// for the slow class.  The table holds a per-SM weight in 1/256 of the median rate; range sizes
+// follow it.  g_sm_w_n == 0 means "not tuned": equal ranges.
+__device__ int g_sm_w[kMaxSm];
+__device__ int g_sm_w_n;
+__device__ unsigned int g_sm_cnt[kMaxSm];
+
+// Every SM streams 8 KiB bulk copies from `scratch` through the same per-warp rings as the
+// attention kernel for a fixed time window and counts what it got.
+__global__ void __launch_bounds__(kWarps * 32, 1)
+sm_rate_probe_kernel(const uint8_t* scratch, unsigned long long chunks, unsigned int window_ns) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  constexpr int kStages = 3, kStage = 8192;
+  __shared__ uint64_t bars[kWarps * kStages];
+  __shared__ unsigned int warp_cnt[kWarps];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (lane == 0) {
+    for (int s = 0; s < kStages; ++s) mbar_init(smem_u32(&bars[warp * kStages + s]), 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  unsigned int smid;
+  asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+  unsigned long long t0, t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+  unsigned long long h = (unsigned long long)(smid * kWarps + warp) * 0x9E3779B97F4A7C15ull + 12345;
+  const uint32_t stage0 = smem_u32(smem + warp * kStages * kStage);
+  auto issue = [&](int n) {
+    h = h * 6364136223846793005ull + 1442695040888963407ull;
+    const unsigned long long c = (h >> 20) % chunks;
+    const uint32_t bar = smem_u32(&bars[warp * kStages + n % kStages]);
+    mbar_expect_tx(bar, kStage);
+    bulk_load(stage0 + (n % kStages) * kStage, scratch + c * kStage, kStage, bar);
+  };
+  unsigned int n = 0;
+  if (lane == 0) for (int s = 0; s < kStages; ++s) issue(s);
+  while (true) {
+    mbar_wait(smem_u32(&bars[warp * kStages + n % kStages]), (n / kStages) & 1);
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    if (t - t0 >= window_ns) break;
+    if (lane == 0) issue(n + kStages);
+    ++n;
+  }
+  // drain what is still in flight so that no bulk copy outlives the CTA
+  for (unsigned int e = n + 1; e < n + kStages; ++e) mbar_wait(smem_u32(&bars[warp * kStages + e % kStages]), (e / kStages) & 1);
+  if (lane == 0) warp_cnt[warp] = n;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned int tot = 0;
+    for (int w2 = 0; w2 < kWarps; ++w2) tot += warp_cnt[w2];
+    if (smid < kMaxSm) atomicMax(&g_sm_cnt[smid], tot);
+  }
+}
+
+// One CTA: raw[s] = count[s] / median count; weight[s] = 256 * (1 + damp * (raw - 1)) rounded to a
+// multiple of 8 (3 %: keeps the table stable from run to run) and clamped to [192, 352].  damp < 1
+// because HBM is a shared, saturated pie: an SM that is given more work also runs longer against
+// fewer competitors, so the probe's rate spread overstates the spread that balances the kernel.
+// SMs that saw no probe CTA get the nominal 256.
+__global__ void sm_rate_finalize_kernel(int n_sm, int reset, int damp_256) {
+  __shared__ unsigned int cnt[kMaxSm];
+  __shared__ unsigned int median;
+  const int t = threadIdx.x;
+  if (reset) {
+    if (t < kMaxSm) { g_sm_w[t] = 256; g_sm_cnt[t] = 0; }
+    if (t == 0) g_sm_w_n = 0;
+    return;
+  }
+  if (t < kMaxSm) cnt[t] = t < n_sm ? g_sm_cnt[t] : 0;
+  if (t == 0) median = 0;
+  __syncthreads();
+  if (t < n_sm && cnt[t] > 0) {
+    int below = 0, valid = 0;
+    for (int u = 0; u < n_sm; ++u)
+      if (cnt[u] > 0) { ++valid; below += (cnt[u] < cnt[t]) || (cnt[u] == cnt[t] && u < t); }
+    if (below == valid / 2) median = cnt[t];
+  }
+  __syncthreads();
+  if (t < kMaxSm) {
+    int w = 256;
+    if (t < n_sm && cnt[t] > 0 && median > 0) {
+      const long long raw = (256ll * cnt[t]) / median;               // 1/256 units
+      long long d = 256 + ((raw - 256) * damp_256) / 256;
+      d = (d + 4) & ~7ll;
+      w = (int)(d < 192 ? 192 : (d > 352 ? 352 : d));
+    }
+    g_sm_w[t] = w;
+    g_sm_cnt[t] = 0;
+  }
+  if (t == 0) { __threadfence(); g_sm_w_n = n_sm; }
+}
+
+// ------------------------------------------------------------------------------------------
 template <int D, int NT>
 __global__ void __launch_bounds__(kWarps * 32, 1)
 attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
@@ -153,14 +249,41 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
   uint64_t* bars = reinterpret_cast<uint64_t*>(q_base + kWarps * C::kQBytes);
   int* cum = reinterpret_cast<int*>(bars + kWarps * (kStages + 1));
   int* slen = cum + (kBMax + 1);
+  int* smlo = slen + kBMax;            // [nC + 1] first tile of each CTA-level range; then [nC+1] = my slot
+  int* my_slot = smlo + kMaxSm + 1;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int B = p.B, Hkv = p.Hkv, G = p.G;
+  const int nC = gridDim.x;
+#ifdef HX_TRACE
+  unsigned long long tr[6] = {0, 0, 0, 0, 0, 0};
+#define HX_STAMP(x) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tr[x]))
+#else
+#define HX_STAMP(x)
+#endif
+  HX_STAMP(0);
+
+  // ---- which CTA-level range is mine.  Not tuned: range blockIdx.x.  Tuned (hx_tune_sm_rates):
+  // range sizes follow the per-SM rate table, so the range of SM s belongs to the CTA running on
+  // SM s; it is claimed with a flag, and a CTA that finds its SM's range taken (two CTAs landed on
+  // one SM) takes any free one, so every range is processed exactly once whatever the placement.
+  const bool tuned = (g_sm_w_n == nC);
+  const int my_w = (tid < nC) ? (tuned ? g_sm_w[tid] : 256) : 0;   // weight of CTA-level range `tid`
+  if (tid == 0) {
+    int slot = blockIdx.x;
+    if (tuned) {
+      unsigned int smid;
+      asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+      slot = (int)(smid % (unsigned)nC);
+      while (atomicCAS(p.claim + slot, 0, 1) != 0) slot = (slot + 1 == nC) ? 0 : slot + 1;
+    }
+    *my_slot = slot;
+  }
 
   // ---- setup: page-count prefix sums (row A4) and barrier init; the only CTA-wide syncs
   {
     constexpr int PER = kBMax / (kWarps * 32);
-    __shared__ int warp_tot[kWarps];
+    __shared__ int warp_tot[kWarps], warp_tot_w[kWarps];
     int np[PER], sum = 0;
 #pragma unroll
     for (int e = 0; e < PER; ++e) {
@@ -170,13 +293,14 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
       np[e] = (n + 15) >> 4;
       sum += np[e];
     }
-    int incl = sum;
+    int incl = sum, incl_w = my_w;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
       const int t = __shfl_up_sync(FULL, incl, o);
-      if (lane >= o) incl += t;
+      const int tw = __shfl_up_sync(FULL, incl_w, o);
+      if (lane >= o) { incl += t; incl_w += tw; }
     }
-    if (lane == 31) warp_tot[warp] = incl;
+    if (lane == 31) { warp_tot[warp] = incl; warp_tot_w[warp] = incl_w; }
     if (lane == 0) {
       const uint32_t b0 = smem_u32(bars + warp * (kStages + 1));
       for (int s = 0; s <= kStages; ++s) mbar_init(b0 + 8 * s, 1);
@@ -193,6 +317,16 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
       if (i < B) cum[i + 1] = off;
     }
     __syncthreads();
+    {
+      // CTA-level range starts: smlo[s] = N * (weights before s) / (all weights)
+      int before = incl_w - my_w, all = 0;
+#pragma unroll
+      for (int w2 = 0; w2 < kWarps; ++w2) { if (w2 < warp) before += warp_tot_w[w2]; all += warp_tot_w[w2]; }
+      const long long Nt = (long long)Hkv * cum[B];
+      if (tid < nC) smlo[tid] = (int)(Nt * before / all);
+      if (tid == nC || (nC == kWarps * 32 && tid == 0)) smlo[nC] = (int)Nt;
+    }
+    __syncthreads();
     // reading S11: an empty context gives a zero output row (no tile ever touches it)
     for (int i = blockIdx.x * (kWarps * 32) + tid; i < B; i += gridDim.x * (kWarps * 32))
       if (slen[i] == 0) {
@@ -201,10 +335,25 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
       }
   }
 
-  const long long N = (long long)Hkv * cum[B];
-  const int w = blockIdx.x * kWarps + warp;
-  const long long k0 = (long long)w * N / p.W, k1 = (long long)(w + 1) * N / p.W;
-  if (k0 >= k1) return;
+  // worker (slot s, warp j) owns [lo(s, j), lo(s, j + 1)): the CTA range cut in 8 equal parts
+  auto w_lo = [&](int ww) -> int {
+    const int s = ww >> 3, j = ww & 7;
+    return smlo[s] + (int)((long long)(smlo[s + 1] - smlo[s]) * j >> 3);
+  };
+  auto owner_of = [&](int k) -> int {                       // worker whose range holds tile k
+    int lo = 0, hi = nC;                                    // smlo[lo] <= k < smlo[hi]
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (smlo[mid] <= k) lo = mid; else hi = mid;
+    }
+    const int len = smlo[lo + 1] - smlo[lo];
+    return lo * 8 + (int)((((unsigned)(k - smlo[lo]) + 1u) * 8u - 1u) / (unsigned)len);   // len < 2^28 (host check)
+  };
+  HX_STAMP(1);
+  const int w = *my_slot * kWarps + warp;
+  const int k0 = w_lo(w), k1 = w_lo(w + 1);
+  do {
+  if (k0 >= k1) break;
 
   uint8_t* my_stage = smem + warp * kStages * C::kStage;
   const uint32_t stage_u32 = smem_u32(my_stage);
@@ -306,6 +455,10 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
       seg_j0 = c.j;
     }
     mbar_wait(bar_u32 + 8 * stage, (idx / kStages) & 1);
+#ifdef HX_TRACE
+    if (idx == 0) HX_STAMP(2);
+    if (ck == k1 - 1) HX_STAMP(3);
+#endif
 
     const uint32_t kb = stage_u32 + stage * C::kStage, vb = kb + kTile;
     const bool last_page = (c.j == c.np - 1);
@@ -417,10 +570,16 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
           }
         }
         // ---- last arriver merges (row A8).  Owners of this pair's tiles [a, b): workers wa..wb.
-        const long long a = (long long)Hkv * cum[c.i] + (long long)c.g * c.np, b = a + c.np;
-        const int W = p.W;
-        const int wa = (int)(((a + 1) * W - 1) / N), wb = (int)((b * W - 1) / N);
-        const int nseg = (N >= W) ? wb - wa + 1 : c.np;          // N < W: one tile per non-empty worker
+        const int a = Hkv * cum[c.i] + c.g * c.np, b = a + c.np;
+        const int wa = owner_of(a), wb = owner_of(b - 1);
+        const bool dense = smlo[nC] >= 16 * nC;                // then every worker's range is non-empty
+        auto next_owner = [&](int ww) -> int {                 // next worker with a tile of the pair
+          if (dense) return ww + 1;
+          const int kn = w_lo(ww + 1);                         // (workers with an empty range own none)
+          return kn >= b ? wb + 1 : owner_of(kn);
+        };
+        int nseg = wb - wa + 1;
+        if (!dense) { nseg = 0; for (int ww = wa; ww <= wb; ww = next_owner(ww)) ++nseg; }
         int* counter = p.counters + c.i * Hkv + c.g;
         __threadfence();
         __syncwarp();
@@ -430,13 +589,9 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         if (old == nseg - 1) {
           if (lane == 0) *counter = 0;                           // leave the workspace clean for the next call
           __threadfence();
-          const bool wa_first = ((long long)wa * N / W) == a;
+          const bool wa_first = (w_lo(wa) == a);
           auto slot_of = [&](int ww) -> const float* {
             return p.partials + (size_t)((ww == wa && !wa_first) ? 2 * ww + 1 : 2 * ww) * C::kSlotFloats;
-          };
-          auto next_owner = [&](int ww) -> int {                 // skips workers with an empty range
-            const long long kn = (long long)(ww + 1) * N / W;
-            return kn >= b ? wb + 1 : (int)(((kn + 1) * W - 1) / N);
           };
           const int hb = 2 * (lane & 3);
 #pragma unroll
@@ -501,6 +656,28 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         c.g = 0;
         do { ++c.i; } while (c.i < B && cum[c.i + 1] == cum[c.i]);
         if (c.i < B) { c.np = cum[c.i + 1] - cum[c.i]; cn = slen[c.i]; }
+      }
+    }
+  }
+  } while (false);
+#ifdef HX_TRACE
+  HX_STAMP(4);
+  if (lane == 0) {
+    unsigned long long* t = reinterpret_cast<unsigned long long*>(p.claim + 2 * kMaxSm) + (size_t)(blockIdx.x * kWarps + warp) * 8;
+    for (int e = 0; e < 5; ++e) t[e] = tr[e];
+    t[5] = (unsigned long long)(k1 - k0);
+    unsigned smid; asm volatile("mov.u32 %0, %%smid;" : "=r"(smid)); t[6] = smid;
+  }
+#endif
+
+  // ---- tuned mode: the last CTA of the grid to finish clears the claim flags for the next call
+  if (tuned) {
+    __syncthreads();
+    if (tid == 0) {
+      __threadfence();
+      if (atomicAdd(p.claim + kMaxSm, 1) == nC - 1) {
+        for (int s = 0; s <= kMaxSm; ++s) p.claim[s] = 0;
+        __threadfence();
       }
     }
   }
@@ -647,9 +824,11 @@ int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream
   if (rc) return rc;
 
   int grid = di.sm_count;
-  if (grid * kWarps > kMaxWorkers) grid = kMaxWorkers / kWarps;
+  if (grid > kMaxSm) grid = kMaxSm;
   char* ws = static_cast<char*>(a.workspace);
   const size_t partial_bytes = (size_t)2 * kMaxWorkers * C::kSlotFloats * sizeof(float);
+  const size_t counter_bytes = ((size_t)kBMax * a.kv_heads * sizeof(int32_t) + 15) & ~(size_t)15;
+  if ((long long)kBMax * a.bt_stride * a.kv_heads >= (1ll << 28)) HX_FAIL(HX_ERR_UNSUPPORTED, "block_table_stride * kv_heads too large");
   for (int b0 = 0; b0 < a.batch; b0 += kBMax) {
     StreamParams p;
     p.B = (a.batch - b0 < kBMax) ? a.batch - b0 : kBMax;
@@ -659,10 +838,10 @@ int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream
     p.lens = a.seq_lens + b0;
     p.partials = reinterpret_cast<float*>(ws);
     p.counters = reinterpret_cast<int32_t*>(ws + partial_bytes);
+    p.claim = reinterpret_cast<int32_t*>(ws + partial_bytes + counter_bytes);
     p.Hq = a.q_heads; p.Hkv = a.kv_heads; p.G = a.q_heads / a.kv_heads; p.bt_stride = a.bt_stride;
     p.layer_row0 = (uint32_t)(rows_per_layer * a.layer);
     p.scale_log2 = a.sm_scale * kLog2e;
-    p.W = grid * kWarps;
     attn_stream_kernel<D, NT><<<grid, kWarps * 32, C::kSmem, stream>>>(tk, tv, p);
     HX_CUDA_OK(cudaGetLastError());
   }
@@ -692,8 +871,36 @@ size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, in
   const int G = q_heads / kv_heads;
   const int nt = G > 8 ? 2 : 1;
   const size_t slot = (size_t)nt * ((head_dim / 16) * 128 + 16) * sizeof(float);
-  const size_t bytes = 2 * (size_t)kMaxWorkers * slot + (size_t)kBMax * kv_heads * sizeof(int32_t);
-  return (bytes + 15) & ~(size_t)15;
+  const size_t counter_bytes = ((size_t)kBMax * kv_heads * sizeof(int32_t) + 15) & ~(size_t)15;
+  return 2 * (size_t)kMaxWorkers * slot + counter_bytes + (size_t)(2 * kMaxSm) * sizeof(int32_t);
+}
+
+int tune_sm_rates(const void* scratch, size_t bytes, cudaStream_t stream) {
+  DeviceInfo di;
+  int rc = device_info(&di);
+  if (rc) return rc;
+  const int grid = di.sm_count < kMaxSm ? di.sm_count : kMaxSm;
+  if (!scratch || bytes == 0) {                              // back to equal ranges
+    sm_rate_finalize_kernel<<<1, kMaxSm, 0, stream>>>(grid, 1, 0);
+    HX_CUDA_OK(cudaGetLastError());
+    return HX_OK;
+  }
+  constexpr int kProbeSmem = kWarps * 3 * 8192;
+  static bool attr_set[64] = {false};
+  if (!attr_set[di.device]) {
+    HX_CUDA_OK(cudaFuncSetAttribute(sm_rate_probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kProbeSmem));
+    attr_set[di.device] = true;
+  }
+  // three windows of 80 us: the counts of a window are max-merged per SM, which drops start-up noise
+  for (int rep = 0; rep < 3; ++rep) {
+    sm_rate_probe_kernel<<<grid, kWarps * 32, kProbeSmem, stream>>>(static_cast<const uint8_t*>(scratch), bytes / 8192, 80000u);
+    HX_CUDA_OK(cudaGetLastError());
+  }
+  int damp = 176;                                           // 0.69 (B200 sweep: 160-192 best), see sm_rate_finalize_kernel
+  if (const char* e = getenv("HX_TUNE_DAMP_256")) damp = atoi(e);   // experiments only
+  sm_rate_finalize_kernel<<<1, kMaxSm, 0, stream>>>(grid, 0, damp);
+  HX_CUDA_OK(cudaGetLastError());
+  return HX_OK;
 }
 
 int launch_attention(const AttnParams& a, cudaStream_t stream) {

@@ -180,6 +180,16 @@ int hx_decode_attention(void* out, const void* q, const hx_paged_cache* cache, i
   return launch_attention(p, static_cast<cudaStream_t>(stream));
 }
 
+int hx_tune_sm_rates(const void* scratch, size_t scratch_bytes, void* stream) {
+  using namespace hx;
+  clear_error();
+  if (scratch && scratch_bytes > 0) {
+    if (!aligned16(scratch)) HX_FAIL(HX_ERR_INVALID_ARG, "hx_tune_sm_rates: scratch must be 16-byte aligned");
+    if (scratch_bytes < ((size_t)256 << 20)) HX_FAIL(HX_ERR_UNSUPPORTED, "hx_tune_sm_rates: scratch of %zu bytes is too small to be HBM-bound (need >= 256 MiB)", scratch_bytes);
+  }
+  return tune_sm_rates(scratch, scratch_bytes, static_cast<cudaStream_t>(stream));
+}
+
 int hx_decode_step_host(const hx_step_host_args* a, void* stream_) {
   using namespace hx;
   clear_error();

@@ -66,5 +66,6 @@ struct AttnParams {
 size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, int32_t head_dim,
                             int32_t max_seq_len, int32_t page_size);
 int launch_attention(const AttnParams& p, cudaStream_t stream);
+int tune_sm_rates(const void* scratch, size_t bytes, cudaStream_t stream);
 
 }  // namespace hx

@@ -186,3 +186,27 @@ def test_ingest_then_attention_end_to_end_tiny(env):
     wa = dict(q=q, k=dk.view(np.float16), v=dv.view(np.float16), block_table=w["block_table"],
               seq_lens=w["seq_lens"], num_pages=w["num_pages"])
     check_attn(env, wa, "tiny e2e")
+
+
+def test_attention_with_tuned_sm_rates(env):
+    """hx_tune_sm_rates changes only how the tile sequence is cut: results stay inside the tolerance,
+    stay bit-identical from run to run and under page permutation, and reset restores equal ranges."""
+    hx, torch, oracle = env
+    c = W.AttnConfig(77, "tuned", 12, 32, 4, 128, 256, "x")
+    w = W.make_attention_inputs(c, lens=np.array([1, 17, 64, 100, 255, 256, 700, 1000, 2000, 3000, 4000, 33], dtype=np.int32))
+    base = run_gpu_attention(hx, torch, w)
+    scratch = torch.empty(320 << 20, dtype=torch.uint8, device="cuda")
+    scratch.random_()
+    try:
+        hx.tune_sm_rates(scratch)
+        torch.cuda.synchronize()
+        got, _ = check_attn(env, w, "tuned")
+        again = run_gpu_attention(hx, torch, w)
+        assert np.array_equal(got.view(np.uint16), again.view(np.uint16))
+        check_attn(env, W.make_attention_inputs(W.CONFIGS["tiny"]), "tuned tiny")
+        with pytest.raises(hx.HxError):
+            hx.tune_sm_rates(scratch[: 1 << 20])                      # too small to be HBM-bound
+    finally:
+        hx.tune_sm_rates(None)
+        torch.cuda.synchronize()
+    assert np.array_equal(base.view(np.uint16), run_gpu_attention(hx, torch, w).view(np.uint16))
