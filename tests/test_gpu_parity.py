@@ -210,3 +210,70 @@ def test_attention_with_tuned_sm_rates(env):
         hx.tune_sm_rates(None)
         torch.cuda.synchronize()
     assert np.array_equal(base.view(np.uint16), run_gpu_attention(hx, torch, w).view(np.uint16))
+
+
+def test_attention_batch_larger_than_one_launch(env):
+    """B above the per-launch request limit (2048) goes out as several launches sharing one workspace."""
+    g = W.rng(78, 0)
+    lens = g.integers(0, 40, size=2100).astype(np.int32)
+    lens[[0, 2047, 2048, 2099]] = [33, 17, 1, 16]
+    c = W.AttnConfig(78, "bigB", len(lens), 8, 2, 64, 4, "x")
+    check_attn(env, W.make_attention_inputs(c, lens=lens), "B=2100")
+
+
+def test_attention_shared_pages_between_requests(env):
+    """Two requests may point at the same physical pages (prefix sharing): attention only reads."""
+    hx, torch, oracle = env
+    c = W.AttnConfig(79, "shared", 3, 8, 1, 128, 8, "x")
+    w = W.make_attention_inputs(c, lens=np.array([64, 64, 100], dtype=np.int32))
+    w["block_table"][1, :4] = w["block_table"][0, :4]
+    w["block_table"][2, :4] = w["block_table"][0, :4]
+    got, ref = check_attn(env, w, "shared pages")
+    assert not np.array_equal(got[0], got[1])            # different q, same KV
+
+
+def test_attention_max_context_single_request(env):
+    """One 8192-token request (512 pages, the cfg5 maximum) split over every worker of the grid."""
+    c = W.AttnConfig(80, "long", 1, 8, 1, 128, 512, "x")
+    check_attn(env, W.make_attention_inputs(c, lens=np.array([8192], dtype=np.int32)), "n=8192")
+
+
+def test_ingest_on_side_stream_while_attention_runs(env):
+    """Ingest into pages disjoint from the active batch may run on another stream."""
+    hx, torch, oracle = env
+    c = W.AttnConfig(81, "overlap", 16, 32, 4, 128, 128, "x")
+    w = W.make_attention_inputs(c, lens=W.rng(81, 1).integers(500, 2000, size=16).astype(np.int32), spare=2.0)
+    base = run_gpu_attention(hx, torch, w)
+    used = set(w["block_table"][w["block_table"] >= 0].tolist())
+    free = np.array([p for p in range(w["num_pages"]) if p not in used], dtype=np.int32)
+    ci = W.IngestConfig(81, "ov", 1, 4, 128, 2, 1, 4, "x")
+    wi = W.make_ingest_inputs(ci, lens=np.array([300, 200, 100, 17], dtype=np.int32), bits=True)
+    need = W.pages_for(wi["seq_lens"])
+    bt = np.full((4, int(need.max())), -1, dtype=np.int32)
+    o = 0
+    for i, k in enumerate(need):
+        bt[i, :k] = free[o:o + k]; o += k
+    from helpers import to_dev, dev_u16
+    k, v = to_dev(w["k"], torch), to_dev(w["v"], torch)
+    cache = hx.PagedCache(k, v)
+    q = to_dev(w["q"], torch); out = torch.empty_like(q)
+    btd = torch.from_numpy(w["block_table"]).cuda(); sl = torch.from_numpy(w["seq_lens"]).cuda()
+    wsb = hx.decode_attention_workspace_bytes(16, 32, 4, 128, 2000)
+    ws = torch.zeros(wsb, dtype=torch.uint8, device="cuda")
+    sk = [to_dev(a, torch) for a in wi["src_k"]]; sv = [to_dev(a, torch) for a in wi["src_v"]]
+    ibt = torch.from_numpy(bt).cuda(); icu = torch.from_numpy(wi["cu_seqlens"]).cuda(); isl = torch.from_numpy(wi["seq_lens"]).cuda()
+    side = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    for _ in range(3):
+        with torch.cuda.stream(side):
+            hx.kv_ingest(sk, sv, layers=1, heads=4, head_dim=128, src_tp=2, dst_tp=1, dst_rank=0, dst=cache, block_table=ibt,
+                         block_table_stride=ibt.shape[1], cu_seqlens=icu, seq_lens=isl, batch=4, total_tokens=617, max_seq_len=300)
+        hx.decode_attention(out, q, cache, layer=0, q_heads=32, block_table=btd, block_table_stride=btd.shape[1], seq_lens=sl,
+                            batch=16, max_seq_len=2000, workspace=ws, workspace_bytes=wsb)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy().view(np.uint16), base.view(np.uint16))
+    # and the ingested pages hold exactly what the oracle puts there
+    ok = w["k"].view(np.uint16).copy(); ov = w["v"].view(np.uint16).copy()
+    oracle.kv_ingest(wi["src_k"], wi["src_v"], ok, ov, heads=4, src_tp=2, dst_tp=1, dst_rank=0, block_table=bt,
+                     cu_seqlens=wi["cu_seqlens"], seq_lens=wi["seq_lens"])
+    assert np.array_equal(dev_u16(k), ok) and np.array_equal(dev_u16(v), ov)
