@@ -277,3 +277,41 @@ def test_ingest_on_side_stream_while_attention_runs(env):
     oracle.kv_ingest(wi["src_k"], wi["src_v"], ok, ov, heads=4, src_tp=2, dst_tp=1, dst_rank=0, block_table=bt,
                      cu_seqlens=wi["cu_seqlens"], seq_lens=wi["seq_lens"])
     assert np.array_equal(dev_u16(k), ok) and np.array_equal(dev_u16(v), ov)
+
+
+def test_decode_step_host_matches_oracle(env):
+    """hx_decode_step_host: host shards + host q in, host out back; ingest lands bit-exact and the
+    attention over the freshly ingested pages matches the oracle (whole path, configs[0] shape)."""
+    hx, torch, oracle = env
+    from helpers import dev_u16
+    wi = W.make_ingest_inputs(W.CONFIGS["tiny_ingest"])
+    P, L, H, D = wi["num_pages"], 1, 4, 64
+    lens = wi["seq_lens"]
+    cache = hx.PagedCache(torch.zeros((L, P, H, 16, D), dtype=torch.float16, device="cuda"),
+                          torch.zeros((L, P, H, 16, D), dtype=torch.float16, device="cuda"))
+    q_np = W.draw_fp16_normal((4, 4, D), 1, W.configs.S_Q)
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    qh, oh = pin(q_np), torch.empty((4, 4, D), dtype=torch.float16).pin_memory()
+    skh = [pin(a.view(np.int16)) for a in wi["src_k"]]; svh = [pin(a.view(np.int16)) for a in wi["src_v"]]
+    skd = [torch.empty_like(a, device="cuda") for a in skh]; svd = [torch.empty_like(a, device="cuda") for a in svh]
+    bth, cuh, slh = pin(wi["block_table"]), pin(wi["cu_seqlens"]), pin(lens)
+    btd, cud, sld = (torch.empty_like(a, device="cuda") for a in (bth, cuh, slh))
+    qd, od = torch.empty_like(qh, device="cuda"), torch.empty_like(oh, device="cuda")
+    wsb = hx.decode_attention_workspace_bytes(4, 4, 4, D, 255)
+    ws = torch.zeros(wsb, dtype=torch.uint8, device="cuda")
+    # the active batch is the 4 prompts just ingested: its device block table / lengths are the staging copies
+    hx.decode_step_host(q_host=qh, out_host=oh, q_dev=qd, out_dev=od, cache=cache, layer=0, q_heads=4,
+                        block_table_dev=btd, block_table_stride=btd.shape[1], seq_lens_dev=sld, batch=4, max_seq_len=255,
+                        sm_scale=0.0, workspace=ws, workspace_bytes=wsb, src_k_host=skh, src_v_host=svh, src_k_dev=skd,
+                        src_v_dev=svd, ing_layers=1, heads=4, src_tp=2, dst_tp=1, dst_rank=0, ing_block_table_host=bth,
+                        ing_block_table_stride=bth.shape[1], ing_cu_seqlens_host=cuh, ing_seq_lens_host=slh,
+                        ing_block_table_dev=btd, ing_cu_seqlens_dev=cud, ing_seq_lens_dev=sld, ing_batch=4,
+                        ing_total_tokens=wi["total_tokens"], ing_max_seq_len=255)
+    torch.cuda.synchronize()
+    ok = np.zeros((L, P, H, 16, D), dtype=np.uint16); ov = np.zeros_like(ok)
+    oracle.kv_ingest(wi["src_k"], wi["src_v"], ok, ov, heads=4, src_tp=2, dst_tp=1, dst_rank=0,
+                     block_table=wi["block_table"], cu_seqlens=wi["cu_seqlens"], seq_lens=lens)
+    assert np.array_equal(dev_u16(cache.k), ok) and np.array_equal(dev_u16(cache.v), ov)
+    ref = oracle.decode_attention(q_np, ok.view(np.float16), ov.view(np.float16), wi["block_table"], lens)
+    max_abs, rel = attn_errors(oh.numpy(), ref)
+    assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (max_abs, rel)
