@@ -22,7 +22,10 @@
  * Pins (tests/test_oracle_pins.py): brute-force dense numpy float64, constant-V, n=1, q=0 mean,
  * page-permutation invariance, GQA==repeated-MHA, split-merge identity, stability under 8x
  * logits, NaN-poison masking, ingest/gather round trip for every (S,R), changed-element count,
- * all-65536-pattern fp16 decode vs numpy, Table-1 byte counts.
+ * all-65536-pattern fp16 decode vs numpy, Table-1 byte counts;
+ * stage ingest: any cut of the model into prefill x decode stages == the one-call ingest, and an
+ * independent numpy restatement; append: ingest of n-1 tokens + append == ingest of n tokens,
+ * changed-element count, attention after append == dense softmax over the concatenation.
  * No function here is "parity unpinned".
  */
 #include <math.h>
@@ -94,6 +97,69 @@ int hxo_kv_ingest(uint16_t* const* src_k, uint16_t* const* src_v,
           }
         }
       }
+    }
+  }
+  return 0;
+}
+
+/* Pipeline-stage ingest ("each GPU containing the j-th layer
+ * within phi_i should transmit its KV cache to the matching GPU housing the j-th layer within
+ * delta_i"; prefill and decode replicas cut the model into different
+ * pipeline stages).  The source buffers hold `src_layers` layers of a prefill stage, the paged
+ * cache holds `dst_layers` layers of a decode stage; `count` consecutive layers move, source
+ * layer src_layer0 + c landing at cache layer dst_layer0 + c, c = 0..count-1.  Everything else
+ * is the ingest equation above.  Written as its own loop nest (not by calling hxo_kv_ingest). */
+int hxo_kv_ingest_stage(uint16_t* const* src_k, uint16_t* const* src_v,
+                        int src_layers, int src_layer0, int dst_layers, int dst_layer0, int count,
+                        int total_tokens, int heads, int head_dim,
+                        int src_tp, int dst_tp, int dst_rank,
+                        uint16_t* dst_k, uint16_t* dst_v, int num_pages, int page_size,
+                        const int32_t* block_table, int block_table_stride,
+                        const int32_t* cu_seqlens, const int32_t* seq_lens, int batch) {
+  if (heads % src_tp || heads % dst_tp || dst_rank < 0 || dst_rank >= dst_tp) return 1;
+  if (count < 0 || src_layer0 < 0 || dst_layer0 < 0 || src_layer0 + count > src_layers ||
+      dst_layer0 + count > dst_layers) return 2;
+  const int hs = heads / src_tp, hd = heads / dst_tp;
+  const int64_t D = head_dim, T = total_tokens, P = num_pages, ps = page_size;
+  for (int c = 0; c < count; ++c) {
+    const int64_t ls = src_layer0 + c, ld = dst_layer0 + c;
+    for (int i = 0; i < batch; ++i)
+      for (int t = 0; t < seq_lens[i]; ++t)
+        for (int h = dst_rank * hd; h < (dst_rank + 1) * hd; ++h)
+          for (int x = 0; x < 2; ++x)
+            for (int e = 0; e < D; ++e) {
+              const int64_t page = block_table[(int64_t)i * block_table_stride + t / ps];
+              const uint16_t* s = (x ? src_v : src_k)[h / hs];
+              uint16_t* d = x ? dst_v : dst_k;
+              d[((((ld * P) + page) * hd + (h % hd)) * ps + (t % ps)) * D + e] =
+                  s[(((ls * T) + cu_seqlens[i] + t) * hs + (h % hs)) * D + e];
+            }
+  }
+  return 0;
+}
+
+/* Append of the decode step's new token ("the decoding phase
+ * generates subsequent tokens by one token at each step", each step's K/V joining the cache,
+ * PAPER.md:L54).  seq_lens[i] = n_i counts the new token (reading S12), so it is
+ * token t = n_i - 1:
+ *     X[layer][ bt[i][(n_i-1) div ps] ][g][(n_i-1) mod ps][:] = x_new[i][g][:],  X in {K, V}
+ * for every request with n_i >= 1 and every local kv head g.  n_i = 0: nothing is written.
+ * k_new, v_new: uint16 [B][Hkv][D].  Nothing else in the cache changes. */
+int hxo_kv_append(const uint16_t* k_new, const uint16_t* v_new, uint16_t* k, uint16_t* v,
+                  int layer, int layers, int num_pages, int kv_heads, int page_size, int head_dim,
+                  const int32_t* block_table, int block_table_stride, const int32_t* seq_lens,
+                  int batch) {
+  if (layer < 0 || layer >= layers) return 1;
+  const int64_t D = head_dim, P = num_pages, ps = page_size;
+  for (int i = 0; i < batch; ++i) {
+    const int n = seq_lens[i];
+    if (n <= 0) continue;
+    const int t = n - 1;
+    const int64_t page = block_table[(int64_t)i * block_table_stride + t / ps];
+    for (int g = 0; g < kv_heads; ++g) {
+      const int64_t d_off = ((((int64_t)layer * P + page) * kv_heads + g) * ps + (t % ps)) * D;
+      const int64_t s_off = ((int64_t)i * kv_heads + g) * D;
+      for (int e = 0; e < D; ++e) { k[d_off + e] = k_new[s_off + e]; v[d_off + e] = v_new[s_off + e]; }
     }
   }
   return 0;

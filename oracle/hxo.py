@@ -93,6 +93,44 @@ def kv_gather(src_k, src_v, dst_k, dst_v, *, heads, src_tp, dst_tp, dst_rank, bl
             gather=1, threads=threads)
 
 
+def kv_ingest_stage(src_k, src_v, dst_k, dst_v, *, heads, src_tp, dst_tp, dst_rank, src_layer0,
+                    dst_layer0, count, block_table, cu_seqlens, seq_lens):
+    """Pipeline-stage ingest (F3): `count` layers, source layer src_layer0+c -> cache layer
+    dst_layer0+c.  Source and cache may hold different numbers of layers."""
+    src_k = [_u16(a) for a in src_k]
+    src_v = [_u16(a) for a in src_v]
+    dst_k, dst_v = _u16(dst_k), _u16(dst_v)
+    Ls, T, hs, D = src_k[0].shape
+    Ld, P, hd, ps, Dd = dst_k.shape
+    assert len(src_k) == src_tp == len(src_v) and hs == heads // src_tp
+    assert (hd, Dd) == (heads // dst_tp, D) and dst_v.shape == dst_k.shape
+    bt = np.ascontiguousarray(block_table, dtype=np.int32)
+    cu = np.ascontiguousarray(cu_seqlens, dtype=np.int32)
+    sl = np.ascontiguousarray(seq_lens, dtype=np.int32)
+    PK = (C.c_void_p * src_tp)(*[a.ctypes.data for a in src_k])
+    PV = (C.c_void_p * src_tp)(*[a.ctypes.data for a in src_v])
+    rc = lib().hxo_kv_ingest_stage(PK, PV, Ls, src_layer0, Ld, dst_layer0, count, T, heads, D, src_tp,
+                                   dst_tp, dst_rank, _p(dst_k), _p(dst_v), P, ps, _p(bt), bt.shape[1],
+                                   _p(cu), _p(sl), len(sl))
+    if rc:
+        raise ValueError(f"hxo_kv_ingest_stage: invalid arguments ({rc})")
+
+
+def kv_append(k_new, v_new, k, v, *, layer, block_table, seq_lens):
+    """Append (F1): writes token n_i-1 of every request with n_i >= 1 into k / v in place."""
+    k_new, v_new, k, v = _u16(k_new), _u16(v_new), _u16(k), _u16(v)
+    B, Hkv, D = k_new.shape
+    Ln, P, Hk, ps, Dk = k.shape
+    assert (Hk, Dk) == (Hkv, D) and v.shape == k.shape and v_new.shape == k_new.shape
+    bt = np.ascontiguousarray(block_table, dtype=np.int32)
+    sl = np.ascontiguousarray(seq_lens, dtype=np.int32)
+    assert len(sl) == B
+    rc = lib().hxo_kv_append(_p(k_new), _p(v_new), _p(k), _p(v), layer, Ln, P, Hkv, ps, D, _p(bt),
+                             bt.shape[1], _p(sl), B)
+    if rc:
+        raise ValueError("hxo_kv_append: invalid arguments")
+
+
 def default_scale(head_dim: int) -> float:
     """(double)(float)(1/sqrt(D)): the constant both sides use (reading S2)."""
     return float(np.float32(1.0) / np.sqrt(np.float32(head_dim)))
