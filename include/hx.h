@@ -48,7 +48,7 @@
 extern "C" {
 #endif
 
-#define HX_VERSION 100 /* 0.1.0 */
+#define HX_VERSION 110 /* 0.1.1: + hx_kv_ingest_stage, hx_stage_overlap, hx_kv_append, hx_decode_attention_append */
 
 typedef enum {
   HX_OK = 0,
@@ -120,6 +120,52 @@ int hx_kv_gather(void* const* src_k, void* const* src_v,
                  int32_t batch, int32_t total_tokens, int32_t max_seq_len,
                  void* stream);
 
+/* ---- (a') pipeline-stage ingest -------------------------------------
+ * PAPER.md:L92 matches layers, not stages: "each GPU containing the j-th layer within phi_i should
+ * transmit its KV cache to the matching GPU housing the j-th layer within delta_i", and prefill
+ * and decode replicas cut the model into different pipeline stages (Table 2:
+ * PP in {1,2,3,5}).  One call moves the layers that ONE prefill stage and
+ * ONE decode stage have in common: the source buffers hold `src_layers` layers
+ * (fp16 [src_layers][total_tokens][heads/src_tp][head_dim]); source layer src_layer0 + c lands at
+ * cache layer dst_layer0 + c for c = 0..layers-1.  Everything else is hx_kv_ingest
+ * (hx_kv_ingest == this with src_layers = layers, src_layer0 = dst_layer0 = 0).
+ * HX_ERR_INVALID_ARG when [src_layer0, src_layer0+layers) leaves [0, src_layers) or
+ * [dst_layer0, dst_layer0+layers) leaves [0, dst->layers).  hx_stage_overlap computes the three
+ * numbers from the two stages' global layer ranges. */
+int hx_kv_ingest_stage(const void* const* src_k, const void* const* src_v,
+                       int32_t src_layers, int32_t src_layer0, int32_t dst_layer0, int32_t layers,
+                       int32_t heads, int32_t head_dim,
+                       int32_t src_tp, int32_t dst_tp, int32_t dst_rank,
+                       const hx_paged_cache* dst,
+                       const int32_t* block_table, int32_t block_table_stride,
+                       const int32_t* cu_seqlens, const int32_t* seq_lens,
+                       int32_t batch, int32_t total_tokens, int32_t max_seq_len,
+                       void* stream);
+
+/* Host helper: a prefill stage holds global layers [src_first, src_first + src_count), a decode
+ * stage [dst_first, dst_first + dst_count).  Writes the arguments of hx_kv_ingest_stage for their
+ * intersection; *layers = 0 when they share none.  Returns HX_ERR_INVALID_ARG on negative input
+ * or NULL outputs. */
+int hx_stage_overlap(int32_t src_first, int32_t src_count, int32_t dst_first, int32_t dst_count,
+                     int32_t* src_layer0, int32_t* dst_layer0, int32_t* layers);
+
+/* ---- (a'') append of the decode step's token -----------------------
+ * "the decoding phase generates subsequent tokens by one token at each step"; the
+ * token's K/V joins the request's cache.  seq_lens[i] = n_i COUNTS the new token
+ * (reading S12), so it is token n_i - 1: for every request with n_i >= 1, local kv head g, X in {K,V}
+ *
+ *   cache->X[layer][ block_table[i][(n_i-1) / ps] ][g][(n_i-1) % ps][:] = x_new[i][g][:]
+ *
+ * A bit copy; n_i == 0 writes nothing; nothing else in the cache changes.
+ * k_new, v_new : device fp16 [batch][kv_heads][head_dim], 16-byte aligned.
+ * Device-side contract: the destination slots of different requests are distinct (the last page
+ * of a request is not shared). */
+int hx_kv_append(const void* k_new, const void* v_new,
+                 const hx_paged_cache* cache, int32_t layer,
+                 const int32_t* block_table, int32_t block_table_stride,
+                 const int32_t* seq_lens, int32_t batch, int32_t max_seq_len,
+                 void* stream);
+
 /* ---- (b) paged decode attention ---------------------------------------------------------
  * PAPER.md:L110 (§4) integrates PagedAttention / FlashAttention and gives no formula; the
  * definition is the textbook one (reading S1).  For request i with n = seq_lens[i]
@@ -148,6 +194,18 @@ int hx_decode_attention(void* out, const void* q,
                         int32_t batch, int32_t max_seq_len, float sm_scale,
                         void* workspace, size_t workspace_bytes,
                         void* stream);
+
+/* Fused append-then-attend (F1): the same result, bit for bit, in the cache AND in `out`, as
+ * hx_kv_append(k_new, v_new, ...) followed by hx_decode_attention(...), in ONE launch: the warp
+ * that streams the last page of (request, kv head) overlays the new K/V row on the tile in shared
+ * memory and stores it to the page.  Arguments as in the two calls. */
+int hx_decode_attention_append(void* out, const void* q, const void* k_new, const void* v_new,
+                               const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
+                               const int32_t* block_table, int32_t block_table_stride,
+                               const int32_t* seq_lens,
+                               int32_t batch, int32_t max_seq_len, float sm_scale,
+                               void* workspace, size_t workspace_bytes,
+                               void* stream);
 
 /* Optional, once per process and device: measure how fast each SM streams from HBM when all SMs
  * load at once, and size hx_decode_attention's per-SM ranges accordingly.  On B200 the SMs fall into

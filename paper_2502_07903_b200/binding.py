@@ -16,6 +16,7 @@ EXPORTS = [
     "hx_kv_gather", "hx_decode_attention_workspace_bytes", "hx_decode_attention", "hx_pool_create",
     "hx_pool_shuffle", "hx_pool_alloc", "hx_pool_free", "hx_pool_num_free", "hx_pool_num_pages",
     "hx_pool_alloc_table", "hx_pool_destroy", "hx_decode_step_host", "hx_tune_sm_rates",
+    "hx_kv_ingest_stage", "hx_stage_overlap", "hx_kv_append", "hx_decode_attention_append",
 ]
 
 
@@ -97,6 +98,20 @@ def lib() -> C.CDLL:
         if not os.environ.get("HX_LIB") or hasattr(L, "hx_tune_sm_rates"):   # older A/B builds lack it
             L.hx_tune_sm_rates.restype = C.c_int
             L.hx_tune_sm_rates.argtypes = [C.c_void_p, C.c_size_t, C.c_void_p]
+        if not os.environ.get("HX_LIB") or hasattr(L, "hx_kv_append"):
+            L.hx_kv_ingest_stage.restype = C.c_int
+            L.hx_kv_ingest_stage.argtypes = [C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)] + [C.c_int32] * 9 + [
+                C.POINTER(_CCache), C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32,
+                C.c_void_p]
+            L.hx_stage_overlap.restype = C.c_int
+            L.hx_stage_overlap.argtypes = [C.c_int32] * 4 + [C.POINTER(C.c_int32)] * 3
+            L.hx_kv_append.restype = C.c_int
+            L.hx_kv_append.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CCache), C.c_int32, C.c_void_p, C.c_int32,
+                                       C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
+            L.hx_decode_attention_append.restype = C.c_int
+            L.hx_decode_attention_append.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(_CCache),
+                                                     C.c_int32, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_int32,
+                                                     C.c_int32, C.c_float, C.c_void_p, C.c_size_t, C.c_void_p]
         L.hx_decode_step_host.restype = C.c_int
         L.hx_decode_step_host.argtypes = [C.POINTER(_CStepArgs), C.c_void_p]
         _lib = L
@@ -193,6 +208,43 @@ def kv_gather(src_k, src_v, *, layers, heads, head_dim, src_tp, dst_tp, dst_rank
     """hx_kv_gather: exact inverse of kv_ingest (writes the shard tensors)."""
     _ingest(lib().hx_kv_gather, src_k, src_v, layers, heads, head_dim, src_tp, dst_tp, dst_rank, dst,
             block_table, block_table_stride, cu_seqlens, seq_lens, batch, total_tokens, max_seq_len, stream)
+
+
+def kv_ingest_stage(src_k, src_v, *, src_layers, src_layer0, dst_layer0, layers, heads, head_dim, src_tp, dst_tp,
+                    dst_rank, dst, block_table, block_table_stride, cu_seqlens, seq_lens, batch, total_tokens,
+                    max_seq_len, stream=None):
+    """hx_kv_ingest_stage (include/hx.h): `layers` layers, source layer src_layer0+c -> cache layer dst_layer0+c."""
+    assert len(src_k) == src_tp and len(src_v) == src_tp
+    _check(lib().hx_kv_ingest_stage(_ptr_array(src_k), _ptr_array(src_v), src_layers, src_layer0, dst_layer0, layers,
+                                    heads, head_dim, src_tp, dst_tp, dst_rank, dst.ref, _ptr(block_table),
+                                    block_table_stride, _ptr(cu_seqlens), _ptr(seq_lens), batch, total_tokens,
+                                    max_seq_len, _stream_ptr(stream)))
+
+
+def stage_overlap(src_first, src_count, dst_first, dst_count):
+    """hx_stage_overlap -> (src_layer0, dst_layer0, layers)."""
+    a, b, n = C.c_int32(), C.c_int32(), C.c_int32()
+    _check(lib().hx_stage_overlap(src_first, src_count, dst_first, dst_count, C.byref(a), C.byref(b), C.byref(n)))
+    return a.value, b.value, n.value
+
+
+def kv_append(k_new, v_new, cache: PagedCache, *, layer, block_table, block_table_stride, seq_lens, batch,
+              max_seq_len, stream=None):
+    """hx_kv_append (include/hx.h): token n_i-1 of every request joins the paged cache."""
+    _check(lib().hx_kv_append(_ptr(k_new), _ptr(v_new), cache.ref, layer, _ptr(block_table), block_table_stride,
+                              _ptr(seq_lens), batch, max_seq_len, _stream_ptr(stream)))
+
+
+def decode_attention_append(out, q, k_new, v_new, cache: PagedCache, *, layer, q_heads, block_table,
+                            block_table_stride, seq_lens, batch, max_seq_len, sm_scale=0.0, workspace=None,
+                            workspace_bytes=None, stream=None):
+    """hx_decode_attention_append: hx_kv_append + hx_decode_attention in one launch."""
+    if workspace_bytes is None:
+        workspace_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    _check(lib().hx_decode_attention_append(_ptr(out), _ptr(q), _ptr(k_new), _ptr(v_new), cache.ref, layer, q_heads,
+                                            _ptr(block_table), block_table_stride, _ptr(seq_lens), batch, max_seq_len,
+                                            C.c_float(sm_scale), _ptr(workspace), workspace_bytes,
+                                            _stream_ptr(stream)))
 
 
 def decode_attention_workspace_bytes(batch, q_heads, kv_heads, head_dim, max_seq_len, page_size=16) -> int:

@@ -21,6 +21,9 @@
 //    starts or ends inside one writes an (m, l, acc) partial and bumps the pair's arrival counter;
 //    the last arriver merges the pair's partials in worker order (= token order, so the result
 //    does not depend on who arrives last), normalises and writes (row A8).  No second launch.
+//  * APPEND (hx_decode_attention_append): the warp that streams the
+//    last page of a (request, kv head) overlays the step's new K/V row on the tile in shared memory
+//    and stores it to the page, so the decode step needs no separate append launch.
 //
 // attn_simple_kernel — one CTA per (request, q head) on CUDA cores; bring-up/debug only
 // (HX_ATTN_IMPL=simple).
@@ -66,6 +69,12 @@ struct StreamParams {
   int32_t B, Hq, Hkv, G, bt_stride;
   uint32_t layer_row0;    // first tensor-map row of the layer
   float scale_log2;
+  // fused append (hx_decode_attention_append): the step's new K/V rows [B][Hkv][D] and the layer's
+  // cache tensors; the owner of the last page of (request, kv head) overlays and stores the row
+  const __half* k_new;
+  const __half* v_new;
+  __half* kc;
+  __half* vc;
 };
 
 // ---------------------------------------------------------------------------- PTX helpers
@@ -237,7 +246,7 @@ __global__ void sm_rate_finalize_kernel(int n_sm, int reset, int damp_256) {
 }
 
 // ------------------------------------------------------------------------------------------
-template <int D, int NT>
+template <int D, int NT, bool APPEND>
 __global__ void __launch_bounds__(kWarps * 32, 1)
 attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
                    const StreamParams p) {
@@ -454,6 +463,20 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
       q_busy = false;
       seg_j0 = c.j;
     }
+    const bool last_page = (c.j == c.np - 1);
+    const int valid = last_page ? cn - 16 * (c.np - 1) : 16;
+    // fused append (F1): token n-1 is the step's new token; its K/V row comes from k_new/v_new, not
+    // from the page.  Fetch it (lanes [0,CH): K chunks, [CH,2CH): V chunks) while the tile lands.
+    int4 new_row = make_int4(0, 0, 0, 0);
+    int new_page = 0;
+    if (APPEND && last_page) {
+      constexpr int CH = D / 8;
+      if (lane < 2 * CH) {
+        const __half* src = (lane < CH ? p.k_new : p.v_new) + ((size_t)c.i * Hkv + c.g) * D + (lane % CH) * 8;
+        new_row = __ldg(reinterpret_cast<const int4*>(src));
+      }
+      new_page = __ldg(p.bt + (size_t)c.i * p.bt_stride + c.j);
+    }
     mbar_wait(bar_u32 + 8 * stage, (idx / kStages) & 1);
 #ifdef HX_TRACE
     if (idx == 0) HX_STAMP(2);
@@ -461,8 +484,20 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
 #endif
 
     const uint32_t kb = stage_u32 + stage * C::kStage, vb = kb + kTile;
-    const bool last_page = (c.j == c.np - 1);
-    const int valid = last_page ? cn - 16 * (c.np - 1) : 16;
+    if (APPEND && last_page) {
+      // overlay the row on the tile in shared memory (same swizzle as the TMA box) and store it to
+      // the page: cache and output both equal hx_kv_append followed by hx_decode_attention
+      constexpr int CH = D / 8;
+      const int r = valid - 1;
+      if (lane < 2 * CH) {
+        const int x = lane >= CH ? 1 : 0, ch = lane - x * CH;
+        *reinterpret_cast<int4*>(my_stage + stage * C::kStage + x * kTile + (ch >> 3) * 2048 + r * 128 +
+                                 (((ch & 7) ^ (r & 7)) << 4)) = new_row;
+        __half* dstg = (x ? p.vc : p.kc) + (((size_t)new_page * Hkv + c.g) * 16 + r) * D + ch * 8;
+        *reinterpret_cast<int4*>(dstg) = new_row;
+      }
+      __syncwarp();
+    }
     if (valid < 16) {
       // tail slots may hold anything (NaN/Inf): P is 0 there, but 0 * Inf = NaN in the PV MMA,
       // so the V rows past the context end are zeroed in shared memory (reading S10).
@@ -540,7 +575,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
 
     // ------------------------------------------------ segment end: output or partial (row A8)
     const bool seg_end = last_page || (ck == k1 - 1);
-    bool wrote_smem = valid < 16;
+    bool wrote_smem = valid < 16 || (APPEND && last_page);
     if (seg_end) {
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt)
@@ -807,13 +842,13 @@ int get_tile_maps(const void* k, const void* v, uint64_t rows, int D, CUtensorMa
   return HX_OK;
 }
 
-template <int D, int NT>
+template <int D, int NT, bool APPEND>
 int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream) {
   using C = Cfg<D, NT>;
   static bool attr_set[64] = {false};
   if (!attr_set[di.device]) {
     if (C::kSmem > di.max_smem_optin) HX_FAIL(HX_ERR_UNSUPPORTED, "device offers %d B shared memory per CTA, kernel needs %d", di.max_smem_optin, C::kSmem);
-    HX_CUDA_OK(cudaFuncSetAttribute(attn_stream_kernel<D, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmem));
+    HX_CUDA_OK(cudaFuncSetAttribute(attn_stream_kernel<D, NT, APPEND>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmem));
     attr_set[di.device] = true;
   }
   const uint64_t rows_per_layer = (uint64_t)a.num_pages * a.kv_heads * 16;
@@ -842,7 +877,12 @@ int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream
     p.Hq = a.q_heads; p.Hkv = a.kv_heads; p.G = a.q_heads / a.kv_heads; p.bt_stride = a.bt_stride;
     p.layer_row0 = (uint32_t)(rows_per_layer * a.layer);
     p.scale_log2 = a.sm_scale * kLog2e;
-    attn_stream_kernel<D, NT><<<grid, kWarps * 32, C::kSmem, stream>>>(tk, tv, p);
+    const size_t layer_elems = (size_t)rows_per_layer * D;
+    p.k_new = APPEND ? static_cast<const __half*>(a.k_new) + (size_t)b0 * a.kv_heads * D : nullptr;
+    p.v_new = APPEND ? static_cast<const __half*>(a.v_new) + (size_t)b0 * a.kv_heads * D : nullptr;
+    p.kc = static_cast<__half*>(const_cast<void*>(a.k_base)) + layer_elems * a.layer;
+    p.vc = static_cast<__half*>(const_cast<void*>(a.v_base)) + layer_elems * a.layer;
+    attn_stream_kernel<D, NT, APPEND><<<grid, kWarps * 32, C::kSmem, stream>>>(tk, tv, p);
     HX_CUDA_OK(cudaGetLastError());
   }
   return HX_OK;
@@ -908,10 +948,15 @@ int launch_attention(const AttnParams& a, cudaStream_t stream) {
   int rc = device_info(&di);
   if (rc) return rc;
   static const bool simple = [] { const char* e = getenv("HX_ATTN_IMPL"); return e && !strcmp(e, "simple"); }();
+  if (simple && a.k_new) HX_FAIL(HX_ERR_UNSUPPORTED, "HX_ATTN_IMPL=simple has no fused append");
   if (simple) return a.head_dim == 128 ? launch_simple<128>(a, stream) : launch_simple<64>(a, stream);
   const int G = a.q_heads / a.kv_heads;
-  if (a.head_dim == 128) return G > 8 ? launch_stream<128, 2>(a, di, stream) : launch_stream<128, 1>(a, di, stream);
-  return G > 8 ? launch_stream<64, 2>(a, di, stream) : launch_stream<64, 1>(a, di, stream);
+  if (a.k_new) {
+    if (a.head_dim == 128) return G > 8 ? launch_stream<128, 2, true>(a, di, stream) : launch_stream<128, 1, true>(a, di, stream);
+    return G > 8 ? launch_stream<64, 2, true>(a, di, stream) : launch_stream<64, 1, true>(a, di, stream);
+  }
+  if (a.head_dim == 128) return G > 8 ? launch_stream<128, 2, false>(a, di, stream) : launch_stream<128, 1, false>(a, di, stream);
+  return G > 8 ? launch_stream<64, 2, false>(a, di, stream) : launch_stream<64, 1, false>(a, di, stream);
 }
 
 }  // namespace hx

@@ -52,8 +52,8 @@ static int ingest_common(const void* const* src_k, const void* const* src_v, int
                          int32_t head_dim, int32_t src_tp, int32_t dst_tp, int32_t dst_rank,
                          const hx_paged_cache* dst, const int32_t* block_table, int32_t stride,
                          const int32_t* cu_seqlens, const int32_t* seq_lens, int32_t batch,
-                         int32_t total_tokens, int32_t max_seq_len, void* stream, bool gather) {
-  const char* who = gather ? "hx_kv_gather" : "hx_kv_ingest";
+                         int32_t total_tokens, int32_t max_seq_len, void* stream, bool gather,
+                         const char* who, int32_t src_layers, int32_t src_layer0, int32_t dst_layer0) {
   clear_error();
   if (layers < 0 || batch < 0 || total_tokens < 0 || max_seq_len < 0)
     HX_FAIL(HX_ERR_INVALID_ARG, "%s: negative size (layers=%d batch=%d total_tokens=%d max_seq_len=%d)", who, layers, batch, total_tokens, max_seq_len);
@@ -66,14 +66,18 @@ static int ingest_common(const void* const* src_k, const void* const* src_v, int
   if (rc) return rc;
   if (dst->head_dim != head_dim) HX_FAIL(HX_ERR_INVALID_ARG, "%s: head_dim %d != cache head_dim %d", who, head_dim, dst->head_dim);
   if (dst->kv_heads != heads / dst_tp) HX_FAIL(HX_ERR_INVALID_ARG, "%s: cache kv_heads %d != heads/dst_tp = %d", who, dst->kv_heads, heads / dst_tp);
-  if (layers > dst->layers) HX_FAIL(HX_ERR_INVALID_ARG, "%s: layers %d > cache layers %d", who, layers, dst->layers);
+  if (src_layers < 0) src_layers = layers;                     // plain ingest: the buffers hold exactly `layers`
+  if (src_layer0 < 0 || dst_layer0 < 0 || (int64_t)src_layer0 + layers > src_layers)
+    HX_FAIL(HX_ERR_INVALID_ARG, "%s: source layers [%d,%d) not inside [0,%d)", who, src_layer0, src_layer0 + layers, src_layers);
+  if ((int64_t)dst_layer0 + layers > dst->layers)
+    HX_FAIL(HX_ERR_INVALID_ARG, "%s: cache layers [%d,%d) not inside [0,%d)", who, dst_layer0, dst_layer0 + layers, dst->layers);
   if (batch == 0 || total_tokens == 0 || layers == 0) return HX_OK;
   if (!src_k || !src_v) HX_FAIL(HX_ERR_INVALID_ARG, "%s: src_k/src_v array is NULL", who);
   if (!block_table || !cu_seqlens || !seq_lens) HX_FAIL(HX_ERR_INVALID_ARG, "%s: block_table/cu_seqlens/seq_lens is NULL", who);
   if (max_seq_len > total_tokens) HX_FAIL(HX_ERR_INVALID_ARG, "%s: max_seq_len %d > total_tokens %d", who, max_seq_len, total_tokens);
   const int32_t ps = dst->page_size;
   if ((int64_t)stride * ps < (int64_t)max_seq_len) HX_FAIL(HX_ERR_INVALID_ARG, "%s: block_table_stride %d < ceil(max_seq_len %d / %d)", who, stride, max_seq_len, ps);
-  if ((int64_t)layers * total_tokens * (heads / src_tp) * head_dim >= (int64_t)1 << 40) HX_FAIL(HX_ERR_UNSUPPORTED, "%s: shard too large", who);
+  if ((int64_t)src_layers * total_tokens * (heads / src_tp) * head_dim >= (int64_t)1 << 40) HX_FAIL(HX_ERR_UNSUPPORTED, "%s: shard too large", who);
 
   IngestParams p;
   memset(&p, 0, sizeof(p));
@@ -87,6 +91,7 @@ static int ingest_common(const void* const* src_k, const void* const* src_v, int
   p.dst_k = dst->k; p.dst_v = dst->v;
   p.block_table = block_table; p.cu_seqlens = cu_seqlens; p.seq_lens = seq_lens;
   p.layers = layers; p.total_tokens = total_tokens; p.batch = batch;
+  p.src_layer0 = src_layer0; p.dst_layer0 = dst_layer0;
   p.head_dim = head_dim; p.page_size = ps; p.num_pages = dst->num_pages; p.bt_stride = stride;
   return launch_ingest(p, gather, static_cast<cudaStream_t>(stream));
 }
@@ -124,7 +129,36 @@ int hx_kv_ingest(const void* const* src_k, const void* const* src_v, int32_t lay
                  const int32_t* block_table, int32_t block_table_stride, const int32_t* cu_seqlens,
                  const int32_t* seq_lens, int32_t batch, int32_t total_tokens, int32_t max_seq_len, void* stream) {
   return hx::ingest_common(src_k, src_v, layers, heads, head_dim, src_tp, dst_tp, dst_rank, dst, block_table,
-                           block_table_stride, cu_seqlens, seq_lens, batch, total_tokens, max_seq_len, stream, false);
+                           block_table_stride, cu_seqlens, seq_lens, batch, total_tokens, max_seq_len, stream, false,
+                           "hx_kv_ingest", -1, 0, 0);
+}
+
+int hx_kv_ingest_stage(const void* const* src_k, const void* const* src_v, int32_t src_layers, int32_t src_layer0,
+                       int32_t dst_layer0, int32_t layers, int32_t heads, int32_t head_dim, int32_t src_tp,
+                       int32_t dst_tp, int32_t dst_rank, const hx_paged_cache* dst, const int32_t* block_table,
+                       int32_t block_table_stride, const int32_t* cu_seqlens, const int32_t* seq_lens,
+                       int32_t batch, int32_t total_tokens, int32_t max_seq_len, void* stream) {
+  if (src_layers < 0) {
+    hx::set_error("hx_kv_ingest_stage: src_layers %d is negative", src_layers);
+    return HX_ERR_INVALID_ARG;
+  }
+  return hx::ingest_common(src_k, src_v, layers, heads, head_dim, src_tp, dst_tp, dst_rank, dst, block_table,
+                           block_table_stride, cu_seqlens, seq_lens, batch, total_tokens, max_seq_len, stream, false,
+                           "hx_kv_ingest_stage", src_layers, src_layer0, dst_layer0);
+}
+
+int hx_stage_overlap(int32_t src_first, int32_t src_count, int32_t dst_first, int32_t dst_count,
+                     int32_t* src_layer0, int32_t* dst_layer0, int32_t* layers) {
+  using namespace hx;
+  clear_error();
+  if (!src_layer0 || !dst_layer0 || !layers) HX_FAIL(HX_ERR_INVALID_ARG, "hx_stage_overlap: NULL output");
+  if (src_first < 0 || src_count < 0 || dst_first < 0 || dst_count < 0) HX_FAIL(HX_ERR_INVALID_ARG, "hx_stage_overlap: negative input");
+  const int64_t lo = src_first > dst_first ? src_first : dst_first;
+  const int64_t se = (int64_t)src_first + src_count, de = (int64_t)dst_first + dst_count;
+  const int64_t hi = se < de ? se : de;
+  if (hi <= lo) { *src_layer0 = 0; *dst_layer0 = 0; *layers = 0; return HX_OK; }
+  *src_layer0 = (int32_t)(lo - src_first); *dst_layer0 = (int32_t)(lo - dst_first); *layers = (int32_t)(hi - lo);
+  return HX_OK;
 }
 
 int hx_kv_gather(void* const* src_k, void* const* src_v, int32_t layers, int32_t heads, int32_t head_dim,
@@ -133,7 +167,7 @@ int hx_kv_gather(void* const* src_k, void* const* src_v, int32_t layers, int32_t
                  const int32_t* seq_lens, int32_t batch, int32_t total_tokens, int32_t max_seq_len, void* stream) {
   return hx::ingest_common(const_cast<const void* const*>(src_k), const_cast<const void* const*>(src_v), layers, heads,
                            head_dim, src_tp, dst_tp, dst_rank, dst, block_table, block_table_stride, cu_seqlens,
-                           seq_lens, batch, total_tokens, max_seq_len, stream, true);
+                           seq_lens, batch, total_tokens, max_seq_len, stream, true, "hx_kv_gather", -1, 0, 0);
 }
 
 size_t hx_decode_attention_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, int32_t head_dim,
@@ -142,12 +176,12 @@ size_t hx_decode_attention_workspace_bytes(int32_t batch, int32_t q_heads, int32
   return hx::attn_workspace_bytes(batch, q_heads, kv_heads, head_dim, max_seq_len, page_size);
 }
 
-int hx_decode_attention(void* out, const void* q, const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
-                        const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
-                        int32_t batch, int32_t max_seq_len, float sm_scale, void* workspace,
-                        size_t workspace_bytes, void* stream) {
+static int attention_common(const char* who, void* out, const void* q, const void* k_new, const void* v_new, bool append,
+                            const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
+                            const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
+                            int32_t batch, int32_t max_seq_len, float sm_scale, void* workspace,
+                            size_t workspace_bytes, void* stream) {
   using namespace hx;
-  const char* who = "hx_decode_attention";
   clear_error();
   if (batch < 0 || max_seq_len < 0) HX_FAIL(HX_ERR_INVALID_ARG, "%s: negative size (batch=%d max_seq_len=%d)", who, batch, max_seq_len);
   int rc = check_cache(cache, who);
@@ -161,6 +195,10 @@ int hx_decode_attention(void* out, const void* q, const hx_paged_cache* cache, i
   if (!out || !q) HX_FAIL(HX_ERR_INVALID_ARG, "%s: out/q is NULL", who);
   if (!aligned16(out) || !aligned16(q)) HX_FAIL(HX_ERR_INVALID_ARG, "%s: out/q must be 16-byte aligned", who);
   if (!block_table || !seq_lens) HX_FAIL(HX_ERR_INVALID_ARG, "%s: block_table/seq_lens is NULL", who);
+  if (append) {
+    if (!k_new || !v_new) HX_FAIL(HX_ERR_INVALID_ARG, "%s: k_new/v_new is NULL", who);
+    if (!aligned16(k_new) || !aligned16(v_new)) HX_FAIL(HX_ERR_INVALID_ARG, "%s: k_new/v_new must be 16-byte aligned", who);
+  }
   if ((int64_t)block_table_stride * cache->page_size < (int64_t)max_seq_len)
     HX_FAIL(HX_ERR_INVALID_ARG, "%s: block_table_stride %d < ceil(max_seq_len %d / %d)", who, block_table_stride, max_seq_len, cache->page_size);
   const size_t need = attn_workspace_bytes(batch, q_heads, cache->kv_heads, cache->head_dim, max_seq_len, cache->page_size);
@@ -177,7 +215,53 @@ int hx_decode_attention(void* out, const void* q, const hx_paged_cache* cache, i
   p.batch = batch; p.q_heads = q_heads; p.kv_heads = cache->kv_heads; p.head_dim = cache->head_dim;
   p.page_size = cache->page_size; p.num_pages = cache->num_pages; p.bt_stride = block_table_stride;
   p.max_seq_len = max_seq_len; p.sm_scale = sm_scale;
+  p.k_new = append ? k_new : nullptr; p.v_new = append ? v_new : nullptr;
   return launch_attention(p, static_cast<cudaStream_t>(stream));
+}
+
+int hx_decode_attention(void* out, const void* q, const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
+                        const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
+                        int32_t batch, int32_t max_seq_len, float sm_scale, void* workspace,
+                        size_t workspace_bytes, void* stream) {
+  return attention_common("hx_decode_attention", out, q, nullptr, nullptr, false, cache, layer, q_heads, block_table,
+                          block_table_stride, seq_lens, batch, max_seq_len, sm_scale, workspace, workspace_bytes, stream);
+}
+
+int hx_decode_attention_append(void* out, const void* q, const void* k_new, const void* v_new,
+                               const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
+                               const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
+                               int32_t batch, int32_t max_seq_len, float sm_scale, void* workspace,
+                               size_t workspace_bytes, void* stream) {
+  return attention_common("hx_decode_attention_append", out, q, k_new, v_new, true, cache, layer, q_heads, block_table,
+                          block_table_stride, seq_lens, batch, max_seq_len, sm_scale, workspace, workspace_bytes, stream);
+}
+
+int hx_kv_append(const void* k_new, const void* v_new, const hx_paged_cache* cache, int32_t layer,
+                 const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens, int32_t batch,
+                 int32_t max_seq_len, void* stream) {
+  using namespace hx;
+  const char* who = "hx_kv_append";
+  clear_error();
+  if (batch < 0 || max_seq_len < 0) HX_FAIL(HX_ERR_INVALID_ARG, "%s: negative size (batch=%d max_seq_len=%d)", who, batch, max_seq_len);
+  int rc = check_cache(cache, who);
+  if (rc) return rc;
+  if (layer < 0 || layer >= cache->layers) HX_FAIL(HX_ERR_INVALID_ARG, "%s: layer %d not in [0,%d)", who, layer, cache->layers);
+  if (batch == 0) return HX_OK;
+  if (!k_new || !v_new) HX_FAIL(HX_ERR_INVALID_ARG, "%s: k_new/v_new is NULL", who);
+  if (!aligned16(k_new) || !aligned16(v_new)) HX_FAIL(HX_ERR_INVALID_ARG, "%s: k_new/v_new must be 16-byte aligned", who);
+  if (!block_table || !seq_lens) HX_FAIL(HX_ERR_INVALID_ARG, "%s: block_table/seq_lens is NULL", who);
+  if ((int64_t)block_table_stride * cache->page_size < (int64_t)max_seq_len)
+    HX_FAIL(HX_ERR_INVALID_ARG, "%s: block_table_stride %d < ceil(max_seq_len %d / %d)", who, block_table_stride, max_seq_len, cache->page_size);
+  if ((int64_t)batch * 2 * cache->kv_heads * (cache->head_dim / 8) >= (int64_t)1 << 31) HX_FAIL(HX_ERR_UNSUPPORTED, "%s: batch too large", who);
+  AppendParams p;
+  const size_t layer_elems = (size_t)cache->num_pages * cache->kv_heads * cache->page_size * cache->head_dim;
+  p.k_new = k_new; p.v_new = v_new;
+  p.k = static_cast<uint16_t*>(cache->k) + layer_elems * layer;
+  p.v = static_cast<uint16_t*>(cache->v) + layer_elems * layer;
+  p.block_table = block_table; p.seq_lens = seq_lens;
+  p.batch = batch; p.kv_heads = cache->kv_heads; p.head_dim = cache->head_dim; p.page_size = cache->page_size;
+  p.bt_stride = block_table_stride;
+  return launch_append(p, static_cast<cudaStream_t>(stream));
 }
 
 int hx_tune_sm_rates(const void* scratch, size_t scratch_bytes, void* stream) {

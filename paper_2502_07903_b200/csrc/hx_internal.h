@@ -45,6 +45,7 @@ struct IngestParams {
   const int32_t* cu_seqlens;
   const int32_t* seq_lens;
   int32_t layers, total_tokens, batch;
+  int32_t src_layer0, dst_layer0;  // first source / cache layer of the call (pipeline-stage ingest)
   int32_t hs, hd, head0;          // heads per source shard, per dest rank, first owned global head
   int32_t head_dim, page_size, num_pages, bt_stride;
 };
@@ -62,10 +63,23 @@ struct AttnParams {
   int32_t batch, q_heads, kv_heads, head_dim, page_size, num_pages, bt_stride, max_seq_len;
   int32_t layer, layers;
   float sm_scale;
+  const void* k_new;              // fused append (hx_decode_attention_append); NULL otherwise
+  const void* v_new;
 };
 size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, int32_t head_dim,
                             int32_t max_seq_len, int32_t page_size);
 int launch_attention(const AttnParams& p, cudaStream_t stream);
 int tune_sm_rates(const void* scratch, size_t bytes, cudaStream_t stream);
+
+struct AppendParams {
+  const void* k_new;
+  const void* v_new;
+  void* k;                        // cache tensors, already offset to the layer
+  void* v;
+  const int32_t* block_table;
+  const int32_t* seq_lens;
+  int32_t batch, kv_heads, head_dim, page_size, bt_stride;
+};
+int launch_append(const AppendParams& p, cudaStream_t stream);
 
 }  // namespace hx

@@ -71,8 +71,8 @@ __global__ void __launch_bounds__(kThreads) ingest_rows_kernel(const __grid_cons
           const int r = h / p.hs;
           const __half* sbase = static_cast<const __half*>(x ? p.src_v[r] : p.src_k[r]);
           const __half* dbase = static_cast<const __half*>(x ? p.dst_v : p.dst_k);
-          const __half* s = sbase + l * src_layer + src_tok + (size_t)(h - r * p.hs) * D;
-          const __half* d = dbase + l * dst_layer + dst_tok + (size_t)j * ps * D;
+          const __half* s = sbase + (size_t)(l + p.src_layer0) * src_layer + src_tok + (size_t)(h - r * p.hs) * D;
+          const __half* d = dbase + (size_t)(l + p.dst_layer0) * dst_layer + dst_tok + (size_t)j * ps * D;
           const __half* from = GATHER ? d : s;
           const __half* to = GATHER ? s : d;
           val[u] = ld_stream(reinterpret_cast<const int4*>(from));
@@ -86,7 +86,38 @@ __global__ void __launch_bounds__(kThreads) ingest_rows_kernel(const __grid_cons
   }
 }
 
+// hx_kv_append: one thread per 16-byte chunk of one
+// (request, K|V, kv head) row of the step's new token; B * 2 * Hkv * D/8 threads in all.
+template <int D>
+__global__ void __launch_bounds__(kThreads) append_kernel(const AppendParams p) {
+  constexpr int CH = D / 8;
+  const int idx = blockIdx.x * kThreads + threadIdx.x;
+  const int per_req = 2 * p.kv_heads * CH;
+  const int i = idx / per_req;
+  if (i >= p.batch) return;
+  const int n = __ldg(p.seq_lens + i);
+  if (n <= 0) return;
+  const int rem = idx - i * per_req;
+  const int x = rem / (p.kv_heads * CH);
+  const int gc = rem - x * (p.kv_heads * CH);
+  const int g = gc / CH, c = gc - g * CH;
+  const int t = n - 1;
+  const int page = __ldg(p.block_table + (size_t)i * p.bt_stride + t / p.page_size);
+  const __half* src = static_cast<const __half*>(x ? p.v_new : p.k_new) + ((size_t)i * p.kv_heads + g) * D + c * 8;
+  __half* dst = static_cast<__half*>(x ? p.v : p.k) + (((size_t)page * p.kv_heads + g) * p.page_size + t % p.page_size) * D + c * 8;
+  st_stream(reinterpret_cast<int4*>(dst), ld_stream(reinterpret_cast<const int4*>(src)));
+}
+
 }  // namespace
+
+int launch_append(const AppendParams& p, cudaStream_t stream) {
+  const long long threads = (long long)p.batch * 2 * p.kv_heads * (p.head_dim / 8);
+  const int grid = (int)((threads + kThreads - 1) / kThreads);
+  if (p.head_dim == 128) append_kernel<128><<<grid, kThreads, 0, stream>>>(p);
+  else                   append_kernel<64><<<grid, kThreads, 0, stream>>>(p);
+  HX_CUDA_OK(cudaGetLastError());
+  return HX_OK;
+}
 
 int launch_ingest(const IngestParams& p, bool gather, cudaStream_t stream) {
   DeviceInfo di;

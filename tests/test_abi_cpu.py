@@ -22,7 +22,7 @@ def test_library_exports_every_declared_symbol():
     L = hx.lib()
     for name in declared:
         assert hasattr(L, name), name
-    assert hx.version() == 100
+    assert hx.version() == 110
     assert hx.status_string(0) == "HX_OK" and hx.status_string(5) == "HX_ERR_NO_PAGES"
     assert hx.status_string(77) == "HX_ERR_UNKNOWN"
 
@@ -152,3 +152,71 @@ def test_ingest_unneeded_shard_may_be_null_and_empty_is_ok():
     _ingest(src=[0, 0x20000], dst_rank=1, batch=0)
     _ingest(total_tokens=0, max_seq_len=0)
     _ingest(layers=0)
+
+
+# ---------------------------------------------------------------- F3 / F1 entry points
+def _stage(cache=None, src=None, **over):
+    kw = dict(src_layers=3, src_layer0=1, dst_layer0=0, layers=2, heads=4, head_dim=128, src_tp=2, dst_tp=2,
+              dst_rank=0, block_table=0x3000, block_table_stride=4, cu_seqlens=0x4000, seq_lens=0x5000, batch=2,
+              total_tokens=100, max_seq_len=64, stream=0)
+    kw.update(over)
+    s = src if src is not None else [0x10000 * (r + 1) for r in range(kw["src_tp"])]
+    hx.kv_ingest_stage(s, list(s), dst=cache or FakeCache(), **kw)
+
+
+@pytest.mark.parametrize("over,status", [
+    (dict(src_layer0=2), B.HX_ERR_INVALID_ARG), (dict(src_layer0=-1), B.HX_ERR_INVALID_ARG),
+    (dict(dst_layer0=1), B.HX_ERR_INVALID_ARG), (dict(dst_layer0=-1), B.HX_ERR_INVALID_ARG),
+    (dict(src_layers=-1), B.HX_ERR_INVALID_ARG), (dict(layers=-1), B.HX_ERR_INVALID_ARG),
+    (dict(layers=3, src_layer0=0), B.HX_ERR_INVALID_ARG), (dict(heads=5), B.HX_ERR_INVALID_ARG),
+    (dict(src=[0, 0x20000]), B.HX_ERR_INVALID_ARG),
+])
+def test_stage_ingest_rejects_invalid_arguments_without_launching(over, status):
+    with pytest.raises(hx.HxError) as e:
+        _stage(**over)
+    assert e.value.status == status, str(e.value)
+    _stage(layers=0)                                                   # nothing to move: OK, no launch
+    _stage(batch=0)
+
+
+def test_stage_overlap_host_helper():
+    # prefill stages of 80 layers cut 27/27/26, decode stages 40/40 (Table 2 has PP=3 and PP=2)
+    src = [(0, 27), (27, 27), (54, 26)]
+    dst = [(0, 40), (40, 40)]
+    covered = np.zeros((80,), dtype=int)
+    for sf, sc in src:
+        for df, dc in dst:
+            a, b, n = hx.stage_overlap(sf, sc, df, dc)
+            if n:
+                assert sf + a == df + b and 0 <= a and a + n <= sc and 0 <= b and b + n <= dc
+                covered[sf + a: sf + a + n] += 1
+    assert (covered == 1).all()                                        # every layer moved exactly once
+    assert hx.stage_overlap(0, 10, 10, 5) == (0, 0, 0)
+    assert hx.stage_overlap(3, 4, 0, 100) == (0, 3, 4)
+    with pytest.raises(hx.HxError):
+        hx.stage_overlap(-1, 4, 0, 100)
+
+
+def _append(cache=None, fused=False, **over):
+    kw = dict(layer=0, block_table=0x3000, block_table_stride=4, seq_lens=0x4000, batch=2, max_seq_len=64, stream=0)
+    kw.update(over)
+    kn, vn = kw.pop("k_new", 0x8000), kw.pop("v_new", 0x9000)
+    if fused:
+        hx.decode_attention_append(kw.pop("out", 0x6000), kw.pop("q", 0x7000), kn, vn, cache or FakeCache(),
+                                   q_heads=4, workspace=0x5000, workspace_bytes=1 << 30, **kw)
+    else:
+        hx.kv_append(kn, vn, cache or FakeCache(), **kw)
+
+
+@pytest.mark.parametrize("fused", [False, True])
+@pytest.mark.parametrize("over,status", [
+    (dict(k_new=0), B.HX_ERR_INVALID_ARG), (dict(v_new=0x9004), B.HX_ERR_INVALID_ARG),
+    (dict(layer=2), B.HX_ERR_INVALID_ARG), (dict(batch=-1), B.HX_ERR_INVALID_ARG),
+    (dict(block_table=0), B.HX_ERR_INVALID_ARG), (dict(seq_lens=0), B.HX_ERR_INVALID_ARG),
+    (dict(block_table_stride=3), B.HX_ERR_INVALID_ARG), (dict(cache=FakeCache(ps=8)), B.HX_ERR_UNSUPPORTED),
+])
+def test_append_rejects_invalid_arguments_without_launching(fused, over, status):
+    with pytest.raises(hx.HxError) as e:
+        _append(fused=fused, **over)
+    assert e.value.status == status, str(e.value)
+    _append(fused=fused, batch=0)
