@@ -151,18 +151,37 @@ def run_hx(args, rank, world, local_rank):
     ing_cu = torch.from_numpy(ing["cu_seqlens"]).to(dev)
     ing_sl = torch.from_numpy(ing["seq_lens"]).to(dev)
     ing_bt_dev = torch.empty((nI, ing_stride), dtype=torch.int32, device=dev)
-    ing_bt_pin = torch.empty((nI, ing_stride), dtype=torch.int32).pin_memory()
+    # the host runs ahead of the GPU: a ring of pinned row buffers, each reused only after the copy
+    # that last read it has completed
+    RING = 16
+    ing_bt_pins = [torch.empty((nI, ing_stride), dtype=torch.int32).pin_memory() for _ in range(RING)]
+    ring_ev = [None] * RING
     pool = st["pool"]
-    prev = {"ids": None}
+    prev = {"ids": None, "n": 0}
 
-    def step(record=None):
-        # A1: free last step's prompts, allocate this step's (host), upload the new rows
+    def next_rows(stream=None):
+        """A1: free last step's prompts, allocate this step's (host), stage the new rows for upload."""
         if prev["ids"] is not None:
             pool.free(prev["ids"])
         rows = pool.alloc_table(st["ing_lens"], ing_stride)
         prev["ids"] = rows[rows >= 0]
-        ing_bt_pin.numpy()[:] = rows
-        ing_bt_dev.copy_(ing_bt_pin, non_blocking=True)
+        slot = prev["n"] % RING
+        prev["n"] += 1
+        if ring_ev[slot] is not None:
+            ring_ev[slot].synchronize()
+        pin = ing_bt_pins[slot]
+        pin.numpy()[:] = rows
+        return pin, slot
+
+    def uploaded(slot):
+        ev = ring_ev[slot] or torch.cuda.Event()
+        ev.record()
+        ring_ev[slot] = ev
+
+    def step(record=None):
+        pin, slot = next_rows()
+        ing_bt_dev.copy_(pin, non_blocking=True)
+        uploaded(slot)
         if record:
             record[0].record()
         hx.kv_ingest(src_k, src_v, layers=1, heads=ci.heads, head_dim=D, src_tp=4, dst_tp=1, dst_rank=0,
@@ -208,13 +227,10 @@ def run_hx(args, rank, world, local_rank):
     main = torch.cuda.current_stream(dev)
 
     def step_two_stream():
-        if prev["ids"] is not None:
-            pool.free(prev["ids"])
-        rows = pool.alloc_table(st["ing_lens"], ing_stride)
-        prev["ids"] = rows[rows >= 0]
-        ing_bt_pin.numpy()[:] = rows
+        pin, slot = next_rows()
         with torch.cuda.stream(side):
-            ing_bt_dev.copy_(ing_bt_pin, non_blocking=True)
+            ing_bt_dev.copy_(pin, non_blocking=True)
+            uploaded(slot)
             hx.kv_ingest(src_k, src_v, layers=1, heads=ci.heads, head_dim=D, src_tp=4, dst_tp=1, dst_rank=0,
                          dst=cache, block_table=ing_bt_dev, block_table_stride=ing_stride, cu_seqlens=ing_cu,
                          seq_lens=ing_sl, batch=nI, total_tokens=TI, max_seq_len=2048)
@@ -245,13 +261,10 @@ def run_hx(args, rank, world, local_rank):
     cu_h = torch.from_numpy(ing["cu_seqlens"]).pin_memory()
     sl_h = torch.from_numpy(ing["seq_lens"]).pin_memory()
 
-    def step_e2e():
-        if prev["ids"] is not None:
-            pool.free(prev["ids"])
-        rows = pool.alloc_table(st["ing_lens"], ing_stride)
-        prev["ids"] = rows[rows >= 0]
-        ing_bt_pin.numpy()[:] = rows
+    def step_e2e(pull):
+        ing_bt_pin, _ = next_rows()                     # (the step synchronises below: no reuse hazard)
         hx.decode_step_host(
+            pull_src=int(pull),
             q_host=qh, out_host=oh, q_dev=q, out_dev=out, cache=cache, layer=0, q_heads=Hq, block_table_dev=bt,
             block_table_stride=bt.shape[1], seq_lens_dev=sl, batch=B, max_seq_len=max_len, sm_scale=0.0,
             workspace=ws, workspace_bytes=ws_bytes, src_k_host=skh, src_v_host=svh, src_k_dev=src_k,
@@ -262,19 +275,26 @@ def run_hx(args, rank, world, local_rank):
         torch.cuda.current_stream().synchronize()      # the step's result is read on the host
         return float(oh[0, 0, 0])
 
-    for _ in range(3):
-        step_e2e()
-    barrier()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(args.steps):
-        step_e2e()
-    e1.record()
-    barrier()
-    e2e_ms = e0.elapsed_time(e1)
-    e2e_ms = max_over_ranks(e2e_ms, world, dev)
+    def time_e2e(pull):
+        for _ in range(3):
+            step_e2e(pull)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            step_e2e(pull)
+        e1.record()
+        barrier()
+        return max_over_ranks(e0.elapsed_time(e1), world, dev)
 
-    h2d = qh.numel() * 2 + sum(a.numel() * 2 for a in skh + svh) + ing_bt_pin.numel() * 4 + cu_h.numel() * 4 + sl_h.numel() * 4
+    # staged: cudaMemcpyAsync of the shards into HBM, then ingest (the headline e2e: the copy engine
+    # drives PCIe a little better than SM loads do).  pull (F2): the ingest kernel reads the pinned
+    # shards over the link itself (transfer + regroup + scatter fused); reported beside it.  The same
+    # bytes cross the link either way.
+    e2e_ms = time_e2e(False)
+    e2e_pull_ms = time_e2e(True)
+
+    h2d = qh.numel() * 2 + sum(a.numel() * 2 for a in skh + svh) + nI * ing_stride * 4 + cu_h.numel() * 4 + sl_h.numel() * 4
     d2h = oh.numel() * 2
     peak, peak_src = measured_peak()
     att_gbs = st["kv_bytes"] / (att_ms * 1e-3) / 1e9
@@ -283,6 +303,21 @@ def run_hx(args, rank, world, local_rank):
     extra = {}
     if rank == 0 and not args.no_extra:
         extra = other_configs(torch, hx, dev, peak)
+        # F1: the decode step's append, as its own launch and fused into the attention kernel
+        kn = torch.empty((B, Hkv, D), dtype=torch.float16, device=dev).normal_()
+        vn = torch.empty((B, Hkv, D), dtype=torch.float16, device=dev).normal_()
+        akw = dict(layer=0, block_table=bt, block_table_stride=bt.shape[1], seq_lens=sl, batch=B, max_seq_len=max_len)
+
+        def two_launches():
+            hx.kv_append(kn, vn, cache, **akw)
+            hx.decode_attention(out, q, cache, q_heads=Hq, workspace=ws, workspace_bytes=ws_bytes, **akw)
+
+        def fused():
+            hx.decode_attention_append(out, q, kn, vn, cache, q_heads=Hq, workspace=ws, workspace_bytes=ws_bytes, **akw)
+        m2, _ = time_kernel(torch, two_launches, iters=20)
+        m1, _ = time_kernel(torch, fused, iters=20)
+        extra["append_cfg5"] = {"append_then_attention_ms": m2, "fused_append_attention_ms": m1,
+                                "note": "hx_kv_append + hx_decode_attention (2 launches) vs hx_decode_attention_append (1 launch)"}
 
     line = {
         "metric": METRIC, "value": whole_job_value(step_bytes, args.steps, world, total_ms), "unit": UNIT,
@@ -297,7 +332,10 @@ def run_hx(args, rank, world, local_rank):
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
         "clocks": clocks,
         "e2e": {"value": whole_job_value(step_bytes, args.steps, world, e2e_ms), "unit": UNIT,
-                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms / args.steps},
+                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms / args.steps,
+                "path": "hx_decode_step_host: shards staged into HBM by cudaMemcpyAsync, then ingest + attention",
+                "pull_mode_ms_per_step": e2e_pull_ms / args.steps,
+                "pull_mode_value": whole_job_value(step_bytes, args.steps, world, e2e_pull_ms)},
         "gpu_launches": int(args.steps * LAUNCHES_PER_STEP),
         "roofline": {"bound": "hbm", "kernel": "hx_decode_attention (attn_stream_kernel, in-kernel merge)",
                      "achieved": att_gbs, "peak": peak, "unit": "GB/s", "frac": att_gbs / peak,

@@ -92,7 +92,10 @@ size_t hx_paged_cache_bytes(int32_t layers, int32_t num_pages, int32_t kv_heads,
  * unowned pages and other layers beyond `layers` keep their contents).
  *
  * src_k, src_v : HOST arrays of src_tp DEVICE pointers (16-byte aligned).  Entries for shards
- *                that hold none of dst_rank's heads may be NULL.
+ *                that hold none of dst_rank's heads may be NULL.  "Device pointer" = any address the
+ *                GPU can load from: its own HBM, a peer GPU's memory (peer access enabled) or pinned
+ *                host memory; the last two make the call a PULL-mode handoff (F2): the shard crosses
+ *                the link once, straight into its pages.
  * layers       : layers present in the source buffers; they land at layers [0, layers) of dst
  *                (a pipeline stage = one call; dst->layers >= layers).
  * heads        : GLOBAL kv heads; must be divisible by src_tp and dst_tp; dst->kv_heads == heads/dst_tp.
@@ -257,6 +260,12 @@ typedef struct {
   const int32_t* ing_cu_seqlens_host;  const int32_t* ing_seq_lens_host;
   int32_t* ing_block_table_dev; int32_t* ing_cu_seqlens_dev; int32_t* ing_seq_lens_dev; /* device staging */
   int32_t ing_batch, ing_total_tokens, ing_max_seq_len;
+  /* F2 pull mode ("asynchronous ... to enable overlapping"): non-zero =
+   * do NOT stage the shards; hx_kv_ingest reads them through src_k_host/src_v_host directly, over
+   * the link, fusing transfer + head regroup + page scatter in one kernel.  The pointers must then
+   * be reachable from the device: pinned host memory (UVA) or a peer GPU's memory with peer access
+   * enabled.  src_k_dev/src_v_dev are ignored. */
+  int32_t pull_src;
 } hx_step_host_args;
 int hx_decode_step_host(const hx_step_host_args* args, void* stream);
 

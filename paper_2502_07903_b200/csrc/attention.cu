@@ -98,10 +98,23 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-__device__ __forceinline__ void tma_tile_3d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2, uint32_t bar) {
+// K/V tiles are read once per call: evict-first keeps them from pushing the block table, Q and the
+// partials out of L2.
+__device__ __forceinline__ uint64_t policy_evict_first() {
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+__device__ __forceinline__ void tma_tile_3d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2, uint32_t bar, uint64_t pol) {
+#ifdef HX_NO_EVICT_FIRST
   asm volatile(
       "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
       ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
+#else
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4}], [%5], %6;"
+      ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "l"(pol) : "memory");
+#endif
 }
 __device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -271,6 +284,10 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
 #define HX_STAMP(x)
 #endif
   HX_STAMP(0);
+  if (tid == 32) {                                   // descriptor fetch off the first TMA's critical path
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&tmK) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&tmV) : "memory");
+  }
 
   // ---- which CTA-level range is mine.  Not tuned: range blockIdx.x.  Tuned (hx_tune_sm_rates):
   // range sizes follow the per-SM rate table, so the range of SM s belongs to the CTA running on
@@ -370,6 +387,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
   const uint32_t q_u32 = smem_u32(my_q);
   const uint32_t bar_u32 = smem_u32(bars + warp * (kStages + 1));
   const uint32_t qbar = bar_u32 + 8 * kStages;
+  const uint64_t kv_policy = policy_evict_first();
 
   // ---- per-lane lookahead: lane L of round r describes tile k0 + 32 r + L
   int page_cur = 0, gpart_cur = 0, meta_cur = 0, page_nxt = 0, gpart_nxt = 0, meta_nxt = 0;
@@ -430,8 +448,8 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         const uint32_t dst = stage_u32 + stage * C::kStage;
         const int row = (int)(p.layer_row0 + (uint32_t)page * (uint32_t)(Hkv * 16) + (uint32_t)gpart);
         mbar_expect_tx(full, 2 * kTile);
-        tma_tile_3d(dst, &tmK, 0, row, 0, full);
-        tma_tile_3d(dst + kTile, &tmV, 0, row, 0, full);
+        tma_tile_3d(dst, &tmK, 0, row, 0, full, kv_policy);
+        tma_tile_3d(dst + kTile, &tmV, 0, row, 0, full, kv_policy);
       }
       if (segstart) q_busy = true;
       ++pk;
@@ -705,16 +723,13 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
   }
 #endif
 
-  // ---- tuned mode: the last CTA of the grid to finish clears the claim flags for the next call
+  // ---- tuned mode: the last CTA of the grid to finish clears the claim flags for the next call.
+  // No fences: every CTA's claim (an atomic whose result it consumed) precedes its own count-up, and
+  // the plain stores below are flushed by kernel completion.
   if (tuned) {
     __syncthreads();
-    if (tid == 0) {
-      __threadfence();
-      if (atomicAdd(p.claim + kMaxSm, 1) == nC - 1) {
-        for (int s = 0; s <= kMaxSm; ++s) p.claim[s] = 0;
-        __threadfence();
-      }
-    }
+    if (tid == 0 && atomicAdd(p.claim + kMaxSm, 1) == nC - 1)
+      for (int s = 0; s <= kMaxSm; ++s) p.claim[s] = 0;
   }
 }
 

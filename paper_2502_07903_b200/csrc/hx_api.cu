@@ -282,14 +282,15 @@ int hx_decode_step_host(const hx_step_host_args* a, void* stream_) {
   if (!a->cache) HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_host: cache is NULL");
   const size_t qbytes = (size_t)a->batch * a->q_heads * a->cache->head_dim * 2;
   if (a->ing_batch > 0) {
-    if (!a->src_k_host || !a->src_v_host || !a->src_k_dev || !a->src_v_dev || !a->ing_block_table_host ||
+    const bool pull = a->pull_src != 0;
+    if (!a->src_k_host || !a->src_v_host || (!pull && (!a->src_k_dev || !a->src_v_dev)) || !a->ing_block_table_host ||
         !a->ing_cu_seqlens_host || !a->ing_seq_lens_host || !a->ing_block_table_dev || !a->ing_cu_seqlens_dev ||
         !a->ing_seq_lens_dev)
       HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_host: ingest buffers missing");
     if (a->src_tp <= 0 || a->src_tp > 16 || a->heads <= 0 || a->heads % a->src_tp)
       HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_host: bad heads/src_tp");
     const size_t shard = (size_t)a->ing_layers * a->ing_total_tokens * (a->heads / a->src_tp) * a->cache->head_dim * 2;
-    for (int r = 0; r < a->src_tp; ++r) {
+    for (int r = 0; r < a->src_tp && !pull; ++r) {
       if (!a->src_k_host[r] || !a->src_k_dev[r]) continue;   // shard not needed by this rank
       HX_CUDA_OK(cudaMemcpyAsync(a->src_k_dev[r], a->src_k_host[r], shard, cudaMemcpyHostToDevice, stream));
       HX_CUDA_OK(cudaMemcpyAsync(a->src_v_dev[r], a->src_v_host[r], shard, cudaMemcpyHostToDevice, stream));
@@ -298,7 +299,8 @@ int hx_decode_step_host(const hx_step_host_args* a, void* stream_) {
                                (size_t)a->ing_batch * a->ing_block_table_stride * 4, cudaMemcpyHostToDevice, stream));
     HX_CUDA_OK(cudaMemcpyAsync(a->ing_cu_seqlens_dev, a->ing_cu_seqlens_host, (size_t)(a->ing_batch + 1) * 4, cudaMemcpyHostToDevice, stream));
     HX_CUDA_OK(cudaMemcpyAsync(a->ing_seq_lens_dev, a->ing_seq_lens_host, (size_t)a->ing_batch * 4, cudaMemcpyHostToDevice, stream));
-    int rc = hx_kv_ingest(const_cast<const void* const*>(a->src_k_dev), const_cast<const void* const*>(a->src_v_dev),
+    int rc = hx_kv_ingest(pull ? a->src_k_host : const_cast<const void* const*>(a->src_k_dev),
+                          pull ? a->src_v_host : const_cast<const void* const*>(a->src_v_dev),
                           a->ing_layers, a->heads, a->cache->head_dim, a->src_tp, a->dst_tp, a->dst_rank, a->cache,
                           a->ing_block_table_dev, a->ing_block_table_stride, a->ing_cu_seqlens_dev,
                           a->ing_seq_lens_dev, a->ing_batch, a->ing_total_tokens, a->ing_max_seq_len, stream_);
