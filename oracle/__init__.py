@@ -6,5 +6,5 @@ Citations and the list of pins are in oracle/hxo.c's header.
 """
 from .hxo import (  # noqa: F401
     build, lib, kv_ingest, kv_gather, decode_attention, partial_attention,
-    half_to_double, max_threads, merge_partials, kv_ingest_stage, kv_append,
+    half_to_double, max_threads, merge_partials, kv_ingest_stage, kv_append, prefill_attention,
 )

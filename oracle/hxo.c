@@ -25,7 +25,9 @@
  * all-65536-pattern fp16 decode vs numpy, Table-1 byte counts;
  * stage ingest: any cut of the model into prefill x decode stages == the one-call ingest, and an
  * independent numpy restatement; append: ingest of n-1 tokens + append == ingest of n tokens,
- * changed-element count, attention after append == dense softmax over the concatenation.
+ * changed-element count, attention after append == dense softmax over the concatenation;
+ * prefill: brute-force causal numpy/scipy, m = 1 == decode attention, first token returns v_0,
+ * future tokens never matter, chunked (m < n) == the tail rows of the whole-prompt result.
  * No function here is "parity unpinned".
  */
 #include <math.h>
@@ -210,6 +212,61 @@ int hxo_decode_attention(double* out, const uint16_t* q, const uint16_t* k, cons
       for (int e = 0; e < D; ++e) o[e] /= l;
       free(s);
     }
+  }
+  return 0;
+}
+
+/* Paged prefill (multi-token) attention, causal ("the prefill phase
+ * processes the request's input tokens all at once", PAPER.md:L110 integrates FlashAttention for it;
+ * the definition is the textbook causal one, reading S24).  Request i has n_i cached tokens
+ * and m_i query tokens, which are its LAST m_i tokens: query r (0 <= r < m_i) sits at position
+ * p = n_i - m_i + r and attends to the cached tokens t = 0..p:
+ *     out[cu_q[i] + r][h] = sum_{t<=p} softmax_t(scale * <q[cu_q[i]+r][h], k_t>) v_t,   g = h div G.
+ * m_i = n_i is a whole-prompt prefill; m_i = 1 is hx's decode attention.  m_i = 0: no rows.
+ * q: uint16 [Tq][Hq][D] packed by request; out: double [Tq][Hq][D].  Two passes, float64. */
+int hxo_prefill_attention(double* out, const uint16_t* q, const uint16_t* k, const uint16_t* v,
+                          int layer, int num_pages, int kv_heads, int page_size, int head_dim,
+                          int q_heads, const int32_t* block_table, int block_table_stride,
+                          const int32_t* seq_lens, const int32_t* q_lens, const int32_t* cu_q,
+                          int batch, double scale, int threads) {
+  if (kv_heads <= 0 || q_heads % kv_heads) return 1;
+  for (int i = 0; i < batch; ++i) if (q_lens[i] < 0 || q_lens[i] > seq_lens[i]) return 2;
+  const int G = q_heads / kv_heads;
+  const int64_t D = head_dim, P = num_pages, ps = page_size;
+#ifdef _OPENMP
+  if (threads <= 0) threads = omp_get_max_threads();
+#pragma omp parallel for num_threads(threads) schedule(dynamic, 1)
+#endif
+  for (int i = 0; i < batch; ++i) {
+    double* s = (double*)malloc(sizeof(double) * (size_t)(seq_lens[i] > 0 ? seq_lens[i] : 1));
+    for (int r = 0; r < q_lens[i]; ++r) {
+      const int p = seq_lens[i] - q_lens[i] + r;           /* position of this query token */
+      for (int h = 0; h < q_heads; ++h) {
+        const int g = h / G;
+        const uint16_t* qh = q + (((int64_t)cu_q[i] + r) * q_heads + h) * D;
+        double* o = out + (((int64_t)cu_q[i] + r) * q_heads + h) * D;
+        double m = -INFINITY;
+        for (int t = 0; t <= p; ++t) {
+          const int64_t page = block_table[(int64_t)i * block_table_stride + t / ps];
+          const uint16_t* kt = k + ((((int64_t)layer * P + page) * kv_heads + g) * ps + (t % ps)) * D;
+          double dot = 0.0;
+          for (int e = 0; e < D; ++e) dot += hxo_half_to_double(qh[e]) * hxo_half_to_double(kt[e]);
+          s[t] = scale * dot;
+          if (s[t] > m) m = s[t];
+        }
+        double l = 0.0;
+        for (int e = 0; e < D; ++e) o[e] = 0.0;
+        for (int t = 0; t <= p; ++t) {
+          const int64_t page = block_table[(int64_t)i * block_table_stride + t / ps];
+          const uint16_t* vt = v + ((((int64_t)layer * P + page) * kv_heads + g) * ps + (t % ps)) * D;
+          const double w = exp(s[t] - m);
+          l += w;
+          for (int e = 0; e < D; ++e) o[e] += w * hxo_half_to_double(vt[e]);
+        }
+        for (int e = 0; e < D; ++e) o[e] /= l;
+      }
+    }
+    free(s);
   }
   return 0;
 }

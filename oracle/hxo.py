@@ -153,6 +153,28 @@ def decode_attention(q, k, v, block_table, seq_lens, *, layer=0, sm_scale=None, 
     return out
 
 
+def prefill_attention(q, k, v, block_table, seq_lens, q_lens, *, layer=0, sm_scale=None, threads=0):
+    """Causal paged attention of the LAST q_lens[i] tokens of each request (F4).
+    q fp16 [sum(q_lens)][Hq][D] packed by request -> float64 of the same shape."""
+    q, k, v = _u16(q), _u16(k), _u16(v)
+    Tq, Hq, D = q.shape
+    Ln, P, Hkv, ps, Dk = k.shape
+    assert Dk == D and v.shape == k.shape and 0 <= layer < Ln
+    bt = np.ascontiguousarray(block_table, dtype=np.int32)
+    sl = np.ascontiguousarray(seq_lens, dtype=np.int32)
+    ql = np.ascontiguousarray(q_lens, dtype=np.int32)
+    cu = np.zeros(len(ql) + 1, dtype=np.int32)
+    np.cumsum(ql, out=cu[1:])
+    assert cu[-1] == Tq and len(ql) == len(sl)
+    scale = default_scale(D) if sm_scale is None or sm_scale <= 0 else float(np.float32(sm_scale))
+    out = np.zeros((Tq, Hq, D), dtype=np.float64)
+    rc = lib().hxo_prefill_attention(_p(out), _p(q), _p(k), _p(v), layer, P, Hkv, ps, D, Hq, _p(bt),
+                                     bt.shape[1], _p(sl), _p(ql), _p(cu), len(sl), C.c_double(scale), int(threads))
+    if rc:
+        raise ValueError(f"hxo_prefill_attention: invalid arguments ({rc})")
+    return out
+
+
 def partial_attention(q_row, k, v, bt_row, g, t0, t1, *, layer=0, scale):
     q_row, k, v = _u16(q_row), _u16(k), _u16(v)
     _, P, Hkv, ps, D = k.shape

@@ -173,3 +173,85 @@ def test_attention_after_append_equals_dense_softmax_over_old_plus_new():
             np.testing.assert_allclose(got[i, h], softmax(Kd @ q[i, h].astype(np.float64) * scale) @ Vd, atol=1e-12)
     # and the generic dense pin still holds on the updated cache
     np.testing.assert_allclose(got, dense_reference(q, kf, vf, bt, lens, layer=2), atol=1e-12)
+
+
+# ---------------------------------------------------------------- F4: causal paged prefill attention
+def _prefill_case(seed, Hq, Hkv, D, lens, qlens, ps=4):
+    lens = np.asarray(lens, dtype=np.int32)
+    _, k, v, bt, lens = small_case(seed, len(lens), Hq, Hkv, D, lens, ps)
+    qlens = np.asarray(qlens, dtype=np.int32)
+    q = np.random.default_rng(seed + 100).standard_normal((int(qlens.sum()), Hq, D)).astype(np.float16)
+    return q, k, v, bt, lens, qlens
+
+
+def dense_causal(q, k, v, bt, lens, qlens):
+    """Brute force with numpy/scipy only: gather the request's K/V densely, mask by position."""
+    Tq, Hq, D = q.shape
+    _, P, Hkv, ps, _ = k.shape
+    G = Hq // Hkv
+    scale = float(np.float32(1.0) / np.sqrt(np.float32(D)))
+    out = np.zeros((Tq, Hq, D))
+    row = 0
+    for i, (n, m) in enumerate(zip(lens, qlens)):
+        t = np.arange(n)
+        Kd = k[0, bt[i, t // ps], :, t % ps].astype(np.float64)        # [n][Hkv][D]
+        Vd = v[0, bt[i, t // ps], :, t % ps].astype(np.float64)
+        for r in range(m):
+            p = n - m + r
+            for h in range(Hq):
+                s = Kd[:p + 1, h // G] @ q[row, h].astype(np.float64) * scale
+                out[row, h] = softmax(s) @ Vd[:p + 1, h // G]
+            row += 1
+    return out
+
+
+@pytest.mark.parametrize("Hq,Hkv,D,lens,qlens", [
+    (2, 2, 8, [5, 1, 9], [5, 1, 9]),            # whole-prompt prefill, MHA
+    (4, 2, 16, [7, 12, 4], [3, 12, 0]),         # chunked / empty
+    (8, 1, 8, [16, 17], [16, 2]),               # GQA, page boundaries
+])
+def test_prefill_equals_bruteforce_causal_dense(Hq, Hkv, D, lens, qlens):
+    q, k, v, bt, lens, qlens = _prefill_case(21, Hq, Hkv, D, lens, qlens)
+    got = oracle.prefill_attention(q, k, v, bt, lens, qlens)
+    np.testing.assert_allclose(got, dense_causal(q, k, v, bt, lens, qlens), atol=1e-12)
+
+
+def test_prefill_with_one_query_token_is_decode_attention():
+    q, k, v, bt, lens, qlens = _prefill_case(22, 4, 2, 16, [1, 6, 13, 8], [1, 1, 1, 1])
+    a = oracle.prefill_attention(q, k, v, bt, lens, qlens)
+    b = oracle.decode_attention(q, k, v, bt, lens)              # q is [B][Hq][D] when every m_i = 1
+    np.testing.assert_allclose(a, b, atol=1e-13)
+
+
+def test_prefill_first_token_returns_v0_and_future_tokens_never_matter():
+    q, k, v, bt, lens, qlens = _prefill_case(23, 2, 1, 8, [11, 6], [11, 6])
+    base = oracle.prefill_attention(q, k, v, bt, lens, qlens)
+    ps = k.shape[3]
+    cu = np.concatenate([[0], np.cumsum(qlens)])
+    for i in range(2):                                                    # position 0 sees only token 0
+        v0 = v[0, bt[i, 0], 0, 0].astype(np.float64)
+        np.testing.assert_array_equal(base[cu[i], 0], v0)
+        np.testing.assert_array_equal(base[cu[i], 1], v0)
+    # poison everything after position 4 of request 0: rows 0..4 must not change, later rows must
+    k2, v2 = k.copy(), v.copy()
+    for t in range(5, 11):
+        k2[0, bt[0, t // ps], :, t % ps] = np.float16(3.0)
+        v2[0, bt[0, t // ps], :, t % ps] = np.float16(-7.0)
+    got = oracle.prefill_attention(q, k2, v2, bt, lens, qlens)
+    np.testing.assert_array_equal(got[:5], base[:5])
+    assert np.abs(got[5:11] - base[5:11]).max() > 1e-3
+    np.testing.assert_array_equal(got[11:], base[11:])
+
+
+def test_chunked_prefill_equals_tail_rows_of_whole_prefill_and_constant_v():
+    q, k, v, bt, lens, qlens = _prefill_case(24, 4, 4, 8, [9, 14], [9, 14])
+    whole = oracle.prefill_attention(q, k, v, bt, lens, qlens)
+    ql2 = np.array([4, 5], dtype=np.int32)
+    q2 = np.concatenate([q[5:9], q[9 + 9:9 + 14]])
+    part = oracle.prefill_attention(q2, k, v, bt, lens, ql2)
+    np.testing.assert_array_equal(part, np.concatenate([whole[5:9], whole[18:23]]))
+    vc = np.broadcast_to(np.linspace(-1, 1, 8).astype(np.float16), v.shape).copy()
+    np.testing.assert_allclose(oracle.prefill_attention(q, k, vc, bt, lens, qlens),
+                               np.broadcast_to(vc[0, 0, 0, 0].astype(np.float64), whole.shape), atol=1e-14)
+    with pytest.raises(ValueError):
+        oracle.prefill_attention(q2, k, v, bt, lens, np.array([10, -1], dtype=np.int32))
