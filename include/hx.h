@@ -48,7 +48,7 @@
 extern "C" {
 #endif
 
-#define HX_VERSION 110 /* 0.1.1: + hx_kv_ingest_stage, hx_stage_overlap, hx_kv_append, hx_decode_attention_append */
+#define HX_VERSION 120 /* 0.1.2: + stage ingest, append, fused append-attend, pull mode, prefill attention */
 
 typedef enum {
   HX_OK = 0,
@@ -209,6 +209,31 @@ int hx_decode_attention_append(void* out, const void* q, const void* k_new, cons
                                int32_t batch, int32_t max_seq_len, float sm_scale,
                                void* workspace, size_t workspace_bytes,
                                void* stream);
+
+/* ---- (c) paged prefill attention -------------------------------------
+ * "the prefill phase processes the request's input tokens all at once" (compute-bound);
+ * PAPER.md:L110 integrates FlashAttention for it.  Causal attention of the LAST q_lens[i] tokens of
+ * request i over its paged context of seq_lens[i] tokens (reading S24): query r (0 <= r < q_lens[i])
+ * sits at position p = seq_lens[i] - q_lens[i] + r and attends to cached tokens t = 0..p,
+ *
+ *   out[cu_q_lens[i] + r][h] = sum_{t<=p} softmax_t(sm_scale * <q[cu_q_lens[i]+r][h], K_t>) V_t
+ *
+ * with K_t, V_t read through the block table as in hx_decode_attention (kv head h / G).  q_lens ==
+ * seq_lens is a whole-prompt prefill over a cache the prompt's K/V were already written to;
+ * q_lens < seq_lens is a chunked prefill; q_lens == 1 equals hx_decode_attention.
+ * Runs on tcgen05 tensor cores (fp16 in, fp32 accumulate in tensor memory, fp16 out).
+ *
+ * out, q       : device fp16 [total_q_tokens][q_heads][head_dim], rows packed by request, 16-byte aligned.
+ * q_lens       : device int32 [batch], 0 <= q_lens[i] <= seq_lens[i] (device-side contract).
+ * cu_q_lens    : device int32 [batch+1], exclusive prefix sums of q_lens.
+ * total_q_tokens, max_q_len, max_seq_len : host copies for launch sizing and checks.
+ * HX_ERR_UNSUPPORTED: head_dim != 128 (this version), group size not in {1,2,4,8,16}. */
+int hx_prefill_attention(void* out, const void* q,
+                         const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
+                         const int32_t* block_table, int32_t block_table_stride,
+                         const int32_t* seq_lens, const int32_t* q_lens, const int32_t* cu_q_lens,
+                         int32_t batch, int32_t total_q_tokens, int32_t max_q_len, int32_t max_seq_len,
+                         float sm_scale, void* stream);
 
 /* Optional, once per process and device: measure how fast each SM streams from HBM when all SMs
  * load at once, and size hx_decode_attention's per-SM ranges accordingly.  On B200 the SMs fall into

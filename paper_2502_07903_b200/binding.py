@@ -17,6 +17,7 @@ EXPORTS = [
     "hx_pool_shuffle", "hx_pool_alloc", "hx_pool_free", "hx_pool_num_free", "hx_pool_num_pages",
     "hx_pool_alloc_table", "hx_pool_destroy", "hx_decode_step_host", "hx_tune_sm_rates",
     "hx_kv_ingest_stage", "hx_stage_overlap", "hx_kv_append", "hx_decode_attention_append",
+    "hx_prefill_attention",
 ]
 
 
@@ -113,6 +114,11 @@ def lib() -> C.CDLL:
             L.hx_decode_attention_append.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(_CCache),
                                                      C.c_int32, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_int32,
                                                      C.c_int32, C.c_float, C.c_void_p, C.c_size_t, C.c_void_p]
+        if not os.environ.get("HX_LIB") or hasattr(L, "hx_prefill_attention"):
+            L.hx_prefill_attention.restype = C.c_int
+            L.hx_prefill_attention.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CCache), C.c_int32, C.c_int32,
+                                               C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
+                                               C.c_int32, C.c_int32, C.c_int32, C.c_float, C.c_void_p]
         L.hx_decode_step_host.restype = C.c_int
         L.hx_decode_step_host.argtypes = [C.POINTER(_CStepArgs), C.c_void_p]
         _lib = L
@@ -246,6 +252,15 @@ def decode_attention_append(out, q, k_new, v_new, cache: PagedCache, *, layer, q
                                             _ptr(block_table), block_table_stride, _ptr(seq_lens), batch, max_seq_len,
                                             C.c_float(sm_scale), _ptr(workspace), workspace_bytes,
                                             _stream_ptr(stream)))
+
+
+def prefill_attention(out, q, cache: PagedCache, *, layer, q_heads, block_table, block_table_stride, seq_lens,
+                      q_lens, cu_q_lens, batch, total_q_tokens, max_q_len, max_seq_len, sm_scale=0.0, stream=None):
+    """hx_prefill_attention (include/hx.h): causal paged attention of the last q_lens[i] tokens."""
+    _check(lib().hx_prefill_attention(_ptr(out), _ptr(q), cache.ref, layer, q_heads, _ptr(block_table),
+                                      block_table_stride, _ptr(seq_lens), _ptr(q_lens), _ptr(cu_q_lens), batch,
+                                      total_q_tokens, max_q_len, max_seq_len, C.c_float(sm_scale),
+                                      _stream_ptr(stream)))
 
 
 def decode_attention_workspace_bytes(batch, q_heads, kv_heads, head_dim, max_seq_len, page_size=16) -> int:

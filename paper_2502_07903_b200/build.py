@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libhx.so")
-SOURCES = ["hx_api.cu", "ingest.cu", "attention.cu", "hx_pool.cpp"]
+SOURCES = ["hx_api.cu", "ingest.cu", "attention.cu", "prefill.cu", "hx_pool.cpp"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
     "-Xcompiler", "-fPIC,-Wall,-Wno-unused-function", "-cudart", "static", "--expt-relaxed-constexpr",

@@ -264,6 +264,41 @@ int hx_kv_append(const void* k_new, const void* v_new, const hx_paged_cache* cac
   return launch_append(p, static_cast<cudaStream_t>(stream));
 }
 
+int hx_prefill_attention(void* out, const void* q, const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
+                         const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
+                         const int32_t* q_lens, const int32_t* cu_q_lens, int32_t batch, int32_t total_q_tokens,
+                         int32_t max_q_len, int32_t max_seq_len, float sm_scale, void* stream) {
+  using namespace hx;
+  const char* who = "hx_prefill_attention";
+  clear_error();
+  if (batch < 0 || total_q_tokens < 0 || max_q_len < 0 || max_seq_len < 0)
+    HX_FAIL(HX_ERR_INVALID_ARG, "%s: negative size (batch=%d total_q_tokens=%d max_q_len=%d max_seq_len=%d)", who, batch, total_q_tokens, max_q_len, max_seq_len);
+  int rc = check_cache(cache, who);
+  if (rc) return rc;
+  if (cache->head_dim != 128) HX_FAIL(HX_ERR_UNSUPPORTED, "%s: head_dim %d != 128", who, cache->head_dim);
+  if (layer < 0 || layer >= cache->layers) HX_FAIL(HX_ERR_INVALID_ARG, "%s: layer %d not in [0,%d)", who, layer, cache->layers);
+  if (q_heads <= 0 || q_heads % cache->kv_heads) HX_FAIL(HX_ERR_INVALID_ARG, "%s: q_heads %d not a positive multiple of kv_heads %d", who, q_heads, cache->kv_heads);
+  const int G = q_heads / cache->kv_heads;
+  if (G != 1 && G != 2 && G != 4 && G != 8 && G != 16) HX_FAIL(HX_ERR_UNSUPPORTED, "%s: group size %d not in {1,2,4,8,16}", who, G);
+  if (!(sm_scale == sm_scale) || sm_scale > 1e30f) HX_FAIL(HX_ERR_INVALID_ARG, "%s: sm_scale is NaN or too large", who);
+  if (max_q_len > max_seq_len || max_q_len > total_q_tokens) HX_FAIL(HX_ERR_INVALID_ARG, "%s: max_q_len %d > max_seq_len %d or total_q_tokens %d", who, max_q_len, max_seq_len, total_q_tokens);
+  if (batch == 0 || total_q_tokens == 0 || max_q_len == 0) return HX_OK;
+  if (!out || !q) HX_FAIL(HX_ERR_INVALID_ARG, "%s: out/q is NULL", who);
+  if (!aligned16(out) || !aligned16(q)) HX_FAIL(HX_ERR_INVALID_ARG, "%s: out/q must be 16-byte aligned", who);
+  if (!block_table || !seq_lens || !q_lens || !cu_q_lens) HX_FAIL(HX_ERR_INVALID_ARG, "%s: block_table/seq_lens/q_lens/cu_q_lens is NULL", who);
+  if ((int64_t)block_table_stride * cache->page_size < (int64_t)max_seq_len)
+    HX_FAIL(HX_ERR_INVALID_ARG, "%s: block_table_stride %d < ceil(max_seq_len %d / %d)", who, block_table_stride, max_seq_len, cache->page_size);
+  if (sm_scale <= 0.f) sm_scale = 1.0f / sqrtf((float)cache->head_dim);
+  PrefillArgs a;
+  memset(&a, 0, sizeof(a));
+  a.out = out; a.q = q; a.k_base = cache->k; a.v_base = cache->v;
+  a.block_table = block_table; a.seq_lens = seq_lens; a.q_lens = q_lens; a.cu_q_lens = cu_q_lens;
+  a.batch = batch; a.q_heads = q_heads; a.kv_heads = cache->kv_heads; a.head_dim = cache->head_dim;
+  a.num_pages = cache->num_pages; a.bt_stride = block_table_stride; a.layer = layer; a.layers = cache->layers;
+  a.total_q = total_q_tokens; a.max_q_len = max_q_len; a.sm_scale = sm_scale;
+  return launch_prefill(a, static_cast<cudaStream_t>(stream));
+}
+
 int hx_tune_sm_rates(const void* scratch, size_t scratch_bytes, void* stream) {
   using namespace hx;
   clear_error();

@@ -71,6 +71,21 @@ size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, in
 int launch_attention(const AttnParams& p, cudaStream_t stream);
 int tune_sm_rates(const void* scratch, size_t bytes, cudaStream_t stream);
 
+struct PrefillArgs {
+  void* out;
+  const void* q;
+  const void* k_base;             // whole cache (all layers)
+  const void* v_base;
+  const int32_t* block_table;
+  const int32_t* seq_lens;
+  const int32_t* q_lens;
+  const int32_t* cu_q_lens;
+  int32_t batch, q_heads, kv_heads, head_dim, num_pages, bt_stride, layer, layers;
+  int32_t total_q, max_q_len;
+  float sm_scale;
+};
+int launch_prefill(const PrefillArgs& a, cudaStream_t stream);
+
 struct AppendParams {
   const void* k_new;
   const void* v_new;

@@ -1,0 +1,404 @@
+// hx_prefill_attention — causal, paged, multi-token attention on the 5th-generation tensor cores
+// ("the prefill phase processes the request's input tokens all at
+// once" and is compute-bound, PAPER.md:L110 integrates FlashAttention for it and gives no kernel:
+// the design below is ours, for sm_100a).
+//
+// Roofline: tensor.  Algorithmic flops = 4 * D per (query row, visible kv token) pair (QK^T and PV),
+// causal pairs only.  Unlike the decode path this IS a dense contraction: 128 query rows share every
+// K/V tile, so it runs on tcgen05.mma with accumulators in TMEM.
+//
+// One CTA = one (request, kv head, tile of 128 query rows); a row is a (token, head-of-the-group)
+// pair, so a GQA group of G heads packs 128/G tokens x G heads into one M = 128 tile and the K/V tile
+// is read once for all of them.  Per 128-token KV tile (8 pages):
+//   TMA     K, V pages -> shared [D/64 halves][128 tokens][128 B], 128-byte swizzle (two tiles in flight)
+//   UMMA 1  S[128 x 128] = Q K^T           (8 x tcgen05.mma M128 N128 K16, f16 in / f32 in TMEM cols 0..127)
+//   softmax tcgen05.ld S (thread = row), causal + length mask, online max/sum in fp32, P -> fp16 ->
+//           shared in the K-major swizzled layout UMMA reads
+//   UMMA 2  O_tile[128 x D] = P V          (V is the MN-major B operand straight from the page layout;
+//           TMEM cols 128..255)
+//   update  tcgen05.ld O_tile, o_acc = o_acc * corr + O_tile in registers (128 fp32 per thread)
+// Epilogue: o_acc / l -> fp16 -> out.  This first version is synchronous per tile (MMA and softmax do
+// not overlap); the measured fraction of the tensor peak is reported by bench.py as it stands.
+#include <cuda.h>
+#include <cuda_fp16.h>
+
+#include <cstring>
+#include <mutex>
+
+#include "hx_internal.h"
+
+namespace hx {
+namespace {
+
+constexpr int kD = 128;                  // head_dim (this version)
+constexpr int kRows = 128;               // query rows per CTA (UMMA M)
+constexpr int kKvTile = 128;             // kv tokens per tile (UMMA N of S, K of PV)
+constexpr int kHalfBytes = kRows * 128;  // one [128 rows][128 B] swizzled region (64 fp16 wide)
+constexpr int kOperandBytes = 2 * kHalfBytes;   // a 128 x 128 fp16 operand
+constexpr int kSmem = 6 * kOperandBytes + 1024 /* alignment slack */ + 64;
+constexpr float kLog2e = 1.4426950408889634f;
+
+struct PrefillParams {
+  __half* out;
+  const int32_t* bt;
+  const int32_t* lens;
+  const int32_t* qlens;
+  const int32_t* cuq;
+  int32_t B, Hq, Hkv, G, bt_stride;
+  uint32_t layer_row0;
+  float scale_log2;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ void tma_3d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+      ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tma_4d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2, int c3, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+      ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar) : "memory");
+}
+__device__ __forceinline__ float ex2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+// ---- tcgen05 wrappers
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void umma_f16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// 32 consecutive fp32 columns of this thread's TMEM lane
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {
+  uint32_t r[32];
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr));
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+  for (int e = 0; e < 32; ++e) v[e] = __uint_as_float(r[e]);
+}
+
+// Shared-memory matrix descriptor (cute::UMMA::SmemDescriptor bit layout): start address >> 4 in
+// [0,14), leading byte offset >> 4 in [16,30), stride byte offset >> 4 in [32,46), version 1 in
+// [46,48), layout type in [61,64) (2 = 128-byte swizzle).
+__device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  return (uint64_t)((addr >> 4) & 0x3fff) | ((uint64_t)((lbo_bytes >> 4) & 0x3fff) << 16) |
+         ((uint64_t)((sbo_bytes >> 4) & 0x3fff) << 32) | (1ull << 46) | (2ull << 61);
+}
+// Instruction descriptor (cute::UMMA::InstrDescriptor): c_format f32 (1 << 4), a/b format f16 (0),
+// a_major bit 15, b_major bit 16 (1 = MN-major), N >> 3 in [17,23), M >> 4 in [24,29).
+constexpr uint32_t kIdescS = (1u << 4) | ((uint32_t)(kKvTile >> 3) << 17) | ((uint32_t)(kRows >> 4) << 24);
+constexpr uint32_t kIdescPV = (1u << 4) | (1u << 16) | ((uint32_t)(kD >> 3) << 17) | ((uint32_t)(kRows >> 4) << 24);
+
+__global__ void __launch_bounds__(128, 1)
+prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
+               const __grid_constant__ CUtensorMap tmV, const PrefillParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  uint8_t* sQ = smem;
+  uint8_t* sK = smem + kOperandBytes;          // [2 buffers]
+  uint8_t* sV = smem + 3 * kOperandBytes;      // [2 buffers]
+  uint8_t* sP = smem + 5 * kOperandBytes;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + 6 * kOperandBytes);   // q, kv[2], mma
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 4);
+
+  const int tid = threadIdx.x, warp = tid >> 5;
+  const int G = p.G, Hkv = p.Hkv;
+  const int TQ = kRows / G;                          // query tokens per tile
+  const int i = blockIdx.z, g = blockIdx.y;
+  const int n = __ldg(p.lens + i), m = __ldg(p.qlens + i);
+  const int qt = (int)gridDim.x - 1 - (int)blockIdx.x;   // heavy (late) tiles first
+  if (qt * TQ >= m) return;
+  const int r0 = qt * TQ;                            // first query token of the tile (within the request's m)
+  const int row_tok0 = __ldg(p.cuq + i) + r0;        // its packed row in q / out
+  const int pos0 = n - m + r0;                       // its position in the context
+  const int pos_last = min(pos0 + TQ - 1, n - 1);
+  const int nkv = pos_last / kKvTile + 1;            // causal: kv tiles 0..nkv-1
+  const int np = (n + 15) >> 4;
+
+  const uint32_t bar_q = smem_u32(bars), bar_kv0 = smem_u32(bars + 1), bar_mma = smem_u32(bars + 3);
+  if (tid == 0) {
+    mbar_init(bar_q, 1); mbar_init(bar_kv0, 1); mbar_init(bar_kv0 + 8, 1); mbar_init(bar_mma, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&tmQ) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&tmK) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&tmV) : "memory");
+  }
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 256;" ::"r"(smem_u32(tmem_slot)) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = *tmem_slot;
+  const uint32_t tS = tmem, tO = tmem + 128;
+  const uint32_t lane_sel = (uint32_t)(warp * 32) << 16;   // this warp's TMEM lanes
+
+  // ---- loads: Q once; K/V tile j into buffer j & 1 (pages past the context end are not loaded)
+  auto issue_kv = [&](int j) {
+    const int buf = j & 1;
+    const uint32_t bar = bar_kv0 + 8 * buf;
+    const int pg0 = j * (kKvTile / 16);
+    const int npg = min(kKvTile / 16, np - pg0);
+    mbar_expect_tx(bar, (uint32_t)(npg * 2 * 16 * kD * 2));
+    for (int pp = 0; pp < npg; ++pp) {
+      const int page = __ldg(p.bt + (size_t)i * p.bt_stride + pg0 + pp);
+      const int row = (int)(p.layer_row0 + (uint32_t)page * (uint32_t)(Hkv * 16) + (uint32_t)(g * 16));
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        tma_3d(smem_u32(sK + buf * kOperandBytes + h * kHalfBytes + pp * 2048), &tmK, 0, row, h, bar);
+        tma_3d(smem_u32(sV + buf * kOperandBytes + h * kHalfBytes + pp * 2048), &tmV, 0, row, h, bar);
+      }
+    }
+  };
+  if (tid == 0) {
+    mbar_expect_tx(bar_q, kOperandBytes);
+    tma_4d(smem_u32(sQ), &tmQ, 0, g * G, row_tok0, 0, bar_q);
+    tma_4d(smem_u32(sQ + kHalfBytes), &tmQ, 0, g * G, row_tok0, 1, bar_q);
+    issue_kv(0);
+    if (nkv > 1) issue_kv(1);
+  }
+
+  // ---- per-row state: thread tid owns row tid = (token r0 + tid / G, head g*G + tid % G)
+  const int my_pos = min(pos0 + tid / G, n - 1);     // rows past the request's last query are never stored
+  float m_run = -INFINITY, l_run = 0.f;
+  float o_acc[kD];
+#pragma unroll
+  for (int e = 0; e < kD; ++e) o_acc[e] = 0.f;
+  uint32_t mma_phase = 0;
+
+  for (int j = 0; j < nkv; ++j) {
+    const int buf = j & 1;
+    const uint32_t kb = smem_u32(sK + buf * kOperandBytes), vb = smem_u32(sV + buf * kOperandBytes);
+    // ---- wait for the tile; clear what the MMA must not see (0 * Inf = NaN in P V): V rows of slots
+    // past the context end and of pages that were not loaded (readings S10)
+    if (j == 0) mbar_wait(bar_q, 0);
+    mbar_wait(bar_kv0 + 8 * buf, (uint32_t)(j >> 1) & 1);
+    const int t0 = j * kKvTile;
+    if (t0 + kKvTile > n) {
+      for (int e = tid; e < (t0 + kKvTile - n) * 16; e += 128) {
+        const int r = (n - t0) + e / 16, ch = e % 16;
+        *reinterpret_cast<int4*>(sV + buf * kOperandBytes + (ch >> 3) * kHalfBytes + r * 128 + (((ch & 7) ^ (r & 7)) << 4)) =
+            make_int4(0, 0, 0, 0);
+      }
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    // ---- UMMA 1: S = Q K^T
+    if (tid == 0) {
+      tc_fence_after();
+#pragma unroll
+      for (int ks = 0; ks < kD / 16; ++ks) {
+        const uint32_t off = (uint32_t)(ks >> 2) * kHalfBytes + (uint32_t)(ks & 3) * 32;
+        umma_f16(tS, smem_desc(smem_u32(sQ) + off, 16, 1024), smem_desc(kb + off, 16, 1024), kIdescS, ks > 0);
+      }
+      umma_commit(bar_mma);
+    }
+    mbar_wait(bar_mma, mma_phase);
+    mma_phase ^= 1;
+    tc_fence_after();
+
+    // ---- softmax on row tid: pass 1 row max, pass 2 weights -> P (fp16, shared) and row sum
+    const bool need_mask = (t0 + kKvTile - 1 > pos0);          // some (row, token) of this tile is masked
+    float mx = -INFINITY;
+#pragma unroll 1
+    for (int c = 0; c < 4; ++c) {
+      float s[32];
+      tmem_ld32(tS + lane_sel + c * 32, s);
+#pragma unroll
+      for (int e = 0; e < 32; ++e) {
+        const float x = (!need_mask || t0 + c * 32 + e <= my_pos) ? s[e] * p.scale_log2 : -INFINITY;
+        mx = fmaxf(mx, x);
+      }
+    }
+    const float m_new = fmaxf(m_run, mx);                       // finite from tile 0 on (token 0 is visible)
+    const float corr = ex2(m_run - m_new);
+    m_run = m_new;
+    float rsum = 0.f;
+#pragma unroll 1
+    for (int c = 0; c < 4; ++c) {
+      float s[32];
+      tmem_ld32(tS + lane_sel + c * 32, s);
+      uint32_t pk[16];
+#pragma unroll
+      for (int e = 0; e < 32; e += 2) {
+        const float x0 = (!need_mask || t0 + c * 32 + e <= my_pos) ? s[e] * p.scale_log2 : -INFINITY;
+        const float x1 = (!need_mask || t0 + c * 32 + e + 1 <= my_pos) ? s[e + 1] * p.scale_log2 : -INFINITY;
+        const __half2 h2 = __floats2half2_rn(ex2(x0 - m_new), ex2(x1 - m_new));
+        rsum += __low2float(h2) + __high2float(h2);             // the ROUNDED weights (reading S22)
+        pk[e >> 1] = *reinterpret_cast<const uint32_t*>(&h2);
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {                             // 4 x 16-byte chunks = 32 tokens of this row
+        const int ch = c * 4 + u;                               // chunk index along the 128 kv tokens
+        *reinterpret_cast<int4*>(sP + (ch >> 3) * kHalfBytes + tid * 128 + (((ch & 7) ^ (tid & 7)) << 4)) =
+            make_int4((int)pk[4 * u], (int)pk[4 * u + 1], (int)pk[4 * u + 2], (int)pk[4 * u + 3]);
+      }
+    }
+    l_run = l_run * corr + rsum;
+#pragma unroll
+    for (int e = 0; e < kD; ++e) o_acc[e] *= corr;
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    tc_fence_before();
+    __syncthreads();
+    // ---- UMMA 2: O_tile = P V  (V: MN-major B, 64-wide N blocks 16 KiB apart, 8-token groups 1 KiB apart)
+    if (tid == 0) {
+      tc_fence_after();
+#pragma unroll
+      for (int ks = 0; ks < kKvTile / 16; ++ks) {
+        const uint32_t aoff = (uint32_t)(ks >> 2) * kHalfBytes + (uint32_t)(ks & 3) * 32;
+        umma_f16(tO, smem_desc(smem_u32(sP) + aoff, 16, 1024), smem_desc(vb + (uint32_t)ks * 2048, kHalfBytes, 1024),
+                 kIdescPV, ks > 0);
+      }
+      umma_commit(bar_mma);
+    }
+    mbar_wait(bar_mma, mma_phase);
+    mma_phase ^= 1;
+    tc_fence_after();
+    // both MMAs of this tile are done: its K/V buffer is free for tile j + 2
+    if (tid == 0 && j + 2 < nkv) issue_kv(j + 2);
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      float v[32];
+      tmem_ld32(tO + lane_sel + c * 32, v);
+#pragma unroll
+      for (int e = 0; e < 32; ++e) o_acc[c * 32 + e] += v[e];
+    }
+  }
+
+  // ---- epilogue: row tid -> out[row_tok0 + tid / G][g*G + tid % G][:]
+  if (r0 + tid / G < m) {
+    const float inv = 1.f / l_run;
+    __half* dst = p.out + ((size_t)(row_tok0 + tid / G) * p.Hq + (size_t)(g * G + tid % G)) * kD;
+#pragma unroll
+    for (int e = 0; e < kD; e += 8) {
+      __half2 h[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) h[u] = __floats2half2_rn(o_acc[e + 2 * u] * inv, o_acc[e + 2 * u + 1] * inv);
+      *reinterpret_cast<int4*>(dst + e) = *reinterpret_cast<const int4*>(h);
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 256;" ::"r"(tmem) : "memory");
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int encode_fn(EncodeTiledFn* out) {
+  static EncodeTiledFn fn = nullptr;
+  static std::mutex mu;
+  std::lock_guard<std::mutex> lock(mu);
+  if (!fn) {
+    void* ptr = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    HX_CUDA_OK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres));
+    if (qres != cudaDriverEntryPointSuccess || !ptr) HX_FAIL(HX_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
+    fn = reinterpret_cast<EncodeTiledFn>(ptr);
+  }
+  *out = fn;
+  return HX_OK;
+}
+
+}  // namespace
+
+int launch_prefill(const PrefillArgs& a, cudaStream_t stream) {
+  DeviceInfo di;
+  int rc = device_info(&di);
+  if (rc) return rc;
+  static bool attr_set[64] = {false};
+  if (!attr_set[di.device]) {
+    if (kSmem > di.max_smem_optin) HX_FAIL(HX_ERR_UNSUPPORTED, "device offers %d B shared memory per CTA, kernel needs %d", di.max_smem_optin, kSmem);
+    HX_CUDA_OK(cudaFuncSetAttribute(prefill_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem));
+    attr_set[di.device] = true;
+  }
+  EncodeTiledFn enc;
+  rc = encode_fn(&enc);
+  if (rc) return rc;
+  const int G = a.q_heads / a.kv_heads;
+  const uint64_t rows_per_layer = (uint64_t)a.num_pages * a.kv_heads * 16;
+  const uint64_t rows = rows_per_layer * a.layers;
+  if (rows >= (1ull << 31)) HX_FAIL(HX_ERR_UNSUPPORTED, "cache too large for one tensor map (%llu rows)", (unsigned long long)rows);
+  CUtensorMap tq, tk, tv;
+  {
+    // K / V cache as [D/64 halves][rows][64]; box = one 64-wide half of one (page, head) tile
+    cuuint64_t dims[3] = {64, rows, (cuuint64_t)(kD / 64)};
+    cuuint64_t strides[2] = {(cuuint64_t)kD * 2, 128};
+    cuuint32_t box[3] = {64, 16, 1};
+    cuuint32_t es[3] = {1, 1, 1};
+    for (int x = 0; x < 2; ++x) {
+      CUresult r = enc(x ? &tv : &tk, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, const_cast<void*>(x ? a.v_base : a.k_base), dims,
+                       strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                       CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      if (r != CUDA_SUCCESS) HX_FAIL(HX_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d) for the K/V cache", (int)r);
+    }
+  }
+  {
+    // Q as [64][Hq heads][Tq tokens][D/64 halves]; box {64, G, 128/G, 1} lands as [token][head][128 B]:
+    // row = token * G + head, the M order of the tile.  Tokens past the end read as zeros.
+    cuuint64_t dims[4] = {64, (cuuint64_t)a.q_heads, (cuuint64_t)a.total_q, (cuuint64_t)(kD / 64)};
+    cuuint64_t strides[3] = {(cuuint64_t)kD * 2, (cuuint64_t)a.q_heads * kD * 2, 128};
+    cuuint32_t box[4] = {64, (cuuint32_t)G, (cuuint32_t)(kRows / G), 1};
+    cuuint32_t es[4] = {1, 1, 1, 1};
+    CUresult r = enc(&tq, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 4, const_cast<void*>(a.q), dims, strides, box, es,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) HX_FAIL(HX_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d) for q", (int)r);
+  }
+  PrefillParams p;
+  p.out = static_cast<__half*>(a.out);
+  p.bt = a.block_table; p.lens = a.seq_lens; p.qlens = a.q_lens; p.cuq = a.cu_q_lens;
+  p.B = a.batch; p.Hq = a.q_heads; p.Hkv = a.kv_heads; p.G = G; p.bt_stride = a.bt_stride;
+  p.layer_row0 = (uint32_t)(rows_per_layer * a.layer);
+  p.scale_log2 = a.sm_scale * kLog2e;
+  const int TQ = kRows / G;
+  const int qtiles = (a.max_q_len + TQ - 1) / TQ;
+  for (int b0 = 0; b0 < a.batch; b0 += 65535) {
+    PrefillParams pb = p;
+    pb.B = (a.batch - b0 < 65535) ? a.batch - b0 : 65535;
+    pb.bt = a.block_table + (size_t)b0 * a.bt_stride;
+    pb.lens = a.seq_lens + b0; pb.qlens = a.q_lens + b0; pb.cuq = a.cu_q_lens + b0;
+    prefill_kernel<<<dim3(qtiles, a.kv_heads, pb.B), 128, kSmem, stream>>>(tq, tk, tv, pb);
+    HX_CUDA_OK(cudaGetLastError());
+  }
+  return HX_OK;
+}
+
+}  // namespace hx

@@ -1,0 +1,92 @@
+"""GPU parity for hx_prefill_attention: the tcgen05 kernel against the float64
+oracle (causal paged attention of the last q_lens[i] tokens), north_star tolerances."""
+import numpy as np
+import pytest
+
+import workloads as W
+from helpers import MAX_ABS_TOL, REL_L2_TOL, attn_errors, to_dev
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device (no CPU fallback exists)")
+    import paper_2502_07903_b200 as hx
+    import oracle
+    oracle.build()
+    return hx, torch, oracle
+
+
+def run_prefill(env, cfgno, Hq, Hkv, lens, qlens, layers=1, layer=0, poison=False, sm_scale=0.0):
+    hx, torch, oracle = env
+    lens = np.asarray(lens, dtype=np.int32)
+    qlens = np.asarray(qlens, dtype=np.int32)
+    c = W.AttnConfig(cfgno, "t", len(lens), Hq, Hkv, 128, 8, "x")
+    w = W.make_attention_inputs(c, lens=lens, layers=layers)
+    Tq = int(qlens.sum())
+    q = W.draw_fp16_normal((Tq, Hq, 128), cfgno, 40)
+    k, v = w["k"], w["v"]
+    if poison:                                   # slots past the context end and unowned pages: NaN / Inf
+        kb, vb = k.view(np.uint16).copy(), v.view(np.uint16).copy()
+        owned = np.zeros((w["num_pages"], 16), dtype=bool)
+        for i, n in enumerate(lens):
+            t = np.arange(n)
+            owned[w["block_table"][i, t // 16], t % 16] = True
+        kb[:].transpose(0, 1, 3, 2, 4)[:, ~owned] = 0x7E00
+        vb[:].transpose(0, 1, 3, 2, 4)[:, ~owned] = 0x7C00
+        k, v = kb.view(np.float16), vb.view(np.float16)
+    ref = oracle.prefill_attention(q, k, v, w["block_table"], lens, qlens, layer=layer,
+                                   sm_scale=sm_scale if sm_scale > 0 else None)
+    cache = hx.PagedCache(to_dev(k, torch), to_dev(v, torch))
+    cu = np.zeros(len(lens) + 1, dtype=np.int32)
+    np.cumsum(qlens, out=cu[1:])
+    qd = to_dev(q, torch)
+    out = torch.full_like(qd, float("nan"))
+    bt = torch.from_numpy(w["block_table"]).cuda()
+    hx.prefill_attention(out, qd, cache, layer=layer, q_heads=Hq, block_table=bt, block_table_stride=bt.shape[1],
+                         seq_lens=torch.from_numpy(lens).cuda(), q_lens=torch.from_numpy(qlens).cuda(),
+                         cu_q_lens=torch.from_numpy(cu).cuda(), batch=len(lens), total_q_tokens=Tq,
+                         max_q_len=int(qlens.max(initial=0)), max_seq_len=int(lens.max(initial=0)), sm_scale=sm_scale)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    assert np.isfinite(got.astype(np.float32)).all()
+    max_abs, rel = attn_errors(got, ref)
+    assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (max_abs, rel)
+    return got, ref
+
+
+@pytest.mark.parametrize("G,Hkv", [(8, 1), (1, 2), (4, 2), (16, 1), (2, 1)])
+def test_prefill_whole_prompts_page_and_tile_boundaries(env, G, Hkv):
+    lens = [1, 15, 16, 17, 127, 128, 129, 255, 257, 300]
+    run_prefill(env, 60 + G, G * Hkv, Hkv, lens, lens)
+
+
+def test_prefill_llama70b_shape_long_prompt(env):
+    run_prefill(env, 70, 16, 2, [1000, 700], [1000, 700])          # G = 8, several kv tiles per q tile
+
+
+def test_prefill_chunked_and_decode_like_and_empty(env):
+    lens = [300, 64, 200, 17, 129]
+    qlens = [44, 1, 200, 0, 128]
+    run_prefill(env, 71, 8, 1, lens, qlens)
+
+
+def test_prefill_layer_and_scale_and_poison(env):
+    run_prefill(env, 72, 8, 1, [100, 260, 31], [100, 260, 31], layers=3, layer=2, sm_scale=0.05)
+    run_prefill(env, 73, 8, 1, [100, 260, 31, 130], [100, 60, 31, 130], poison=True)
+
+
+def test_prefill_one_query_token_matches_decode_kernel(env):
+    """q_lens = 1: the tensor-memory kernel and the streaming decode kernel answer the same question."""
+    hx, torch, oracle = env
+    lens = np.array([1, 16, 100, 513, 129], dtype=np.int32)
+    got, ref = run_prefill(env, 74, 8, 1, lens, np.ones(5, dtype=np.int32))
+    ref_dec = None
+    c = W.AttnConfig(74, "t", 5, 8, 1, 128, 8, "x")
+    w = W.make_attention_inputs(c, lens=lens)
+    q = W.draw_fp16_normal((5, 8, 128), 74, 40)
+    ref_dec = oracle.decode_attention(q, w["k"], w["v"], w["block_table"], lens)
+    np.testing.assert_allclose(ref, ref_dec, atol=1e-13)
