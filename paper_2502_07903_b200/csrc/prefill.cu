@@ -9,16 +9,17 @@
 //
 // One CTA = one (request, kv head, tile of 128 query rows); a row is a (token, head-of-the-group)
 // pair, so a GQA group of G heads packs 128/G tokens x G heads into one M = 128 tile and the K/V tile
-// is read once for all of them.  Per 128-token KV tile (8 pages):
-//   TMA     K, V pages -> shared [D/64 halves][128 tokens][128 B], 128-byte swizzle (two tiles in flight)
-//   UMMA 1  S[128 x 128] = Q K^T           (8 x tcgen05.mma M128 N128 K16, f16 in / f32 in TMEM cols 0..127)
+// is read once for all of them.  Per 64-token KV tile (4 pages):
+//   TMA     K, V pages -> shared [D/64 halves][64 tokens][128 B], 128-byte swizzle (two tiles in flight)
+//   UMMA 1  S[128 x 64] = Q K^T            (8 x tcgen05.mma M128 N64 K16, f16 in / f32 in TMEM cols 0..63)
 //   softmax tcgen05.ld S (thread = row), causal + length mask, online max/sum in fp32, P -> fp16 ->
 //           shared in the K-major swizzled layout UMMA reads
 //   UMMA 2  O_tile[128 x D] = P V          (V is the MN-major B operand straight from the page layout;
 //           TMEM cols 128..255)
 //   update  tcgen05.ld O_tile, o_acc = o_acc * corr + O_tile in registers (128 fp32 per thread)
-// Epilogue: o_acc / l -> fp16 -> out.  This first version is synchronous per tile (MMA and softmax do
-// not overlap); the measured fraction of the tensor peak is reported by bench.py as it stands.
+// Epilogue: o_acc / l -> fp16 -> out.  Within a CTA the tile steps are synchronous; two CTAs share an
+// SM (112 KiB of shared memory and 256 TMEM columns each) so that one's MMAs run under the other's
+// softmax.  The measured fraction of the tensor peak is reported by bench.py as it stands.
 #include <cuda.h>
 #include <cuda_fp16.h>
 
@@ -32,10 +33,14 @@ namespace {
 
 constexpr int kD = 128;                  // head_dim (this version)
 constexpr int kRows = 128;               // query rows per CTA (UMMA M)
-constexpr int kKvTile = 128;             // kv tokens per tile (UMMA N of S, K of PV)
-constexpr int kHalfBytes = kRows * 128;  // one [128 rows][128 B] swizzled region (64 fp16 wide)
-constexpr int kOperandBytes = 2 * kHalfBytes;   // a 128 x 128 fp16 operand
-constexpr int kSmem = 6 * kOperandBytes + 1024 /* alignment slack */ + 64;
+constexpr int kKvTile = 64;              // kv tokens per tile (UMMA N of S, K of PV): 4 pages
+constexpr int kHalfBytes = kRows * 128;  // Q: one [128 rows][128 B] swizzled region (64 fp16 wide)
+constexpr int kQBytes = 2 * kHalfBytes;  // Q tile, 128 rows x 128 fp16
+constexpr int kKvHalfBytes = kKvTile * 128;      // K or V: one [64 tokens][128 B] region
+constexpr int kKvBytes = 2 * kKvHalfBytes;       // a K or V tile, 64 tokens x 128 fp16
+constexpr int kPBytes = kRows * kKvTile * 2;     // P tile, 128 rows x 64 fp16 = one swizzled region
+// Q + 2 x (K + V) + P + barriers = 112 KiB + 64 B: two CTAs per SM (their MMA and softmax phases overlap)
+constexpr int kSmem = kQBytes + 4 * kKvBytes + kPBytes + 64;
 constexpr float kLog2e = 1.4426950408889634f;
 
 struct PrefillParams {
@@ -123,16 +128,16 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo_bytes,
 constexpr uint32_t kIdescS = (1u << 4) | ((uint32_t)(kKvTile >> 3) << 17) | ((uint32_t)(kRows >> 4) << 24);
 constexpr uint32_t kIdescPV = (1u << 4) | (1u << 16) | ((uint32_t)(kD >> 3) << 17) | ((uint32_t)(kRows >> 4) << 24);
 
-__global__ void __launch_bounds__(128, 1)
+__global__ void __launch_bounds__(128, 2)
 prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                const __grid_constant__ CUtensorMap tmV, const PrefillParams p) {
-  extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  extern __shared__ __align__(1024) uint8_t smem[];
+  if ((smem_u32(smem) & 1023u) != 0) __trap();   // the 128-byte swizzle needs 1 KiB-aligned regions
   uint8_t* sQ = smem;
-  uint8_t* sK = smem + kOperandBytes;          // [2 buffers]
-  uint8_t* sV = smem + 3 * kOperandBytes;      // [2 buffers]
-  uint8_t* sP = smem + 5 * kOperandBytes;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + 6 * kOperandBytes);   // q, kv[2], mma
+  uint8_t* sK = smem + kQBytes;                // [2 buffers]
+  uint8_t* sV = sK + 2 * kKvBytes;             // [2 buffers]
+  uint8_t* sP = sV + 2 * kKvBytes;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sP + kPBytes);   // q, kv[2], mma
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 4);
 
   const int tid = threadIdx.x, warp = tid >> 5;
@@ -180,13 +185,13 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       const int row = (int)(p.layer_row0 + (uint32_t)page * (uint32_t)(Hkv * 16) + (uint32_t)(g * 16));
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
-        tma_3d(smem_u32(sK + buf * kOperandBytes + h * kHalfBytes + pp * 2048), &tmK, 0, row, h, bar);
-        tma_3d(smem_u32(sV + buf * kOperandBytes + h * kHalfBytes + pp * 2048), &tmV, 0, row, h, bar);
+        tma_3d(smem_u32(sK + buf * kKvBytes + h * kKvHalfBytes + pp * 2048), &tmK, 0, row, h, bar);
+        tma_3d(smem_u32(sV + buf * kKvBytes + h * kKvHalfBytes + pp * 2048), &tmV, 0, row, h, bar);
       }
     }
   };
   if (tid == 0) {
-    mbar_expect_tx(bar_q, kOperandBytes);
+    mbar_expect_tx(bar_q, kQBytes);
     tma_4d(smem_u32(sQ), &tmQ, 0, g * G, row_tok0, 0, bar_q);
     tma_4d(smem_u32(sQ + kHalfBytes), &tmQ, 0, g * G, row_tok0, 1, bar_q);
     issue_kv(0);
@@ -203,7 +208,7 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
 
   for (int j = 0; j < nkv; ++j) {
     const int buf = j & 1;
-    const uint32_t kb = smem_u32(sK + buf * kOperandBytes), vb = smem_u32(sV + buf * kOperandBytes);
+    const uint32_t kb = smem_u32(sK + buf * kKvBytes), vb = smem_u32(sV + buf * kKvBytes);
     // ---- wait for the tile; clear what the MMA must not see (0 * Inf = NaN in P V): V rows of slots
     // past the context end and of pages that were not loaded (readings S10)
     if (j == 0) mbar_wait(bar_q, 0);
@@ -212,7 +217,7 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     if (t0 + kKvTile > n) {
       for (int e = tid; e < (t0 + kKvTile - n) * 16; e += 128) {
         const int r = (n - t0) + e / 16, ch = e % 16;
-        *reinterpret_cast<int4*>(sV + buf * kOperandBytes + (ch >> 3) * kHalfBytes + r * 128 + (((ch & 7) ^ (r & 7)) << 4)) =
+        *reinterpret_cast<int4*>(sV + buf * kKvBytes + (ch >> 3) * kKvHalfBytes + r * 128 + (((ch & 7) ^ (r & 7)) << 4)) =
             make_int4(0, 0, 0, 0);
       }
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -224,8 +229,9 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       tc_fence_after();
 #pragma unroll
       for (int ks = 0; ks < kD / 16; ++ks) {
-        const uint32_t off = (uint32_t)(ks >> 2) * kHalfBytes + (uint32_t)(ks & 3) * 32;
-        umma_f16(tS, smem_desc(smem_u32(sQ) + off, 16, 1024), smem_desc(kb + off, 16, 1024), kIdescS, ks > 0);
+        const uint32_t koff = (uint32_t)(ks & 3) * 32;
+        umma_f16(tS, smem_desc(smem_u32(sQ) + (uint32_t)(ks >> 2) * kHalfBytes + koff, 16, 1024),
+                 smem_desc(kb + (uint32_t)(ks >> 2) * kKvHalfBytes + koff, 16, 1024), kIdescS, ks > 0);
       }
       umma_commit(bar_mma);
     }
@@ -233,57 +239,64 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     mma_phase ^= 1;
     tc_fence_after();
 
-    // ---- softmax on row tid: pass 1 row max, pass 2 weights -> P (fp16, shared) and row sum
+    // ---- softmax on row tid: pass 1 row max (raw scores: the scale is positive), pass 2 weights ->
+    // P (fp16, shared) and row sum.  Only the diagonal / last tiles pay for the mask.
     const bool need_mask = (t0 + kKvTile - 1 > pos0);          // some (row, token) of this tile is masked
     float mx = -INFINITY;
 #pragma unroll 1
-    for (int c = 0; c < 4; ++c) {
+    for (int c = 0; c < kKvTile / 32; ++c) {
       float s[32];
       tmem_ld32(tS + lane_sel + c * 32, s);
+      if (need_mask) {
 #pragma unroll
-      for (int e = 0; e < 32; ++e) {
-        const float x = (!need_mask || t0 + c * 32 + e <= my_pos) ? s[e] * p.scale_log2 : -INFINITY;
-        mx = fmaxf(mx, x);
+        for (int e = 0; e < 32; ++e) mx = fmaxf(mx, (t0 + c * 32 + e <= my_pos) ? s[e] : -INFINITY);
+      } else {
+#pragma unroll
+        for (int e = 0; e < 32; ++e) mx = fmaxf(mx, s[e]);
       }
     }
-    const float m_new = fmaxf(m_run, mx);                       // finite from tile 0 on (token 0 is visible)
+    const float m_new = fmaxf(m_run, mx * p.scale_log2);        // finite from tile 0 on (token 0 is visible)
     const float corr = ex2(m_run - m_new);
     m_run = m_new;
     float rsum = 0.f;
 #pragma unroll 1
-    for (int c = 0; c < 4; ++c) {
+    for (int c = 0; c < kKvTile / 32; ++c) {
       float s[32];
       tmem_ld32(tS + lane_sel + c * 32, s);
       uint32_t pk[16];
 #pragma unroll
       for (int e = 0; e < 32; e += 2) {
-        const float x0 = (!need_mask || t0 + c * 32 + e <= my_pos) ? s[e] * p.scale_log2 : -INFINITY;
-        const float x1 = (!need_mask || t0 + c * 32 + e + 1 <= my_pos) ? s[e + 1] * p.scale_log2 : -INFINITY;
-        const __half2 h2 = __floats2half2_rn(ex2(x0 - m_new), ex2(x1 - m_new));
+        float w0 = ex2(fmaf(s[e], p.scale_log2, -m_new)), w1 = ex2(fmaf(s[e + 1], p.scale_log2, -m_new));
+        if (need_mask) {
+          w0 = (t0 + c * 32 + e <= my_pos) ? w0 : 0.f;
+          w1 = (t0 + c * 32 + e + 1 <= my_pos) ? w1 : 0.f;
+        }
+        const __half2 h2 = __floats2half2_rn(w0, w1);
         rsum += __low2float(h2) + __high2float(h2);             // the ROUNDED weights (reading S22)
         pk[e >> 1] = *reinterpret_cast<const uint32_t*>(&h2);
       }
 #pragma unroll
       for (int u = 0; u < 4; ++u) {                             // 4 x 16-byte chunks = 32 tokens of this row
-        const int ch = c * 4 + u;                               // chunk index along the 128 kv tokens
-        *reinterpret_cast<int4*>(sP + (ch >> 3) * kHalfBytes + tid * 128 + (((ch & 7) ^ (tid & 7)) << 4)) =
+        const int ch = c * 4 + u;                               // chunk index along the tile's kv tokens (< 8)
+        *reinterpret_cast<int4*>(sP + tid * 128 + ((ch ^ (tid & 7)) << 4)) =
             make_int4((int)pk[4 * u], (int)pk[4 * u + 1], (int)pk[4 * u + 2], (int)pk[4 * u + 3]);
       }
     }
     l_run = l_run * corr + rsum;
+    if (__any_sync(0xffffffffu, corr != 1.f)) {
 #pragma unroll
-    for (int e = 0; e < kD; ++e) o_acc[e] *= corr;
+      for (int e = 0; e < kD; ++e) o_acc[e] *= corr;
+    }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     tc_fence_before();
     __syncthreads();
-    // ---- UMMA 2: O_tile = P V  (V: MN-major B, 64-wide N blocks 16 KiB apart, 8-token groups 1 KiB apart)
+    // ---- UMMA 2: O_tile = P V  (V: MN-major B, 64-wide N blocks 8 KiB apart, 8-token groups 1 KiB apart)
     if (tid == 0) {
       tc_fence_after();
 #pragma unroll
       for (int ks = 0; ks < kKvTile / 16; ++ks) {
-        const uint32_t aoff = (uint32_t)(ks >> 2) * kHalfBytes + (uint32_t)(ks & 3) * 32;
-        umma_f16(tO, smem_desc(smem_u32(sP) + aoff, 16, 1024), smem_desc(vb + (uint32_t)ks * 2048, kHalfBytes, 1024),
-                 kIdescPV, ks > 0);
+        umma_f16(tO, smem_desc(smem_u32(sP) + (uint32_t)ks * 32, 16, 1024),
+                 smem_desc(vb + (uint32_t)ks * 2048, kKvHalfBytes, 1024), kIdescPV, ks > 0);
       }
       umma_commit(bar_mma);
     }
