@@ -14,12 +14,13 @@
 //   UMMA 1  S[128 x 64] = Q K^T            (8 x tcgen05.mma M128 N64 K16, f16 in / f32 in TMEM cols 0..63)
 //   softmax tcgen05.ld S (thread = row), causal + length mask, online max/sum in fp32, P -> fp16 ->
 //           shared in the K-major swizzled layout UMMA reads
-//   UMMA 2  O_tile[128 x D] = P V          (V is the MN-major B operand straight from the page layout;
-//           TMEM cols 128..255)
-//   update  tcgen05.ld O_tile, o_acc = o_acc * corr + O_tile in registers (128 fp32 per thread)
-// Epilogue: o_acc / l -> fp16 -> out.  Within a CTA the tile steps are synchronous; two CTAs share an
-// SM (112 KiB of shared memory and 256 TMEM columns each) so that one's MMAs run under the other's
-// softmax.  The measured fraction of the tensor peak is reported by bench.py as it stands.
+//   UMMA 2  O[128 x D] += P V              (V is the MN-major B operand straight from the page layout;
+//           O stays in TMEM cols 128..255 for the whole CTA)
+//   rescale O and l only when a row max has moved by more than 2^8 since the scale was last set
+//           (tcgen05.ld / st; rare): the stale scale cancels in O / l.
+// Epilogue: tcgen05.ld O, O / l -> fp16 -> out.  S is double-buffered in TMEM, so the tensor pipe runs
+// S_{j+1} and P V_{j-1} under step j's softmax; two CTAs share an SM (112 KiB of shared memory and
+// 256 TMEM columns each).  The measured fraction of the tensor peak is reported by bench.py as it stands.
 #include <cuda.h>
 #include <cuda_fp16.h>
 
@@ -40,7 +41,7 @@ constexpr int kKvHalfBytes = kKvTile * 128;      // K or V: one [64 tokens][128 
 constexpr int kKvBytes = 2 * kKvHalfBytes;       // a K or V tile, 64 tokens x 128 fp16
 constexpr int kPBytes = kRows * kKvTile * 2;     // P tile, 128 rows x 64 fp16 = one swizzled region
 // Q + 2 x (K + V) + P + barriers = 112 KiB + 64 B: two CTAs per SM (their MMA and softmax phases overlap)
-constexpr int kSmem = kQBytes + 4 * kKvBytes + kPBytes + 64;
+constexpr int kSmem = kQBytes + 4 * kKvBytes + kPBytes + 80;   // 8 mbarriers + the TMEM address
 constexpr float kLog2e = 1.4426950408889634f;
 
 struct PrefillParams {
@@ -116,6 +117,34 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {
   for (int e = 0; e < 32; ++e) v[e] = __uint_as_float(r[e]);
 }
 
+__device__ __forceinline__ void tmem_ld32_issue(uint32_t taddr, uint32_t (&r)[32]) {   // no wait
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32]) {   // no wait
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+      "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
+      ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),
+        "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]),
+        "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]),
+        "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31]) : "memory");
+}
+__device__ __forceinline__ void tmem_ld64(uint32_t taddr, float (&v)[64]) {
+  uint32_t a[32], b[32];
+  tmem_ld32_issue(taddr, a);
+  tmem_ld32_issue(taddr + 32, b);
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+  for (int e = 0; e < 32; ++e) { v[e] = __uint_as_float(a[e]); v[32 + e] = __uint_as_float(b[e]); }
+}
+
 // Shared-memory matrix descriptor (cute::UMMA::SmemDescriptor bit layout): start address >> 4 in
 // [0,14), leading byte offset >> 4 in [16,30), stride byte offset >> 4 in [32,46), version 1 in
 // [46,48), layout type in [61,64) (2 = 128-byte swizzle).
@@ -137,8 +166,8 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   uint8_t* sK = smem + kQBytes;                // [2 buffers]
   uint8_t* sV = sK + 2 * kKvBytes;             // [2 buffers]
   uint8_t* sP = sV + 2 * kKvBytes;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(sP + kPBytes);   // q, kv[2], mma
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 4);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sP + kPBytes);   // q, k[2], v[2], s[2], o
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 8);
 
   const int tid = threadIdx.x, warp = tid >> 5;
   const int G = p.G, Hkv = p.Hkv;
@@ -154,9 +183,10 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   const int nkv = pos_last / kKvTile + 1;            // causal: kv tiles 0..nkv-1
   const int np = (n + 15) >> 4;
 
-  const uint32_t bar_q = smem_u32(bars), bar_kv0 = smem_u32(bars + 1), bar_mma = smem_u32(bars + 3);
+  const uint32_t bar_q = smem_u32(bars), bar_k0 = smem_u32(bars + 1), bar_v0 = smem_u32(bars + 3);
+  const uint32_t bar_s0 = smem_u32(bars + 5), bar_o = smem_u32(bars + 7);
   if (tid == 0) {
-    mbar_init(bar_q, 1); mbar_init(bar_kv0, 1); mbar_init(bar_kv0 + 8, 1); mbar_init(bar_mma, 1);
+    for (int e = 0; e < 8; ++e) mbar_init(bar_q + 8 * e, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tmQ) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tmK) : "memory");
@@ -170,160 +200,195 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = *tmem_slot;
-  const uint32_t tS = tmem, tO = tmem + 128;
+  const uint32_t tO = tmem + 128;                          // S_j lives at columns 64 * (j & 1)
   const uint32_t lane_sel = (uint32_t)(warp * 32) << 16;   // this warp's TMEM lanes
 
-  // ---- loads: Q once; K/V tile j into buffer j & 1 (pages past the context end are not loaded)
-  auto issue_kv = [&](int j) {
-    const int buf = j & 1;
-    const uint32_t bar = bar_kv0 + 8 * buf;
-    const int pg0 = j * (kKvTile / 16);
-    const int npg = min(kKvTile / 16, np - pg0);
-    mbar_expect_tx(bar, (uint32_t)(npg * 2 * 16 * kD * 2));
-    for (int pp = 0; pp < npg; ++pp) {
-      const int page = __ldg(p.bt + (size_t)i * p.bt_stride + pg0 + pp);
-      const int row = (int)(p.layer_row0 + (uint32_t)page * (uint32_t)(Hkv * 16) + (uint32_t)(g * 16));
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        tma_3d(smem_u32(sK + buf * kKvBytes + h * kKvHalfBytes + pp * 2048), &tmK, 0, row, h, bar);
-        tma_3d(smem_u32(sV + buf * kKvBytes + h * kKvHalfBytes + pp * 2048), &tmV, 0, row, h, bar);
-      }
-    }
+  // ---- loads: Q once; K tile t / V tile t into their buffers t & 1, each on its own barrier (pages
+  // past the context end are not loaded).  Warp 0 issues them: lane l < 4 owns page l of the tile and
+  // fetched its block-table entry a step earlier, so no global-load latency sits in the issue path.
+  const int lane = tid & 31;
+  auto load_page = [&](int t) -> int {
+    const int pg = t * (kKvTile / 16) + lane;
+    return (warp == 0 && lane < kKvTile / 16 && t < nkv && pg < np) ? __ldg(p.bt + (size_t)i * p.bt_stride + pg) : 0;
   };
-  if (tid == 0) {
-    mbar_expect_tx(bar_q, kQBytes);
-    tma_4d(smem_u32(sQ), &tmQ, 0, g * G, row_tok0, 0, bar_q);
-    tma_4d(smem_u32(sQ + kHalfBytes), &tmQ, 0, g * G, row_tok0, 1, bar_q);
-    issue_kv(0);
-    if (nkv > 1) issue_kv(1);
+  auto issue_tile = [&](int t, bool is_v, int page) {            // call from all of warp 0
+    const int buf = t & 1;
+    const uint32_t bar = (is_v ? bar_v0 : bar_k0) + 8 * buf;
+    const int npg = min(kKvTile / 16, np - t * (kKvTile / 16));
+    if (lane == 0) mbar_expect_tx(bar, (uint32_t)(npg * 16 * kD * 2));
+    if (lane < npg) {
+      uint8_t* dstb = (is_v ? sV : sK) + buf * kKvBytes + lane * 2048;
+      const int row = (int)(p.layer_row0 + (uint32_t)page * (uint32_t)(Hkv * 16) + (uint32_t)(g * 16));
+      tma_3d(smem_u32(dstb), is_v ? &tmV : &tmK, 0, row, 0, bar);
+      tma_3d(smem_u32(dstb + kKvHalfBytes), is_v ? &tmV : &tmK, 0, row, 1, bar);
+    }
+    __syncwarp();
+  };
+  // S_t = Q K_t^T into TMEM columns [64 * (t & 1), +64); completion -> bar_s[t & 1]  (one thread)
+  auto issue_s = [&](int t) {
+    const uint32_t kb = smem_u32(sK + (t & 1) * kKvBytes);
+    tc_fence_after();
+#pragma unroll
+    for (int ks = 0; ks < kD / 16; ++ks) {
+      const uint32_t koff = (uint32_t)(ks & 3) * 32;
+      umma_f16(tmem + 64 * (t & 1), smem_desc(smem_u32(sQ) + (uint32_t)(ks >> 2) * kHalfBytes + koff, 16, 1024),
+               smem_desc(kb + (uint32_t)(ks >> 2) * kKvHalfBytes + koff, 16, 1024), kIdescS, ks > 0);
+    }
+    umma_commit(bar_s0 + 8 * (t & 1));   // two barriers: S_{t+1} may finish before every thread has seen S_t
+  };
+  int pgA = 0, pgB = 0;                                          // warp 0: pages of tiles j + 2 and j + 1
+  if (warp == 0) {
+    const int pg0 = load_page(0);
+    pgB = load_page(1);
+    pgA = load_page(2);
+    if (lane == 0) {
+      mbar_expect_tx(bar_q, kQBytes);
+      tma_4d(smem_u32(sQ), &tmQ, 0, g * G, row_tok0, 0, bar_q);
+      tma_4d(smem_u32(sQ + kHalfBytes), &tmQ, 0, g * G, row_tok0, 1, bar_q);
+    }
+    issue_tile(0, false, pg0);
+    issue_tile(0, true, pg0);
+    if (nkv > 1) { issue_tile(1, false, pgB); issue_tile(1, true, pgB); }
+    if (lane == 0) {
+      mbar_wait(bar_q, 0);
+      mbar_wait(bar_k0, 0);
+      issue_s(0);
+    }
+    __syncwarp();
   }
 
-  // ---- per-row state: thread tid owns row tid = (token r0 + tid / G, head g*G + tid % G)
+  // ---- per-row state: thread tid owns row tid = (token r0 + tid / G, head g*G + tid % G).  The
+  // output accumulator O lives in TMEM (columns 128..255) across all tiles: P V_j accumulates into it.
+  // Its scale is m_used, a STALE row max that is moved (and O, l rescaled) only when the true max has
+  // run ahead of it by more than 2^8: the weights 2^(s - m_used) then stay <= 256, exact in fp16's
+  // relative precision, and the result is the same softmax average (the factor cancels in O / l).
   const int my_pos = min(pos0 + tid / G, n - 1);     // rows past the request's last query are never stored
-  float m_run = -INFINITY, l_run = 0.f;
-  float o_acc[kD];
-#pragma unroll
-  for (int e = 0; e < kD; ++e) o_acc[e] = 0.f;
-  uint32_t mma_phase = 0;
+  float m_used = -INFINITY, l_run = 0.f;
 
+  // Schedule of step j (the tensor pipe runs S_{j+1} and P V_{j-1} under this step's softmax):
+  //   wait S_j | free K buffer j&1 -> load K_{j+2} | issue S_{j+1} | row max of S_j | wait P V_{j-1},
+  //   load V_{j+1} | (rarely) rescale O | P_j -> shared | wait V_j | issue P V_j (accumulating)
   for (int j = 0; j < nkv; ++j) {
     const int buf = j & 1;
-    const uint32_t kb = smem_u32(sK + buf * kKvBytes), vb = smem_u32(sV + buf * kKvBytes);
-    // ---- wait for the tile; clear what the MMA must not see (0 * Inf = NaN in P V): V rows of slots
-    // past the context end and of pages that were not loaded (readings S10)
-    if (j == 0) mbar_wait(bar_q, 0);
-    mbar_wait(bar_kv0 + 8 * buf, (uint32_t)(j >> 1) & 1);
     const int t0 = j * kKvTile;
+    mbar_wait(bar_s0 + 8 * buf, (uint32_t)(j >> 1) & 1);
+    tc_fence_after();
+    if (warp == 0) {
+      if (j + 2 < nkv) issue_tile(j + 2, false, pgA);           // S_j is done: its K buffer is free
+      if (lane == 0 && j + 1 < nkv) {
+        mbar_wait(bar_k0 + 8 * ((j + 1) & 1), (uint32_t)((j + 1) >> 1) & 1);
+        issue_s(j + 1);                                        // (S_{j-1}, same TMEM columns, was read a step ago)
+      }
+      __syncwarp();
+    }
+    // ---- softmax on row tid: row max on the raw scores (the scale is positive), then the weights ->
+    // P (fp16, shared) and the row sum.  Only the diagonal / last tiles pay for the mask.
+    const bool need_mask = (t0 + kKvTile - 1 > pos0);          // some (row, token) of this tile is masked
+    float s[kKvTile];
+    tmem_ld64(tmem + 64 * buf + lane_sel, s);
+    float mx = -INFINITY;
+    if (need_mask) {
+#pragma unroll
+      for (int e = 0; e < kKvTile; ++e) mx = fmaxf(mx, (t0 + e <= my_pos) ? s[e] : -INFINITY);
+    } else {
+#pragma unroll
+      for (int e = 0; e < kKvTile; ++e) mx = fmaxf(mx, s[e]);
+    }
+    const float m_tile = mx * p.scale_log2;
+    if (j == 0) {
+      m_used = m_tile;                                         // finite: token 0 is visible to every row
+    } else {
+      mbar_wait(bar_o, (uint32_t)(j - 1) & 1);                  // P V_{j-1} done: sP and V buffer (j+1)&1 are free
+      tc_fence_after();
+      if (warp == 0) {
+        if (j + 1 < nkv) issue_tile(j + 1, true, pgB);
+        pgB = pgA;
+        pgA = load_page(j + 3);
+      }
+      const bool move = m_tile > m_used + 8.f;
+      if (__any_sync(0xffffffffu, move)) {                      // rare after the first tiles
+        const float corr = move ? ex2(m_used - m_tile) : 1.f;
+        if (move) m_used = m_tile;
+        l_run *= corr;
+#pragma unroll 1
+        for (int c = 0; c < 4; ++c) {
+          uint32_t r[32];
+          tmem_ld32_issue(tO + lane_sel + c * 32, r);
+          asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+          for (int e = 0; e < 32; ++e) r[e] = __float_as_uint(__uint_as_float(r[e]) * corr);
+          tmem_st32(tO + lane_sel + c * 32, r);
+        }
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+      }
+    }
+    if (j == 0 && warp == 0) { pgB = pgA; pgA = load_page(3); }
+    float rsum = 0.f;
+#pragma unroll
+    for (int u = 0; u < kKvTile / 8; ++u) {                     // 16-byte chunks of 8 tokens of this row
+      uint32_t pk[4];
+#pragma unroll
+      for (int e2 = 0; e2 < 4; ++e2) {
+        const int e = u * 8 + e2 * 2;
+        float w0 = ex2(fmaf(s[e], p.scale_log2, -m_used)), w1 = ex2(fmaf(s[e + 1], p.scale_log2, -m_used));
+        if (need_mask) {
+          w0 = (t0 + e <= my_pos) ? w0 : 0.f;
+          w1 = (t0 + e + 1 <= my_pos) ? w1 : 0.f;
+        }
+        const __half2 h2 = __floats2half2_rn(w0, w1);
+        rsum += __low2float(h2) + __high2float(h2);             // the ROUNDED weights (reading S22)
+        pk[e2] = *reinterpret_cast<const uint32_t*>(&h2);
+      }
+      *reinterpret_cast<int4*>(sP + tid * 128 + ((u ^ (tid & 7)) << 4)) = make_int4((int)pk[0], (int)pk[1], (int)pk[2], (int)pk[3]);
+    }
+    l_run += rsum;
+    // ---- V_j must have landed; clear what the MMA must not see (0 * Inf = NaN in P V): V rows of
+    // slots past the context end and of pages that were not loaded (reading S10)
+    mbar_wait(bar_v0 + 8 * buf, (uint32_t)(j >> 1) & 1);
     if (t0 + kKvTile > n) {
       for (int e = tid; e < (t0 + kKvTile - n) * 16; e += 128) {
         const int r = (n - t0) + e / 16, ch = e % 16;
         *reinterpret_cast<int4*>(sV + buf * kKvBytes + (ch >> 3) * kKvHalfBytes + r * 128 + (((ch & 7) ^ (r & 7)) << 4)) =
             make_int4(0, 0, 0, 0);
       }
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    }
-    tc_fence_before();
-    __syncthreads();
-    // ---- UMMA 1: S = Q K^T
-    if (tid == 0) {
-      tc_fence_after();
-#pragma unroll
-      for (int ks = 0; ks < kD / 16; ++ks) {
-        const uint32_t koff = (uint32_t)(ks & 3) * 32;
-        umma_f16(tS, smem_desc(smem_u32(sQ) + (uint32_t)(ks >> 2) * kHalfBytes + koff, 16, 1024),
-                 smem_desc(kb + (uint32_t)(ks >> 2) * kKvHalfBytes + koff, 16, 1024), kIdescS, ks > 0);
-      }
-      umma_commit(bar_mma);
-    }
-    mbar_wait(bar_mma, mma_phase);
-    mma_phase ^= 1;
-    tc_fence_after();
-
-    // ---- softmax on row tid: pass 1 row max (raw scores: the scale is positive), pass 2 weights ->
-    // P (fp16, shared) and row sum.  Only the diagonal / last tiles pay for the mask.
-    const bool need_mask = (t0 + kKvTile - 1 > pos0);          // some (row, token) of this tile is masked
-    float mx = -INFINITY;
-#pragma unroll 1
-    for (int c = 0; c < kKvTile / 32; ++c) {
-      float s[32];
-      tmem_ld32(tS + lane_sel + c * 32, s);
-      if (need_mask) {
-#pragma unroll
-        for (int e = 0; e < 32; ++e) mx = fmaxf(mx, (t0 + c * 32 + e <= my_pos) ? s[e] : -INFINITY);
-      } else {
-#pragma unroll
-        for (int e = 0; e < 32; ++e) mx = fmaxf(mx, s[e]);
-      }
-    }
-    const float m_new = fmaxf(m_run, mx * p.scale_log2);        // finite from tile 0 on (token 0 is visible)
-    const float corr = ex2(m_run - m_new);
-    m_run = m_new;
-    float rsum = 0.f;
-#pragma unroll 1
-    for (int c = 0; c < kKvTile / 32; ++c) {
-      float s[32];
-      tmem_ld32(tS + lane_sel + c * 32, s);
-      uint32_t pk[16];
-#pragma unroll
-      for (int e = 0; e < 32; e += 2) {
-        float w0 = ex2(fmaf(s[e], p.scale_log2, -m_new)), w1 = ex2(fmaf(s[e + 1], p.scale_log2, -m_new));
-        if (need_mask) {
-          w0 = (t0 + c * 32 + e <= my_pos) ? w0 : 0.f;
-          w1 = (t0 + c * 32 + e + 1 <= my_pos) ? w1 : 0.f;
-        }
-        const __half2 h2 = __floats2half2_rn(w0, w1);
-        rsum += __low2float(h2) + __high2float(h2);             // the ROUNDED weights (reading S22)
-        pk[e >> 1] = *reinterpret_cast<const uint32_t*>(&h2);
-      }
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {                             // 4 x 16-byte chunks = 32 tokens of this row
-        const int ch = c * 4 + u;                               // chunk index along the tile's kv tokens (< 8)
-        *reinterpret_cast<int4*>(sP + tid * 128 + ((ch ^ (tid & 7)) << 4)) =
-            make_int4((int)pk[4 * u], (int)pk[4 * u + 1], (int)pk[4 * u + 2], (int)pk[4 * u + 3]);
-      }
-    }
-    l_run = l_run * corr + rsum;
-    if (__any_sync(0xffffffffu, corr != 1.f)) {
-#pragma unroll
-      for (int e = 0; e < kD; ++e) o_acc[e] *= corr;
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     tc_fence_before();
     __syncthreads();
-    // ---- UMMA 2: O_tile = P V  (V: MN-major B, 64-wide N blocks 8 KiB apart, 8-token groups 1 KiB apart)
+    // ---- UMMA 2: O += P V  (V: MN-major B, 64-wide N blocks 8 KiB apart, 8-token groups 1 KiB apart)
     if (tid == 0) {
+      const uint32_t vb = smem_u32(sV + buf * kKvBytes);
       tc_fence_after();
 #pragma unroll
-      for (int ks = 0; ks < kKvTile / 16; ++ks) {
+      for (int ks = 0; ks < kKvTile / 16; ++ks)
         umma_f16(tO, smem_desc(smem_u32(sP) + (uint32_t)ks * 32, 16, 1024),
-                 smem_desc(vb + (uint32_t)ks * 2048, kKvHalfBytes, 1024), kIdescPV, ks > 0);
-      }
-      umma_commit(bar_mma);
-    }
-    mbar_wait(bar_mma, mma_phase);
-    mma_phase ^= 1;
-    tc_fence_after();
-    // both MMAs of this tile are done: its K/V buffer is free for tile j + 2
-    if (tid == 0 && j + 2 < nkv) issue_kv(j + 2);
-#pragma unroll
-    for (int c = 0; c < 4; ++c) {
-      float v[32];
-      tmem_ld32(tO + lane_sel + c * 32, v);
-#pragma unroll
-      for (int e = 0; e < 32; ++e) o_acc[c * 32 + e] += v[e];
+                 smem_desc(vb + (uint32_t)ks * 2048, kKvHalfBytes, 1024), kIdescPV, (j > 0 || ks > 0) ? 1u : 0u);
+      umma_commit(bar_o);
     }
   }
+  mbar_wait(bar_o, (uint32_t)(nkv - 1) & 1);
+  tc_fence_after();
 
-  // ---- epilogue: row tid -> out[row_tok0 + tid / G][g*G + tid % G][:]
-  if (r0 + tid / G < m) {
+  // ---- epilogue: row tid -> out[row_tok0 + tid / G][g*G + tid % G][:]   (all warps load: .sync.aligned)
+  {
     const float inv = 1.f / l_run;
+    const bool store = r0 + tid / G < m;
     __half* dst = p.out + ((size_t)(row_tok0 + tid / G) * p.Hq + (size_t)(g * G + tid % G)) * kD;
+#pragma unroll 1
+    for (int c = 0; c < 4; ++c) {
+      uint32_t r[32];
+      tmem_ld32_issue(tO + lane_sel + c * 32, r);
+      asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+      if (store) {
 #pragma unroll
-    for (int e = 0; e < kD; e += 8) {
-      __half2 h[4];
+        for (int e = 0; e < 32; e += 8) {
+          __half2 h[4];
 #pragma unroll
-      for (int u = 0; u < 4; ++u) h[u] = __floats2half2_rn(o_acc[e + 2 * u] * inv, o_acc[e + 2 * u + 1] * inv);
-      *reinterpret_cast<int4*>(dst + e) = *reinterpret_cast<const int4*>(h);
+          for (int u = 0; u < 4; ++u)
+            h[u] = __floats2half2_rn(__uint_as_float(r[e + 2 * u]) * inv, __uint_as_float(r[e + 2 * u + 1]) * inv);
+          *reinterpret_cast<int4*>(dst + c * 32 + e) = *reinterpret_cast<const int4*>(h);
+        }
+      }
     }
   }
   tc_fence_before();
