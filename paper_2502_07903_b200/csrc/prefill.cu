@@ -12,7 +12,7 @@
 // is read once for all of them.  Per 64-token KV tile (4 pages):
 //   TMA     K, V pages -> shared [D/64 halves][64 tokens][128 B], 128-byte swizzle (two tiles in flight)
 //   UMMA 1  S[128 x 64] = Q K^T            (8 x tcgen05.mma M128 N64 K16, f16 in / f32 in TMEM cols 0..63)
-//   softmax tcgen05.ld S (thread = row), causal + length mask, online max/sum in fp32, P -> fp16 ->
+//   softmax tcgen05.ld S (two threads per row, 32 columns each), causal + length mask, online max/sum in fp32, P -> fp16 ->
 //           shared in the K-major swizzled layout UMMA reads
 //   UMMA 2  O[128 x D] += P V              (V is the MN-major B operand straight from the page layout;
 //           O stays in TMEM cols 128..255 for the whole CTA)
@@ -22,6 +22,7 @@
 // S_{j+1} and P V_{j-1} under step j's softmax; two CTAs share an SM (112 KiB of shared memory and
 // 256 TMEM columns each).  The measured fraction of the tensor peak is reported by bench.py as it stands.
 #include <cuda.h>
+#include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
 #include <cstring>
@@ -41,8 +42,9 @@ constexpr int kKvHalfBytes = kKvTile * 128;      // K or V: one [64 tokens][128 
 constexpr int kKvBytes = 2 * kKvHalfBytes;       // a K or V tile, 64 tokens x 128 fp16
 constexpr int kPBytes = kRows * kKvTile * 2;     // P tile, 128 rows x 64 fp16 = one swizzled region
 // Q + 2 x (K + V) + P + barriers = 112 KiB + 64 B: two CTAs per SM (their MMA and softmax phases overlap)
-constexpr int kSmem = kQBytes + 4 * kKvBytes + kPBytes + 80;   // 8 mbarriers + the TMEM address
+constexpr int kSmem = kQBytes + 4 * kKvBytes + kPBytes + 80 + 512;   // + the row-max exchange (bf16 [2][128])   // 8 mbarriers + the TMEM address
 constexpr float kLog2e = 1.4426950408889634f;
+constexpr int kIssuer = 8;               // warp 8 issues TMA and MMA; warps 0..7 do the softmax (two threads per row)
 
 struct PrefillParams {
   __half* out;
@@ -157,7 +159,14 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo_bytes,
 constexpr uint32_t kIdescS = (1u << 4) | ((uint32_t)(kKvTile >> 3) << 17) | ((uint32_t)(kRows >> 4) << 24);
 constexpr uint32_t kIdescPV = (1u << 4) | (1u << 16) | ((uint32_t)(kD >> 3) << 17) | ((uint32_t)(kRows >> 4) << 24);
 
-__global__ void __launch_bounds__(128, 2)
+#ifdef HX_PF_TRACE
+__device__ unsigned long long g_pf_trace[16];
+#define PF_T(k) do { if (tid == HX_PF_TID) { long long t_ = clock64(); pf_acc[k] += t_ - pf_last; pf_last = t_; } } while (0)
+#else
+#define PF_T(k)
+#endif
+
+__global__ void __launch_bounds__(288, 2)
 prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                const __grid_constant__ CUtensorMap tmV, const PrefillParams p) {
   extern __shared__ __align__(1024) uint8_t smem[];
@@ -168,6 +177,7 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   uint8_t* sP = sV + 2 * kKvBytes;
   uint64_t* bars = reinterpret_cast<uint64_t*>(sP + kPBytes);   // q, k[2], v[2], s[2], o
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 8);
+  __nv_bfloat16* xch = reinterpret_cast<__nv_bfloat16*>(bars + 10);     // [2 column halves][128 rows]
 
   const int tid = threadIdx.x, warp = tid >> 5;
   const int G = p.G, Hkv = p.Hkv;
@@ -201,7 +211,9 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   tc_fence_after();
   const uint32_t tmem = *tmem_slot;
   const uint32_t tO = tmem + 128;                          // S_j lives at columns 64 * (j & 1)
-  const uint32_t lane_sel = (uint32_t)(warp * 32) << 16;   // this warp's TMEM lanes
+  // 8 warps: warp w and warp w + 4 share TMEM lanes 32 (w & 3) .. +31 (= rows) and split the columns
+  const int row = tid & 127, ch_half = warp >> 2;
+  const uint32_t lane_sel = (uint32_t)((warp & 3) * 32) << 16;
 
   // ---- loads: Q once; K tile t / V tile t into their buffers t & 1, each on its own barrier (pages
   // past the context end are not loaded).  Warp 0 issues them: lane l < 4 owns page l of the tile and
@@ -209,9 +221,9 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   const int lane = tid & 31;
   auto load_page = [&](int t) -> int {
     const int pg = t * (kKvTile / 16) + lane;
-    return (warp == 0 && lane < kKvTile / 16 && t < nkv && pg < np) ? __ldg(p.bt + (size_t)i * p.bt_stride + pg) : 0;
+    return (warp == kIssuer && lane < kKvTile / 16 && t < nkv && pg < np) ? __ldg(p.bt + (size_t)i * p.bt_stride + pg) : 0;
   };
-  auto issue_tile = [&](int t, bool is_v, int page) {            // call from all of warp 0
+  auto issue_tile = [&](int t, bool is_v, int page) {            // call from all of the issuer warp
     const int buf = t & 1;
     const uint32_t bar = (is_v ? bar_v0 : bar_k0) + 8 * buf;
     const int npg = min(kKvTile / 16, np - t * (kKvTile / 16));
@@ -236,8 +248,8 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     }
     umma_commit(bar_s0 + 8 * (t & 1));   // two barriers: S_{t+1} may finish before every thread has seen S_t
   };
-  int pgA = 0, pgB = 0;                                          // warp 0: pages of tiles j + 2 and j + 1
-  if (warp == 0) {
+  int pgA = 0, pgB = 0;                                          // issuer: pages of tiles j + 2 and j + 1
+  if (warp == kIssuer) {
     const int pg0 = load_page(0);
     pgB = load_page(1);
     pgA = load_page(2);
@@ -262,122 +274,163 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   // Its scale is m_used, a STALE row max that is moved (and O, l rescaled) only when the true max has
   // run ahead of it by more than 2^8: the weights 2^(s - m_used) then stay <= 256, exact in fp16's
   // relative precision, and the result is the same softmax average (the factor cancels in O / l).
-  const int my_pos = min(pos0 + tid / G, n - 1);     // rows past the request's last query are never stored
+  const int my_pos = min(pos0 + row / G, n - 1);     // rows past the request's last query are never stored
   float m_used = -INFINITY, l_run = 0.f;
 
   // Schedule of step j (the tensor pipe runs S_{j+1} and P V_{j-1} under this step's softmax):
   //   wait S_j | free K buffer j&1 -> load K_{j+2} | issue S_{j+1} | row max of S_j | wait P V_{j-1},
   //   load V_{j+1} | (rarely) rescale O | P_j -> shared | wait V_j | issue P V_j (accumulating)
-  for (int j = 0; j < nkv; ++j) {
-    const int buf = j & 1;
-    const int t0 = j * kKvTile;
-    mbar_wait(bar_s0 + 8 * buf, (uint32_t)(j >> 1) & 1);
-    tc_fence_after();
-    if (warp == 0) {
+#ifdef HX_PF_TRACE
+  long long pf_acc[10] = {0,0,0,0,0,0,0,0,0,0}; long long pf_last = clock64();
+#endif
+  if (warp == kIssuer) {
+    // ===== issuer warp: its tcgen05 / TMA queue never sits in front of a softmax thread's TMEM load
+    for (int j = 0; j < nkv; ++j) {
+      const int buf = j & 1;
+      if (lane == 0) mbar_wait(bar_s0 + 8 * buf, (uint32_t)(j >> 1) & 1);
+      __syncwarp();
       if (j + 2 < nkv) issue_tile(j + 2, false, pgA);           // S_j is done: its K buffer is free
       if (lane == 0 && j + 1 < nkv) {
         mbar_wait(bar_k0 + 8 * ((j + 1) & 1), (uint32_t)((j + 1) >> 1) & 1);
         issue_s(j + 1);                                        // (S_{j-1}, same TMEM columns, was read a step ago)
       }
       __syncwarp();
+      if (j > 0) {
+        if (lane == 0) mbar_wait(bar_o, (uint32_t)(j - 1) & 1);   // P V_{j-1} done: V buffer (j+1)&1 is free
+        __syncwarp();
+        if (j + 1 < nkv) issue_tile(j + 1, true, pgB);
+      }
+      pgB = pgA;
+      pgA = load_page(j + 3);
+      if (lane == 0) mbar_wait(bar_v0 + 8 * buf, (uint32_t)(j >> 1) & 1);
+      tc_fence_before();
+      __syncthreads();                                         // P_j is in shared memory, V_j's tail is cleared
+      if (lane == 0) {
+        const uint32_t vb = smem_u32(sV + buf * kKvBytes);
+        tc_fence_after();
+#pragma unroll
+        for (int ks = 0; ks < kKvTile / 16; ++ks)
+          umma_f16(tO, smem_desc(smem_u32(sP) + (uint32_t)ks * 32, 16, 1024),
+                   smem_desc(vb + (uint32_t)ks * 2048, kKvHalfBytes, 1024), kIdescPV, (j > 0 || ks > 0) ? 1u : 0u);
+        umma_commit(bar_o);
+      }
+      __syncwarp();
     }
-    // ---- softmax on row tid: row max on the raw scores (the scale is positive), then the weights ->
-    // P (fp16, shared) and the row sum.  Only the diagonal / last tiles pay for the mask.
+  } else {
+  for (int j = 0; j < nkv; ++j) {
+    const int buf = j & 1;
+    const int t0 = j * kKvTile;
+    PF_T(0);
+    mbar_wait(bar_s0 + 8 * buf, (uint32_t)(j >> 1) & 1);
+    tc_fence_after();
+    PF_T(1);
+    PF_T(2);
+    // ---- softmax: thread (row, ch_half) owns 32 of the row's 64 scores.  Row max on the raw scores
+    // (the scale is positive), exchanged with the other half through shared memory (rounded to bf16
+    // on both sides, so both halves use the SAME scale; it only has to be near the max), then the
+    // weights -> P (fp16, shared) and this half's row sum.  Only diagonal / last tiles pay for the mask.
     const bool need_mask = (t0 + kKvTile - 1 > pos0);          // some (row, token) of this tile is masked
-    float s[kKvTile];
-    tmem_ld64(tmem + 64 * buf + lane_sel, s);
-    float mx = -INFINITY;
+    const int tk0 = t0 + ch_half * 32;                          // first kv token of this thread's columns
+    PF_T(2);
+    float s[32];
+    tmem_ld32(tmem + 64 * buf + ch_half * 32 + lane_sel, s);
+    PF_T(3);
+    float mx4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
     if (need_mask) {
 #pragma unroll
-      for (int e = 0; e < kKvTile; ++e) mx = fmaxf(mx, (t0 + e <= my_pos) ? s[e] : -INFINITY);
+      for (int e = 0; e < 32; ++e) mx4[e & 3] = fmaxf(mx4[e & 3], (tk0 + e <= my_pos) ? s[e] : -INFINITY);
     } else {
 #pragma unroll
-      for (int e = 0; e < kKvTile; ++e) mx = fmaxf(mx, s[e]);
+      for (int e = 0; e < 32; ++e) mx4[e & 3] = fmaxf(mx4[e & 3], s[e]);
     }
-    const float m_tile = mx * p.scale_log2;
+    const __nv_bfloat16 mine = __float2bfloat16_rn(fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * p.scale_log2);
+    xch[ch_half * 128 + row] = mine;
+    asm volatile("bar.sync %0, 64;" ::"r"(1 + (warp & 3)) : "memory");     // the two warps of these 32 rows
+    PF_T(4);
+    const float m_tile = fmaxf(__bfloat162float(mine), __bfloat162float(xch[(ch_half ^ 1) * 128 + row]));
     if (j == 0) {
       m_used = m_tile;                                         // finite: token 0 is visible to every row
     } else {
       mbar_wait(bar_o, (uint32_t)(j - 1) & 1);                  // P V_{j-1} done: sP and V buffer (j+1)&1 are free
       tc_fence_after();
-      if (warp == 0) {
-        if (j + 1 < nkv) issue_tile(j + 1, true, pgB);
-        pgB = pgA;
-        pgA = load_page(j + 3);
-      }
       const bool move = m_tile > m_used + 8.f;
       if (__any_sync(0xffffffffu, move)) {                      // rare after the first tiles
         const float corr = move ? ex2(m_used - m_tile) : 1.f;
         if (move) m_used = m_tile;
         l_run *= corr;
 #pragma unroll 1
-        for (int c = 0; c < 4; ++c) {
+        for (int c = 0; c < 2; ++c) {                           // this half's 64 columns of O
           uint32_t r[32];
-          tmem_ld32_issue(tO + lane_sel + c * 32, r);
+          tmem_ld32_issue(tO + lane_sel + ch_half * 64 + c * 32, r);
           asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
           for (int e = 0; e < 32; ++e) r[e] = __float_as_uint(__uint_as_float(r[e]) * corr);
-          tmem_st32(tO + lane_sel + c * 32, r);
+          tmem_st32(tO + lane_sel + ch_half * 64 + c * 32, r);
         }
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
       }
     }
-    if (j == 0 && warp == 0) { pgB = pgA; pgA = load_page(3); }
-    float rsum = 0.f;
+    PF_T(5);
+    float rs4[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-    for (int u = 0; u < kKvTile / 8; ++u) {                     // 16-byte chunks of 8 tokens of this row
+    for (int u = 0; u < 4; ++u) {                               // 16-byte chunks of 8 tokens of this row
       uint32_t pk[4];
 #pragma unroll
       for (int e2 = 0; e2 < 4; ++e2) {
         const int e = u * 8 + e2 * 2;
         float w0 = ex2(fmaf(s[e], p.scale_log2, -m_used)), w1 = ex2(fmaf(s[e + 1], p.scale_log2, -m_used));
         if (need_mask) {
-          w0 = (t0 + e <= my_pos) ? w0 : 0.f;
-          w1 = (t0 + e + 1 <= my_pos) ? w1 : 0.f;
+          w0 = (tk0 + e <= my_pos) ? w0 : 0.f;
+          w1 = (tk0 + e + 1 <= my_pos) ? w1 : 0.f;
         }
         const __half2 h2 = __floats2half2_rn(w0, w1);
-        rsum += __low2float(h2) + __high2float(h2);             // the ROUNDED weights (reading S22)
+        rs4[e2] += __low2float(h2) + __high2float(h2);          // the ROUNDED weights (reading S22)
         pk[e2] = *reinterpret_cast<const uint32_t*>(&h2);
       }
-      *reinterpret_cast<int4*>(sP + tid * 128 + ((u ^ (tid & 7)) << 4)) = make_int4((int)pk[0], (int)pk[1], (int)pk[2], (int)pk[3]);
+      const int ch = ch_half * 4 + u;
+      *reinterpret_cast<int4*>(sP + row * 128 + ((ch ^ (row & 7)) << 4)) = make_int4((int)pk[0], (int)pk[1], (int)pk[2], (int)pk[3]);
     }
-    l_run += rsum;
+    l_run += (rs4[0] + rs4[1]) + (rs4[2] + rs4[3]);
+    PF_T(6);
     // ---- V_j must have landed; clear what the MMA must not see (0 * Inf = NaN in P V): V rows of
     // slots past the context end and of pages that were not loaded (reading S10)
     mbar_wait(bar_v0 + 8 * buf, (uint32_t)(j >> 1) & 1);
     if (t0 + kKvTile > n) {
-      for (int e = tid; e < (t0 + kKvTile - n) * 16; e += 128) {
+      for (int e = tid; e < (t0 + kKvTile - n) * 16; e += 256) {
         const int r = (n - t0) + e / 16, ch = e % 16;
         *reinterpret_cast<int4*>(sV + buf * kKvBytes + (ch >> 3) * kKvHalfBytes + r * 128 + (((ch & 7) ^ (r & 7)) << 4)) =
             make_int4(0, 0, 0, 0);
       }
     }
+    PF_T(7);
+#ifndef HX_EXP_NOPROXYFENCE
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+#endif
     tc_fence_before();
     __syncthreads();
-    // ---- UMMA 2: O += P V  (V: MN-major B, 64-wide N blocks 8 KiB apart, 8-token groups 1 KiB apart)
-    if (tid == 0) {
-      const uint32_t vb = smem_u32(sV + buf * kKvBytes);
-      tc_fence_after();
-#pragma unroll
-      for (int ks = 0; ks < kKvTile / 16; ++ks)
-        umma_f16(tO, smem_desc(smem_u32(sP) + (uint32_t)ks * 32, 16, 1024),
-                 smem_desc(vb + (uint32_t)ks * 2048, kKvHalfBytes, 1024), kIdescPV, (j > 0 || ks > 0) ? 1u : 0u);
-      umma_commit(bar_o);
-    }
+    PF_T(8);
+    PF_T(9);
+  }
   }
   mbar_wait(bar_o, (uint32_t)(nkv - 1) & 1);
   tc_fence_after();
+#ifdef HX_PF_TRACE
+  if (tid == HX_PF_TID) { for (int k = 0; k < 10; ++k) atomicAdd(&g_pf_trace[k], (unsigned long long)pf_acc[k]); atomicAdd(&g_pf_trace[10], (unsigned long long)nkv); }
+#endif
 
-  // ---- epilogue: row tid -> out[row_tok0 + tid / G][g*G + tid % G][:]   (all warps load: .sync.aligned)
+  // ---- epilogue: thread (row, ch_half) -> 64 columns of out[row_tok0 + row / G][g*G + row % G][:];
+  // the two halves' row sums meet in shared memory (sP is free now)
   {
-    const float inv = 1.f / l_run;
-    const bool store = r0 + tid / G < m;
-    __half* dst = p.out + ((size_t)(row_tok0 + tid / G) * p.Hq + (size_t)(g * G + tid % G)) * kD;
+    float* lsum = reinterpret_cast<float*>(sP);
+    if (warp != kIssuer) lsum[ch_half * 128 + row] = l_run;
+    __syncthreads();
+    const float inv = 1.f / (lsum[row] + lsum[128 + row]);
+    const bool store = warp != kIssuer && r0 + row / G < m;
+    __half* dst = p.out + ((size_t)(row_tok0 + row / G) * p.Hq + (size_t)(g * G + row % G)) * kD + ch_half * 64;
 #pragma unroll 1
-    for (int c = 0; c < 4; ++c) {
+    for (int c = 0; c < 2 && warp != kIssuer; ++c) {
       uint32_t r[32];
-      tmem_ld32_issue(tO + lane_sel + c * 32, r);
+      tmem_ld32_issue(tO + lane_sel + ch_half * 64 + c * 32, r);
       asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
       if (store) {
 #pragma unroll
@@ -416,6 +469,14 @@ int encode_fn(EncodeTiledFn* out) {
 }
 
 }  // namespace
+
+#ifdef HX_PF_TRACE
+extern "C" int hx_debug_pf_trace(unsigned long long* out, int reset) {
+  cudaMemcpyFromSymbol(out, g_pf_trace, sizeof(g_pf_trace));
+  if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(g_pf_trace, z, sizeof(z)); }
+  return 0;
+}
+#endif
 
 int launch_prefill(const PrefillArgs& a, cudaStream_t stream) {
   DeviceInfo di;
@@ -473,7 +534,7 @@ int launch_prefill(const PrefillArgs& a, cudaStream_t stream) {
     pb.B = (a.batch - b0 < 65535) ? a.batch - b0 : 65535;
     pb.bt = a.block_table + (size_t)b0 * a.bt_stride;
     pb.lens = a.seq_lens + b0; pb.qlens = a.q_lens + b0; pb.cuq = a.cu_q_lens + b0;
-    prefill_kernel<<<dim3(qtiles, a.kv_heads, pb.B), 128, kSmem, stream>>>(tq, tk, tv, pb);
+    prefill_kernel<<<dim3(qtiles, a.kv_heads, pb.B), 288, kSmem, stream>>>(tq, tk, tv, pb);
     HX_CUDA_OK(cudaGetLastError());
   }
   return HX_OK;
