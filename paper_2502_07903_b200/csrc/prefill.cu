@@ -44,7 +44,8 @@ constexpr int kPBytes = kRows * kKvTile * 2;     // P tile, 128 rows x 64 fp16 =
 // Q + 2 x (K + V) + P + barriers = 112 KiB + 64 B: two CTAs per SM (their MMA and softmax phases overlap)
 constexpr int kSmem = kQBytes + 4 * kKvBytes + kPBytes + 80 + 512;   // + the row-max exchange (bf16 [2][128])   // 8 mbarriers + the TMEM address
 constexpr float kLog2e = 1.4426950408889634f;
-constexpr int kIssuer = 8;               // warp 8 issues TMA and MMA; warps 0..7 do the softmax (two threads per row)
+constexpr int kIssuer = 8;               // warp 8 issues tcgen05.mma, warp 9 TMA; warps 0..7 do the softmax (two threads per row)
+constexpr int kLoader = 9;
 
 struct PrefillParams {
   __half* out;
@@ -166,7 +167,7 @@ __device__ unsigned long long g_pf_trace[16];
 #define PF_T(k)
 #endif
 
-__global__ void __launch_bounds__(288, 2)
+__global__ void __launch_bounds__(320, 2)
 prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                const __grid_constant__ CUtensorMap tmV, const PrefillParams p) {
   extern __shared__ __align__(1024) uint8_t smem[];
@@ -176,7 +177,7 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   uint8_t* sV = sK + 2 * kKvBytes;             // [2 buffers]
   uint8_t* sP = sV + 2 * kKvBytes;
   uint64_t* bars = reinterpret_cast<uint64_t*>(sP + kPBytes);   // q, k[2], v[2], s[2], o
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 8);
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 9);
   __nv_bfloat16* xch = reinterpret_cast<__nv_bfloat16*>(bars + 10);     // [2 column halves][128 rows]
 
   const int tid = threadIdx.x, warp = tid >> 5;
@@ -194,9 +195,9 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   const int np = (n + 15) >> 4;
 
   const uint32_t bar_q = smem_u32(bars), bar_k0 = smem_u32(bars + 1), bar_v0 = smem_u32(bars + 3);
-  const uint32_t bar_s0 = smem_u32(bars + 5), bar_o = smem_u32(bars + 7);
+  const uint32_t bar_s0 = smem_u32(bars + 5), bar_o0 = smem_u32(bars + 7);   // q, k[2], v[2], s[2], o[2]
   if (tid == 0) {
-    for (int e = 0; e < 8; ++e) mbar_init(bar_q + 8 * e, 1);
+    for (int e = 0; e < 9; ++e) mbar_init(bar_q + 8 * e, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tmQ) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tmK) : "memory");
@@ -221,9 +222,9 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   const int lane = tid & 31;
   auto load_page = [&](int t) -> int {
     const int pg = t * (kKvTile / 16) + lane;
-    return (warp == kIssuer && lane < kKvTile / 16 && t < nkv && pg < np) ? __ldg(p.bt + (size_t)i * p.bt_stride + pg) : 0;
+    return (warp == kLoader && lane < kKvTile / 16 && t < nkv && pg < np) ? __ldg(p.bt + (size_t)i * p.bt_stride + pg) : 0;
   };
-  auto issue_tile = [&](int t, bool is_v, int page) {            // call from all of the issuer warp
+  auto issue_tile = [&](int t, bool is_v, int page) {            // call from all of the loader warp
     const int buf = t & 1;
     const uint32_t bar = (is_v ? bar_v0 : bar_k0) + 8 * buf;
     const int npg = min(kKvTile / 16, np - t * (kKvTile / 16));
@@ -248,8 +249,8 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     }
     umma_commit(bar_s0 + 8 * (t & 1));   // two barriers: S_{t+1} may finish before every thread has seen S_t
   };
-  int pgA = 0, pgB = 0;                                          // issuer: pages of tiles j + 2 and j + 1
-  if (warp == kIssuer) {
+  int pgA = 0, pgB = 0;                                          // loader: pages of tiles j + 2 and j + 1
+  if (warp == kLoader) {
     const int pg0 = load_page(0);
     pgB = load_page(1);
     pgA = load_page(2);
@@ -261,6 +262,7 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     issue_tile(0, false, pg0);
     issue_tile(0, true, pg0);
     if (nkv > 1) { issue_tile(1, false, pgB); issue_tile(1, true, pgB); }
+  } else if (warp == kIssuer) {
     if (lane == 0) {
       mbar_wait(bar_q, 0);
       mbar_wait(bar_k0, 0);
@@ -283,28 +285,38 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
 #ifdef HX_PF_TRACE
   long long pf_acc[10] = {0,0,0,0,0,0,0,0,0,0}; long long pf_last = clock64();
 #endif
-  if (warp == kIssuer) {
-    // ===== issuer warp: its tcgen05 / TMA queue never sits in front of a softmax thread's TMEM load
+  // The step barrier (named barrier 5) joins the 8 softmax warps and the MMA warp; the loader warp
+  // follows the mbarriers only.
+  if (warp == kLoader) {
+    // ===== loader warp: K_{j+2} once S_j is done (its K buffer is free), V_{j+1} once P V_{j-1} is done
     for (int j = 0; j < nkv; ++j) {
-      const int buf = j & 1;
-      if (lane == 0) mbar_wait(bar_s0 + 8 * buf, (uint32_t)(j >> 1) & 1);
-      __syncwarp();
-      if (j + 2 < nkv) issue_tile(j + 2, false, pgA);           // S_j is done: its K buffer is free
-      if (lane == 0 && j + 1 < nkv) {
-        mbar_wait(bar_k0 + 8 * ((j + 1) & 1), (uint32_t)((j + 1) >> 1) & 1);
-        issue_s(j + 1);                                        // (S_{j-1}, same TMEM columns, was read a step ago)
-      }
-      __syncwarp();
-      if (j > 0) {
-        if (lane == 0) mbar_wait(bar_o, (uint32_t)(j - 1) & 1);   // P V_{j-1} done: V buffer (j+1)&1 is free
+      if (j + 2 < nkv) {
+        if (lane == 0) mbar_wait(bar_s0 + 8 * (j & 1), (uint32_t)(j >> 1) & 1);
         __syncwarp();
-        if (j + 1 < nkv) issue_tile(j + 1, true, pgB);
+        issue_tile(j + 2, false, pgA);
+      }
+      if (j > 0 && j + 1 < nkv) {
+        if (lane == 0) mbar_wait(bar_o0 + 8 * ((j - 1) & 1), (uint32_t)((j - 1) >> 1) & 1);
+        __syncwarp();
+        issue_tile(j + 1, true, pgB);
       }
       pgB = pgA;
       pgA = load_page(j + 3);
-      if (lane == 0) mbar_wait(bar_v0 + 8 * buf, (uint32_t)(j >> 1) & 1);
+    }
+  } else if (warp == kIssuer) {
+    // ===== MMA warp: one lane issues; the tensor pipe runs S_{j+1} and P V_j in issue order
+    for (int j = 0; j < nkv; ++j) {
+      const int buf = j & 1;
+      PF_T(0);
+      if (lane == 0 && j + 1 < nkv) {
+        mbar_wait(bar_k0 + 8 * ((j + 1) & 1), (uint32_t)((j + 1) >> 1) & 1);
+        issue_s(j + 1);                      // its TMEM columns held S_{j-1}, read before the last step barrier
+      }
+      __syncwarp();
+      PF_T(1);
       tc_fence_before();
-      __syncthreads();                                         // P_j is in shared memory, V_j's tail is cleared
+      asm volatile("bar.sync 5, 288;" ::: "memory");             // P_j is in shared memory, V_j landed and its tail is cleared
+      PF_T(2);
       if (lane == 0) {
         const uint32_t vb = smem_u32(sV + buf * kKvBytes);
         tc_fence_after();
@@ -312,9 +324,10 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
         for (int ks = 0; ks < kKvTile / 16; ++ks)
           umma_f16(tO, smem_desc(smem_u32(sP) + (uint32_t)ks * 32, 16, 1024),
                    smem_desc(vb + (uint32_t)ks * 2048, kKvHalfBytes, 1024), kIdescPV, (j > 0 || ks > 0) ? 1u : 0u);
-        umma_commit(bar_o);
+        umma_commit(bar_o0 + 8 * buf);      // two barriers: the loader may look for P V_{j-1} after P V_j is done
       }
       __syncwarp();
+      PF_T(3);
     }
   } else {
   for (int j = 0; j < nkv; ++j) {
@@ -351,7 +364,7 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     if (j == 0) {
       m_used = m_tile;                                         // finite: token 0 is visible to every row
     } else {
-      mbar_wait(bar_o, (uint32_t)(j - 1) & 1);                  // P V_{j-1} done: sP and V buffer (j+1)&1 are free
+      mbar_wait(bar_o0 + 8 * ((j - 1) & 1), (uint32_t)((j - 1) >> 1) & 1);   // P V_{j-1} done: sP is free
       tc_fence_after();
       const bool move = m_tile > m_used + 8.f;
       if (__any_sync(0xffffffffu, move)) {                      // rare after the first tiles
@@ -407,12 +420,12 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 #endif
     tc_fence_before();
-    __syncthreads();
+    asm volatile("bar.sync 5, 288;" ::: "memory");
     PF_T(8);
     PF_T(9);
   }
   }
-  mbar_wait(bar_o, (uint32_t)(nkv - 1) & 1);
+  mbar_wait(bar_o0 + 8 * ((nkv - 1) & 1), (uint32_t)((nkv - 1) >> 1) & 1);
   tc_fence_after();
 #ifdef HX_PF_TRACE
   if (tid == HX_PF_TID) { for (int k = 0; k < 10; ++k) atomicAdd(&g_pf_trace[k], (unsigned long long)pf_acc[k]); atomicAdd(&g_pf_trace[10], (unsigned long long)nkv); }
@@ -422,13 +435,13 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   // the two halves' row sums meet in shared memory (sP is free now)
   {
     float* lsum = reinterpret_cast<float*>(sP);
-    if (warp != kIssuer) lsum[ch_half * 128 + row] = l_run;
+    if (warp < kIssuer) lsum[ch_half * 128 + row] = l_run;
     __syncthreads();
     const float inv = 1.f / (lsum[row] + lsum[128 + row]);
-    const bool store = warp != kIssuer && r0 + row / G < m;
+    const bool store = warp < kIssuer && r0 + row / G < m;
     __half* dst = p.out + ((size_t)(row_tok0 + row / G) * p.Hq + (size_t)(g * G + row % G)) * kD + ch_half * 64;
 #pragma unroll 1
-    for (int c = 0; c < 2 && warp != kIssuer; ++c) {
+    for (int c = 0; c < 2 && warp < kIssuer; ++c) {
       uint32_t r[32];
       tmem_ld32_issue(tO + lane_sel + ch_half * 64 + c * 32, r);
       asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
@@ -534,7 +547,7 @@ int launch_prefill(const PrefillArgs& a, cudaStream_t stream) {
     pb.B = (a.batch - b0 < 65535) ? a.batch - b0 : 65535;
     pb.bt = a.block_table + (size_t)b0 * a.bt_stride;
     pb.lens = a.seq_lens + b0; pb.qlens = a.q_lens + b0; pb.cuq = a.cu_q_lens + b0;
-    prefill_kernel<<<dim3(qtiles, a.kv_heads, pb.B), 288, kSmem, stream>>>(tq, tk, tv, pb);
+    prefill_kernel<<<dim3(qtiles, a.kv_heads, pb.B), 320, kSmem, stream>>>(tq, tk, tv, pb);
     HX_CUDA_OK(cudaGetLastError());
   }
   return HX_OK;
