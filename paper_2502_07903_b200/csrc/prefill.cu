@@ -42,7 +42,7 @@ constexpr int kKvHalfBytes = kKvTile * 128;      // K or V: one [64 tokens][128 
 constexpr int kKvBytes = 2 * kKvHalfBytes;       // a K or V tile, 64 tokens x 128 fp16
 constexpr int kPBytes = kRows * kKvTile * 2;     // P tile, 128 rows x 64 fp16 = one swizzled region
 // Q + 2 x (K + V) + P + barriers = 112 KiB + 64 B: two CTAs per SM (their MMA and softmax phases overlap)
-constexpr int kSmem = kQBytes + 4 * kKvBytes + kPBytes + 80 + 512;   // + the row-max exchange (bf16 [2][128])   // 8 mbarriers + the TMEM address
+constexpr int kSmem = kQBytes + 4 * kKvBytes + 80 + 512;   // + the row-max exchange (bf16 [2][128])   // 8 mbarriers + the TMEM address
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr int kIssuer = 8;               // warp 8 issues tcgen05.mma, warp 9 TMA; warps 0..7 do the softmax (two threads per row)
 constexpr int kLoader = 9;
@@ -100,6 +100,20 @@ __device__ __forceinline__ void umma_f16(uint32_t d_tmem, uint64_t a_desc, uint6
       "setp.ne.b32 p, %4, 0;\n\t"
       "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
       ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// A operand from TMEM (128 lanes = rows, two fp16 per 32-bit column along K), B from shared memory
+__device__ __forceinline__ void umma_f16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+      ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16]) {   // no wait
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+      ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),
+        "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]) : "memory");
 }
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
@@ -175,8 +189,7 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   uint8_t* sQ = smem;
   uint8_t* sK = smem + kQBytes;                // [2 buffers]
   uint8_t* sV = sK + 2 * kKvBytes;             // [2 buffers]
-  uint8_t* sP = sV + 2 * kKvBytes;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(sP + kPBytes);   // q, k[2], v[2], s[2], o
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sV + 2 * kKvBytes);   // q, k[2], v[2], s[2], o
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 9);
   __nv_bfloat16* xch = reinterpret_cast<__nv_bfloat16*>(bars + 10);     // [2 column halves][128 rows]
 
@@ -322,8 +335,8 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
         tc_fence_after();
 #pragma unroll
         for (int ks = 0; ks < kKvTile / 16; ++ks)
-          umma_f16(tO, smem_desc(smem_u32(sP) + (uint32_t)ks * 32, 16, 1024),
-                   smem_desc(vb + (uint32_t)ks * 2048, kKvHalfBytes, 1024), kIdescPV, (j > 0 || ks > 0) ? 1u : 0u);
+          umma_f16_ts(tO, tmem + 64 * buf + ks * 8, smem_desc(vb + (uint32_t)ks * 2048, kKvHalfBytes, 1024), kIdescPV,
+                      (j > 0 || ks > 0) ? 1u : 0u);
         umma_commit(bar_o0 + 8 * buf);      // two barriers: the loader may look for P V_{j-1} after P V_j is done
       }
       __syncwarp();
@@ -364,7 +377,7 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     if (j == 0) {
       m_used = m_tile;                                         // finite: token 0 is visible to every row
     } else {
-      mbar_wait(bar_o0 + 8 * ((j - 1) & 1), (uint32_t)((j - 1) >> 1) & 1);   // P V_{j-1} done: sP is free
+      mbar_wait(bar_o0 + 8 * ((j - 1) & 1), (uint32_t)((j - 1) >> 1) & 1);   // P V_{j-1} done: O may be rescaled
       tc_fence_after();
       const bool move = m_tile > m_used + 8.f;
       if (__any_sync(0xffffffffu, move)) {                      // rare after the first tiles
@@ -385,24 +398,22 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     }
     PF_T(5);
     float rs4[4] = {0.f, 0.f, 0.f, 0.f};
+    uint32_t pk[16];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {                               // 16-byte chunks of 8 tokens of this row
-      uint32_t pk[4];
-#pragma unroll
-      for (int e2 = 0; e2 < 4; ++e2) {
-        const int e = u * 8 + e2 * 2;
-        float w0 = ex2(fmaf(s[e], p.scale_log2, -m_used)), w1 = ex2(fmaf(s[e + 1], p.scale_log2, -m_used));
-        if (need_mask) {
-          w0 = (tk0 + e <= my_pos) ? w0 : 0.f;
-          w1 = (tk0 + e + 1 <= my_pos) ? w1 : 0.f;
-        }
-        const __half2 h2 = __floats2half2_rn(w0, w1);
-        rs4[e2] += __low2float(h2) + __high2float(h2);          // the ROUNDED weights (reading S22)
-        pk[e2] = *reinterpret_cast<const uint32_t*>(&h2);
+    for (int e = 0; e < 32; e += 2) {
+      float w0 = ex2(fmaf(s[e], p.scale_log2, -m_used)), w1 = ex2(fmaf(s[e + 1], p.scale_log2, -m_used));
+      if (need_mask) {
+        w0 = (tk0 + e <= my_pos) ? w0 : 0.f;
+        w1 = (tk0 + e + 1 <= my_pos) ? w1 : 0.f;
       }
-      const int ch = ch_half * 4 + u;
-      *reinterpret_cast<int4*>(sP + row * 128 + ((ch ^ (row & 7)) << 4)) = make_int4((int)pk[0], (int)pk[1], (int)pk[2], (int)pk[3]);
+      const __half2 h2 = __floats2half2_rn(w0, w1);
+      rs4[(e >> 1) & 3] += __low2float(h2) + __high2float(h2);  // the ROUNDED weights (reading S22)
+      pk[e >> 1] = *reinterpret_cast<const uint32_t*>(&h2);
     }
+    // P_j overwrites the first 32 columns of S_j's TMEM buffer (both halves of the row have loaded
+    // their scores: the pair barrier above); it is the A operand of P V_j, read from tensor memory
+    tmem_st16(tmem + 64 * buf + ch_half * 16 + lane_sel, pk);
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     l_run += (rs4[0] + rs4[1]) + (rs4[2] + rs4[3]);
     PF_T(6);
     // ---- V_j must have landed; clear what the MMA must not see (0 * Inf = NaN in P V): V rows of
@@ -414,11 +425,9 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
         *reinterpret_cast<int4*>(sV + buf * kKvBytes + (ch >> 3) * kKvHalfBytes + r * 128 + (((ch & 7) ^ (r & 7)) << 4)) =
             make_int4(0, 0, 0, 0);
       }
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
     PF_T(7);
-#ifndef HX_EXP_NOPROXYFENCE
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-#endif
     tc_fence_before();
     asm volatile("bar.sync 5, 288;" ::: "memory");
     PF_T(8);
@@ -432,9 +441,9 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
 #endif
 
   // ---- epilogue: thread (row, ch_half) -> 64 columns of out[row_tok0 + row / G][g*G + row % G][:];
-  // the two halves' row sums meet in shared memory (sP is free now)
+  // the two halves' row sums meet in shared memory
   {
-    float* lsum = reinterpret_cast<float*>(sP);
+    float* lsum = reinterpret_cast<float*>(sK);                  // every MMA is done: the K buffers are free
     if (warp < kIssuer) lsum[ch_half * 128 + row] = l_run;
     __syncthreads();
     const float inv = 1.f / (lsum[row] + lsum[128 + row]);
