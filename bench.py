@@ -44,6 +44,49 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def measured_tensor_peak():
+    """Dense bf16/fp16 tensor peak in TFLOP/s (burst figure: the prefill kernel is timed alone)."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["bf16_tflops"]), "measured (MEASURED_PEAKS.json bf16_tflops, cuBLAS 8192^3 burst)"
+    except Exception:
+        return 1590.0, "fallback (B200_PROFILING.md 1.59 PFLOP/s)"
+
+
+def prefill_extra(torch, hx, dev):
+    """F4: hx_prefill_attention on the prefill that produced cfg5's new prompts: 16 prompts x
+    2048 tokens, LLaMA-2-70B, one layer, K/V already in the paged cache.  Algorithmic flops = 4*D per causal
+    (query, kv token) pair per q head; nothing padded or masked is counted."""
+    res = {}
+    peak, src = measured_tensor_peak()
+    for name, (B, n, Hq, Hkv) in {"llama70b_tp1_16x2048": (16, 2048, 64, 8), "llama70b_prefill_tp4_16x2048": (16, 2048, 16, 2),
+                                  "opt30b_tp4_16x2048": (16, 2048, 14, 14)}.items():
+        D = 128
+        pages = B * ((n + 15) // 16)
+        k = torch.empty((1, pages, Hkv, 16, D), dtype=torch.float16, device=dev).normal_()
+        v = torch.empty_like(k).normal_()
+        cache = hx.PagedCache(k, v)
+        g = torch.Generator(device=dev)
+        g.manual_seed(7)
+        bt = torch.randperm(pages, device=dev, generator=g).to(torch.int32).reshape(B, -1).contiguous()
+        lens = torch.full((B,), n, dtype=torch.int32, device=dev)
+        cu = torch.arange(B + 1, dtype=torch.int32, device=dev) * n
+        q = torch.empty((B * n, Hq, D), dtype=torch.float16, device=dev).normal_()
+        out = torch.empty_like(q)
+
+        def fn():
+            hx.prefill_attention(out, q, cache, layer=0, q_heads=Hq, block_table=bt, block_table_stride=bt.shape[1],
+                                 seq_lens=lens, q_lens=lens, cu_q_lens=cu, batch=B, total_q_tokens=B * n, max_q_len=n,
+                                 max_seq_len=n)
+        med, mn = time_kernel(torch, fn, iters=10, warm=3)
+        flops = B * Hq * (n * (n + 1) // 2) * 4 * D
+        res[name] = {"ms_median": med, "ms_min": mn, "algorithmic_flops": flops, "TFLOPs": flops / med / 1e9,
+                     "roofline": {"bound": "tensor", "achieved": flops / med / 1e9, "peak": peak, "unit": "TFLOP/s",
+                                  "frac": flops / med / 1e9 / peak, "peak_source": src}}
+        del k, v, cache, q, out
+    return res
+
+
 def max_over_ranks(ms: float, world: int, device) -> float:
     """Multi-GPU numbers are the MAX over ranks of the device time (never wall clock)."""
     if world <= 1:
@@ -316,6 +359,7 @@ def run_hx(args, rank, world, local_rank):
             hx.decode_attention_append(out, q, kn, vn, cache, q_heads=Hq, workspace=ws, workspace_bytes=ws_bytes, **akw)
         m2, _ = time_kernel(torch, two_launches, iters=20)
         m1, _ = time_kernel(torch, fused, iters=20)
+        extra["prefill"] = prefill_extra(torch, hx, dev)
         extra["append_cfg5"] = {"append_then_attention_ms": m2, "fused_append_attention_ms": m1,
                                 "note": "hx_kv_append + hx_decode_attention (2 launches) vs hx_decode_attention_append (1 launch)"}
 

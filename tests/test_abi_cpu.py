@@ -220,3 +220,29 @@ def test_append_rejects_invalid_arguments_without_launching(fused, over, status)
         _append(fused=fused, **over)
     assert e.value.status == status, str(e.value)
     _append(fused=fused, batch=0)
+
+
+# ---------------------------------------------------------------- F4 entry point
+def _prefill(cache=None, **over):
+    kw = dict(layer=0, q_heads=4, block_table=0x3000, block_table_stride=4, seq_lens=0x4000, q_lens=0x4100,
+              cu_q_lens=0x4200, batch=2, total_q_tokens=100, max_q_len=64, max_seq_len=64, sm_scale=0.0, stream=0)
+    kw.update(over)
+    out, q = kw.pop("out", 0x6000), kw.pop("q", 0x7000)
+    hx.prefill_attention(out, q, cache or FakeCache(), **kw)
+
+
+@pytest.mark.parametrize("over,status", [
+    (dict(out=0), B.HX_ERR_INVALID_ARG), (dict(q=0x7004), B.HX_ERR_INVALID_ARG),
+    (dict(layer=2), B.HX_ERR_INVALID_ARG), (dict(q_heads=3), B.HX_ERR_INVALID_ARG),
+    (dict(q_heads=6), B.HX_ERR_UNSUPPORTED), (dict(batch=-1), B.HX_ERR_INVALID_ARG),
+    (dict(q_lens=0), B.HX_ERR_INVALID_ARG), (dict(cu_q_lens=0), B.HX_ERR_INVALID_ARG),
+    (dict(max_q_len=65), B.HX_ERR_INVALID_ARG), (dict(max_q_len=101, max_seq_len=200, block_table_stride=13), B.HX_ERR_INVALID_ARG),
+    (dict(block_table_stride=3), B.HX_ERR_INVALID_ARG), (dict(sm_scale=float("nan")), B.HX_ERR_INVALID_ARG),
+    (dict(cache=FakeCache(D=64)), B.HX_ERR_UNSUPPORTED), (dict(cache=FakeCache(ps=32)), B.HX_ERR_UNSUPPORTED),
+])
+def test_prefill_rejects_invalid_arguments_without_launching(over, status):
+    with pytest.raises(hx.HxError) as e:
+        _prefill(**over)
+    assert e.value.status == status, str(e.value)
+    _prefill(batch=0, out=0, q=0)                       # HX_OK, nothing launched
+    _prefill(total_q_tokens=0, max_q_len=0)
