@@ -115,6 +115,38 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16
       ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),
         "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]) : "memory");
 }
+// Warp-uniform issue: every lane of the MMA warp executes these with identical operands and ONE elected
+// lane issues.  With uniform control flow ptxas keeps the descriptors in uniform registers; under an
+// `if (lane == 0)` it cannot prove uniformity and emits a waterfall loop (ELECT / R2UR.BROADCAST / BRA)
+// of a dozen instructions around every UTCHMMA.
+__device__ __forceinline__ uint32_t elect_one() {     // 1 in exactly one lane of a converged warp
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(pred));
+  return pred;
+}
+// (`me` = 1 in the issuing lane, 0 elsewhere.)
+__device__ __forceinline__ void umma_f16_u(uint32_t me, uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p, q;\n\t"
+      "setp.ne.b32 q, %5, 0;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "@q tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate), "r"(me) : "memory");
+}
+__device__ __forceinline__ void umma_f16_ts_u(uint32_t me, uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p, q;\n\t"
+      "setp.ne.b32 q, %5, 0;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "@q tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+      ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate), "r"(me) : "memory");
+}
+__device__ __forceinline__ void umma_commit_u(uint32_t me, uint32_t bar) {
+  asm volatile(
+      "{\n\t.reg .pred q;\n\t"
+      "setp.ne.b32 q, %1, 0;\n\t"
+      "@q tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t}" ::"r"(bar), "r"(me) : "memory");
+}
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
@@ -250,17 +282,22 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     }
     __syncwarp();
   };
-  // S_t = Q K_t^T into TMEM columns [64 * (t & 1), +64); completion -> bar_s[t & 1]  (one thread)
+  const uint32_t tmem_u = __shfl_sync(0xffffffffu, tmem, 0);     // the same value, provably warp-uniform
+  const uint32_t me = (lane == 0) ? 1u : 0u;                     // the issuing lane of the MMA warp
+  // S_t = Q K_t^T into TMEM columns [64 * (t & 1), +64); completion -> bar_s[t & 1]  (whole MMA warp, one lane issues)
   auto issue_s = [&](int t) {
     const uint32_t kb = smem_u32(sK + (t & 1) * kKvBytes);
     tc_fence_after();
+    if (elect_one()) {
 #pragma unroll
-    for (int ks = 0; ks < kD / 16; ++ks) {
-      const uint32_t koff = (uint32_t)(ks & 3) * 32;
-      umma_f16(tmem + 64 * (t & 1), smem_desc(smem_u32(sQ) + (uint32_t)(ks >> 2) * kHalfBytes + koff, 16, 1024),
-               smem_desc(kb + (uint32_t)(ks >> 2) * kKvHalfBytes + koff, 16, 1024), kIdescS, ks > 0);
+      for (int ks = 0; ks < kD / 16; ++ks) {
+        const uint32_t koff = (uint32_t)(ks & 3) * 32;
+        umma_f16(tmem_u + 64 * (t & 1), smem_desc(smem_u32(sQ) + (uint32_t)(ks >> 2) * kHalfBytes + koff, 16, 1024),
+                 smem_desc(kb + (uint32_t)(ks >> 2) * kKvHalfBytes + koff, 16, 1024), kIdescS, ks > 0);
+      }
+      umma_commit(bar_s0 + 8 * (t & 1));
     }
-    umma_commit(bar_s0 + 8 * (t & 1));   // two barriers: S_{t+1} may finish before every thread has seen S_t
+    __syncwarp();   // two barriers: S_{t+1} may finish before every thread has seen S_t
   };
   int pgA = 0, pgB = 0;                                          // loader: pages of tiles j + 2 and j + 1
   if (warp == kLoader) {
@@ -276,12 +313,9 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     issue_tile(0, true, pg0);
     if (nkv > 1) { issue_tile(1, false, pgB); issue_tile(1, true, pgB); }
   } else if (warp == kIssuer) {
-    if (lane == 0) {
-      mbar_wait(bar_q, 0);
-      mbar_wait(bar_k0, 0);
-      issue_s(0);
-    }
-    __syncwarp();
+    mbar_wait(bar_q, 0);
+    mbar_wait(bar_k0, 0);
+    issue_s(0);
   }
 
   // ---- per-row state: thread tid owns row tid = (token r0 + tid / G, head g*G + tid % G).  The
@@ -321,25 +355,26 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     for (int j = 0; j < nkv; ++j) {
       const int buf = j & 1;
       PF_T(0);
-      if (lane == 0 && j + 1 < nkv) {
+      if (j + 1 < nkv) {
         mbar_wait(bar_k0 + 8 * ((j + 1) & 1), (uint32_t)((j + 1) >> 1) & 1);
         issue_s(j + 1);                      // its TMEM columns held S_{j-1}, read before the last step barrier
       }
-      __syncwarp();
       PF_T(1);
       tc_fence_before();
       asm volatile("bar.sync 5, 288;" ::: "memory");             // P_j is in shared memory, V_j landed and its tail is cleared
       PF_T(2);
-      if (lane == 0) {
+      {
         const uint32_t vb = smem_u32(sV + buf * kKvBytes);
         tc_fence_after();
+        if (elect_one()) {
 #pragma unroll
-        for (int ks = 0; ks < kKvTile / 16; ++ks)
-          umma_f16_ts(tO, tmem + 64 * buf + ks * 8, smem_desc(vb + (uint32_t)ks * 2048, kKvHalfBytes, 1024), kIdescPV,
-                      (j > 0 || ks > 0) ? 1u : 0u);
-        umma_commit(bar_o0 + 8 * buf);      // two barriers: the loader may look for P V_{j-1} after P V_j is done
+          for (int ks = 0; ks < kKvTile / 16; ++ks)
+            umma_f16_ts(tmem_u + 128, tmem_u + 64 * buf + ks * 8, smem_desc(vb + (uint32_t)ks * 2048, kKvHalfBytes, 1024), kIdescPV,
+                        (j > 0 || ks > 0) ? 1u : 0u);
+          umma_commit(bar_o0 + 8 * buf);    // two barriers: the loader may look for P V_{j-1} after P V_j is done
+        }
+        __syncwarp();
       }
-      __syncwarp();
       PF_T(3);
     }
   } else {
