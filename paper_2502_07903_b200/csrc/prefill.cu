@@ -412,10 +412,12 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     if (j == 0) {
       m_used = m_tile;                                         // finite: token 0 is visible to every row
     } else {
-      mbar_wait(bar_o0 + 8 * ((j - 1) & 1), (uint32_t)((j - 1) >> 1) & 1);   // P V_{j-1} done: O may be rescaled
-      tc_fence_after();
       const bool move = m_tile > m_used + 8.f;
       if (__any_sync(0xffffffffu, move)) {                      // rare after the first tiles
+        // only the rescale touches O, so only it waits for P V_{j-1}; P_j itself goes to the OTHER S
+        // buffer than the P_{j-1} that MMA may still be reading
+        mbar_wait(bar_o0 + 8 * ((j - 1) & 1), (uint32_t)((j - 1) >> 1) & 1);
+        tc_fence_after();
         const float corr = move ? ex2(m_used - m_tile) : 1.f;
         if (move) m_used = m_tile;
         l_run *= corr;
