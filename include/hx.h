@@ -48,7 +48,7 @@
 extern "C" {
 #endif
 
-#define HX_VERSION 120 /* 0.1.2: + stage ingest, append, fused append-attend, pull mode, prefill attention */
+#define HX_VERSION 121 /* 0.1.2.1: + stage ingest, append, fused append-attend, pull mode, prefill attention, overlapped handoff */
 
 typedef enum {
   HX_OK = 0,
@@ -291,6 +291,12 @@ typedef struct {
    * be reachable from the device: pinned host memory (UVA) or a peer GPU's memory with peer access
    * enabled.  src_k_dev/src_v_dev are ignored. */
   int32_t pull_src;
+  /* non-zero = the step's attention does NOT read the pages this step ingests (the new prompts join the
+   * batch later; "asynchronous ... to enable overlapping between computation and
+   * communication"): the shard transfer + ingest run on a library-owned side stream, forked from `stream`
+   * at entry and joined to it before return, so PCIe and the ingest overlap the attention.  0 = everything
+   * in order on `stream` (the attention may read the freshly ingested pages). */
+  int32_t overlap_ingest;
 } hx_step_host_args;
 int hx_decode_step_host(const hx_step_host_args* args, void* stream);
 

@@ -47,7 +47,7 @@ class _CStepArgs(C.Structure):
         ("ing_cu_seqlens_host", C.c_void_p), ("ing_seq_lens_host", C.c_void_p),
         ("ing_block_table_dev", C.c_void_p), ("ing_cu_seqlens_dev", C.c_void_p), ("ing_seq_lens_dev", C.c_void_p),
         ("ing_batch", C.c_int32), ("ing_total_tokens", C.c_int32), ("ing_max_seq_len", C.c_int32),
-        ("pull_src", C.c_int32),
+        ("pull_src", C.c_int32), ("overlap_ingest", C.c_int32),
     ]
 
 

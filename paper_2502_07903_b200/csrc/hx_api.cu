@@ -316,6 +316,30 @@ int hx_decode_step_host(const hx_step_host_args* a, void* stream_) {
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
   if (!a->cache) HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_host: cache is NULL");
   const size_t qbytes = (size_t)a->batch * a->q_heads * a->cache->head_dim * 2;
+  // overlap_ingest: fork a library-owned side stream (one per device, created on first use) for the handoff
+  cudaStream_t main_stream = stream;
+  const bool fork = a->overlap_ingest != 0 && a->ing_batch > 0 && a->batch > 0;
+  static std::mutex mu;
+  static cudaStream_t side_streams[64] = {nullptr};
+  static cudaEvent_t ev_fork[64] = {nullptr}, ev_join[64] = {nullptr};
+  int dev = 0;
+  if (fork) {
+    HX_CUDA_OK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) HX_FAIL(HX_ERR_CUDA, "device id %d out of range", dev);
+    std::lock_guard<std::mutex> lock(mu);
+    if (!side_streams[dev]) {
+      HX_CUDA_OK(cudaStreamCreateWithFlags(&side_streams[dev], cudaStreamNonBlocking));
+      HX_CUDA_OK(cudaEventCreateWithFlags(&ev_fork[dev], cudaEventDisableTiming));
+      HX_CUDA_OK(cudaEventCreateWithFlags(&ev_join[dev], cudaEventDisableTiming));
+    }
+    HX_CUDA_OK(cudaEventRecord(ev_fork[dev], main_stream));
+    HX_CUDA_OK(cudaStreamWaitEvent(side_streams[dev], ev_fork[dev], 0));
+    // the attention's small q upload goes first on the main stream so that it is not queued behind the shards
+    if (!a->q_host || !a->q_dev) HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_host: q/out buffers missing");
+    HX_CUDA_OK(cudaMemcpyAsync(a->q_dev, a->q_host, qbytes, cudaMemcpyHostToDevice, main_stream));
+    stream = side_streams[dev];
+    stream_ = static_cast<void*>(stream);
+  }
   if (a->ing_batch > 0) {
     const bool pull = a->pull_src != 0;
     if (!a->src_k_host || !a->src_v_host || (!pull && (!a->src_k_dev || !a->src_v_dev)) || !a->ing_block_table_host ||
@@ -341,15 +365,21 @@ int hx_decode_step_host(const hx_step_host_args* a, void* stream_) {
                           a->ing_seq_lens_dev, a->ing_batch, a->ing_total_tokens, a->ing_max_seq_len, stream_);
     if (rc) return rc;
   }
+  if (fork) {
+    HX_CUDA_OK(cudaEventRecord(ev_join[dev], stream));
+    stream = main_stream;
+    stream_ = static_cast<void*>(stream);
+  }
   if (a->batch > 0) {
     if (!a->q_host || !a->out_host || !a->q_dev || !a->out_dev) HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_host: q/out buffers missing");
-    HX_CUDA_OK(cudaMemcpyAsync(a->q_dev, a->q_host, qbytes, cudaMemcpyHostToDevice, stream));
+    if (!fork) HX_CUDA_OK(cudaMemcpyAsync(a->q_dev, a->q_host, qbytes, cudaMemcpyHostToDevice, stream));
     int rc = hx_decode_attention(a->out_dev, a->q_dev, a->cache, a->layer, a->q_heads, a->block_table_dev,
                                  a->block_table_stride, a->seq_lens_dev, a->batch, a->max_seq_len, a->sm_scale,
                                  a->workspace, a->workspace_bytes, stream_);
     if (rc) return rc;
     HX_CUDA_OK(cudaMemcpyAsync(a->out_host, a->out_dev, qbytes, cudaMemcpyDeviceToHost, stream));
   }
+  if (fork) HX_CUDA_OK(cudaStreamWaitEvent(main_stream, ev_join[dev], 0));     // join: `stream` now covers the handoff too
   return HX_OK;
 }
 

@@ -224,3 +224,55 @@ def test_pull_mode_ingest_from_mapped_host_memory(env):
         oracle.kv_ingest(w["src_k"], w["src_v"], ok, ov, heads=8, src_tp=4, dst_tp=2, dst_rank=qrank,
                          block_table=w["block_table"], cu_seqlens=w["cu_seqlens"], seq_lens=lens)
         assert np.array_equal(dev_u16(cache.k), ok) and np.array_equal(dev_u16(cache.v), ov)
+
+
+def test_decode_step_host_overlapped_handoff(env):
+    """hx_decode_step_host(overlap_ingest=1): the new prompts' handoff runs on the library's side stream
+    under the attention of an active batch whose pages are disjoint from it.  After the stream is
+    synchronised both results are the oracle's: the new pages bit for bit, the batch's output within tolerance,
+    staged and pull mode alike, twice in a row (the fork/join events are reused)."""
+    hx, torch, oracle = env
+    Hkv, D, Hq = 2, 128, 16
+    ca = W.AttnConfig(99, "t", 6, Hq, Hkv, D, 64, "x")
+    wa = W.make_attention_inputs(ca, lens=np.array([5, 100, 257, 600, 16, 1000], dtype=np.int32), spare=3.0)
+    ci = W.IngestConfig(99, "t", 1, Hkv, D, 2, 1, 3, "x")
+    ilens = np.array([33, 500, 128], dtype=np.int32)
+    used = wa["block_table"][wa["block_table"] >= 0]
+    wi = W.make_ingest_inputs(ci, lens=ilens)
+    free = np.setdiff1d(np.arange(wa["num_pages"]), used)
+    ibt = np.full((3, 32), -1, dtype=np.int32)
+    o = 0
+    for r, n in enumerate(ilens):
+        k = (n + 15) // 16
+        ibt[r, :k] = free[o:o + k]
+        o += k
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    ref_out = oracle.decode_attention(wa["q"], wa["k"], wa["v"], wa["block_table"], wa["seq_lens"])
+    ok, ov = wa["k"].view(np.uint16).copy(), wa["v"].view(np.uint16).copy()
+    oracle.kv_ingest(wi["src_k"], wi["src_v"], ok, ov, heads=Hkv, src_tp=2, dst_tp=1, dst_rank=0, block_table=ibt,
+                     cu_seqlens=wi["cu_seqlens"], seq_lens=ilens)
+    for pull in (0, 1):
+        cache = hx.PagedCache(to_dev(wa["k"], torch), to_dev(wa["v"], torch))
+        qh, oh = pin(wa["q"]), torch.empty(wa["q"].shape, dtype=torch.float16).pin_memory()
+        skh = [pin(a.view(np.int16)) for a in wi["src_k"]]; svh = [pin(a.view(np.int16)) for a in wi["src_v"]]
+        skd = [torch.empty_like(a, device="cuda") for a in skh]; svd = [torch.empty_like(a, device="cuda") for a in svh]
+        bth, cuh, slh = pin(ibt), pin(wi["cu_seqlens"]), pin(ilens)
+        btd, cud, sld = (torch.empty_like(a, device="cuda") for a in (bth, cuh, slh))
+        qd, od = torch.empty_like(qh, device="cuda"), torch.empty_like(oh, device="cuda")
+        abt, asl = torch.from_numpy(wa["block_table"]).cuda(), torch.from_numpy(wa["seq_lens"]).cuda()
+        wsb = hx.decode_attention_workspace_bytes(6, Hq, Hkv, D, 1000)
+        ws = torch.zeros(wsb, dtype=torch.uint8, device="cuda")
+        for rep in range(2):
+            oh.zero_()
+            hx.decode_step_host(q_host=qh, out_host=oh, q_dev=qd, out_dev=od, cache=cache, layer=0, q_heads=Hq,
+                                block_table_dev=abt, block_table_stride=abt.shape[1], seq_lens_dev=asl, batch=6,
+                                max_seq_len=1000, sm_scale=0.0, workspace=ws, workspace_bytes=wsb, src_k_host=skh,
+                                src_v_host=svh, src_k_dev=skd, src_v_dev=svd, ing_layers=1, heads=Hkv, src_tp=2, dst_tp=1,
+                                dst_rank=0, ing_block_table_host=bth, ing_block_table_stride=32, ing_cu_seqlens_host=cuh,
+                                ing_seq_lens_host=slh, ing_block_table_dev=btd, ing_cu_seqlens_dev=cud, ing_seq_lens_dev=sld,
+                                ing_batch=3, ing_total_tokens=wi["total_tokens"], ing_max_seq_len=500, pull_src=pull,
+                                overlap_ingest=1)
+            torch.cuda.current_stream().synchronize()          # the join makes the caller's stream cover the handoff
+            assert np.array_equal(dev_u16(cache.k), ok) and np.array_equal(dev_u16(cache.v), ov), (pull, rep)
+            max_abs, rel = attn_errors(oh.numpy(), ref_out)
+            assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (pull, rep, max_abs, rel)
