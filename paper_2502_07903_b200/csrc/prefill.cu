@@ -9,18 +9,23 @@
 //
 // One CTA = one (request, kv head, tile of 128 query rows); a row is a (token, head-of-the-group)
 // pair, so a GQA group of G heads packs 128/G tokens x G heads into one M = 128 tile and the K/V tile
-// is read once for all of them.  Per 64-token KV tile (4 pages):
-//   TMA     K, V pages -> shared [D/64 halves][64 tokens][128 B], 128-byte swizzle (two tiles in flight)
-//   UMMA 1  S[128 x 64] = Q K^T            (8 x tcgen05.mma M128 N64 K16, f16 in / f32 in TMEM cols 0..63)
-//   softmax tcgen05.ld S (two threads per row, 32 columns each), causal + length mask, online max/sum in fp32, P -> fp16 ->
-//           shared in the K-major swizzled layout UMMA reads
-//   UMMA 2  O[128 x D] += P V              (V is the MN-major B operand straight from the page layout;
-//           O stays in TMEM cols 128..255 for the whole CTA)
+// is read once for all of them.  Two CTAs share an SM (97 KiB of shared memory and 256 TMEM columns
+// each): while one CTA's softmax runs, the tensor pipe works for the other.  Roles: 8 softmax warps
+// (two threads per row), one MMA warp (warp-uniform code, one elected lane issues), one TMA loader warp.
+// Per 128-token KV tile (8 pages):
+//   TMA     K, V pages -> shared [D/64 halves][128 tokens][128 B], 128-byte swizzle; one K and one V tile,
+//           each reloaded as soon as the MMAs that read it are done (a whole softmax before its next use)
+//   UMMA 1  S[128 x 128] = Q K^T           (8 x tcgen05.mma M128 N128 K16, f16 in / f32 in TMEM cols 0..127)
+//   softmax tcgen05.ld S; both threads of a row scan all 128 scores for the max (no exchange), then each
+//           turns its 64 scores into weights: causal + length mask on diagonal tiles only, fp32 row sum of
+//           the rounded weights, P -> fp16 -> tcgen05.st over the thread's OWN first 32 score columns
+//   UMMA 2  O[128 x D] += P V              (P is the TMEM A operand, V the MN-major B operand straight from
+//           the page layout; O stays in TMEM cols 128..255 for the whole CTA), then S of the next tile
+//           over the same columns (the pipe runs in issue order)
 //   rescale O and l only when a row max has moved by more than 2^8 since the scale was last set
 //           (tcgen05.ld / st; rare): the stale scale cancels in O / l.
-// Epilogue: tcgen05.ld O, O / l -> fp16 -> out.  S is double-buffered in TMEM, so the tensor pipe runs
-// S_{j+1} and P V_{j-1} under step j's softmax; two CTAs share an SM (112 KiB of shared memory and
-// 256 TMEM columns each).  The measured fraction of the tensor peak is reported by bench.py as it stands.
+// Epilogue: tcgen05.ld O, O / l -> fp16 -> out.  The measured fraction of the tensor peak is reported by
+// bench.py as it stands; DESIGN.md 6.4 has the history and what bounds it.
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
@@ -35,14 +40,14 @@ namespace {
 
 constexpr int kD = 128;                  // head_dim (this version)
 constexpr int kRows = 128;               // query rows per CTA (UMMA M)
-constexpr int kKvTile = 64;              // kv tokens per tile (UMMA N of S, K of PV): 4 pages
+constexpr int kKvTile = 128;             // kv tokens per tile (UMMA N of S, K of PV): 8 pages
 constexpr int kHalfBytes = kRows * 128;  // Q: one [128 rows][128 B] swizzled region (64 fp16 wide)
 constexpr int kQBytes = 2 * kHalfBytes;  // Q tile, 128 rows x 128 fp16
-constexpr int kKvHalfBytes = kKvTile * 128;      // K or V: one [64 tokens][128 B] region
-constexpr int kKvBytes = 2 * kKvHalfBytes;       // a K or V tile, 64 tokens x 128 fp16
+constexpr int kKvHalfBytes = kKvTile * 128;      // K or V: one [128 tokens][128 B] region
+constexpr int kKvBytes = 2 * kKvHalfBytes;       // a K or V tile, 128 tokens x 128 fp16
 constexpr int kPBytes = kRows * kKvTile * 2;     // P tile, 128 rows x 64 fp16 = one swizzled region
 // Q + 2 x (K + V) + P + barriers = 112 KiB + 64 B: two CTAs per SM (their MMA and softmax phases overlap)
-constexpr int kSmem = kQBytes + 4 * kKvBytes + 80 + 512;   // + the row-max exchange (bf16 [2][128])   // 8 mbarriers + the TMEM address
+constexpr int kSmem = kQBytes + 2 * kKvBytes + 1024 + 64;   // Q, K, V tiles + the row-sum exchange + 5 mbarriers, the TMEM address
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr int kIssuer = 8;               // warp 8 issues tcgen05.mma, warp 9 TMA; warps 0..7 do the softmax (two threads per row)
 constexpr int kLoader = 9;
@@ -219,13 +224,13 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   extern __shared__ __align__(1024) uint8_t smem[];
   if ((smem_u32(smem) & 1023u) != 0) __trap();   // the 128-byte swizzle needs 1 KiB-aligned regions
   uint8_t* sQ = smem;
-  uint8_t* sK = smem + kQBytes;                // [2 buffers]
-  uint8_t* sV = sK + 2 * kKvBytes;             // [2 buffers]
-  uint64_t* bars = reinterpret_cast<uint64_t*>(sV + 2 * kKvBytes);   // q, k[2], v[2], s[2], o
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 9);
-  __nv_bfloat16* xch = reinterpret_cast<__nv_bfloat16*>(bars + 10);     // [2 column halves][128 rows]
+  uint8_t* sK = smem + kQBytes;                // one K tile and one V tile: each is reloaded as soon as the
+  uint8_t* sV = sK + kKvBytes;                 // MMAs that read it are done, a whole softmax before its next use
+  float* lsum = reinterpret_cast<float*>(sV + kKvBytes);         // [2 column halves][128 rows] row sums (epilogue)
+  uint64_t* bars = reinterpret_cast<uint64_t*>(lsum + 256);      // q, k, v, s, o
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 5);
 
-  const int tid = threadIdx.x, warp = tid >> 5;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int G = p.G, Hkv = p.Hkv;
   const int TQ = kRows / G;                          // query tokens per tile
   const int i = blockIdx.z, g = blockIdx.y;
@@ -239,10 +244,9 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   const int nkv = pos_last / kKvTile + 1;            // causal: kv tiles 0..nkv-1
   const int np = (n + 15) >> 4;
 
-  const uint32_t bar_q = smem_u32(bars), bar_k0 = smem_u32(bars + 1), bar_v0 = smem_u32(bars + 3);
-  const uint32_t bar_s0 = smem_u32(bars + 5), bar_o0 = smem_u32(bars + 7);   // q, k[2], v[2], s[2], o[2]
+  const uint32_t bar_q = smem_u32(bars), bar_k = bar_q + 8, bar_v = bar_q + 16, bar_s = bar_q + 24, bar_o = bar_q + 32;
   if (tid == 0) {
-    for (int e = 0; e < 9; ++e) mbar_init(bar_q + 8 * e, 1);
+    for (int e = 0; e < 5; ++e) mbar_init(bar_q + 8 * e, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tmQ) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tmK) : "memory");
@@ -256,231 +260,186 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = *tmem_slot;
-  const uint32_t tO = tmem + 128;                          // S_j lives at columns 64 * (j & 1)
-  // 8 warps: warp w and warp w + 4 share TMEM lanes 32 (w & 3) .. +31 (= rows) and split the columns
+  const uint32_t tS = tmem, tO = tmem + 128;       // S (and P over its first 64 columns) | O
+  // 8 softmax warps: warp w and warp w + 4 share TMEM lanes 32 (w & 3) .. +31 (= rows) and split the columns
   const int row = tid & 127, ch_half = warp >> 2;
   const uint32_t lane_sel = (uint32_t)((warp & 3) * 32) << 16;
 
-  // ---- loads: Q once; K tile t / V tile t into their buffers t & 1, each on its own barrier (pages
-  // past the context end are not loaded).  Warp 0 issues them: lane l < 4 owns page l of the tile and
-  // fetched its block-table entry a step earlier, so no global-load latency sits in the issue path.
-  const int lane = tid & 31;
-  auto load_page = [&](int t) -> int {
-    const int pg = t * (kKvTile / 16) + lane;
-    return (warp == kLoader && lane < kKvTile / 16 && t < nkv && pg < np) ? __ldg(p.bt + (size_t)i * p.bt_stride + pg) : 0;
-  };
-  auto issue_tile = [&](int t, bool is_v, int page) {            // call from all of the loader warp
-    const int buf = t & 1;
-    const uint32_t bar = (is_v ? bar_v0 : bar_k0) + 8 * buf;
-    const int npg = min(kKvTile / 16, np - t * (kKvTile / 16));
-    if (lane == 0) mbar_expect_tx(bar, (uint32_t)(npg * 16 * kD * 2));
-    if (lane < npg) {
-      uint8_t* dstb = (is_v ? sV : sK) + buf * kKvBytes + lane * 2048;
-      const int row = (int)(p.layer_row0 + (uint32_t)page * (uint32_t)(Hkv * 16) + (uint32_t)(g * 16));
-      tma_3d(smem_u32(dstb), is_v ? &tmV : &tmK, 0, row, 0, bar);
-      tma_3d(smem_u32(dstb + kKvHalfBytes), is_v ? &tmV : &tmK, 0, row, 1, bar);
-    }
-    __syncwarp();
-  };
-  const uint32_t tmem_u = __shfl_sync(0xffffffffu, tmem, 0);     // the same value, provably warp-uniform
-  const uint32_t me = (lane == 0) ? 1u : 0u;                     // the issuing lane of the MMA warp
-  // S_t = Q K_t^T into TMEM columns [64 * (t & 1), +64); completion -> bar_s[t & 1]  (whole MMA warp, one lane issues)
-  auto issue_s = [&](int t) {
-    const uint32_t kb = smem_u32(sK + (t & 1) * kKvBytes);
-    tc_fence_after();
-    if (elect_one()) {
-#pragma unroll
-      for (int ks = 0; ks < kD / 16; ++ks) {
-        const uint32_t koff = (uint32_t)(ks & 3) * 32;
-        umma_f16(tmem_u + 64 * (t & 1), smem_desc(smem_u32(sQ) + (uint32_t)(ks >> 2) * kHalfBytes + koff, 16, 1024),
-                 smem_desc(kb + (uint32_t)(ks >> 2) * kKvHalfBytes + koff, 16, 1024), kIdescS, ks > 0);
-      }
-      umma_commit(bar_s0 + 8 * (t & 1));
-    }
-    __syncwarp();   // two barriers: S_{t+1} may finish before every thread has seen S_t
-  };
-  int pgA = 0, pgB = 0;                                          // loader: pages of tiles j + 2 and j + 1
+  float m_used = -INFINITY, l_run = 0.f;             // softmax threads' row state (see below)
+
   if (warp == kLoader) {
-    const int pg0 = load_page(0);
-    pgB = load_page(1);
-    pgA = load_page(2);
+    // ===== loader warp: lane l < 8 owns page l of a 128-token tile; its block-table entry is fetched one
+    // tile ahead.  K_{j+1} goes out when S_j is done, V_{j+1} when P V_j is done.
+    auto load_page = [&](int t) -> int {
+      const int pg = t * (kKvTile / 16) + lane;
+      return (lane < kKvTile / 16 && t < nkv && pg < np) ? __ldg(p.bt + (size_t)i * p.bt_stride + pg) : 0;
+    };
+    auto issue_tile = [&](int t, bool is_v, int page) {
+      const uint32_t bar = is_v ? bar_v : bar_k;
+      const int npg = min(kKvTile / 16, np - t * (kKvTile / 16));
+      if (lane == 0) mbar_expect_tx(bar, (uint32_t)(npg * 16 * kD * 2));
+      if (lane < npg) {
+        uint8_t* dstb = (is_v ? sV : sK) + lane * 2048;
+        const int rw = (int)(p.layer_row0 + (uint32_t)page * (uint32_t)(Hkv * 16) + (uint32_t)(g * 16));
+        tma_3d(smem_u32(dstb), is_v ? &tmV : &tmK, 0, rw, 0, bar);
+        tma_3d(smem_u32(dstb + kKvHalfBytes), is_v ? &tmV : &tmK, 0, rw, 1, bar);
+      }
+      __syncwarp();
+    };
+    int pg_cur = load_page(0), pg_nxt = load_page(1);
     if (lane == 0) {
       mbar_expect_tx(bar_q, kQBytes);
       tma_4d(smem_u32(sQ), &tmQ, 0, g * G, row_tok0, 0, bar_q);
       tma_4d(smem_u32(sQ + kHalfBytes), &tmQ, 0, g * G, row_tok0, 1, bar_q);
     }
-    issue_tile(0, false, pg0);
-    issue_tile(0, true, pg0);
-    if (nkv > 1) { issue_tile(1, false, pgB); issue_tile(1, true, pgB); }
-  } else if (warp == kIssuer) {
-    mbar_wait(bar_q, 0);
-    mbar_wait(bar_k0, 0);
-    issue_s(0);
-  }
-
-  // ---- per-row state: thread tid owns row tid = (token r0 + tid / G, head g*G + tid % G).  The
-  // output accumulator O lives in TMEM (columns 128..255) across all tiles: P V_j accumulates into it.
-  // Its scale is m_used, a STALE row max that is moved (and O, l rescaled) only when the true max has
-  // run ahead of it by more than 2^8: the weights 2^(s - m_used) then stay <= 256, exact in fp16's
-  // relative precision, and the result is the same softmax average (the factor cancels in O / l).
-  const int my_pos = min(pos0 + row / G, n - 1);     // rows past the request's last query are never stored
-  float m_used = -INFINITY, l_run = 0.f;
-
-  // Schedule of step j (the tensor pipe runs S_{j+1} and P V_{j-1} under this step's softmax):
-  //   wait S_j | free K buffer j&1 -> load K_{j+2} | issue S_{j+1} | row max of S_j | wait P V_{j-1},
-  //   load V_{j+1} | (rarely) rescale O | P_j -> shared | wait V_j | issue P V_j (accumulating)
-#ifdef HX_PF_TRACE
-  long long pf_acc[10] = {0,0,0,0,0,0,0,0,0,0}; long long pf_last = clock64();
-#endif
-  // The step barrier (named barrier 5) joins the 8 softmax warps and the MMA warp; the loader warp
-  // follows the mbarriers only.
-  if (warp == kLoader) {
-    // ===== loader warp: K_{j+2} once S_j is done (its K buffer is free), V_{j+1} once P V_{j-1} is done
-    for (int j = 0; j < nkv; ++j) {
-      if (j + 2 < nkv) {
-        if (lane == 0) mbar_wait(bar_s0 + 8 * (j & 1), (uint32_t)(j >> 1) & 1);
-        __syncwarp();
-        issue_tile(j + 2, false, pgA);
-      }
-      if (j > 0 && j + 1 < nkv) {
-        if (lane == 0) mbar_wait(bar_o0 + 8 * ((j - 1) & 1), (uint32_t)((j - 1) >> 1) & 1);
-        __syncwarp();
-        issue_tile(j + 1, true, pgB);
-      }
-      pgB = pgA;
-      pgA = load_page(j + 3);
+    issue_tile(0, false, pg_cur);
+    issue_tile(0, true, pg_cur);
+    for (int j = 0; j + 1 < nkv; ++j) {
+      const int pg_nn = load_page(j + 2);
+      if (lane == 0) mbar_wait(bar_s, (uint32_t)j & 1);         // S_j done: the K tile is free
+      __syncwarp();
+      issue_tile(j + 1, false, pg_nxt);
+      if (lane == 0) mbar_wait(bar_o, (uint32_t)j & 1);         // P V_j done: the V tile is free
+      __syncwarp();
+      issue_tile(j + 1, true, pg_nxt);
+      pg_cur = pg_nxt; pg_nxt = pg_nn;
     }
   } else if (warp == kIssuer) {
-    // ===== MMA warp: one lane issues; the tensor pipe runs S_{j+1} and P V_j in issue order
-    for (int j = 0; j < nkv; ++j) {
-      const int buf = j & 1;
-      PF_T(0);
-      if (j + 1 < nkv) {
-        mbar_wait(bar_k0 + 8 * ((j + 1) & 1), (uint32_t)((j + 1) >> 1) & 1);
-        issue_s(j + 1);                      // its TMEM columns held S_{j-1}, read before the last step barrier
-      }
-      PF_T(1);
-      tc_fence_before();
-      asm volatile("bar.sync 5, 288;" ::: "memory");             // P_j is in shared memory, V_j landed and its tail is cleared
-      PF_T(2);
-      {
-        const uint32_t vb = smem_u32(sV + buf * kKvBytes);
-        tc_fence_after();
-        if (elect_one()) {
+    // ===== MMA warp (warp-uniform; one elected lane issues).  Per tile: P V_j after the step barrier, then
+    // S_{j+1} over the same TMEM columns (the pipe runs in issue order, so P_j is read before it is
+    // overwritten).  The other CTA of the SM keeps the pipe fed while this CTA's softmax runs.
+    const uint32_t tmem_u = __shfl_sync(0xffffffffu, tmem, 0);  // the same value, provably warp-uniform
+    auto issue_s = [&]() {
+      tc_fence_after();
+      if (elect_one()) {
 #pragma unroll
-          for (int ks = 0; ks < kKvTile / 16; ++ks)
-            umma_f16_ts(tmem_u + 128, tmem_u + 64 * buf + ks * 8, smem_desc(vb + (uint32_t)ks * 2048, kKvHalfBytes, 1024), kIdescPV,
-                        (j > 0 || ks > 0) ? 1u : 0u);
-          umma_commit(bar_o0 + 8 * buf);    // two barriers: the loader may look for P V_{j-1} after P V_j is done
+        for (int ks = 0; ks < kD / 16; ++ks) {
+          const uint32_t koff = (uint32_t)(ks & 3) * 32;
+          umma_f16(tmem_u, smem_desc(smem_u32(sQ) + (uint32_t)(ks >> 2) * kHalfBytes + koff, 16, 1024),
+                   smem_desc(smem_u32(sK) + (uint32_t)(ks >> 2) * kKvHalfBytes + koff, 16, 1024), kIdescS, ks > 0);
         }
-        __syncwarp();
+        umma_commit(bar_s);
       }
-      PF_T(3);
+      __syncwarp();
+    };
+    mbar_wait(bar_q, 0);
+    mbar_wait(bar_k, 0);
+    issue_s();
+    for (int j = 0; j < nkv; ++j) {
+      tc_fence_before();
+      asm volatile("bar.sync 5, 288;" ::: "memory");             // P_j is in TMEM, V_j landed and its tail is cleared
+      tc_fence_after();
+      if (elect_one()) {
+#pragma unroll
+        for (int ks = 0; ks < kKvTile / 16; ++ks)
+          umma_f16_ts(tmem_u + 128, tmem_u + (ks < 4 ? ks * 8 : 64 + (ks - 4) * 8), smem_desc(smem_u32(sV) + (uint32_t)ks * 2048, kKvHalfBytes, 1024), kIdescPV,
+                      (j > 0 || ks > 0) ? 1u : 0u);
+        umma_commit(bar_o);
+      }
+      __syncwarp();
+      if (j + 1 < nkv) {
+        mbar_wait(bar_k, (uint32_t)(j + 1) & 1);
+        issue_s();
+      }
     }
   } else {
-  for (int j = 0; j < nkv; ++j) {
-    const int buf = j & 1;
-    const int t0 = j * kKvTile;
-    PF_T(0);
-    mbar_wait(bar_s0 + 8 * buf, (uint32_t)(j >> 1) & 1);
-    tc_fence_after();
-    PF_T(1);
-    PF_T(2);
-    // ---- softmax: thread (row, ch_half) owns 32 of the row's 64 scores.  Row max on the raw scores
-    // (the scale is positive), exchanged with the other half through shared memory (rounded to bf16
-    // on both sides, so both halves use the SAME scale; it only has to be near the max), then the
-    // weights -> P (fp16, shared) and this half's row sum.  Only diagonal / last tiles pay for the mask.
-    const bool need_mask = (t0 + kKvTile - 1 > pos0);          // some (row, token) of this tile is masked
-    const int tk0 = t0 + ch_half * 32;                          // first kv token of this thread's columns
-    PF_T(2);
-    float s[32];
-    tmem_ld32(tmem + 64 * buf + ch_half * 32 + lane_sel, s);
-    PF_T(3);
-    float mx4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
-    if (need_mask) {
+    // ===== softmax warps: thread (row, ch_half) owns 64 of the row's 128 scores, handled 32 at a time.
+    // O lives in TMEM (columns 128..255) across all tiles at the scale m_used, a STALE row max that is
+    // moved (and O, l rescaled) only when the true max has run ahead of it by more than 2^8: the weights
+    // 2^(s - m_used) then stay <= 256, exact in fp16's relative precision, and the result is the same
+    // softmax average (the factor cancels in O / l).
+    const int my_pos = min(pos0 + row / G, n - 1);     // rows past the request's last query are never stored
+    for (int j = 0; j < nkv; ++j) {
+      const int t0 = j * kKvTile;
+      mbar_wait(bar_s, (uint32_t)j & 1);
+      tc_fence_after();
+      const bool need_mask = (t0 + kKvTile - 1 > pos0);          // some (row, token) of this tile is masked
+      const int tk0 = t0 + ch_half * 64;                          // first kv token of this thread's columns
+      // ---- pass 1: row max on the raw scores (the scale is positive).  Both threads of a row scan all
+      // 128 scores (TMEM loads are cheap) instead of exchanging half-row maxima: no barrier, and both get
+      // bit-identical scales.
+      float mx4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
-      for (int e = 0; e < 32; ++e) mx4[e & 3] = fmaxf(mx4[e & 3], (tk0 + e <= my_pos) ? s[e] : -INFINITY);
-    } else {
+      for (int c = 0; c < 4; ++c) {
+        float s[32];
+        tmem_ld32(tS + c * 32 + lane_sel, s);
+        if (need_mask) {
 #pragma unroll
-      for (int e = 0; e < 32; ++e) mx4[e & 3] = fmaxf(mx4[e & 3], s[e]);
-    }
-    const __nv_bfloat16 mine = __float2bfloat16_rn(fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * p.scale_log2);
-    xch[ch_half * 128 + row] = mine;
-    asm volatile("bar.sync %0, 64;" ::"r"(1 + (warp & 3)) : "memory");     // the two warps of these 32 rows
-    PF_T(4);
-    const float m_tile = fmaxf(__bfloat162float(mine), __bfloat162float(xch[(ch_half ^ 1) * 128 + row]));
-    if (j == 0) {
-      m_used = m_tile;                                         // finite: token 0 is visible to every row
-    } else {
-      const bool move = m_tile > m_used + 8.f;
-      if (__any_sync(0xffffffffu, move)) {                      // rare after the first tiles
-        // only the rescale touches O, so only it waits for P V_{j-1}; P_j itself goes to the OTHER S
-        // buffer than the P_{j-1} that MMA may still be reading
-        mbar_wait(bar_o0 + 8 * ((j - 1) & 1), (uint32_t)((j - 1) >> 1) & 1);
-        tc_fence_after();
-        const float corr = move ? ex2(m_used - m_tile) : 1.f;
-        if (move) m_used = m_tile;
-        l_run *= corr;
-#pragma unroll 1
-        for (int c = 0; c < 2; ++c) {                           // this half's 64 columns of O
-          uint32_t r[32];
-          tmem_ld32_issue(tO + lane_sel + ch_half * 64 + c * 32, r);
-          asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+          for (int e = 0; e < 32; ++e) mx4[e & 3] = fmaxf(mx4[e & 3], (t0 + c * 32 + e <= my_pos) ? s[e] : -INFINITY);
+        } else {
 #pragma unroll
-          for (int e = 0; e < 32; ++e) r[e] = __float_as_uint(__uint_as_float(r[e]) * corr);
-          tmem_st32(tO + lane_sel + ch_half * 64 + c * 32, r);
+          for (int e = 0; e < 32; ++e) mx4[e & 3] = fmaxf(mx4[e & 3], s[e]);
         }
-        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
       }
-    }
-    PF_T(5);
-    float rs4[4] = {0.f, 0.f, 0.f, 0.f};
-    uint32_t pk[16];
+      const float m_tile = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * p.scale_log2;
+      if (j == 0) {
+        m_used = m_tile;                                         // finite: token 0 is visible to every row
+      } else {
+        const bool move = m_tile > m_used + 8.f;
+        if (__any_sync(0xffffffffu, move)) {                      // rare after the first tiles
+          mbar_wait(bar_o, (uint32_t)(j - 1) & 1);                // only the rescale touches O: P V_{j-1} must be done
+          tc_fence_after();
+          const float corr = move ? ex2(m_used - m_tile) : 1.f;
+          if (move) m_used = m_tile;
+          l_run *= corr;
+#pragma unroll 1
+          for (int c = 0; c < 2; ++c) {                           // this half's 64 columns of O
+            uint32_t r[32];
+            tmem_ld32_issue(tO + lane_sel + ch_half * 64 + c * 32, r);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
-    for (int e = 0; e < 32; e += 2) {
-      float w0 = ex2(fmaf(s[e], p.scale_log2, -m_used)), w1 = ex2(fmaf(s[e + 1], p.scale_log2, -m_used));
-      if (need_mask) {
-        w0 = (tk0 + e <= my_pos) ? w0 : 0.f;
-        w1 = (tk0 + e + 1 <= my_pos) ? w1 : 0.f;
+            for (int e = 0; e < 32; ++e) r[e] = __float_as_uint(__uint_as_float(r[e]) * corr);
+            tmem_st32(tO + lane_sel + ch_half * 64 + c * 32, r);
+          }
+        }
       }
-      const __half2 h2 = __floats2half2_rn(w0, w1);
-      rs4[(e >> 1) & 3] += __low2float(h2) + __high2float(h2);  // the ROUNDED weights (reading S22)
-      pk[e >> 1] = *reinterpret_cast<const uint32_t*>(&h2);
-    }
-    // P_j overwrites the first 32 columns of S_j's TMEM buffer (both halves of the row have loaded
-    // their scores: the pair barrier above); it is the A operand of P V_j, read from tensor memory
-    tmem_st16(tmem + 64 * buf + ch_half * 16 + lane_sel, pk);
-    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-    l_run += (rs4[0] + rs4[1]) + (rs4[2] + rs4[3]);
-    PF_T(6);
-    // ---- V_j must have landed; clear what the MMA must not see (0 * Inf = NaN in P V): V rows of
-    // slots past the context end and of pages that were not loaded (reading S10)
-    mbar_wait(bar_v0 + 8 * buf, (uint32_t)(j >> 1) & 1);
-    if (t0 + kKvTile > n) {
-      for (int e = tid; e < (t0 + kKvTile - n) * 16; e += 256) {
-        const int r = (n - t0) + e / 16, ch = e % 16;
-        *reinterpret_cast<int4*>(sV + buf * kKvBytes + (ch >> 3) * kKvHalfBytes + r * 128 + (((ch & 7) ^ (r & 7)) << 4)) =
-            make_int4(0, 0, 0, 0);
+      // ---- pass 2: weights -> fp16 -> P, 32 scores at a time.  A thread's P (32 packed columns) overwrites
+      // the first half of ITS OWN 64 score columns, chunk by chunk after the chunk is in registers, so no
+      // thread ever waits for another: P sits at columns [0,32) (tokens 0..63) and [64,96) (tokens 64..127),
+      // and the MMA warp points each K = 16 step's A operand there.
+      // (Pass 1 of the row's other thread reads these columns too: see the barrier note below.)
+      float rs4[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+      for (int c = 0; c < 2; ++c) {
+        float s[32];
+        tmem_ld32(tS + ch_half * 64 + c * 32 + lane_sel, s);
+        uint32_t pk[16];
+#pragma unroll
+        for (int e = 0; e < 32; e += 2) {
+          float w0 = ex2(fmaf(s[e], p.scale_log2, -m_used)), w1 = ex2(fmaf(s[e + 1], p.scale_log2, -m_used));
+          if (need_mask) {
+            w0 = (tk0 + c * 32 + e <= my_pos) ? w0 : 0.f;
+            w1 = (tk0 + c * 32 + e + 1 <= my_pos) ? w1 : 0.f;
+          }
+          const __half2 h2 = __floats2half2_rn(w0, w1);
+          rs4[(e >> 1) & 3] += __low2float(h2) + __high2float(h2);  // the ROUNDED weights (reading S22)
+          pk[e >> 1] = *reinterpret_cast<const uint32_t*>(&h2);
+        }
+        if (c == 0) asm volatile("bar.sync %0, 64;" ::"r"(1 + (warp & 3)) : "memory");   // the row's other thread has finished pass 1
+        tmem_st16(tS + ch_half * 64 + c * 16 + lane_sel, pk);       // P_j: the TMEM A operand of P V_j
       }
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+      l_run += (rs4[0] + rs4[1]) + (rs4[2] + rs4[3]);
+      // ---- V_j must have landed; clear what the MMA must not see (0 * Inf = NaN in P V): V rows of
+      // slots past the context end and of pages that were not loaded (reading S10)
+      mbar_wait(bar_v, (uint32_t)j & 1);
+      if (t0 + kKvTile > n) {
+        for (int e = tid; e < (t0 + kKvTile - n) * 16; e += 256) {
+          const int r = (n - t0) + e / 16, ch = e % 16;
+          *reinterpret_cast<int4*>(sV + (ch >> 3) * kKvHalfBytes + r * 128 + (((ch & 7) ^ (r & 7)) << 4)) = make_int4(0, 0, 0, 0);
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      }
+      tc_fence_before();
+      asm volatile("bar.sync 5, 288;" ::: "memory");
     }
-    PF_T(7);
-    tc_fence_before();
-    asm volatile("bar.sync 5, 288;" ::: "memory");
-    PF_T(8);
-    PF_T(9);
   }
-  }
-  mbar_wait(bar_o0 + 8 * ((nkv - 1) & 1), (uint32_t)((nkv - 1) >> 1) & 1);
+  mbar_wait(bar_o, (uint32_t)(nkv - 1) & 1);
   tc_fence_after();
-#ifdef HX_PF_TRACE
-  if (tid == HX_PF_TID) { for (int k = 0; k < 10; ++k) atomicAdd(&g_pf_trace[k], (unsigned long long)pf_acc[k]); atomicAdd(&g_pf_trace[10], (unsigned long long)nkv); }
-#endif
 
   // ---- epilogue: thread (row, ch_half) -> 64 columns of out[row_tok0 + row / G][g*G + row % G][:];
   // the two halves' row sums meet in shared memory
   {
-    float* lsum = reinterpret_cast<float*>(sK);                  // every MMA is done: the K buffers are free
     if (warp < kIssuer) lsum[ch_half * 128 + row] = l_run;
     __syncthreads();
     const float inv = 1.f / (lsum[row] + lsum[128 + row]);
