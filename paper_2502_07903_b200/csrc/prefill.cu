@@ -266,6 +266,9 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   const uint32_t lane_sel = (uint32_t)((warp & 3) * 32) << 16;
 
   float m_used = -INFINITY, l_run = 0.f;             // softmax threads' row state (see below)
+#ifdef HX_PF_TRACE
+  long long pf_acc[10] = {0,0,0,0,0,0,0,0,0,0}; long long pf_last = clock64();
+#endif
 
   if (warp == kLoader) {
     // ===== loader warp: lane l < 8 owns page l of a 128-token tile; its block-table entry is fetched one
@@ -326,9 +329,11 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     mbar_wait(bar_k, 0);
     issue_s();
     for (int j = 0; j < nkv; ++j) {
+      PF_T(0);
       tc_fence_before();
       asm volatile("bar.sync 5, 288;" ::: "memory");             // P_j is in TMEM, V_j landed and its tail is cleared
       tc_fence_after();
+      PF_T(1);
       if (elect_one()) {
 #pragma unroll
         for (int ks = 0; ks < kKvTile / 16; ++ks)
@@ -337,9 +342,12 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
         umma_commit(bar_o);
       }
       __syncwarp();
+      PF_T(2);
       if (j + 1 < nkv) {
         mbar_wait(bar_k, (uint32_t)(j + 1) & 1);
+        PF_T(3);
         issue_s();
+        PF_T(4);
       }
     }
   } else {
@@ -351,8 +359,10 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     const int my_pos = min(pos0 + row / G, n - 1);     // rows past the request's last query are never stored
     for (int j = 0; j < nkv; ++j) {
       const int t0 = j * kKvTile;
+      PF_T(0);
       mbar_wait(bar_s, (uint32_t)j & 1);
       tc_fence_after();
+      PF_T(1);
       const bool need_mask = (t0 + kKvTile - 1 > pos0);          // some (row, token) of this tile is masked
       const int tk0 = t0 + ch_half * 64;                          // first kv token of this thread's columns
       // ---- pass 1: row max on the raw scores (the scale is positive).  Both threads of a row scan all
@@ -372,6 +382,7 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
         }
       }
       const float m_tile = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * p.scale_log2;
+      PF_T(2);
       if (j == 0) {
         m_used = m_tile;                                         // finite: token 0 is visible to every row
       } else {
@@ -398,6 +409,7 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       // thread ever waits for another: P sits at columns [0,32) (tokens 0..63) and [64,96) (tokens 64..127),
       // and the MMA warp points each K = 16 step's A operand there.
       // (Pass 1 of the row's other thread reads these columns too: see the barrier note below.)
+      PF_T(3);
       float rs4[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
       for (int c = 0; c < 2; ++c) {
@@ -420,9 +432,11 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       }
       asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
       l_run += (rs4[0] + rs4[1]) + (rs4[2] + rs4[3]);
+      PF_T(4);
       // ---- V_j must have landed; clear what the MMA must not see (0 * Inf = NaN in P V): V rows of
       // slots past the context end and of pages that were not loaded (reading S10)
       mbar_wait(bar_v, (uint32_t)j & 1);
+      PF_T(5);
       if (t0 + kKvTile > n) {
         for (int e = tid; e < (t0 + kKvTile - n) * 16; e += 256) {
           const int r = (n - t0) + e / 16, ch = e % 16;
@@ -432,10 +446,14 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       }
       tc_fence_before();
       asm volatile("bar.sync 5, 288;" ::: "memory");
+      PF_T(6);
     }
   }
   mbar_wait(bar_o, (uint32_t)(nkv - 1) & 1);
   tc_fence_after();
+#ifdef HX_PF_TRACE
+  if (tid == HX_PF_TID) { for (int k = 0; k < 10; ++k) atomicAdd(&g_pf_trace[k], (unsigned long long)pf_acc[k]); atomicAdd(&g_pf_trace[10], (unsigned long long)nkv); }
+#endif
 
   // ---- epilogue: thread (row, ch_half) -> 64 columns of out[row_tok0 + row / G][g*G + row % G][:];
   // the two halves' row sums meet in shared memory
