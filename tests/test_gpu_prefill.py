@@ -90,3 +90,10 @@ def test_prefill_one_query_token_matches_decode_kernel(env):
     q = W.draw_fp16_normal((5, 8, 128), 74, 40)
     ref_dec = oracle.decode_attention(q, w["k"], w["v"], w["block_table"], lens)
     np.testing.assert_allclose(ref, ref_dec, atol=1e-13)
+
+
+def test_prefill_chunk_on_a_long_context_and_wide_group(env):
+    """A 300-token chunk at the end of a 5000-token context (most kv tiles carry no mask at all), and a
+    G = 16 group (8 tokens x 16 heads per row tile)."""
+    run_prefill(env, 75, 8, 1, [5000, 4097], [300, 1])
+    run_prefill(env, 76, 16, 1, [700, 129, 33], [700, 129, 33])
