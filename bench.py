@@ -53,6 +53,20 @@ def measured_tensor_peak():
         return 1590.0, "fallback (B200_PROFILING.md 1.59 PFLOP/s)"
 
 
+def stream_peaks(torch, dev):
+    """Read-only and write-only HBM stream rates of this GPU in this run: the attention kernel
+    only reads, so it can exceed the copy figure.  torch ops over 4 GiB (context numbers, not the product)."""
+    n = 1 << 30                                            # 4 GiB of int32
+    x = torch.empty(n, dtype=torch.int32, device=dev)
+    x.zero_()
+    res = {}
+    for name, fn in (("write_only_fill", lambda: x.zero_()), ("read_only_sum", lambda: x.sum())):
+        med, mn = time_kernel(torch, fn, iters=5, warm=2)
+        res[name + "_GBps"] = 4 * n / mn / 1e6
+    del x
+    return res
+
+
 def prefill_extra(torch, hx, dev):
     """F4: hx_prefill_attention on the prefill that produced cfg5's new prompts: 16 prompts x
     2048 tokens, LLaMA-2-70B, one layer, K/V already in the paged cache.  Algorithmic flops = 4*D per causal
@@ -364,6 +378,7 @@ def run_hx(args, rank, world, local_rank):
         m2, _ = time_kernel(torch, two_launches, iters=20)
         m1, _ = time_kernel(torch, fused, iters=20)
         extra["prefill"] = prefill_extra(torch, hx, dev)
+        extra["stream_peaks"] = stream_peaks(torch, dev)
         extra["append_cfg5"] = {"append_then_attention_ms": m2, "fused_append_attention_ms": m1,
                                 "note": "hx_kv_append + hx_decode_attention (2 launches) vs hx_decode_attention_append (1 launch)"}
 
