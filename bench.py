@@ -56,8 +56,8 @@ def measured_tensor_peak():
 def stream_peaks(torch, dev):
     """Read-only and write-only HBM stream rates of this GPU in this run: the attention kernel
     only reads, so it can exceed the copy figure.  torch ops over 4 GiB (context numbers, not the product)."""
-    n = 1 << 30                                            # 4 GiB of int32
-    x = torch.empty(n, dtype=torch.int32, device=dev)
+    n = 1 << 30                                            # 4 GiB of float32
+    x = torch.empty(n, dtype=torch.float32, device=dev)
     x.zero_()
     res = {}
     for name, fn in (("write_only_fill", lambda: x.zero_()), ("read_only_sum", lambda: x.sum())):
