@@ -27,7 +27,6 @@
 // Epilogue: tcgen05.ld O, O / l -> fp16 -> out.  The measured fraction of the tensor peak is reported by
 // bench.py as it stands; DESIGN.md 6.4 has the history and what bounds it.
 #include <cuda.h>
-#include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
 #include <cstring>
@@ -45,11 +44,10 @@ constexpr int kHalfBytes = kRows * 128;  // Q: one [128 rows][128 B] swizzled re
 constexpr int kQBytes = 2 * kHalfBytes;  // Q tile, 128 rows x 128 fp16
 constexpr int kKvHalfBytes = kKvTile * 128;      // K or V: one [128 tokens][128 B] region
 constexpr int kKvBytes = 2 * kKvHalfBytes;       // a K or V tile, 128 tokens x 128 fp16
-constexpr int kPBytes = kRows * kKvTile * 2;     // P tile, 128 rows x 64 fp16 = one swizzled region
-// Q + 2 x (K + V) + P + barriers = 112 KiB + 64 B: two CTAs per SM (their MMA and softmax phases overlap)
+// Q + K + V tiles = 96 KiB (+ exchange, barriers): two CTAs per SM (their MMA and softmax phases overlap)
 constexpr int kSmem = kQBytes + 2 * kKvBytes + 1024 + 64;   // Q, K, V tiles + the row-sum exchange + 5 mbarriers, the TMEM address
 constexpr float kLog2e = 1.4426950408889634f;
-constexpr int kIssuer = 8;               // warp 8 issues tcgen05.mma, warp 9 TMA; warps 0..7 do the softmax (two threads per row)
+constexpr int kIssuer = 8;               // warps 0..7: softmax (two threads per row); warp 8 issues tcgen05.mma, warp 9 TMA
 constexpr int kLoader = 9;
 
 struct PrefillParams {
@@ -135,29 +133,6 @@ __device__ __forceinline__ uint32_t elect_one() {     // 1 in exactly one lane o
   asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(pred));
   return pred;
 }
-// (`me` = 1 in the issuing lane, 0 elsewhere.)
-__device__ __forceinline__ void umma_f16_u(uint32_t me, uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
-  asm volatile(
-      "{\n\t.reg .pred p, q;\n\t"
-      "setp.ne.b32 q, %5, 0;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "@q tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-      ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate), "r"(me) : "memory");
-}
-__device__ __forceinline__ void umma_f16_ts_u(uint32_t me, uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
-  asm volatile(
-      "{\n\t.reg .pred p, q;\n\t"
-      "setp.ne.b32 q, %5, 0;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "@q tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
-      ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate), "r"(me) : "memory");
-}
-__device__ __forceinline__ void umma_commit_u(uint32_t me, uint32_t bar) {
-  asm volatile(
-      "{\n\t.reg .pred q;\n\t"
-      "setp.ne.b32 q, %1, 0;\n\t"
-      "@q tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t}" ::"r"(bar), "r"(me) : "memory");
-}
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
@@ -196,15 +171,6 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32
         "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]),
         "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31]) : "memory");
 }
-__device__ __forceinline__ void tmem_ld64(uint32_t taddr, float (&v)[64]) {
-  uint32_t a[32], b[32];
-  tmem_ld32_issue(taddr, a);
-  tmem_ld32_issue(taddr + 32, b);
-  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-  for (int e = 0; e < 32; ++e) { v[e] = __uint_as_float(a[e]); v[32 + e] = __uint_as_float(b[e]); }
-}
-
 // Shared-memory matrix descriptor (cute::UMMA::SmemDescriptor bit layout): start address >> 4 in
 // [0,14), leading byte offset >> 4 in [16,30), stride byte offset >> 4 in [32,46), version 1 in
 // [46,48), layout type in [61,64) (2 = 128-byte swizzle).
@@ -216,13 +182,6 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo_bytes,
 // a_major bit 15, b_major bit 16 (1 = MN-major), N >> 3 in [17,23), M >> 4 in [24,29).
 constexpr uint32_t kIdescS = (1u << 4) | ((uint32_t)(kKvTile >> 3) << 17) | ((uint32_t)(kRows >> 4) << 24);
 constexpr uint32_t kIdescPV = (1u << 4) | (1u << 16) | ((uint32_t)(kD >> 3) << 17) | ((uint32_t)(kRows >> 4) << 24);
-
-#ifdef HX_PF_TRACE
-__device__ unsigned long long g_pf_trace[16];
-#define PF_T(k) do { if (tid == HX_PF_TID) { long long t_ = clock64(); pf_acc[k] += t_ - pf_last; pf_last = t_; } } while (0)
-#else
-#define PF_T(k)
-#endif
 
 __global__ void __launch_bounds__(320, 2)
 prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
@@ -272,9 +231,6 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   const uint32_t lane_sel = (uint32_t)((warp & 3) * 32) << 16;
 
   float m_used = -INFINITY, l_run = 0.f;             // softmax threads' row state (see below)
-#ifdef HX_PF_TRACE
-  long long pf_acc[10] = {0,0,0,0,0,0,0,0,0,0}; long long pf_last = clock64();
-#endif
 
   if (warp == kLoader) {
     // ===== loader warp: lane l < 8 owns page l of a 128-token tile; its block-table entry is fetched one
@@ -335,11 +291,9 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     mbar_wait(bar_k, 0);
     issue_s();
     for (int j = 0; j < nkv; ++j) {
-      PF_T(0);
       tc_fence_before();
       asm volatile("bar.sync 5, 288;" ::: "memory");             // P_j is in TMEM, V_j landed and its tail is cleared
       tc_fence_after();
-      PF_T(1);
       if (elect_one()) {
 #pragma unroll
         for (int ks = 0; ks < kKvTile / 16; ++ks)
@@ -348,12 +302,9 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
         umma_commit(bar_o);
       }
       __syncwarp();
-      PF_T(2);
       if (j + 1 < nkv) {
         mbar_wait(bar_k, (uint32_t)(j + 1) & 1);
-        PF_T(3);
         issue_s();
-        PF_T(4);
       }
     }
   } else {
@@ -365,10 +316,8 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     const int my_pos = min(pos0 + row / G, n - 1);     // rows past the request's last query are never stored
     for (int j = 0; j < nkv; ++j) {
       const int t0 = j * kKvTile;
-      PF_T(0);
       mbar_wait(bar_s, (uint32_t)j & 1);
       tc_fence_after();
-      PF_T(1);
       const bool need_mask = (t0 + kKvTile - 1 > pos0);          // some (row, token) of this tile is masked
       const int tk0 = t0 + ch_half * 64;                          // first kv token of this thread's columns
       // ---- pass 1: row max on the raw scores (the scale is positive).  Both threads of a row scan all
@@ -388,7 +337,6 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
         }
       }
       const float m_tile = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * p.scale_log2;
-      PF_T(2);
       if (j == 0) {
         m_used = m_tile;                                         // finite: token 0 is visible to every row
       } else {
@@ -415,7 +363,6 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       // thread ever waits for another: P sits at columns [0,32) (tokens 0..63) and [64,96) (tokens 64..127),
       // and the MMA warp points each K = 16 step's A operand there.
       // (Pass 1 of the row's other thread reads these columns too: see the barrier note below.)
-      PF_T(3);
       float rs4[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
       for (int c = 0; c < 2; ++c) {
@@ -438,11 +385,9 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       }
       asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
       l_run += (rs4[0] + rs4[1]) + (rs4[2] + rs4[3]);
-      PF_T(4);
       // ---- V_j must have landed; clear what the MMA must not see (0 * Inf = NaN in P V): V rows of
       // slots past the context end and of pages that were not loaded (reading S10)
       mbar_wait(bar_v, (uint32_t)j & 1);
-      PF_T(5);
       if (t0 + kKvTile > n) {
         for (int e = tid; e < (t0 + kKvTile - n) * 16; e += 256) {
           const int r = (n - t0) + e / 16, ch = e % 16;
@@ -452,14 +397,10 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       }
       tc_fence_before();
       asm volatile("bar.sync 5, 288;" ::: "memory");
-      PF_T(6);
     }
   }
   mbar_wait(bar_o, (uint32_t)(nkv - 1) & 1);
   tc_fence_after();
-#ifdef HX_PF_TRACE
-  if (tid == HX_PF_TID) { for (int k = 0; k < 10; ++k) atomicAdd(&g_pf_trace[k], (unsigned long long)pf_acc[k]); atomicAdd(&g_pf_trace[10], (unsigned long long)nkv); }
-#endif
 
   // ---- epilogue: thread (row, ch_half) -> 64 columns of out[row_tok0 + row / G][g*G + row % G][:];
   // the two halves' row sums meet in shared memory
@@ -511,14 +452,6 @@ int encode_fn(EncodeTiledFn* out) {
 }
 
 }  // namespace
-
-#ifdef HX_PF_TRACE
-extern "C" int hx_debug_pf_trace(unsigned long long* out, int reset) {
-  cudaMemcpyFromSymbol(out, g_pf_trace, sizeof(g_pf_trace));
-  if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(g_pf_trace, z, sizeof(z)); }
-  return 0;
-}
-#endif
 
 int launch_prefill(const PrefillArgs& a, cudaStream_t stream) {
   DeviceInfo di;
