@@ -276,3 +276,68 @@ def test_decode_step_host_overlapped_handoff(env):
             assert np.array_equal(dev_u16(cache.k), ok) and np.array_equal(dev_u16(cache.v), ov), (pull, rep)
             max_abs, rel = attn_errors(oh.numpy(), ref_out)
             assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (pull, rep, max_abs, rel)
+
+
+def test_decode_step_in_a_cuda_graph(env):
+    """The calls only enqueue work and keep no per-call host state, so a whole decode step (ingest of new
+    prompts, append + attention of the active batch) can be captured once in a CUDA graph and replayed; each
+    replay sees the CURRENT contents of the device buffers.  Two replays with different inputs, both checked
+    against the oracle."""
+    hx, torch, oracle = env
+    Hkv, D, Hq = 2, 128, 16
+    ca = W.AttnConfig(87, "t", 5, Hq, Hkv, D, 64, "x")
+    wa = W.make_attention_inputs(ca, lens=np.array([40, 100, 257, 600, 16], dtype=np.int32), spare=3.0)
+    ci = W.IngestConfig(87, "t", 1, Hkv, D, 2, 1, 2, "x")
+    ilens = np.array([33, 200], dtype=np.int32)
+    used = wa["block_table"][wa["block_table"] >= 0]
+    free = np.setdiff1d(np.arange(wa["num_pages"]), used)
+    ibt = np.full((2, 16), -1, dtype=np.int32)
+    o = 0
+    for r, n in enumerate(ilens):
+        k = (n + 15) // 16
+        ibt[r, :k] = free[o:o + k]
+        o += k
+    cache = hx.PagedCache(to_dev(wa["k"], torch), to_dev(wa["v"], torch))
+    B = 5
+    qd = torch.empty((B, Hq, D), dtype=torch.float16, device="cuda")
+    kn = torch.empty((B, Hkv, D), dtype=torch.float16, device="cuda")
+    vn = torch.empty_like(kn)
+    out = torch.empty_like(qd)
+    wi0 = W.make_ingest_inputs(ci, lens=ilens)
+    sk = [torch.empty(a.shape, dtype=torch.float16, device="cuda") for a in wi0["src_k"]]
+    sv = [torch.empty(a.shape, dtype=torch.float16, device="cuda") for a in wi0["src_v"]]
+    abt, asl = torch.from_numpy(wa["block_table"]).cuda(), torch.from_numpy(wa["seq_lens"]).cuda()
+    ibt_d, icu, isl = torch.from_numpy(ibt).cuda(), torch.from_numpy(wi0["cu_seqlens"]).cuda(), torch.from_numpy(ilens).cuda()
+    wsb = hx.decode_attention_workspace_bytes(B, Hq, Hkv, D, 600)
+    ws = torch.zeros(wsb, dtype=torch.uint8, device="cuda")
+
+    def step():
+        hx.kv_ingest(sk, sv, layers=1, heads=Hkv, head_dim=D, src_tp=2, dst_tp=1, dst_rank=0, dst=cache, block_table=ibt_d,
+                     block_table_stride=16, cu_seqlens=icu, seq_lens=isl, batch=2, total_tokens=int(ilens.sum()), max_seq_len=200)
+        hx.decode_attention_append(out, qd, kn, vn, cache, layer=0, q_heads=Hq, block_table=abt, block_table_stride=abt.shape[1],
+                                   seq_lens=asl, batch=B, max_seq_len=600, workspace=ws)
+
+    step()                                          # warm-up outside capture (function attributes, tensor maps)
+    torch.cuda.synchronize()
+    cache.k.copy_(to_dev(wa["k"], torch)); cache.v.copy_(to_dev(wa["v"], torch))
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        step()
+    ok, ov = wa["k"].view(np.uint16).copy(), wa["v"].view(np.uint16).copy()
+    for rep in range(2):
+        wi = W.make_ingest_inputs(ci, lens=ilens, seed_extra=10 + rep)
+        q = W.draw_fp16_normal((B, Hq, D), 87, 70, rep)
+        k1 = W.draw_fp16_normal((B, Hkv, D), 87, 71, rep)
+        v1 = W.draw_fp16_normal((B, Hkv, D), 87, 72, rep)
+        qd.copy_(to_dev(q, torch)); kn.copy_(to_dev(k1, torch)); vn.copy_(to_dev(v1, torch))
+        for r in range(2):
+            sk[r].copy_(to_dev(wi["src_k"][r], torch)); sv[r].copy_(to_dev(wi["src_v"][r], torch))
+        g.replay()
+        torch.cuda.synchronize()
+        oracle.kv_ingest(wi["src_k"], wi["src_v"], ok, ov, heads=Hkv, src_tp=2, dst_tp=1, dst_rank=0, block_table=ibt,
+                         cu_seqlens=wi["cu_seqlens"], seq_lens=ilens)
+        oracle.kv_append(k1, v1, ok, ov, layer=0, block_table=wa["block_table"], seq_lens=wa["seq_lens"])
+        ref = oracle.decode_attention(q, ok.view(np.float16), ov.view(np.float16), wa["block_table"], wa["seq_lens"])
+        assert np.array_equal(dev_u16(cache.k), ok) and np.array_equal(dev_u16(cache.v), ov), rep
+        max_abs, rel = attn_errors(out.cpu().numpy(), ref)
+        assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (rep, max_abs, rel)
