@@ -227,7 +227,7 @@ int hx_decode_attention_append(void* out, const void* q, const void* k_new, cons
  * q_lens       : device int32 [batch], 0 <= q_lens[i] <= seq_lens[i] (device-side contract).
  * cu_q_lens    : device int32 [batch+1], exclusive prefix sums of q_lens.
  * total_q_tokens, max_q_len, max_seq_len : host copies for launch sizing and checks.
- * HX_ERR_UNSUPPORTED: head_dim != 128 (this version), group size not in {1,2,4,8,16}. */
+ * HX_ERR_UNSUPPORTED: head_dim not in {64,128}, group size not in {1,2,4,8,16}. */
 int hx_prefill_attention(void* out, const void* q,
                          const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
                          const int32_t* block_table, int32_t block_table_stride,

@@ -275,7 +275,6 @@ int hx_prefill_attention(void* out, const void* q, const hx_paged_cache* cache, 
     HX_FAIL(HX_ERR_INVALID_ARG, "%s: negative size (batch=%d total_q_tokens=%d max_q_len=%d max_seq_len=%d)", who, batch, total_q_tokens, max_q_len, max_seq_len);
   int rc = check_cache(cache, who);
   if (rc) return rc;
-  if (cache->head_dim != 128) HX_FAIL(HX_ERR_UNSUPPORTED, "%s: head_dim %d != 128", who, cache->head_dim);
   if (layer < 0 || layer >= cache->layers) HX_FAIL(HX_ERR_INVALID_ARG, "%s: layer %d not in [0,%d)", who, layer, cache->layers);
   if (q_heads <= 0 || q_heads % cache->kv_heads) HX_FAIL(HX_ERR_INVALID_ARG, "%s: q_heads %d not a positive multiple of kv_heads %d", who, q_heads, cache->kv_heads);
   const int G = q_heads / cache->kv_heads;

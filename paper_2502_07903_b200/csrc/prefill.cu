@@ -37,15 +37,21 @@
 namespace hx {
 namespace {
 
-constexpr int kD = 128;                  // head_dim (this version)
 constexpr int kRows = 128;               // query rows per CTA (UMMA M)
 constexpr int kKvTile = 128;             // kv tokens per tile (UMMA N of S, K of PV): 8 pages
 constexpr int kHalfBytes = kRows * 128;  // Q: one [128 rows][128 B] swizzled region (64 fp16 wide)
-constexpr int kQBytes = 2 * kHalfBytes;  // Q tile, 128 rows x 128 fp16
 constexpr int kKvHalfBytes = kKvTile * 128;      // K or V: one [128 tokens][128 B] region
-constexpr int kKvBytes = 2 * kKvHalfBytes;       // a K or V tile, 128 tokens x 128 fp16
-// Q + K + V tiles = 96 KiB (+ exchange, barriers): two CTAs per SM (their MMA and softmax phases overlap)
-constexpr int kSmem = kQBytes + 2 * kKvBytes + 1024 + 64;   // Q, K, V tiles + the row-sum exchange + 5 mbarriers, the TMEM address
+// Sizes that depend on head_dim D (64 or 128): operands are stored as D/64 regions of [128 rows][128 B].
+template <int D>
+struct PfCfg {
+  static constexpr int kHalves = D / 64;
+  static constexpr int kQBytes = kHalves * kHalfBytes;       // Q tile, 128 rows x D fp16
+  static constexpr int kKvBytes = kHalves * kKvHalfBytes;    // a K or V tile, 128 tokens x D fp16
+  // Q + K + V tiles (96 KiB at D = 128) + the row-sum exchange + 5 mbarriers, the TMEM address: two CTAs per SM
+  static constexpr int kSmem = kQBytes + 2 * kKvBytes + 1024 + 64;
+  // UMMA instruction descriptor of O += P V: N = D, B operand MN-major
+  static constexpr uint32_t kIdescPV = (1u << 4) | (1u << 16) | ((uint32_t)(D >> 3) << 17) | ((uint32_t)(kRows >> 4) << 24);
+};
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr int kIssuer = 8;               // warps 0..7: softmax (two threads per row); warp 8 issues tcgen05.mma, warp 9 TMA
 constexpr int kLoader = 9;
@@ -181,17 +187,19 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo_bytes,
 // Instruction descriptor (cute::UMMA::InstrDescriptor): c_format f32 (1 << 4), a/b format f16 (0),
 // a_major bit 15, b_major bit 16 (1 = MN-major), N >> 3 in [17,23), M >> 4 in [24,29).
 constexpr uint32_t kIdescS = (1u << 4) | ((uint32_t)(kKvTile >> 3) << 17) | ((uint32_t)(kRows >> 4) << 24);
-constexpr uint32_t kIdescPV = (1u << 4) | (1u << 16) | ((uint32_t)(kD >> 3) << 17) | ((uint32_t)(kRows >> 4) << 24);
 
+template <int D>
 __global__ void __launch_bounds__(320, 2)
 prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                const __grid_constant__ CUtensorMap tmV, const PrefillParams p) {
+  using C = PfCfg<D>;
+  constexpr int kHalves = C::kHalves;
   extern __shared__ __align__(1024) uint8_t smem[];
   if ((smem_u32(smem) & 1023u) != 0) __trap();   // the 128-byte swizzle needs 1 KiB-aligned regions
   uint8_t* sQ = smem;
-  uint8_t* sK = smem + kQBytes;                // one K tile and one V tile: each is reloaded as soon as the
-  uint8_t* sV = sK + kKvBytes;                 // MMAs that read it are done, a whole softmax before its next use
-  float* lsum = reinterpret_cast<float*>(sV + kKvBytes);         // [2 column halves][128 rows] row sums (epilogue)
+  uint8_t* sK = smem + C::kQBytes;                // one K tile and one V tile: each is reloaded as soon as the
+  uint8_t* sV = sK + C::kKvBytes;                 // MMAs that read it are done, a whole softmax before its next use
+  float* lsum = reinterpret_cast<float*>(sV + C::kKvBytes);         // [2 column halves][128 rows] row sums (epilogue)
   uint64_t* bars = reinterpret_cast<uint64_t*>(lsum + 256);      // q, k, v, s, o
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 5);
 
@@ -242,20 +250,20 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     auto issue_tile = [&](int t, bool is_v, int page) {
       const uint32_t bar = is_v ? bar_v : bar_k;
       const int npg = min(kKvTile / 16, np - t * (kKvTile / 16));
-      if (lane == 0) mbar_expect_tx(bar, (uint32_t)(npg * 16 * kD * 2));
+      if (lane == 0) mbar_expect_tx(bar, (uint32_t)(npg * 16 * D * 2));
       if (lane < npg) {
         uint8_t* dstb = (is_v ? sV : sK) + lane * 2048;
         const int rw = (int)(p.layer_row0 + (uint32_t)page * (uint32_t)(Hkv * 16) + (uint32_t)(g * 16));
-        tma_3d(smem_u32(dstb), is_v ? &tmV : &tmK, 0, rw, 0, bar);
-        tma_3d(smem_u32(dstb + kKvHalfBytes), is_v ? &tmV : &tmK, 0, rw, 1, bar);
+#pragma unroll
+        for (int h = 0; h < kHalves; ++h) tma_3d(smem_u32(dstb + h * kKvHalfBytes), is_v ? &tmV : &tmK, 0, rw, h, bar);
       }
       __syncwarp();
     };
     int pg_cur = load_page(0), pg_nxt = load_page(1);
     if (lane == 0) {
-      mbar_expect_tx(bar_q, kQBytes);
-      tma_4d(smem_u32(sQ), &tmQ, 0, g * G, row_tok0, 0, bar_q);
-      tma_4d(smem_u32(sQ + kHalfBytes), &tmQ, 0, g * G, row_tok0, 1, bar_q);
+      mbar_expect_tx(bar_q, C::kQBytes);
+#pragma unroll
+      for (int h = 0; h < kHalves; ++h) tma_4d(smem_u32(sQ + h * kHalfBytes), &tmQ, 0, g * G, row_tok0, h, bar_q);
     }
     issue_tile(0, false, pg_cur);
     issue_tile(0, true, pg_cur);
@@ -278,7 +286,7 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       tc_fence_after();
       if (elect_one()) {
 #pragma unroll
-        for (int ks = 0; ks < kD / 16; ++ks) {
+        for (int ks = 0; ks < D / 16; ++ks) {
           const uint32_t koff = (uint32_t)(ks & 3) * 32;
           umma_f16(tmem_u, smem_desc(smem_u32(sQ) + (uint32_t)(ks >> 2) * kHalfBytes + koff, 16, 1024),
                    smem_desc(smem_u32(sK) + (uint32_t)(ks >> 2) * kKvHalfBytes + koff, 16, 1024), kIdescS, ks > 0);
@@ -297,7 +305,7 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       if (elect_one()) {
 #pragma unroll
         for (int ks = 0; ks < kKvTile / 16; ++ks)
-          umma_f16_ts(tmem_u + 128, tmem_u + (ks < 4 ? ks * 8 : 64 + (ks - 4) * 8), smem_desc(smem_u32(sV) + (uint32_t)ks * 2048, kKvHalfBytes, 1024), kIdescPV,
+          umma_f16_ts(tmem_u + 128, tmem_u + (ks < 4 ? ks * 8 : 64 + (ks - 4) * 8), smem_desc(smem_u32(sV) + (uint32_t)ks * 2048, kKvHalfBytes, 1024), C::kIdescPV,
                       (j > 0 || ks > 0) ? 1u : 0u);
         umma_commit(bar_o);
       }
@@ -348,13 +356,13 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
           if (move) m_used = m_tile;
           l_run *= corr;
 #pragma unroll 1
-          for (int c = 0; c < 2; ++c) {                           // this half's 64 columns of O
+          for (int c = 0; c < D / 64; ++c) {                      // this half's D/2 columns of O
             uint32_t r[32];
-            tmem_ld32_issue(tO + lane_sel + ch_half * 64 + c * 32, r);
+            tmem_ld32_issue(tO + lane_sel + ch_half * (D / 2) + c * 32, r);
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
             for (int e = 0; e < 32; ++e) r[e] = __float_as_uint(__uint_as_float(r[e]) * corr);
-            tmem_st32(tO + lane_sel + ch_half * 64 + c * 32, r);
+            tmem_st32(tO + lane_sel + ch_half * (D / 2) + c * 32, r);
           }
         }
       }
@@ -389,8 +397,8 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
       // slots past the context end and of pages that were not loaded (reading S10)
       mbar_wait(bar_v, (uint32_t)j & 1);
       if (t0 + kKvTile > n) {
-        for (int e = tid; e < (t0 + kKvTile - n) * 16; e += 256) {
-          const int r = (n - t0) + e / 16, ch = e % 16;
+        for (int e = tid; e < (t0 + kKvTile - n) * (D / 8); e += 256) {
+          const int r = (n - t0) + e / (D / 8), ch = e % (D / 8);
           *reinterpret_cast<int4*>(sV + (ch >> 3) * kKvHalfBytes + r * 128 + (((ch & 7) ^ (r & 7)) << 4)) = make_int4(0, 0, 0, 0);
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -402,18 +410,18 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   mbar_wait(bar_o, (uint32_t)(nkv - 1) & 1);
   tc_fence_after();
 
-  // ---- epilogue: thread (row, ch_half) -> 64 columns of out[row_tok0 + row / G][g*G + row % G][:];
+  // ---- epilogue: thread (row, ch_half) -> D/2 columns of out[row_tok0 + row / G][g*G + row % G][:];
   // the two halves' row sums meet in shared memory
   {
     if (warp < kIssuer) lsum[ch_half * 128 + row] = l_run;
     __syncthreads();
     const float inv = 1.f / (lsum[row] + lsum[128 + row]);
     const bool store = warp < kIssuer && r0 + row / G < m;
-    __half* dst = p.out + ((size_t)(row_tok0 + row / G) * p.Hq + (size_t)(g * G + row % G)) * kD + ch_half * 64;
+    __half* dst = p.out + ((size_t)(row_tok0 + row / G) * p.Hq + (size_t)(g * G + row % G)) * D + ch_half * (D / 2);
 #pragma unroll 1
-    for (int c = 0; c < 2 && warp < kIssuer; ++c) {
+    for (int c = 0; c < D / 64 && warp < kIssuer; ++c) {
       uint32_t r[32];
-      tmem_ld32_issue(tO + lane_sel + ch_half * 64 + c * 32, r);
+      tmem_ld32_issue(tO + lane_sel + ch_half * (D / 2) + c * 32, r);
       asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
       if (store) {
 #pragma unroll
@@ -453,14 +461,16 @@ int encode_fn(EncodeTiledFn* out) {
 
 }  // namespace
 
-int launch_prefill(const PrefillArgs& a, cudaStream_t stream) {
+template <int D>
+static int launch_prefill_d(const PrefillArgs& a, cudaStream_t stream) {
+  constexpr int kSmem = PfCfg<D>::kSmem;
   DeviceInfo di;
   int rc = device_info(&di);
   if (rc) return rc;
   static bool attr_set[64] = {false};
   if (!attr_set[di.device]) {
     if (kSmem > di.max_smem_optin) HX_FAIL(HX_ERR_UNSUPPORTED, "device offers %d B shared memory per CTA, kernel needs %d", di.max_smem_optin, kSmem);
-    HX_CUDA_OK(cudaFuncSetAttribute(prefill_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem));
+    HX_CUDA_OK(cudaFuncSetAttribute(prefill_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem));
     attr_set[di.device] = true;
   }
   EncodeTiledFn enc;
@@ -473,8 +483,8 @@ int launch_prefill(const PrefillArgs& a, cudaStream_t stream) {
   CUtensorMap tq, tk, tv;
   {
     // K / V cache as [D/64 halves][rows][64]; box = one 64-wide half of one (page, head) tile
-    cuuint64_t dims[3] = {64, rows, (cuuint64_t)(kD / 64)};
-    cuuint64_t strides[2] = {(cuuint64_t)kD * 2, 128};
+    cuuint64_t dims[3] = {64, rows, (cuuint64_t)(D / 64)};
+    cuuint64_t strides[2] = {(cuuint64_t)D * 2, 128};
     cuuint32_t box[3] = {64, 16, 1};
     cuuint32_t es[3] = {1, 1, 1};
     for (int x = 0; x < 2; ++x) {
@@ -487,8 +497,8 @@ int launch_prefill(const PrefillArgs& a, cudaStream_t stream) {
   {
     // Q as [64][Hq heads][Tq tokens][D/64 halves]; box {64, G, 128/G, 1} lands as [token][head][128 B]:
     // row = token * G + head, the M order of the tile.  Tokens past the end read as zeros.
-    cuuint64_t dims[4] = {64, (cuuint64_t)a.q_heads, (cuuint64_t)a.total_q, (cuuint64_t)(kD / 64)};
-    cuuint64_t strides[3] = {(cuuint64_t)kD * 2, (cuuint64_t)a.q_heads * kD * 2, 128};
+    cuuint64_t dims[4] = {64, (cuuint64_t)a.q_heads, (cuuint64_t)a.total_q, (cuuint64_t)(D / 64)};
+    cuuint64_t strides[3] = {(cuuint64_t)D * 2, (cuuint64_t)a.q_heads * D * 2, 128};
     cuuint32_t box[4] = {64, (cuuint32_t)G, (cuuint32_t)(kRows / G), 1};
     cuuint32_t es[4] = {1, 1, 1, 1};
     CUresult r = enc(&tq, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 4, const_cast<void*>(a.q), dims, strides, box, es,
@@ -509,10 +519,14 @@ int launch_prefill(const PrefillArgs& a, cudaStream_t stream) {
     pb.B = (a.batch - b0 < 65535) ? a.batch - b0 : 65535;
     pb.bt = a.block_table + (size_t)b0 * a.bt_stride;
     pb.lens = a.seq_lens + b0; pb.qlens = a.q_lens + b0; pb.cuq = a.cu_q_lens + b0;
-    prefill_kernel<<<dim3(qtiles, a.kv_heads, pb.B), 320, kSmem, stream>>>(tq, tk, tv, pb);
+    prefill_kernel<D><<<dim3(qtiles, a.kv_heads, pb.B), 320, kSmem, stream>>>(tq, tk, tv, pb);
     HX_CUDA_OK(cudaGetLastError());
   }
   return HX_OK;
+}
+
+int launch_prefill(const PrefillArgs& a, cudaStream_t stream) {
+  return a.head_dim == 128 ? launch_prefill_d<128>(a, stream) : launch_prefill_d<64>(a, stream);
 }
 
 }  // namespace hx

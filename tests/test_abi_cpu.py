@@ -238,7 +238,7 @@ def _prefill(cache=None, **over):
     (dict(q_lens=0), B.HX_ERR_INVALID_ARG), (dict(cu_q_lens=0), B.HX_ERR_INVALID_ARG),
     (dict(max_q_len=65), B.HX_ERR_INVALID_ARG), (dict(max_q_len=101, max_seq_len=200, block_table_stride=13), B.HX_ERR_INVALID_ARG),
     (dict(block_table_stride=3), B.HX_ERR_INVALID_ARG), (dict(sm_scale=float("nan")), B.HX_ERR_INVALID_ARG),
-    (dict(cache=FakeCache(D=64)), B.HX_ERR_UNSUPPORTED), (dict(cache=FakeCache(ps=32)), B.HX_ERR_UNSUPPORTED),
+    (dict(cache=FakeCache(D=96)), B.HX_ERR_UNSUPPORTED), (dict(cache=FakeCache(ps=32)), B.HX_ERR_UNSUPPORTED),
 ])
 def test_prefill_rejects_invalid_arguments_without_launching(over, status):
     with pytest.raises(hx.HxError) as e:

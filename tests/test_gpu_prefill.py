@@ -20,14 +20,14 @@ def env():
     return hx, torch, oracle
 
 
-def run_prefill(env, cfgno, Hq, Hkv, lens, qlens, layers=1, layer=0, poison=False, sm_scale=0.0):
+def run_prefill(env, cfgno, Hq, Hkv, lens, qlens, layers=1, layer=0, poison=False, sm_scale=0.0, D=128):
     hx, torch, oracle = env
     lens = np.asarray(lens, dtype=np.int32)
     qlens = np.asarray(qlens, dtype=np.int32)
-    c = W.AttnConfig(cfgno, "t", len(lens), Hq, Hkv, 128, 8, "x")
+    c = W.AttnConfig(cfgno, "t", len(lens), Hq, Hkv, D, 8, "x")
     w = W.make_attention_inputs(c, lens=lens, layers=layers)
     Tq = int(qlens.sum())
-    q = W.draw_fp16_normal((Tq, Hq, 128), cfgno, 40)
+    q = W.draw_fp16_normal((Tq, Hq, D), cfgno, 40)
     k, v = w["k"], w["v"]
     if poison:                                   # slots past the context end and unowned pages: NaN / Inf
         kb, vb = k.view(np.uint16).copy(), v.view(np.uint16).copy()
@@ -97,3 +97,11 @@ def test_prefill_chunk_on_a_long_context_and_wide_group(env):
     G = 16 group (8 tokens x 16 heads per row tile)."""
     run_prefill(env, 75, 8, 1, [5000, 4097], [300, 1])
     run_prefill(env, 76, 16, 1, [700, 129, 33], [700, 129, 33])
+
+
+@pytest.mark.parametrize("G,Hkv", [(1, 4), (8, 1), (4, 2)])
+def test_prefill_head_dim_64(env, G, Hkv):
+    """head_dim 64 (the shape of BASELINE.json configs[0]): one 64-wide operand region instead of two."""
+    lens = [17, 64, 100, 255, 129, 300]
+    run_prefill(env, 80 + G, G * Hkv, Hkv, lens, lens, D=64)
+    run_prefill(env, 84 + G, G * Hkv, Hkv, [300, 64, 200], [44, 1, 200], D=64, poison=True)
