@@ -207,7 +207,8 @@ prefill_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   const int G = p.G, Hkv = p.Hkv;
   const int TQ = kRows / G;                          // query tokens per tile
   const int i = blockIdx.z, g = blockIdx.y;
-  const int n = __ldg(p.lens + i), m = __ldg(p.qlens + i);
+  const int n = max(__ldg(p.lens + i), 0);
+  const int m = min(__ldg(p.qlens + i), n);          // (q_lens > seq_lens breaks the contract: clamped, never a hang)
   const int qt = (int)gridDim.x - 1 - (int)blockIdx.x;   // heavy (late) tiles first
   if (qt * TQ >= m) return;
   const int r0 = qt * TQ;                            // first query token of the tile (within the request's m)
