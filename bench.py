@@ -185,6 +185,7 @@ def run_hx(args, rank, world, local_rank):
     import paper_2502_07903_b200 as hx
 
     torch.cuda.set_device(local_rank)
+    torch.manual_seed(1234 + rank)                 # every device-side draw below (K/V/Q fills of the extras) is seeded
     dev = torch.device("cuda", local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
