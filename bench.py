@@ -12,6 +12,13 @@ batch (64 q / 8 kv heads, head_dim 128).  Inputs are seeded synthetic data (work
 Prints ONE JSON line (rank 0).  `value` = (attention KV bytes + ingest read+write bytes) per
 step x K / device time, inputs resident in HBM.  N > 1 (torchrun): independent replicas, one per
 GPU, no collective on the data path ("replicas only"); value sums over ranks.
+
+Beside the contract keys (roofline, e2e, cpu_baseline, clocks, gpu_launches) the line carries:
+`two_stream` (the step with the ingest on a side stream), `cuda_graph` (the single-stream step replayed as
+a CUDA graph), `e2e.*` (hx_decode_step_host from pinned host buffers: handoff overlapped / in order / pulled
+by the kernel over PCIe) and `other_configs`: configs[1], [2] (attention) and [3] (80-layer ingest) kernel-only,
+`prefill` (hx_prefill_attention against the tensor roofline), `append_cfg5` (fused append + attention) and
+`stream_peaks` (read-only / write-only HBM rates of the run).
 """
 from __future__ import annotations
 
