@@ -48,7 +48,7 @@
 extern "C" {
 #endif
 
-#define HX_VERSION 121 /* 0.1.2.1: + stage ingest, append, fused append-attend, pull mode, prefill attention, overlapped handoff */
+#define HX_VERSION 122 /* 0.1.2.1: + stage ingest, append, fused append-attend, pull mode, prefill attention, overlapped handoff */
 
 typedef enum {
   HX_OK = 0,
@@ -197,6 +197,21 @@ int hx_decode_attention(void* out, const void* q,
                         int32_t batch, int32_t max_seq_len, float sm_scale,
                         void* workspace, size_t workspace_bytes,
                         void* stream);
+
+/* hx_decode_attention that may OVERLAP the kernel enqueued just before it on `stream` (
+ * PAPER.md:L110 "asynchronous ... to enable overlapping between computation and communication").  Same arguments
+ * and result as hx_decode_attention.  The grid is launched as a programmatic dependent of the preceding kernel:
+ * if that kernel is hx_kv_ingest's (which signals its dependents at once) the attention starts while the handoff
+ * is still landing; after any other kernel it starts when that kernel ends, as usual.  The CALLER asserts that
+ * this call reads nothing the preceding kernel writes — the step's new prompts live in pages disjoint from the
+ * active batch's.  Work enqueued after this call is ordered after both kernels. */
+int hx_decode_attention_overlapped(void* out, const void* q,
+                                   const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
+                                   const int32_t* block_table, int32_t block_table_stride,
+                                   const int32_t* seq_lens,
+                                   int32_t batch, int32_t max_seq_len, float sm_scale,
+                                   void* workspace, size_t workspace_bytes,
+                                   void* stream);
 
 /* Fused append-then-attend (F1): the same result, bit for bit, in the cache AND in `out`, as
  * hx_kv_append(k_new, v_new, ...) followed by hx_decode_attention(...), in ONE launch: the warp

@@ -17,7 +17,7 @@ EXPORTS = [
     "hx_pool_shuffle", "hx_pool_alloc", "hx_pool_free", "hx_pool_num_free", "hx_pool_num_pages",
     "hx_pool_alloc_table", "hx_pool_destroy", "hx_decode_step_host", "hx_tune_sm_rates",
     "hx_kv_ingest_stage", "hx_stage_overlap", "hx_kv_append", "hx_decode_attention_append",
-    "hx_prefill_attention",
+    "hx_prefill_attention", "hx_decode_attention_overlapped",
 ]
 
 
@@ -119,6 +119,9 @@ def lib() -> C.CDLL:
             L.hx_prefill_attention.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CCache), C.c_int32, C.c_int32,
                                                C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
                                                C.c_int32, C.c_int32, C.c_int32, C.c_float, C.c_void_p]
+        if not os.environ.get("HX_LIB") or hasattr(L, "hx_decode_attention_overlapped"):
+            L.hx_decode_attention_overlapped.restype = C.c_int
+            L.hx_decode_attention_overlapped.argtypes = L.hx_decode_attention.argtypes
         L.hx_decode_step_host.restype = C.c_int
         L.hx_decode_step_host.argtypes = [C.POINTER(_CStepArgs), C.c_void_p]
         _lib = L
@@ -275,6 +278,17 @@ def decode_attention(out, q, cache: PagedCache, *, layer, q_heads, block_table, 
     _check(lib().hx_decode_attention(_ptr(out), _ptr(q), cache.ref, layer, q_heads, _ptr(block_table),
                                      block_table_stride, _ptr(seq_lens), batch, max_seq_len,
                                      C.c_float(sm_scale), _ptr(workspace), workspace_bytes, _stream_ptr(stream)))
+
+
+def decode_attention_overlapped(out, q, cache: PagedCache, *, layer, q_heads, block_table, block_table_stride, seq_lens,
+                                batch, max_seq_len, sm_scale=0.0, workspace=None, workspace_bytes=None, stream=None):
+    """hx_decode_attention_overlapped: may overlap the kernel enqueued just before it (see include/hx.h)."""
+    if workspace_bytes is None:
+        workspace_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    _check(lib().hx_decode_attention_overlapped(_ptr(out), _ptr(q), cache.ref, layer, q_heads, _ptr(block_table),
+                                                block_table_stride, _ptr(seq_lens), batch, max_seq_len,
+                                                C.c_float(sm_scale), _ptr(workspace), workspace_bytes,
+                                                _stream_ptr(stream)))
 
 
 def tune_sm_rates(scratch=None, scratch_bytes=None, stream=None):

@@ -897,7 +897,20 @@ int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream
     p.v_new = APPEND ? static_cast<const __half*>(a.v_new) + (size_t)b0 * a.kv_heads * D : nullptr;
     p.kc = static_cast<__half*>(const_cast<void*>(a.k_base)) + layer_elems * a.layer;
     p.vc = static_cast<__half*>(const_cast<void*>(a.v_base)) + layer_elems * a.layer;
-    attn_stream_kernel<D, NT, APPEND><<<grid, kWarps * 32, C::kSmem, stream>>>(tk, tv, p);
+    if (a.overlap_prev && b0 == 0) {
+      // programmatic dependent launch: this grid may start while the preceding kernel of the stream (one that has
+      // executed griddepcontrol.launch_dependents, e.g. hx_kv_ingest's) is still running.  The kernel never waits
+      // on it: the caller asserted that it reads nothing that kernel writes.
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kWarps * 32); cfg.dynamicSmemBytes = C::kSmem; cfg.stream = stream;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+      at[0].val.programmaticStreamSerializationAllowed = 1;
+      cfg.attrs = at; cfg.numAttrs = 1;
+      HX_CUDA_OK(cudaLaunchKernelEx(&cfg, attn_stream_kernel<D, NT, APPEND>, tk, tv, p));
+    } else {
+      attn_stream_kernel<D, NT, APPEND><<<grid, kWarps * 32, C::kSmem, stream>>>(tk, tv, p);
+    }
     HX_CUDA_OK(cudaGetLastError());
   }
   return HX_OK;

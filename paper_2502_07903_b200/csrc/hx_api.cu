@@ -176,7 +176,7 @@ size_t hx_decode_attention_workspace_bytes(int32_t batch, int32_t q_heads, int32
   return hx::attn_workspace_bytes(batch, q_heads, kv_heads, head_dim, max_seq_len, page_size);
 }
 
-static int attention_common(const char* who, void* out, const void* q, const void* k_new, const void* v_new, bool append,
+static int attention_common(const char* who, void* out, const void* q, const void* k_new, const void* v_new, bool append, bool overlap,
                             const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
                             const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
                             int32_t batch, int32_t max_seq_len, float sm_scale, void* workspace,
@@ -216,6 +216,7 @@ static int attention_common(const char* who, void* out, const void* q, const voi
   p.page_size = cache->page_size; p.num_pages = cache->num_pages; p.bt_stride = block_table_stride;
   p.max_seq_len = max_seq_len; p.sm_scale = sm_scale;
   p.k_new = append ? k_new : nullptr; p.v_new = append ? v_new : nullptr;
+  p.overlap_prev = overlap ? 1 : 0;
   return launch_attention(p, static_cast<cudaStream_t>(stream));
 }
 
@@ -223,7 +224,7 @@ int hx_decode_attention(void* out, const void* q, const hx_paged_cache* cache, i
                         const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
                         int32_t batch, int32_t max_seq_len, float sm_scale, void* workspace,
                         size_t workspace_bytes, void* stream) {
-  return attention_common("hx_decode_attention", out, q, nullptr, nullptr, false, cache, layer, q_heads, block_table,
+  return attention_common("hx_decode_attention", out, q, nullptr, nullptr, false, false, cache, layer, q_heads, block_table,
                           block_table_stride, seq_lens, batch, max_seq_len, sm_scale, workspace, workspace_bytes, stream);
 }
 
@@ -232,8 +233,17 @@ int hx_decode_attention_append(void* out, const void* q, const void* k_new, cons
                                const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
                                int32_t batch, int32_t max_seq_len, float sm_scale, void* workspace,
                                size_t workspace_bytes, void* stream) {
-  return attention_common("hx_decode_attention_append", out, q, k_new, v_new, true, cache, layer, q_heads, block_table,
+  return attention_common("hx_decode_attention_append", out, q, k_new, v_new, true, false, cache, layer, q_heads, block_table,
                           block_table_stride, seq_lens, batch, max_seq_len, sm_scale, workspace, workspace_bytes, stream);
+}
+
+int hx_decode_attention_overlapped(void* out, const void* q, const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
+                                   const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
+                                   int32_t batch, int32_t max_seq_len, float sm_scale, void* workspace,
+                                   size_t workspace_bytes, void* stream) {
+  return attention_common("hx_decode_attention_overlapped", out, q, nullptr, nullptr, false, true, cache, layer, q_heads,
+                          block_table, block_table_stride, seq_lens, batch, max_seq_len, sm_scale, workspace,
+                          workspace_bytes, stream);
 }
 
 int hx_kv_append(const void* k_new, const void* v_new, const hx_paged_cache* cache, int32_t layer,

@@ -65,6 +65,7 @@ struct AttnParams {
   float sm_scale;
   const void* k_new;              // fused append (hx_decode_attention_append); NULL otherwise
   const void* v_new;
+  int32_t overlap_prev;           // launch as a programmatic dependent of the preceding kernel (hx_decode_attention_overlapped)
 };
 size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, int32_t head_dim,
                             int32_t max_seq_len, int32_t page_size);

@@ -42,6 +42,9 @@ template <int D, bool GATHER>
 __global__ void __launch_bounds__(kThreads) ingest_rows_kernel(const __grid_constant__ IngestParams p, int layer_splits) {
   constexpr int CH = D / 8;                 // 16-byte chunks per row
   constexpr int TOK = kThreads / CH;        // packed tokens per CTA tile
+  // a kernel launched as a programmatic dependent of this one (hx_decode_attention_overlapped) may start now;
+  // without such a launch this is a no-op
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const int dc = threadIdx.x % CH;
   const int tk = blockIdx.x * TOK + threadIdx.x / CH;
   if (tk >= p.total_tokens) return;

@@ -341,3 +341,48 @@ def test_decode_step_in_a_cuda_graph(env):
         assert np.array_equal(dev_u16(cache.k), ok) and np.array_equal(dev_u16(cache.v), ov), rep
         max_abs, rel = attn_errors(out.cpu().numpy(), ref)
         assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (rep, max_abs, rel)
+
+
+def test_attention_overlapped_with_the_ingest_before_it(env):
+    """hx_decode_attention_overlapped right after hx_kv_ingest on one stream: the attention may start while the
+    ingest is still landing (programmatic dependent launch).  The new prompts' pages are disjoint from the
+    batch's, so both results must be the oracle's; a copy enqueued afterwards sees both finished.  Repeated so
+    that the overlap really happens in some iterations."""
+    hx, torch, oracle = env
+    Hkv, D, Hq = 4, 128, 32
+    ca = W.AttnConfig(86, "t", 8, Hq, Hkv, D, 256, "x")
+    wa = W.make_attention_inputs(ca, lens=np.array([3000, 100, 257, 1600, 16, 2222, 900, 64], dtype=np.int32), spare=2.5)
+    ci = W.IngestConfig(86, "t", 1, Hkv, D, 2, 1, 3, "x")
+    ilens = np.array([1024, 2000, 128], dtype=np.int32)
+    wi = W.make_ingest_inputs(ci, lens=ilens, bits=True)
+    used = wa["block_table"][wa["block_table"] >= 0]
+    free = np.setdiff1d(np.arange(wa["num_pages"]), used)
+    ibt = np.full((3, 128), -1, dtype=np.int32)
+    o = 0
+    for r, n in enumerate(ilens):
+        k = (n + 15) // 16
+        ibt[r, :k] = free[o:o + k]
+        o += k
+    ref_out = oracle.decode_attention(wa["q"], wa["k"], wa["v"], wa["block_table"], wa["seq_lens"])
+    ok, ov = wa["k"].view(np.uint16).copy(), wa["v"].view(np.uint16).copy()
+    oracle.kv_ingest(wi["src_k"], wi["src_v"], ok, ov, heads=Hkv, src_tp=2, dst_tp=1, dst_rank=0, block_table=ibt,
+                     cu_seqlens=wi["cu_seqlens"], seq_lens=ilens)
+    sk = [to_dev(a, torch) for a in wi["src_k"]]; sv = [to_dev(a, torch) for a in wi["src_v"]]
+    bt_i, cu_i, sl_i = torch.from_numpy(ibt).cuda(), torch.from_numpy(wi["cu_seqlens"]).cuda(), torch.from_numpy(ilens).cuda()
+    abt, asl = torch.from_numpy(wa["block_table"]).cuda(), torch.from_numpy(wa["seq_lens"]).cuda()
+    qd = to_dev(wa["q"], torch)
+    wsb = hx.decode_attention_workspace_bytes(8, Hq, Hkv, D, 3000)
+    ws = torch.zeros(wsb, dtype=torch.uint8, device="cuda")
+    for rep in range(4):
+        cache = hx.PagedCache(to_dev(wa["k"], torch), to_dev(wa["v"], torch))
+        out = torch.full_like(qd, float("nan"))
+        hx.kv_ingest(sk, sv, layers=1, heads=Hkv, head_dim=D, src_tp=2, dst_tp=1, dst_rank=0, dst=cache, block_table=bt_i,
+                     block_table_stride=128, cu_seqlens=cu_i, seq_lens=sl_i, batch=3, total_tokens=int(ilens.sum()),
+                     max_seq_len=2000)
+        hx.decode_attention_overlapped(out, qd, cache, layer=0, q_heads=Hq, block_table=abt, block_table_stride=abt.shape[1],
+                                       seq_lens=asl, batch=8, max_seq_len=3000, workspace=ws)
+        k_after = cache.k.clone()                    # stream-ordered after BOTH kernels
+        torch.cuda.synchronize()
+        assert np.array_equal(dev_u16(k_after), ok) and np.array_equal(dev_u16(cache.v), ov), rep
+        max_abs, rel = attn_errors(out.cpu().numpy(), ref_out)
+        assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (rep, max_abs, rel)
