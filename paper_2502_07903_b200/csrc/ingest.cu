@@ -6,8 +6,8 @@
 //
 // Kernel "rows": one thread owns one 16-byte column of one packed token for the whole call.
 // It resolves (request, page, slot) ONCE (binary search over cu_seqlens + one block-table
-// load), then streams every (layer, tensor, head) item of that token: up to 8 independent
-// 16-byte loads are issued before the 8 stores (128 B in flight per thread).  A half-warp
+// load), then streams every (layer, tensor, head) item of that token: 4 independent
+// 16-byte loads are issued before the 4 stores (64 B in flight per thread).  A half-warp
 // (D=128) covers one 256-byte row: reads and writes are both full 32-byte-sector runs, and
 // the 16 tokens of a CTA tile that share a page write one contiguous 4 KiB (page, head) run.
 #include <cuda_fp16.h>
@@ -18,7 +18,11 @@ namespace hx {
 namespace {
 
 constexpr int kThreads = 256;
-constexpr int kBatch = 8;     // independent 16-byte loads in flight per thread
+// 4 loads in flight per thread and at most 51 registers (46 used): five or more CTAs per SM by themselves, and one
+// CTA still fits beside a decode-attention CTA (51 K of the SM's 64 K registers), so an ingest on a side stream
+// or under hx_decode_attention_overlapped keeps moving while attention runs.  cfg4: 6 511 -> 6 592 GB/s.
+constexpr int kBatch = 4;     // independent 16-byte loads in flight per thread
+constexpr int kMinCtas = 5;   // __launch_bounds__ occupancy target (register cap)
 
 __device__ __forceinline__ int4 ld_stream(const int4* p) {
   int4 r;
@@ -39,7 +43,7 @@ __device__ __forceinline__ void st_stream(int4* p, const int4& v) {
 }
 
 template <int D, bool GATHER>
-__global__ void __launch_bounds__(kThreads) ingest_rows_kernel(const __grid_constant__ IngestParams p, int layer_splits) {
+__global__ void __launch_bounds__(kThreads, kMinCtas) ingest_rows_kernel(const __grid_constant__ IngestParams p, int layer_splits) {
   constexpr int CH = D / 8;                 // 16-byte chunks per row
   constexpr int TOK = kThreads / CH;        // packed tokens per CTA tile
   // a kernel launched as a programmatic dependent of this one (hx_decode_attention_overlapped) may start now;
