@@ -505,7 +505,7 @@ def run_hx(args, rank, world, local_rank):
 
 
 LAUNCHES_PER_STEP = 2          # ingest rows kernel + attention stream kernel (merge is in-kernel)
-NCU_TRAFFIC_BYTES = 2348147000  # dram read+write bytes per attention launch, ncu --set full (profiles/r01_launches_v5.md)
+NCU_TRAFFIC_BYTES = 2348367000  # dram read+write bytes per attention launch, ncu --set full (profiles/r01_launches_v6.md)
 
 
 def time_kernel(torch, fn, iters=20, warm=5):
