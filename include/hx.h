@@ -10,9 +10,14 @@
  * Conventions (all entry points)
  *  - Payload is IEEE fp16 (B_type = 2).  fp32 accumulation inside attention.
  *  - DEVICE pointers are marked "device"; everything else is host memory.  The caller owns all
- *    device memory, including the workspace.  The library allocates no device memory; its only
- *    device state is the optional SM rate table of hx_tune_sm_rates (a static __device__ array).
- *    hx_page_pool is the only heap object (host).
+ *    device memory, including the workspace.  The library allocates no device memory.  Its state:
+ *    (1) the optional SM rate table of hx_tune_sm_rates (a static __device__ array); (2) per device, one
+ *    side stream and two events, created by the first hx_decode_step / hx_decode_step_host call that
+ *    asks for an overlapped handoff and destroyed by hx_shutdown(); (3) host-side caches of device
+ *    properties and TMA descriptors.  hx_page_pool is the only heap object the caller owns (host).
+ *  - Thread safety: every entry point may be called from several host threads (on different streams);
+ *    hx_decode_step* serialise on one library mutex while they enqueue.  An hx_page_pool and an attention
+ *    workspace each serve one caller at a time.
  *  - hx_kv_ingest / hx_kv_gather / hx_decode_attention only ENQUEUE work on `stream`
  *    (a cudaStream_t passed as void*, NULL = legacy default stream) and return.  They never
  *    synchronise and never read device memory from the host; this is why sizes that only
@@ -48,7 +53,7 @@
 extern "C" {
 #endif
 
-#define HX_VERSION 122 /* 0.1.2.1: + stage ingest, append, fused append-attend, pull mode, prefill attention, overlapped handoff */
+#define HX_VERSION 130 /* 0.1.3.0: + hx_decode_step (device buffers), hx_shutdown; overlapped launch waits for the ingest */
 
 typedef enum {
   HX_OK = 0,
@@ -56,7 +61,7 @@ typedef enum {
   HX_ERR_UNSUPPORTED = 2, /* head_dim not in {64,128}; page_size != 16; group size not in {1,2,4,8,16}; tp > heads */
   HX_ERR_WORKSPACE = 3,   /* workspace NULL or smaller than hx_decode_attention_workspace_bytes() */
   HX_ERR_CUDA = 4,        /* a CUDA call failed; text in hx_last_error() */
-  HX_ERR_NO_PAGES = 5     /* hx_pool_alloc: not enough free pages; nothing was taken */
+  HX_ERR_NO_PAGES = 5     /* hx_pool_alloc: not enough free pages, nothing was taken; hx_pool_create: out of host memory */
 } hx_status;
 
 int hx_version(void);
@@ -198,13 +203,16 @@ int hx_decode_attention(void* out, const void* q,
                         void* workspace, size_t workspace_bytes,
                         void* stream);
 
-/* hx_decode_attention that may OVERLAP the kernel enqueued just before it on `stream` (
- * PAPER.md:L110 "asynchronous ... to enable overlapping between computation and communication").  Same arguments
- * and result as hx_decode_attention.  The grid is launched as a programmatic dependent of the preceding kernel:
- * if that kernel is hx_kv_ingest's (which signals its dependents at once) the attention starts while the handoff
- * is still landing; after any other kernel it starts when that kernel ends, as usual.  The CALLER asserts that
- * this call reads nothing the preceding kernel writes — the step's new prompts live in pages disjoint from the
- * active batch's.  Work enqueued after this call is ordered after both kernels. */
+/* hx_decode_attention that may OVERLAP the hx_kv_ingest enqueued just before it on `stream` (SURVEY.md §8(a) row
+ * A9; "asynchronous ... to enable overlapping between computation and communication").  Same
+ * arguments and result as hx_decode_attention.  When the LAST library call of this host thread was a launching
+ * hx_kv_ingest / hx_kv_ingest_stage on the same `stream`, and the caller enqueued nothing on `stream` in between
+ * (precondition), the grid is launched as a programmatic dependent of the ingest kernel (which signals its
+ * dependents at once) and starts while the handoff is still landing; every CTA executes griddepcontrol.wait before
+ * it exits, so the grid completes only after the ingest has completed and its writes are visible: work enqueued
+ * after this call is ordered after BOTH kernels.  In every other case (ingest of an empty batch, another call in
+ * between, another thread or stream) this is exactly hx_decode_attention.  The CALLER asserts that this call
+ * reads nothing the ingest writes: the step's new prompts live in pages disjoint from the active batch's. */
 int hx_decode_attention_overlapped(void* out, const void* q,
                                    const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
                                    const int32_t* block_table, int32_t block_table_stride,
@@ -274,6 +282,42 @@ int     hx_pool_alloc_table(hx_page_pool* pool, const int32_t* seq_lens, int32_t
                             int32_t page_size, int32_t* block_table, int32_t stride);
 void    hx_pool_destroy(hx_page_pool* pool);
 
+/* ---- whole decode step on DEVICE buffers (bench.py's timed step) --------
+ * KV cache communication is asynchronous "to enable overlapping between computation and
+ * communication".  One call = hx_kv_ingest of the step's new prompts (ing_* arguments; skipped when
+ * ing_batch == 0) + hx_decode_attention over the active batch (skipped when batch == 0).  Every argument means
+ * what it means in those two calls.  overlap_ingest != 0: the caller asserts that the attention does NOT read
+ * the pages this step ingests (the new prompts join the batch in a later step); the ingest then runs on a
+ * library-owned side stream, forked from `stream` at entry (so it sees everything enqueued on `stream` so
+ * far, e.g. the upload of ing_block_table) and joined to `stream` before return, on every path: work enqueued
+ * on `stream` afterwards is ordered after both kernels.  overlap_ingest == 0: both in order on `stream`.
+ * Every host-side check of both calls runs first; nothing is enqueued unless all pass.  Capturable in a CUDA
+ * graph (the fork/join is the standard event pattern). */
+typedef struct {
+  /* attention over the active batch (hx_decode_attention) */
+  void*       out;               /* device fp16 [batch][q_heads][head_dim] */
+  const void* q;                 /* device fp16 [batch][q_heads][head_dim] */
+  const hx_paged_cache* cache;
+  int32_t layer, q_heads;
+  const int32_t* block_table; int32_t block_table_stride;   /* device */
+  const int32_t* seq_lens;       /* device [batch] */
+  int32_t batch, max_seq_len;
+  float sm_scale;
+  void* workspace; size_t workspace_bytes;
+  /* handoff of the step's new prompts (hx_kv_ingest into `cache`, layers [0, ing_layers)) */
+  const void* const* src_k; const void* const* src_v;       /* host arrays of src_tp device pointers */
+  int32_t ing_layers, heads, src_tp, dst_tp, dst_rank;
+  const int32_t* ing_block_table; int32_t ing_block_table_stride;   /* device [ing_batch][stride] */
+  const int32_t* ing_cu_seqlens;  const int32_t* ing_seq_lens;      /* device */
+  int32_t ing_batch, ing_total_tokens, ing_max_seq_len;
+  int32_t overlap_ingest;
+} hx_step_args;
+int hx_decode_step(const hx_step_args* args, void* stream);
+
+/* Destroys the library-owned side streams and events of every device (after synchronising them).  Optional:
+ * call when no hx_decode_step* call is in flight; a later call re-creates them. */
+int hx_shutdown(void);
+
 /* ---- whole decode step with HOST inputs (bench.py "e2e") --------
  * Copies q, the new prompts' block-table rows / lengths and the source shards from (pinned)
  * host memory to caller-provided device staging buffers, runs hx_kv_ingest for the new
@@ -309,8 +353,9 @@ typedef struct {
   /* non-zero = the step's attention does NOT read the pages this step ingests (the new prompts join the
    * batch later; "asynchronous ... to enable overlapping between computation and
    * communication"): the shard transfer + ingest run on a library-owned side stream, forked from `stream`
-   * at entry and joined to it before return, so PCIe and the ingest overlap the attention.  0 = everything
-   * in order on `stream` (the attention may read the freshly ingested pages). */
+   * at entry and joined to it before return (on every path, errors included), so PCIe and the ingest overlap
+   * the attention.  0 = everything in order on `stream` (the attention may read the freshly ingested pages).
+   * As in hx_decode_step, every host-side check runs before anything is enqueued. */
   int32_t overlap_ingest;
 } hx_step_host_args;
 int hx_decode_step_host(const hx_step_host_args* args, void* stream);

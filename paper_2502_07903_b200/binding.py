@@ -6,7 +6,7 @@ import os
 from typing import Optional, Sequence
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.environ.get("HX_LIB") or os.path.join(_HERE, "libhx.so")   # HX_LIB: load another build (A/B timing)
+_SO = os.path.join(_HERE, "libhx.so")
 
 HX_OK, HX_ERR_INVALID_ARG, HX_ERR_UNSUPPORTED, HX_ERR_WORKSPACE, HX_ERR_CUDA, HX_ERR_NO_PAGES = range(6)
 
@@ -17,7 +17,7 @@ EXPORTS = [
     "hx_pool_shuffle", "hx_pool_alloc", "hx_pool_free", "hx_pool_num_free", "hx_pool_num_pages",
     "hx_pool_alloc_table", "hx_pool_destroy", "hx_decode_step_host", "hx_tune_sm_rates",
     "hx_kv_ingest_stage", "hx_stage_overlap", "hx_kv_append", "hx_decode_attention_append",
-    "hx_prefill_attention", "hx_decode_attention_overlapped",
+    "hx_prefill_attention", "hx_decode_attention_overlapped", "hx_decode_step", "hx_shutdown",
 ]
 
 
@@ -48,6 +48,21 @@ class _CStepArgs(C.Structure):
         ("ing_block_table_dev", C.c_void_p), ("ing_cu_seqlens_dev", C.c_void_p), ("ing_seq_lens_dev", C.c_void_p),
         ("ing_batch", C.c_int32), ("ing_total_tokens", C.c_int32), ("ing_max_seq_len", C.c_int32),
         ("pull_src", C.c_int32), ("overlap_ingest", C.c_int32),
+    ]
+
+
+class _CStepDevArgs(C.Structure):
+    _fields_ = [
+        ("out", C.c_void_p), ("q", C.c_void_p), ("cache", C.POINTER(_CCache)), ("layer", C.c_int32), ("q_heads", C.c_int32),
+        ("block_table", C.c_void_p), ("block_table_stride", C.c_int32), ("seq_lens", C.c_void_p),
+        ("batch", C.c_int32), ("max_seq_len", C.c_int32), ("sm_scale", C.c_float),
+        ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
+        ("src_k", C.POINTER(C.c_void_p)), ("src_v", C.POINTER(C.c_void_p)),
+        ("ing_layers", C.c_int32), ("heads", C.c_int32), ("src_tp", C.c_int32), ("dst_tp", C.c_int32), ("dst_rank", C.c_int32),
+        ("ing_block_table", C.c_void_p), ("ing_block_table_stride", C.c_int32),
+        ("ing_cu_seqlens", C.c_void_p), ("ing_seq_lens", C.c_void_p),
+        ("ing_batch", C.c_int32), ("ing_total_tokens", C.c_int32), ("ing_max_seq_len", C.c_int32),
+        ("overlap_ingest", C.c_int32),
     ]
 
 
@@ -97,33 +112,32 @@ def lib() -> C.CDLL:
         L.hx_pool_alloc_table.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32]
         L.hx_pool_destroy.restype = None
         L.hx_pool_destroy.argtypes = [C.c_void_p]
-        if not os.environ.get("HX_LIB") or hasattr(L, "hx_tune_sm_rates"):   # older A/B builds lack it
-            L.hx_tune_sm_rates.restype = C.c_int
-            L.hx_tune_sm_rates.argtypes = [C.c_void_p, C.c_size_t, C.c_void_p]
-        if not os.environ.get("HX_LIB") or hasattr(L, "hx_kv_append"):
-            L.hx_kv_ingest_stage.restype = C.c_int
-            L.hx_kv_ingest_stage.argtypes = [C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)] + [C.c_int32] * 9 + [
-                C.POINTER(_CCache), C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32,
-                C.c_void_p]
-            L.hx_stage_overlap.restype = C.c_int
-            L.hx_stage_overlap.argtypes = [C.c_int32] * 4 + [C.POINTER(C.c_int32)] * 3
-            L.hx_kv_append.restype = C.c_int
-            L.hx_kv_append.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CCache), C.c_int32, C.c_void_p, C.c_int32,
-                                       C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
-            L.hx_decode_attention_append.restype = C.c_int
-            L.hx_decode_attention_append.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(_CCache),
-                                                     C.c_int32, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_int32,
-                                                     C.c_int32, C.c_float, C.c_void_p, C.c_size_t, C.c_void_p]
-        if not os.environ.get("HX_LIB") or hasattr(L, "hx_prefill_attention"):
-            L.hx_prefill_attention.restype = C.c_int
-            L.hx_prefill_attention.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CCache), C.c_int32, C.c_int32,
-                                               C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
-                                               C.c_int32, C.c_int32, C.c_int32, C.c_float, C.c_void_p]
-        if not os.environ.get("HX_LIB") or hasattr(L, "hx_decode_attention_overlapped"):
-            L.hx_decode_attention_overlapped.restype = C.c_int
-            L.hx_decode_attention_overlapped.argtypes = L.hx_decode_attention.argtypes
+        L.hx_tune_sm_rates.restype = C.c_int
+        L.hx_tune_sm_rates.argtypes = [C.c_void_p, C.c_size_t, C.c_void_p]
+        L.hx_kv_ingest_stage.restype = C.c_int
+        L.hx_kv_ingest_stage.argtypes = [C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)] + [C.c_int32] * 9 + [
+            C.POINTER(_CCache), C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32,
+            C.c_void_p]
+        L.hx_stage_overlap.restype = C.c_int
+        L.hx_stage_overlap.argtypes = [C.c_int32] * 4 + [C.POINTER(C.c_int32)] * 3
+        L.hx_kv_append.restype = C.c_int
+        L.hx_kv_append.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CCache), C.c_int32, C.c_void_p, C.c_int32,
+                                   C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
+        L.hx_decode_attention_append.restype = C.c_int
+        L.hx_decode_attention_append.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(_CCache),
+                                                 C.c_int32, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_int32,
+                                                 C.c_int32, C.c_float, C.c_void_p, C.c_size_t, C.c_void_p]
+        L.hx_prefill_attention.restype = C.c_int
+        L.hx_prefill_attention.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CCache), C.c_int32, C.c_int32,
+                                           C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
+                                           C.c_int32, C.c_int32, C.c_int32, C.c_float, C.c_void_p]
+        L.hx_decode_attention_overlapped.restype = C.c_int
+        L.hx_decode_attention_overlapped.argtypes = L.hx_decode_attention.argtypes
         L.hx_decode_step_host.restype = C.c_int
         L.hx_decode_step_host.argtypes = [C.POINTER(_CStepArgs), C.c_void_p]
+        L.hx_decode_step.restype = C.c_int
+        L.hx_decode_step.argtypes = [C.POINTER(_CStepDevArgs), C.c_void_p]
+        L.hx_shutdown.restype = C.c_int
         _lib = L
     return _lib
 
@@ -301,19 +315,16 @@ def tune_sm_rates(scratch=None, scratch_bytes=None, stream=None):
     _check(lib().hx_tune_sm_rates(_ptr(scratch), scratch_bytes, _stream_ptr(stream)))
 
 
-def decode_step_host(**kw):
-    """hx_decode_step_host: one whole decode step from HOST buffers (see hx_step_host_args).
-    Keyword names are the struct's field names; `cache` is a PagedCache; src_* are lists."""
-    a = _CStepArgs()
+def _fill_struct(a, kw):
+    """Keyword names are the struct's field names; `cache` is a PagedCache; src_* are lists of tensors."""
     keep = []
-    stream = kw.pop("stream", None)
-    for name, ctype in _CStepArgs._fields_:
+    for name, ctype in a._fields_:
         if name not in kw:
             continue
         val = kw.pop(name)
         if name == "cache":
             a.cache = C.pointer(val.c)
-        elif name in ("src_k_host", "src_v_host", "src_k_dev", "src_v_dev"):
+        elif ctype is C.POINTER(C.c_void_p):
             arr = _ptr_array(val)
             keep.append(arr)
             setattr(a, name, arr)
@@ -322,7 +333,38 @@ def decode_step_host(**kw):
         else:
             setattr(a, name, val)
     assert not kw, f"unknown fields: {list(kw)}"
+    return keep
+
+
+def decode_step_host(**kw):
+    """hx_decode_step_host: one whole decode step from HOST buffers (see hx_step_host_args)."""
+    a = _CStepArgs()
+    stream = kw.pop("stream", None)
+    keep = _fill_struct(a, kw)
     _check(lib().hx_decode_step_host(C.byref(a), _stream_ptr(stream)))
+    del keep
+
+
+class DecodeStep:
+    """hx_decode_step with its argument struct built once (the per-step host cost is then one ctypes call).
+    Keyword names are hx_step_args' field names."""
+
+    def __init__(self, **kw):
+        self.a = _CStepDevArgs()
+        self._keep = _fill_struct(self.a, dict(kw))
+        self._refs = kw                      # keeps the tensors behind the raw pointers alive
+
+    def __call__(self, stream=None):
+        _check(lib().hx_decode_step(C.byref(self.a), _stream_ptr(stream)))
+
+
+def decode_step(stream=None, **kw):
+    """hx_decode_step (include/hx.h): ingest of the step's new prompts + attention over the active batch."""
+    DecodeStep(**kw)(stream)
+
+
+def shutdown():
+    _check(lib().hx_shutdown())
 
 
 class PagePool:

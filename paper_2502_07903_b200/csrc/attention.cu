@@ -24,14 +24,9 @@
 //  * APPEND (hx_decode_attention_append): the warp that streams the
 //    last page of a (request, kv head) overlays the step's new K/V row on the tile in shared memory
 //    and stores it to the page, so the decode step needs no separate append launch.
-//
-// attn_simple_kernel — one CTA per (request, q head) on CUDA cores; bring-up/debug only
-// (HX_ATTN_IMPL=simple).
 #include <cuda.h>
 #include <cuda_fp16.h>
 
-#include <cstdlib>
-#include <cstring>
 #include <mutex>
 
 #include "hx_internal.h"
@@ -75,6 +70,10 @@ struct StreamParams {
   const __half* v_new;
   __half* kc;
   __half* vc;
+  // hx_decode_attention_overlapped: this grid was launched as a programmatic dependent of the ingest kernel and
+  // reads nothing that kernel writes; every CTA executes griddepcontrol.wait before it exits, so completion of this
+  // grid implies completion (and visibility) of the ingest
+  int32_t pdl_wait_at_end;
 };
 
 // ---------------------------------------------------------------------------- PTX helpers
@@ -106,15 +105,9 @@ __device__ __forceinline__ uint64_t policy_evict_first() {
   return pol;
 }
 __device__ __forceinline__ void tma_tile_3d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2, uint32_t bar, uint64_t pol) {
-#ifdef HX_NO_EVICT_FIRST
-  asm volatile(
-      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-      ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
-#else
   asm volatile(
       "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4}], [%5], %6;"
       ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "l"(pol) : "memory");
-#endif
 }
 __device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -277,13 +270,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int B = p.B, Hkv = p.Hkv, G = p.G;
   const int nC = gridDim.x;
-#ifdef HX_TRACE
-  unsigned long long tr[6] = {0, 0, 0, 0, 0, 0};
-#define HX_STAMP(x) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tr[x]))
-#else
-#define HX_STAMP(x)
-#endif
-  HX_STAMP(0);
+  if ((smem_u32(smem) & 1023u) != 0) __trap();       // the 128-byte-swizzle address math assumes a 1 KiB-aligned base
   if (tid == 32) {                                   // descriptor fetch off the first TMA's critical path
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tmK) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tmV) : "memory");
@@ -375,7 +362,6 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     const int len = smlo[lo + 1] - smlo[lo];
     return lo * 8 + (int)((((unsigned)(k - smlo[lo]) + 1u) * 8u - 1u) / (unsigned)len);   // len < 2^28 (host check)
   };
-  HX_STAMP(1);
   const int w = *my_slot * kWarps + warp;
   const int k0 = w_lo(w), k1 = w_lo(w + 1);
   do {
@@ -496,10 +482,6 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
       new_page = __ldg(p.bt + (size_t)c.i * p.bt_stride + c.j);
     }
     mbar_wait(bar_u32 + 8 * stage, (idx / kStages) & 1);
-#ifdef HX_TRACE
-    if (idx == 0) HX_STAMP(2);
-    if (ck == k1 - 1) HX_STAMP(3);
-#endif
 
     const uint32_t kb = stage_u32 + stage * C::kStage, vb = kb + kTile;
     if (APPEND && last_page) {
@@ -713,15 +695,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     }
   }
   } while (false);
-#ifdef HX_TRACE
-  HX_STAMP(4);
-  if (lane == 0) {
-    unsigned long long* t = reinterpret_cast<unsigned long long*>(p.claim + 2 * kMaxSm) + (size_t)(blockIdx.x * kWarps + warp) * 8;
-    for (int e = 0; e < 5; ++e) t[e] = tr[e];
-    t[5] = (unsigned long long)(k1 - k0);
-    unsigned smid; asm volatile("mov.u32 %0, %%smid;" : "=r"(smid)); t[6] = smid;
-  }
-#endif
+  if (p.pdl_wait_at_end) asm volatile("griddepcontrol.wait;" ::: "memory");
 
   // ---- tuned mode: the last CTA of the grid to finish clears the claim flags for the next call.
   // No fences: every CTA's claim (an atomic whose result it consumed) precedes its own count-up, and
@@ -730,66 +704,6 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     __syncthreads();
     if (tid == 0 && atomicAdd(p.claim + kMaxSm, 1) == nC - 1)
       for (int s = 0; s <= kMaxSm; ++s) p.claim[s] = 0;
-  }
-}
-
-// ------------------------------------------------------------------------------------------
-// Kernel "simple": one CTA per (request, query head), CUDA-core dot products, no split.
-// ------------------------------------------------------------------------------------------
-struct SimpleParams {
-  const __half* q; __half* out; const __half* k; const __half* v;
-  const int32_t* bt; const int32_t* lens;
-  int32_t q_heads, kv_heads, bt_stride;
-  float scale_log2;
-};
-
-template <int D>
-__global__ void __launch_bounds__(128) attn_simple_kernel(const SimpleParams p) {
-  constexpr int E = D / 32;
-  const int h = blockIdx.x, i = blockIdx.y;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int n = p.lens[i];
-  const int g = h / (p.q_heads / p.kv_heads);
-  const __half* qrow = p.q + ((size_t)i * p.q_heads + h) * D;
-  __half* orow = p.out + ((size_t)i * p.q_heads + h) * D;
-  float qf[E], acc[E];
-#pragma unroll
-  for (int e = 0; e < E; ++e) { qf[e] = __half2float(qrow[lane * E + e]); acc[e] = 0.f; }
-  float m = -INFINITY, l = 0.f;
-  for (int t = warp; t < n; t += 4) {
-    const int page = p.bt[(size_t)i * p.bt_stride + (t >> 4)];
-    const size_t off = (((size_t)page * p.kv_heads + g) * 16 + (t & 15)) * D + lane * E;
-    float dot = 0.f;
-#pragma unroll
-    for (int e = 0; e < E; ++e) dot += qf[e] * __half2float(p.k[off + e]);
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) dot += __shfl_xor_sync(0xffffffffu, dot, o);
-    const float s = dot * p.scale_log2;
-    const float m_new = fmaxf(m, s);
-    const float corr = exp2f(m - m_new), wgt = exp2f(s - m_new);
-    l = l * corr + wgt;
-#pragma unroll
-    for (int e = 0; e < E; ++e) acc[e] = acc[e] * corr + wgt * __half2float(p.v[off + e]);
-    m = m_new;
-  }
-  __shared__ float sm_m[4], sm_l[4], sm_acc[4][D];
-  if (lane == 0) { sm_m[warp] = m; sm_l[warp] = l; }
-#pragma unroll
-  for (int e = 0; e < E; ++e) sm_acc[warp][lane * E + e] = acc[e];
-  __syncthreads();
-  if (warp == 0) {
-    const float mm = fmaxf(fmaxf(sm_m[0], sm_m[1]), fmaxf(sm_m[2], sm_m[3]));
-    float ll = 0.f, o[E];
-#pragma unroll
-    for (int e = 0; e < E; ++e) o[e] = 0.f;
-    for (int w = 0; w < 4; ++w) {
-      const float c = (sm_m[w] == -INFINITY) ? 0.f : exp2f(sm_m[w] - mm);
-      ll += sm_l[w] * c;
-#pragma unroll
-      for (int e = 0; e < E; ++e) o[e] += sm_acc[w][lane * E + e] * c;
-    }
-#pragma unroll
-    for (int e = 0; e < E; ++e) orow[lane * E + e] = __float2half_rn(n > 0 ? o[e] / ll : 0.f);
   }
 }
 
@@ -860,11 +774,15 @@ int get_tile_maps(const void* k, const void* v, uint64_t rows, int D, CUtensorMa
 template <int D, int NT, bool APPEND>
 int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream) {
   using C = Cfg<D, NT>;
-  static bool attr_set[64] = {false};
-  if (!attr_set[di.device]) {
-    if (C::kSmem > di.max_smem_optin) HX_FAIL(HX_ERR_UNSUPPORTED, "device offers %d B shared memory per CTA, kernel needs %d", di.max_smem_optin, C::kSmem);
-    HX_CUDA_OK(cudaFuncSetAttribute(attn_stream_kernel<D, NT, APPEND>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmem));
-    attr_set[di.device] = true;
+  {
+    static std::mutex mu;
+    static bool attr_set[64] = {false};
+    std::lock_guard<std::mutex> lock(mu);
+    if (!attr_set[di.device]) {
+      if (C::kSmem > di.max_smem_optin) HX_FAIL(HX_ERR_UNSUPPORTED, "device offers %d B shared memory per CTA, kernel needs %d", di.max_smem_optin, C::kSmem);
+      HX_CUDA_OK(cudaFuncSetAttribute(attn_stream_kernel<D, NT, APPEND>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmem));
+      attr_set[di.device] = true;
+    }
   }
   const uint64_t rows_per_layer = (uint64_t)a.num_pages * a.kv_heads * 16;
   const uint64_t rows = rows_per_layer * a.layers;
@@ -897,10 +815,12 @@ int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream
     p.v_new = APPEND ? static_cast<const __half*>(a.v_new) + (size_t)b0 * a.kv_heads * D : nullptr;
     p.kc = static_cast<__half*>(const_cast<void*>(a.k_base)) + layer_elems * a.layer;
     p.vc = static_cast<__half*>(const_cast<void*>(a.v_base)) + layer_elems * a.layer;
-    if (a.overlap_prev && b0 == 0) {
-      // programmatic dependent launch: this grid may start while the preceding kernel of the stream (one that has
-      // executed griddepcontrol.launch_dependents, e.g. hx_kv_ingest's) is still running.  The kernel never waits
-      // on it: the caller asserted that it reads nothing that kernel writes.
+    p.pdl_wait_at_end = (a.overlap_prev && b0 == 0) ? 1 : 0;
+    if (p.pdl_wait_at_end) {
+      // programmatic dependent launch: this grid may start while the ingest kernel enqueued just before it (which
+      // executes griddepcontrol.launch_dependents at once) is still running.  The caller asserted that it reads
+      // nothing that kernel writes; each CTA waits for the ingest's completion before it exits, so that whatever is
+      // ordered after this grid is ordered after the ingest too.
       cudaLaunchConfig_t cfg = {};
       cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kWarps * 32); cfg.dynamicSmemBytes = C::kSmem; cfg.stream = stream;
       cudaLaunchAttribute at[1];
@@ -913,21 +833,6 @@ int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream
     }
     HX_CUDA_OK(cudaGetLastError());
   }
-  return HX_OK;
-}
-
-template <int D>
-int launch_simple(const AttnParams& a, cudaStream_t stream) {
-  SimpleParams p;
-  const size_t layer_elems = (size_t)a.num_pages * a.kv_heads * 16 * D;
-  p.q = static_cast<const __half*>(a.q); p.out = static_cast<__half*>(a.out);
-  p.k = static_cast<const __half*>(a.k_base) + layer_elems * a.layer;
-  p.v = static_cast<const __half*>(a.v_base) + layer_elems * a.layer;
-  p.bt = a.block_table; p.lens = a.seq_lens;
-  p.q_heads = a.q_heads; p.kv_heads = a.kv_heads; p.bt_stride = a.bt_stride;
-  p.scale_log2 = a.sm_scale * kLog2e;
-  attn_simple_kernel<D><<<dim3(a.q_heads, a.batch), 128, 0, stream>>>(p);
-  HX_CUDA_OK(cudaGetLastError());
   return HX_OK;
 }
 
@@ -954,18 +859,21 @@ int tune_sm_rates(const void* scratch, size_t bytes, cudaStream_t stream) {
     return HX_OK;
   }
   constexpr int kProbeSmem = kWarps * 3 * 8192;
-  static bool attr_set[64] = {false};
-  if (!attr_set[di.device]) {
-    HX_CUDA_OK(cudaFuncSetAttribute(sm_rate_probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kProbeSmem));
-    attr_set[di.device] = true;
+  {
+    static std::mutex mu;
+    static bool attr_set[64] = {false};
+    std::lock_guard<std::mutex> lock(mu);
+    if (!attr_set[di.device]) {
+      HX_CUDA_OK(cudaFuncSetAttribute(sm_rate_probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kProbeSmem));
+      attr_set[di.device] = true;
+    }
   }
   // three windows of 80 us: the counts of a window are max-merged per SM, which drops start-up noise
   for (int rep = 0; rep < 3; ++rep) {
     sm_rate_probe_kernel<<<grid, kWarps * 32, kProbeSmem, stream>>>(static_cast<const uint8_t*>(scratch), bytes / 8192, 80000u);
     HX_CUDA_OK(cudaGetLastError());
   }
-  int damp = 176;                                           // 0.69 (B200 sweep: 160-192 best), see sm_rate_finalize_kernel
-  if (const char* e = getenv("HX_TUNE_DAMP_256")) damp = atoi(e);   // experiments only
+  const int damp = 176;                                     // 0.69 (B200 sweep: 160-192 best), see sm_rate_finalize_kernel
   sm_rate_finalize_kernel<<<1, kMaxSm, 0, stream>>>(grid, 0, damp);
   HX_CUDA_OK(cudaGetLastError());
   return HX_OK;
@@ -975,9 +883,6 @@ int launch_attention(const AttnParams& a, cudaStream_t stream) {
   DeviceInfo di;
   int rc = device_info(&di);
   if (rc) return rc;
-  static const bool simple = [] { const char* e = getenv("HX_ATTN_IMPL"); return e && !strcmp(e, "simple"); }();
-  if (simple && a.k_new) HX_FAIL(HX_ERR_UNSUPPORTED, "HX_ATTN_IMPL=simple has no fused append");
-  if (simple) return a.head_dim == 128 ? launch_simple<128>(a, stream) : launch_simple<64>(a, stream);
   const int G = a.q_heads / a.kv_heads;
   if (a.k_new) {
     if (a.head_dim == 128) return G > 8 ? launch_stream<128, 2, true>(a, di, stream) : launch_stream<128, 1, true>(a, di, stream);

@@ -18,6 +18,12 @@ void set_error(const char* fmt, ...) {
 }
 void clear_error() { g_err[0] = 0; }
 
+// What this host thread enqueued last through the library, and where.  hx_decode_attention_overlapped launches as a
+// programmatic dependent only when that was an ingest kernel on the same stream (include/hx.h).
+enum LaunchKind { kLaunchNone = 0, kLaunchIngest = 1, kLaunchOther = 2 };
+static thread_local struct { void* stream; int kind; } g_last = {nullptr, kLaunchNone};
+static void note_launch(void* stream, int kind) { g_last.stream = stream; g_last.kind = kind; }
+
 int device_info(DeviceInfo* out) {
   static std::mutex mu;
   static DeviceInfo cache[64];
@@ -53,7 +59,8 @@ static int ingest_common(const void* const* src_k, const void* const* src_v, int
                          const hx_paged_cache* dst, const int32_t* block_table, int32_t stride,
                          const int32_t* cu_seqlens, const int32_t* seq_lens, int32_t batch,
                          int32_t total_tokens, int32_t max_seq_len, void* stream, bool gather,
-                         const char* who, int32_t src_layers, int32_t src_layer0, int32_t dst_layer0) {
+                         const char* who, int32_t src_layers, int32_t src_layer0, int32_t dst_layer0,
+                         bool dry_run = false) {
   clear_error();
   if (layers < 0 || batch < 0 || total_tokens < 0 || max_seq_len < 0)
     HX_FAIL(HX_ERR_INVALID_ARG, "%s: negative size (layers=%d batch=%d total_tokens=%d max_seq_len=%d)", who, layers, batch, total_tokens, max_seq_len);
@@ -93,7 +100,10 @@ static int ingest_common(const void* const* src_k, const void* const* src_v, int
   p.layers = layers; p.total_tokens = total_tokens; p.batch = batch;
   p.src_layer0 = src_layer0; p.dst_layer0 = dst_layer0;
   p.head_dim = head_dim; p.page_size = ps; p.num_pages = dst->num_pages; p.bt_stride = stride;
-  return launch_ingest(p, gather, static_cast<cudaStream_t>(stream));
+  if (dry_run) return HX_OK;                                   // checks only (hx_decode_step validates before it enqueues)
+  rc = launch_ingest(p, gather, static_cast<cudaStream_t>(stream));
+  if (rc == HX_OK) note_launch(stream, gather ? kLaunchOther : kLaunchIngest);
+  return rc;
 }
 
 }  // namespace hx
@@ -180,7 +190,7 @@ static int attention_common(const char* who, void* out, const void* q, const voi
                             const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
                             const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
                             int32_t batch, int32_t max_seq_len, float sm_scale, void* workspace,
-                            size_t workspace_bytes, void* stream) {
+                            size_t workspace_bytes, void* stream, bool dry_run = false) {
   using namespace hx;
   clear_error();
   if (batch < 0 || max_seq_len < 0) HX_FAIL(HX_ERR_INVALID_ARG, "%s: negative size (batch=%d max_seq_len=%d)", who, batch, max_seq_len);
@@ -216,8 +226,12 @@ static int attention_common(const char* who, void* out, const void* q, const voi
   p.page_size = cache->page_size; p.num_pages = cache->num_pages; p.bt_stride = block_table_stride;
   p.max_seq_len = max_seq_len; p.sm_scale = sm_scale;
   p.k_new = append ? k_new : nullptr; p.v_new = append ? v_new : nullptr;
-  p.overlap_prev = overlap ? 1 : 0;
-  return launch_attention(p, static_cast<cudaStream_t>(stream));
+  // a programmatic dependent launch only directly behind an ingest kernel this thread enqueued on this stream
+  p.overlap_prev = (overlap && g_last.kind == kLaunchIngest && g_last.stream == stream) ? 1 : 0;
+  if (dry_run) return HX_OK;
+  rc = launch_attention(p, static_cast<cudaStream_t>(stream));
+  if (rc == HX_OK) note_launch(stream, kLaunchOther);
+  return rc;
 }
 
 int hx_decode_attention(void* out, const void* q, const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
@@ -271,7 +285,9 @@ int hx_kv_append(const void* k_new, const void* v_new, const hx_paged_cache* cac
   p.block_table = block_table; p.seq_lens = seq_lens;
   p.batch = batch; p.kv_heads = cache->kv_heads; p.head_dim = cache->head_dim; p.page_size = cache->page_size;
   p.bt_stride = block_table_stride;
-  return launch_append(p, static_cast<cudaStream_t>(stream));
+  rc = launch_append(p, static_cast<cudaStream_t>(stream));
+  if (rc == HX_OK) note_launch(stream, kLaunchOther);
+  return rc;
 }
 
 int hx_prefill_attention(void* out, const void* q, const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
@@ -305,7 +321,9 @@ int hx_prefill_attention(void* out, const void* q, const hx_paged_cache* cache, 
   a.batch = batch; a.q_heads = q_heads; a.kv_heads = cache->kv_heads; a.head_dim = cache->head_dim;
   a.num_pages = cache->num_pages; a.bt_stride = block_table_stride; a.layer = layer; a.layers = cache->layers;
   a.total_q = total_q_tokens; a.max_q_len = max_q_len; a.sm_scale = sm_scale;
-  return launch_prefill(a, static_cast<cudaStream_t>(stream));
+  rc = launch_prefill(a, static_cast<cudaStream_t>(stream));
+  if (rc == HX_OK) note_launch(stream, kLaunchOther);
+  return rc;
 }
 
 int hx_tune_sm_rates(const void* scratch, size_t scratch_bytes, void* stream) {
@@ -315,80 +333,166 @@ int hx_tune_sm_rates(const void* scratch, size_t scratch_bytes, void* stream) {
     if (!aligned16(scratch)) HX_FAIL(HX_ERR_INVALID_ARG, "hx_tune_sm_rates: scratch must be 16-byte aligned");
     if (scratch_bytes < ((size_t)256 << 20)) HX_FAIL(HX_ERR_UNSUPPORTED, "hx_tune_sm_rates: scratch of %zu bytes is too small to be HBM-bound (need >= 256 MiB)", scratch_bytes);
   }
-  return tune_sm_rates(scratch, scratch_bytes, static_cast<cudaStream_t>(stream));
+  const int rc = tune_sm_rates(scratch, scratch_bytes, static_cast<cudaStream_t>(stream));
+  if (rc == HX_OK) note_launch(stream, kLaunchOther);
+  return rc;
 }
 
-int hx_decode_step_host(const hx_step_host_args* a, void* stream_) {
+// ---- whole decode step (row A9): library-owned side stream per device for the overlapped handoff ----
+namespace {
+struct SideStream { cudaStream_t stream = nullptr; cudaEvent_t fork = nullptr, join = nullptr; };
+std::mutex g_step_mu;                 // held from fork to join: one step is enqueued at a time per process
+SideStream g_side[64];
+
+int side_stream(int* dev_out, SideStream** out) {
   using namespace hx;
-  clear_error();
-  if (!a) HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_host: args is NULL");
-  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
-  if (!a->cache) HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_host: cache is NULL");
-  const size_t qbytes = (size_t)a->batch * a->q_heads * a->cache->head_dim * 2;
-  // overlap_ingest: fork a library-owned side stream (one per device, created on first use) for the handoff
-  cudaStream_t main_stream = stream;
-  const bool fork = a->overlap_ingest != 0 && a->ing_batch > 0 && a->batch > 0;
-  static std::mutex mu;
-  static cudaStream_t side_streams[64] = {nullptr};
-  static cudaEvent_t ev_fork[64] = {nullptr}, ev_join[64] = {nullptr};
+  int dev = 0;
+  HX_CUDA_OK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) HX_FAIL(HX_ERR_CUDA, "device id %d out of range", dev);
+  SideStream& s = g_side[dev];
+  if (!s.stream) {
+    HX_CUDA_OK(cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking));
+    HX_CUDA_OK(cudaEventCreateWithFlags(&s.fork, cudaEventDisableTiming));
+    HX_CUDA_OK(cudaEventCreateWithFlags(&s.join, cudaEventDisableTiming));
+  }
+  *dev_out = dev; *out = &s;
+  return HX_OK;
+}
+
+// The step on device buffers.  `h` (optional) adds the host<->device copies of hx_decode_step_host.
+int step_impl(const char* who, const hx_step_args* a, const hx_step_host_args* h, void* stream_) {
+  using namespace hx;
+  cudaStream_t main_stream = static_cast<cudaStream_t>(stream_);
+  const bool do_ing = a->ing_batch > 0, do_att = a->batch > 0;
+  // ---- every host-side check first: nothing is enqueued unless the whole step is valid
+  if (a->batch < 0 || a->ing_batch < 0) HX_FAIL(HX_ERR_INVALID_ARG, "%s: negative batch", who);
+  if (!a->cache) HX_FAIL(HX_ERR_INVALID_ARG, "%s: cache is NULL", who);
+  int rc;
+  if (do_ing) {
+    if (!a->src_k || !a->src_v) HX_FAIL(HX_ERR_INVALID_ARG, "%s: src_k/src_v is NULL", who);
+    rc = ingest_common(a->src_k, a->src_v, a->ing_layers, a->heads, a->cache->head_dim, a->src_tp, a->dst_tp, a->dst_rank,
+                       a->cache, a->ing_block_table, a->ing_block_table_stride, a->ing_cu_seqlens, a->ing_seq_lens,
+                       a->ing_batch, a->ing_total_tokens, a->ing_max_seq_len, stream_, false, who, -1, 0, 0, /*dry_run=*/true);
+    if (rc) return rc;
+  }
+  if (do_att) {
+    rc = attention_common(who, a->out, a->q, nullptr, nullptr, false, false, a->cache, a->layer, a->q_heads, a->block_table,
+                          a->block_table_stride, a->seq_lens, a->batch, a->max_seq_len, a->sm_scale, a->workspace,
+                          a->workspace_bytes, stream_, /*dry_run=*/true);
+    if (rc) return rc;
+  }
+  size_t qbytes = 0, shard = 0;
+  if (h) {
+    if (do_att && (!h->q_host || !h->out_host)) HX_FAIL(HX_ERR_INVALID_ARG, "%s: q_host/out_host is NULL", who);
+    qbytes = (size_t)a->batch * a->q_heads * a->cache->head_dim * 2;
+    if (do_ing) {
+      if (!h->src_k_host || !h->src_v_host || !h->ing_block_table_host || !h->ing_cu_seqlens_host || !h->ing_seq_lens_host)
+        HX_FAIL(HX_ERR_INVALID_ARG, "%s: host ingest buffers missing", who);
+      if (!h->pull_src && (!h->src_k_dev || !h->src_v_dev)) HX_FAIL(HX_ERR_INVALID_ARG, "%s: device staging for the shards missing", who);
+      shard = (size_t)a->ing_layers * a->ing_total_tokens * (a->heads / a->src_tp) * a->cache->head_dim * 2;
+    }
+  }
+
+  // ---- enqueue.  overlap_ingest: the handoff goes to the side stream, forked from and joined to the caller's
+  // stream; once forked, every exit path joins, so the caller's stream always covers whatever was enqueued.
+  std::lock_guard<std::mutex> lock(g_step_mu);
+  const bool fork = a->overlap_ingest != 0 && do_ing && do_att;
+  SideStream* ss = nullptr;
+  cudaStream_t ing_stream = main_stream;
   int dev = 0;
   if (fork) {
-    HX_CUDA_OK(cudaGetDevice(&dev));
-    if (dev < 0 || dev >= 64) HX_FAIL(HX_ERR_CUDA, "device id %d out of range", dev);
-    std::lock_guard<std::mutex> lock(mu);
-    if (!side_streams[dev]) {
-      HX_CUDA_OK(cudaStreamCreateWithFlags(&side_streams[dev], cudaStreamNonBlocking));
-      HX_CUDA_OK(cudaEventCreateWithFlags(&ev_fork[dev], cudaEventDisableTiming));
-      HX_CUDA_OK(cudaEventCreateWithFlags(&ev_join[dev], cudaEventDisableTiming));
-    }
-    HX_CUDA_OK(cudaEventRecord(ev_fork[dev], main_stream));
-    HX_CUDA_OK(cudaStreamWaitEvent(side_streams[dev], ev_fork[dev], 0));
-    // the attention's small q upload goes first on the main stream so that it is not queued behind the shards
-    if (!a->q_host || !a->q_dev) HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_host: q/out buffers missing");
-    HX_CUDA_OK(cudaMemcpyAsync(a->q_dev, a->q_host, qbytes, cudaMemcpyHostToDevice, main_stream));
-    stream = side_streams[dev];
-    stream_ = static_cast<void*>(stream);
-  }
-  if (a->ing_batch > 0) {
-    const bool pull = a->pull_src != 0;
-    if (!a->src_k_host || !a->src_v_host || (!pull && (!a->src_k_dev || !a->src_v_dev)) || !a->ing_block_table_host ||
-        !a->ing_cu_seqlens_host || !a->ing_seq_lens_host || !a->ing_block_table_dev || !a->ing_cu_seqlens_dev ||
-        !a->ing_seq_lens_dev)
-      HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_host: ingest buffers missing");
-    if (a->src_tp <= 0 || a->src_tp > 16 || a->heads <= 0 || a->heads % a->src_tp)
-      HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_host: bad heads/src_tp");
-    const size_t shard = (size_t)a->ing_layers * a->ing_total_tokens * (a->heads / a->src_tp) * a->cache->head_dim * 2;
-    for (int r = 0; r < a->src_tp && !pull; ++r) {
-      if (!a->src_k_host[r] || !a->src_k_dev[r]) continue;   // shard not needed by this rank
-      HX_CUDA_OK(cudaMemcpyAsync(a->src_k_dev[r], a->src_k_host[r], shard, cudaMemcpyHostToDevice, stream));
-      HX_CUDA_OK(cudaMemcpyAsync(a->src_v_dev[r], a->src_v_host[r], shard, cudaMemcpyHostToDevice, stream));
-    }
-    HX_CUDA_OK(cudaMemcpyAsync(a->ing_block_table_dev, a->ing_block_table_host,
-                               (size_t)a->ing_batch * a->ing_block_table_stride * 4, cudaMemcpyHostToDevice, stream));
-    HX_CUDA_OK(cudaMemcpyAsync(a->ing_cu_seqlens_dev, a->ing_cu_seqlens_host, (size_t)(a->ing_batch + 1) * 4, cudaMemcpyHostToDevice, stream));
-    HX_CUDA_OK(cudaMemcpyAsync(a->ing_seq_lens_dev, a->ing_seq_lens_host, (size_t)a->ing_batch * 4, cudaMemcpyHostToDevice, stream));
-    int rc = hx_kv_ingest(pull ? a->src_k_host : const_cast<const void* const*>(a->src_k_dev),
-                          pull ? a->src_v_host : const_cast<const void* const*>(a->src_v_dev),
-                          a->ing_layers, a->heads, a->cache->head_dim, a->src_tp, a->dst_tp, a->dst_rank, a->cache,
-                          a->ing_block_table_dev, a->ing_block_table_stride, a->ing_cu_seqlens_dev,
-                          a->ing_seq_lens_dev, a->ing_batch, a->ing_total_tokens, a->ing_max_seq_len, stream_);
+    rc = side_stream(&dev, &ss);
     if (rc) return rc;
+    HX_CUDA_OK(cudaEventRecord(ss->fork, main_stream));
+    HX_CUDA_OK(cudaStreamWaitEvent(ss->stream, ss->fork, 0));
+    ing_stream = ss->stream;
   }
-  if (fork) {
-    HX_CUDA_OK(cudaEventRecord(ev_join[dev], stream));
-    stream = main_stream;
-    stream_ = static_cast<void*>(stream);
+  rc = HX_OK;
+  cudaError_t ce = cudaSuccess;
+  const char* what = "";
+#define STEP_CUDA(expr) do { if (rc == HX_OK && ce == cudaSuccess) { ce = (expr); if (ce != cudaSuccess) what = #expr; } } while (0)
+  // the attention's small q upload goes first on the caller's stream so that it is not queued behind the shards
+  if (h && do_att) STEP_CUDA(cudaMemcpyAsync(const_cast<void*>(a->q), h->q_host, qbytes, cudaMemcpyHostToDevice, main_stream));
+  if (do_ing) {
+    if (h) {
+      for (int r = 0; r < a->src_tp && !h->pull_src; ++r) {
+        if (!h->src_k_host[r] || !h->src_k_dev[r]) continue;   // shard not needed by this rank
+        STEP_CUDA(cudaMemcpyAsync(h->src_k_dev[r], h->src_k_host[r], shard, cudaMemcpyHostToDevice, ing_stream));
+        STEP_CUDA(cudaMemcpyAsync(h->src_v_dev[r], h->src_v_host[r], shard, cudaMemcpyHostToDevice, ing_stream));
+      }
+      STEP_CUDA(cudaMemcpyAsync(const_cast<int32_t*>(a->ing_block_table), h->ing_block_table_host,
+                                (size_t)a->ing_batch * a->ing_block_table_stride * 4, cudaMemcpyHostToDevice, ing_stream));
+      STEP_CUDA(cudaMemcpyAsync(const_cast<int32_t*>(a->ing_cu_seqlens), h->ing_cu_seqlens_host, (size_t)(a->ing_batch + 1) * 4,
+                                cudaMemcpyHostToDevice, ing_stream));
+      STEP_CUDA(cudaMemcpyAsync(const_cast<int32_t*>(a->ing_seq_lens), h->ing_seq_lens_host, (size_t)a->ing_batch * 4,
+                                cudaMemcpyHostToDevice, ing_stream));
+    }
+    if (rc == HX_OK && ce == cudaSuccess)
+      rc = ingest_common(a->src_k, a->src_v, a->ing_layers, a->heads, a->cache->head_dim, a->src_tp, a->dst_tp, a->dst_rank,
+                         a->cache, a->ing_block_table, a->ing_block_table_stride, a->ing_cu_seqlens, a->ing_seq_lens,
+                         a->ing_batch, a->ing_total_tokens, a->ing_max_seq_len, static_cast<void*>(ing_stream), false, who, -1, 0, 0);
   }
-  if (a->batch > 0) {
-    if (!a->q_host || !a->out_host || !a->q_dev || !a->out_dev) HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_host: q/out buffers missing");
-    if (!fork) HX_CUDA_OK(cudaMemcpyAsync(a->q_dev, a->q_host, qbytes, cudaMemcpyHostToDevice, stream));
-    int rc = hx_decode_attention(a->out_dev, a->q_dev, a->cache, a->layer, a->q_heads, a->block_table_dev,
-                                 a->block_table_stride, a->seq_lens_dev, a->batch, a->max_seq_len, a->sm_scale,
-                                 a->workspace, a->workspace_bytes, stream_);
-    if (rc) return rc;
-    HX_CUDA_OK(cudaMemcpyAsync(a->out_host, a->out_dev, qbytes, cudaMemcpyDeviceToHost, stream));
+  if (do_att && rc == HX_OK && ce == cudaSuccess) {
+    rc = attention_common(who, a->out, a->q, nullptr, nullptr, false, false, a->cache, a->layer, a->q_heads, a->block_table,
+                          a->block_table_stride, a->seq_lens, a->batch, a->max_seq_len, a->sm_scale, a->workspace,
+                          a->workspace_bytes, stream_);
+    if (h) STEP_CUDA(cudaMemcpyAsync(h->out_host, a->out, qbytes, cudaMemcpyDeviceToHost, main_stream));
   }
-  if (fork) HX_CUDA_OK(cudaStreamWaitEvent(main_stream, ev_join[dev], 0));     // join: `stream` now covers the handoff too
+#undef STEP_CUDA
+  if (fork) {                                                   // join on every path, error or not
+    cudaError_t j = cudaEventRecord(ss->join, ss->stream);
+    if (j == cudaSuccess) j = cudaStreamWaitEvent(main_stream, ss->join, 0);
+    if (j != cudaSuccess && rc == HX_OK && ce == cudaSuccess) { ce = j; what = "join of the side stream"; }
+  }
+  if (rc != HX_OK) return rc;                                   // hx_last_error() already holds the detail
+  if (ce != cudaSuccess) HX_FAIL(HX_ERR_CUDA, "%s: %s: %s", who, what, cudaGetErrorString(ce));
+  return HX_OK;
+}
+}  // namespace
+
+int hx_decode_step(const hx_step_args* a, void* stream) {
+  using namespace hx;
+  clear_error();
+  if (!a) HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step: args is NULL");
+  return step_impl("hx_decode_step", a, nullptr, stream);
+}
+
+int hx_decode_step_host(const hx_step_host_args* h, void* stream) {
+  using namespace hx;
+  clear_error();
+  if (!h) HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_host: args is NULL");
+  hx_step_args a;
+  memset(&a, 0, sizeof(a));
+  a.out = h->out_dev; a.q = h->q_dev; a.cache = h->cache; a.layer = h->layer; a.q_heads = h->q_heads;
+  a.block_table = h->block_table_dev; a.block_table_stride = h->block_table_stride; a.seq_lens = h->seq_lens_dev;
+  a.batch = h->batch; a.max_seq_len = h->max_seq_len; a.sm_scale = h->sm_scale;
+  a.workspace = h->workspace; a.workspace_bytes = h->workspace_bytes;
+  // pull mode (F2): the ingest kernel reads the host shards over the link itself
+  a.src_k = h->pull_src ? h->src_k_host : const_cast<const void* const*>(h->src_k_dev);
+  a.src_v = h->pull_src ? h->src_v_host : const_cast<const void* const*>(h->src_v_dev);
+  a.ing_layers = h->ing_layers; a.heads = h->heads; a.src_tp = h->src_tp; a.dst_tp = h->dst_tp; a.dst_rank = h->dst_rank;
+  a.ing_block_table = h->ing_block_table_dev; a.ing_block_table_stride = h->ing_block_table_stride;
+  a.ing_cu_seqlens = h->ing_cu_seqlens_dev; a.ing_seq_lens = h->ing_seq_lens_dev;
+  a.ing_batch = h->ing_batch; a.ing_total_tokens = h->ing_total_tokens; a.ing_max_seq_len = h->ing_max_seq_len;
+  a.overlap_ingest = h->overlap_ingest;
+  return step_impl("hx_decode_step_host", &a, h, stream);
+}
+
+int hx_shutdown(void) {
+  using namespace hx;
+  clear_error();
+  std::lock_guard<std::mutex> lock(g_step_mu);
+  int cur = 0;
+  HX_CUDA_OK(cudaGetDevice(&cur));
+  for (int d = 0; d < 64; ++d) {
+    SideStream& s = g_side[d];
+    if (!s.stream) continue;
+    HX_CUDA_OK(cudaSetDevice(d));
+    cudaStreamSynchronize(s.stream);
+    cudaEventDestroy(s.fork); cudaEventDestroy(s.join); cudaStreamDestroy(s.stream);
+    s = SideStream();
+  }
+  HX_CUDA_OK(cudaSetDevice(cur));
   return HX_OK;
 }
 

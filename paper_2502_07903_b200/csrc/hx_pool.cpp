@@ -2,7 +2,6 @@
 // Paging is by citation only in the paper; running out of pages is the OOM the
 // paper avoids by capping the online rate -> HX_ERR_NO_PAGES, all-or-nothing.
 #include <cstdint>
-#include <new>
 #include <vector>
 
 #include "hx.h"
@@ -19,12 +18,20 @@ extern "C" {
 
 int hx_pool_create(hx_page_pool** out, int32_t num_pages) {
   if (!out || num_pages < 0) { hx::set_error("hx_pool_create: out=%p num_pages=%d", (void*)out, num_pages); return HX_ERR_INVALID_ARG; }
-  hx_page_pool* p = new (std::nothrow) hx_page_pool();
-  if (!p) { hx::set_error("hx_pool_create: out of host memory"); return HX_ERR_INVALID_ARG; }
-  p->num_pages = num_pages;
-  p->free_list.resize(num_pages);
-  for (int32_t i = 0; i < num_pages; ++i) p->free_list[i] = num_pages - 1 - i;   // page 0 first
-  p->is_free.assign(num_pages, 1);
+  // No C++ exception may cross the C ABI: the only allocations of the pool's lifetime happen here (free_list is
+  // sized to num_pages once, so hx_pool_free's push_back never reallocates) and are caught.
+  hx_page_pool* p = nullptr;
+  try {
+    p = new hx_page_pool();
+    p->num_pages = num_pages;
+    p->free_list.resize(num_pages);
+    for (int32_t i = 0; i < num_pages; ++i) p->free_list[i] = num_pages - 1 - i;   // page 0 first
+    p->is_free.assign(num_pages, 1);
+  } catch (...) {
+    delete p;
+    hx::set_error("hx_pool_create: out of host memory for %d pages", num_pages);
+    return HX_ERR_NO_PAGES;
+  }
   *out = p;
   return HX_OK;
 }
@@ -71,7 +78,7 @@ int hx_pool_free(hx_page_pool* p, const int32_t* ids, int32_t n) {
     }
     p->is_free[id] = 1;    // provisional mark also catches duplicates within ids[]
   }
-  for (int32_t i = 0; i < n; ++i) p->free_list.push_back(ids[i]);
+  for (int32_t i = 0; i < n; ++i) p->free_list.push_back(ids[i]);   // within the capacity reserved at create: no allocation
   return HX_OK;
 }
 

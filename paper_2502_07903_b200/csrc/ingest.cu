@@ -26,15 +26,10 @@ constexpr int kMinCtas = 5;   // __launch_bounds__ occupancy target (register ca
 
 __device__ __forceinline__ int4 ld_stream(const int4* p) {
   int4 r;
-#ifndef HX_NO_EVICT_FIRST
   uint64_t pol;                                   // the source shards are read once: evict-first in L2
   asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
   asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.L2::128B.v4.s32 {%0,%1,%2,%3}, [%4], %5;"
                : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p), "l"(pol));
-  return r;
-#endif
-  asm volatile("ld.global.nc.L1::no_allocate.L2::128B.v4.s32 {%0,%1,%2,%3}, [%4];"
-               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
   return r;
 }
 __device__ __forceinline__ void st_stream(int4* p, const int4& v) {

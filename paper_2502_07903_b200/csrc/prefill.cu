@@ -468,11 +468,15 @@ static int launch_prefill_d(const PrefillArgs& a, cudaStream_t stream) {
   DeviceInfo di;
   int rc = device_info(&di);
   if (rc) return rc;
-  static bool attr_set[64] = {false};
-  if (!attr_set[di.device]) {
-    if (kSmem > di.max_smem_optin) HX_FAIL(HX_ERR_UNSUPPORTED, "device offers %d B shared memory per CTA, kernel needs %d", di.max_smem_optin, kSmem);
-    HX_CUDA_OK(cudaFuncSetAttribute(prefill_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem));
-    attr_set[di.device] = true;
+  {
+    static std::mutex mu;
+    static bool attr_set[64] = {false};
+    std::lock_guard<std::mutex> lock(mu);
+    if (!attr_set[di.device]) {
+      if (kSmem > di.max_smem_optin) HX_FAIL(HX_ERR_UNSUPPORTED, "device offers %d B shared memory per CTA, kernel needs %d", di.max_smem_optin, kSmem);
+      HX_CUDA_OK(cudaFuncSetAttribute(prefill_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem));
+      attr_set[di.device] = true;
+    }
   }
   EncodeTiledFn enc;
   rc = encode_fn(&enc);
