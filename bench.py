@@ -3,28 +3,34 @@
 
 A "step" = the whole hot path over one batch: the host page
 allocator frees last step's 16 prompts and allocates 16 new ones (2048 tokens each), their
-block-table rows are uploaded, hx_kv_ingest lands their KV (prefill TP=4 -> decode TP=1, one
-layer) in the paged cache, and hx_decode_attention runs over the fixed 256-request heavy-tailed
-batch (64 q / 8 kv heads, head_dim 128).  Inputs are seeded synthetic data (workloads/).
+block-table rows are uploaded, and ONE C-ABI call, hx_decode_step(overlap_ingest=1), lands their KV
+(hx_kv_ingest: prefill TP=4 -> decode TP=1, one layer, on the library's side stream) while
+hx_decode_attention runs over the fixed 256-request heavy-tailed batch (64 q / 8 kv heads,
+head_dim 128); the new prompts' pages are disjoint from the batch's (the handoff
+is asynchronous "to enable overlapping").  Inputs are seeded synthetic data (workloads/).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl hx|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl hx|reference] [--oracle-table]
 
 Prints ONE JSON line (rank 0).  `value` = (attention KV bytes + ingest read+write bytes) per
-step x K / device time, inputs resident in HBM.  N > 1 (torchrun): independent replicas, one per
-GPU, no collective on the data path ("replicas only"); value sums over ranks.
+step x K / device time, inputs resident in HBM.  N > 1: independent replicas, one per GPU, no
+collective on the data path ("replicas only"); value sums over ranks.  Without torchrun
+(`WORLD_SIZE` unset) `--gpus N` re-executes itself under torch.distributed.run with N ranks.
 
 Beside the contract keys (roofline, e2e, cpu_baseline, clocks, gpu_launches) the line carries:
-`two_stream` (the step with the ingest on a side stream), `cuda_graph` (the single-stream step replayed as
-a CUDA graph), `e2e.*` (hx_decode_step_host from pinned host buffers: handoff overlapped / in order / pulled
-by the kernel over PCIe) and `other_configs`: configs[1], [2] (attention) and [3] (80-layer ingest) kernel-only,
-`prefill` (hx_prefill_attention against the tensor roofline), `append_cfg5` (fused append + attention) and
-`stream_peaks` (read-only / write-only HBM rates of the run).
+`in_order` (the same step with both kernels on one stream, which also gives each kernel's time alone),
+`overlapped_launch` (one stream, programmatic dependent launch), `cuda_graph` (the headline step replayed as a
+CUDA graph), `e2e.*` (hx_decode_step_host from pinned host buffers) and `other_configs`: configs[1], [2]
+(attention) and [3] (80-layer ingest) kernel-only, `prefill` (hx_prefill_attention against the tensor roofline),
+`append_cfg5` (fused append + attention) and `stream_peaks` (read-only / write-only HBM rates of the run).
+`--oracle-table` prints the oracle's time per config at 1 thread and at all cores instead.
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -125,18 +131,20 @@ def whole_job_value(bytes_per_step_per_rank: int, steps: int, world: int, ms_max
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+    """nvidia-smi clocks / throttle reasons, sampled every 20 ms over the WHOLE run; stop() reports the samples that
+    fell inside the timed window [mark_begin, mark_end] (and the whole run beside them)."""
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
 
     def __init__(self, index: int):
-        self.index, self.rows, self.proc = index, [], None
+        self.index, self.rows, self.proc, self.t0, self.t1 = index, [], None, None, None
 
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+                                          "-i", str(self.index), "-lms", "20"], stdout=subprocess.PIPE, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
         except Exception:
@@ -144,20 +152,65 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append([x.strip() for x in line.split(",")])
+            self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
+
+    def mark_begin(self):
+        self.t0 = time.time()
+
+    def mark_end(self):
+        self.t1 = time.time()
+
+    @classmethod
+    def _summary(cls, rows):
+        sm = [float(r[1]) for r in rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        reasons = [n for j, n in enumerate(cls.NAMES) if any(len(r) > 4 + j and r[4 + j].startswith("Active") for r in rows)]
+        return sm, reasons
 
     def stop(self):
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
+        time.sleep(0.1)
         self.proc.terminate()
         self.t.join(timeout=2)
-        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
-        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = [n for j, n in enumerate(names) if any(len(r) > 3 + j and r[3 + j].startswith("Active") for r in self.rows)]
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": reasons, "samples": len(sm)}
+        rows = [r for _, r in self.rows]
+        mx = [float(r[2]) for r in rows if len(r) > 2 and r[2].replace(".", "").isdigit()]
+        # a sample is attributed to the window if it was read inside it (+- one sampling period)
+        win = [r for t, r in self.rows if self.t0 is not None and self.t0 - 0.02 <= t <= self.t1 + 0.04]
+        sm_all, reasons_all = self._summary(rows)
+        sm_win, reasons_win = self._summary(win)
+        busy = [x for x in sm_all if x >= 0.5 * max(mx, default=0)]           # samples with the GPU clocked up
+        return {"sm_mhz": float(np.median(sm_win)) if sm_win else (float(np.median(busy)) if busy else None),
+                "sm_max_mhz": max(mx) if mx else None, "reasons": reasons_win if win else reasons_all,
+                "samples": len(sm_all), "samples_in_timed_window": len(sm_win),
+                "whole_run": {"sm_mhz_median": float(np.median(sm_all)) if sm_all else None, "reasons": reasons_all,
+                              "seconds": (self.rows[-1][0] - self.rows[0][0]) if len(self.rows) > 1 else 0.0}}
+
+
+NCU_TRAFFIC_FILE = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+
+
+def kernel_source_hash() -> str:
+    """sha256 over the CUDA sources of the two hot kernels: ties an ncu capture to the tree it was taken on."""
+    h = hashlib.sha256()
+    for f in ("attention.cu", "ingest.cu"):
+        with open(os.path.join(ROOT, "paper_2502_07903_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()
+
+
+def ncu_traffic():
+    """dram read+write bytes per attention launch from the committed ncu --set full capture — only if that capture
+    was taken on THIS tree's kernels (profiles/ncu_traffic.json stores their source hash); else null, loudly."""
+    try:
+        with open(NCU_TRAFFIC_FILE) as f:
+            d = json.load(f)
+    except Exception:
+        return None, "no profiles/ncu_traffic.json"
+    if d.get("kernel_source_sha256") != kernel_source_hash():
+        print("bench.py: WARNING: profiles/ncu_traffic.json was captured on other kernel sources; roofline.traffic = null",
+              file=sys.stderr, flush=True)
+        return None, "stale: profiles/ncu_traffic.json was captured on other kernel sources"
+    return int(d["attn_dram_bytes_per_launch"]), f"ncu --set full capture {d.get('capture')} (same kernel sources, not measured in this run)"
 
 
 # ----------------------------------------------------------------------------------------------
@@ -196,6 +249,8 @@ def run_hx(args, rank, world, local_rank):
     dev = torch.device("cuda", local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
+    sampler = ClockSampler(local_rank)             # samples the whole run; the timed window is marked below
+    sampler.start()
     st = build_step_workload(torch, hx, seed_extra=rank)
     ca, ci, ing = st["ca"], st["ci"], st["ing"]
     B, Hq, Hkv, D = ca.batch, ca.q_heads, ca.kv_heads, ca.head_dim
@@ -224,7 +279,7 @@ def run_hx(args, rank, world, local_rank):
     pool = st["pool"]
     prev = {"ids": None, "n": 0}
 
-    def next_rows(stream=None):
+    def next_rows():
         """A1: free last step's prompts, allocate this step's (host), stage the new rows for upload."""
         if prev["ids"] is not None:
             pool.free(prev["ids"])
@@ -238,92 +293,71 @@ def run_hx(args, rank, world, local_rank):
         pin.numpy()[:] = rows
         return pin, slot
 
-    def uploaded(slot):
+    def upload_rows():
+        pin, slot = next_rows()
+        ing_bt_dev.copy_(pin, non_blocking=True)
         ev = ring_ev[slot] or torch.cuda.Event()
         ev.record()
         ring_ev[slot] = ev
 
-    def step(record=None):
-        pin, slot = next_rows()
-        ing_bt_dev.copy_(pin, non_blocking=True)
-        uploaded(slot)
-        if record:
-            record[0].record()
-        hx.kv_ingest(src_k, src_v, layers=1, heads=ci.heads, head_dim=D, src_tp=4, dst_tp=1, dst_rank=0,
-                     dst=cache, block_table=ing_bt_dev, block_table_stride=ing_stride, cu_seqlens=ing_cu,
-                     seq_lens=ing_sl, batch=nI, total_tokens=TI, max_seq_len=2048)
-        if record:
-            record[1].record()
-        hx.decode_attention(out, q, cache, layer=0, q_heads=Hq, block_table=bt, block_table_stride=bt.shape[1],
-                            seq_lens=sl, batch=B, max_seq_len=max_len, workspace=ws, workspace_bytes=ws_bytes)
-        if record:
-            record[2].record()
+    step_kw = dict(out=out, q=q, cache=cache, layer=0, q_heads=Hq, block_table=bt, block_table_stride=bt.shape[1],
+                   seq_lens=sl, batch=B, max_seq_len=max_len, sm_scale=0.0, workspace=ws, workspace_bytes=ws_bytes,
+                   src_k=src_k, src_v=src_v, ing_layers=1, heads=ci.heads, src_tp=4, dst_tp=1, dst_rank=0,
+                   ing_block_table=ing_bt_dev, ing_block_table_stride=ing_stride, ing_cu_seqlens=ing_cu, ing_seq_lens=ing_sl,
+                   ing_batch=nI, ing_total_tokens=TI, ing_max_seq_len=2048)
+    # the headline step: ONE hx_decode_step call, the handoff overlapped on the library's side stream
+    stepper = hx.DecodeStep(overlap_ingest=1, **step_kw)
+    stepper_in_order = hx.DecodeStep(overlap_ingest=0, **step_kw)
+    EV = ("ev_ingest_begin", "ev_ingest_end", "ev_attention_begin", "ev_attention_end")
+
+    def step(which=stepper, events=None):
+        upload_rows()
+        for j, name in enumerate(EV):
+            setattr(which.a, name, events[j].cuda_event if events else None)
+        which()
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
-        step()
-    barrier()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
-    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    t0.record()
-    for s in range(args.steps):
-        step(ev[s])
-    t1.record()
-    barrier()
-    clocks = sampler.stop()
-    total_ms = t0.elapsed_time(t1)
-    ing_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
-    att_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in ev]))
-    att_min_ms = float(np.min([e[1].elapsed_time(e[2]) for e in ev]))
-    total_ms = max_over_ranks(total_ms, world, dev)
+    def new_events(n):
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(n)]
+        for row in evs:
+            for e in row:
+                e.record()                        # creates the handle the library records into
+        return evs
 
+    def timed_steps(which):
+        for _ in range(max(args.warmup, 3)):
+            step(which)
+        barrier()
+        ev = new_events(args.steps)
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        if which is stepper:
+            sampler.mark_begin()
+        t0.record()
+        for s_ in range(args.steps):
+            step(which, ev[s_])
+        t1.record()
+        barrier()
+        if which is stepper:
+            sampler.mark_end()
+        ing = [e[0].elapsed_time(e[1]) for e in ev]
+        att = [e[2].elapsed_time(e[3]) for e in ev]
+        return max_over_ranks(t0.elapsed_time(t1), world, dev), float(np.mean(ing)), float(np.mean(att)), float(np.min(att))
+
+    total_ms, ing_ms, att_ms, att_min_ms = timed_steps(stepper)
     step_bytes = st["kv_bytes"] + 2 * st["ing_payload"]
 
-    # ---- extra: the same steps with the ingest on a side stream (its pages are disjoint from the active
-    # batch, "overlapping between computation and communication")
-    side = torch.cuda.Stream(device=dev)
-    main = torch.cuda.current_stream(dev)
+    # ---- extra: the same step with both kernels in order on one stream (each kernel's time alone, in the step)
+    ser_ms, ser_ing_ms, ser_att_ms, _ = timed_steps(stepper_in_order)
 
-    def step_two_stream():
-        pin, slot = next_rows()
-        with torch.cuda.stream(side):
-            ing_bt_dev.copy_(pin, non_blocking=True)
-            uploaded(slot)
-            hx.kv_ingest(src_k, src_v, layers=1, heads=ci.heads, head_dim=D, src_tp=4, dst_tp=1, dst_rank=0,
-                         dst=cache, block_table=ing_bt_dev, block_table_stride=ing_stride, cu_seqlens=ing_cu,
-                         seq_lens=ing_sl, batch=nI, total_tokens=TI, max_seq_len=2048)
-        hx.decode_attention(out, q, cache, layer=0, q_heads=Hq, block_table=bt, block_table_stride=bt.shape[1],
-                            seq_lens=sl, batch=B, max_seq_len=max_len, workspace=ws, workspace_bytes=ws_bytes)
-
-    barrier()
-    side.wait_stream(main)
-    for _ in range(3):
-        step_two_stream()
-    main.wait_stream(side)
-    barrier()
-    s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    s0.record()
-    side.wait_stream(main)
-    for _ in range(args.steps):
-        step_two_stream()
-    main.wait_stream(side)
-    s1.record()
-    barrier()
-    two_ms = max_over_ranks(s0.elapsed_time(s1), world, dev)
-
-    # ---- extra: the single-stream step with hx_decode_attention_overlapped: the attention grid is a programmatic
-    # dependent of the ingest kernel and starts while the handoff is still landing (disjoint pages)
+    # ---- extra: single stream with hx_decode_attention_overlapped: the attention grid is a programmatic dependent of the
+    # ingest kernel and starts while the handoff is still landing (disjoint pages)
     def step_pdl():
-        pin, slot = next_rows()
-        ing_bt_dev.copy_(pin, non_blocking=True)
-        uploaded(slot)
+        upload_rows()
         hx.kv_ingest(src_k, src_v, layers=1, heads=ci.heads, head_dim=D, src_tp=4, dst_tp=1, dst_rank=0,
                      dst=cache, block_table=ing_bt_dev, block_table_stride=ing_stride, cu_seqlens=ing_cu,
                      seq_lens=ing_sl, batch=nI, total_tokens=TI, max_seq_len=2048)
@@ -342,28 +376,28 @@ def run_hx(args, rank, world, local_rank):
     barrier()
     pdl_ms = max_over_ranks(p0.elapsed_time(p1), world, dev)
 
-    # ---- extra: the same single-stream step captured once in a CUDA graph (row upload + ingest + attention as
-    # three nodes) and replayed; two graphs alternate so that the host can stage step n+1's rows while step n runs
+    # ---- extra: the headline step captured once in a CUDA graph (row upload + hx_decode_step: the fork/join becomes
+    # graph edges) and replayed; two graphs alternate so that the host can stage step n+1's rows while step n runs
+    main = torch.cuda.current_stream(dev)
     graphs = []
     cap = torch.cuda.Stream(device=dev)
+    for name in EV:
+        setattr(stepper.a, name, None)
     for gi in range(2):
         pin_g = torch.empty((nI, ing_stride), dtype=torch.int32).pin_memory()
         dev_g = torch.empty((nI, ing_stride), dtype=torch.int32, device=dev)
         pin_g.numpy()[:] = ing_bt_pins[0].numpy()
+        gstep = hx.DecodeStep(overlap_ingest=1, **dict(step_kw, ing_block_table=dev_g))
         gr = torch.cuda.CUDAGraph()
         cap.wait_stream(main)
         with torch.cuda.graph(gr, stream=cap):
             dev_g.copy_(pin_g, non_blocking=True)
-            hx.kv_ingest(src_k, src_v, layers=1, heads=ci.heads, head_dim=D, src_tp=4, dst_tp=1, dst_rank=0, dst=cache,
-                         block_table=dev_g, block_table_stride=ing_stride, cu_seqlens=ing_cu, seq_lens=ing_sl, batch=nI,
-                         total_tokens=TI, max_seq_len=2048)
-            hx.decode_attention(out, q, cache, layer=0, q_heads=Hq, block_table=bt, block_table_stride=bt.shape[1],
-                                seq_lens=sl, batch=B, max_seq_len=max_len, workspace=ws, workspace_bytes=ws_bytes)
-        graphs.append((gr, pin_g, torch.cuda.Event()))
+            gstep(stream=cap)
+        graphs.append((gr, pin_g, torch.cuda.Event(), gstep))
     main.wait_stream(cap)
 
     def step_graph(n):
-        gr, pin_g, ev = graphs[n & 1]
+        gr, pin_g, ev, _ = graphs[n & 1]
         if prev["ids"] is not None:
             pool.free(prev["ids"])
         rows = pool.alloc_table(st["ing_lens"], ing_stride)
@@ -436,6 +470,7 @@ def run_hx(args, rank, world, local_rank):
     peak, peak_src = measured_peak()
     att_gbs = st["kv_bytes"] / (att_ms * 1e-3) / 1e9
     ing_gbs = 2 * st["ing_payload"] / (ing_ms * 1e-3) / 1e9
+    traffic, traffic_note = ncu_traffic()
 
     extra = {}
     if rank == 0 and not args.no_extra:
@@ -451,12 +486,20 @@ def run_hx(args, rank, world, local_rank):
 
         def fused():
             hx.decode_attention_append(out, q, kn, vn, cache, q_heads=Hq, workspace=ws, workspace_bytes=ws_bytes, **akw)
+
+        def alone():
+            hx.decode_attention(out, q, cache, q_heads=Hq, workspace=ws, workspace_bytes=ws_bytes, **akw)
         m2, _ = time_kernel(torch, two_launches, iters=20)
         m1, _ = time_kernel(torch, fused, iters=20)
+        m0, m0min = time_kernel(torch, alone, iters=20)
+        extra["attention_cfg5_alone"] = {"ms_median": m0, "ms_min": m0min, "kv_GBps": st["kv_bytes"] / m0 / 1e6,
+                                         "frac_of_measured": st["kv_bytes"] / m0 / 1e6 / peak,
+                                         "timing": "one CUDA-event pair per call, nothing else on the GPU"}
         extra["prefill"] = prefill_extra(torch, hx, dev)
         extra["stream_peaks"] = stream_peaks(torch, dev)
         extra["append_cfg5"] = {"append_then_attention_ms": m2, "fused_append_attention_ms": m1,
                                 "note": "hx_kv_append + hx_decode_attention (2 launches) vs hx_decode_attention_append (1 launch)"}
+    clocks = sampler.stop()
 
     line = {
         "metric": METRIC, "value": whole_job_value(step_bytes, args.steps, world, total_ms), "unit": UNIT,
@@ -465,6 +508,7 @@ def run_hx(args, rank, world, local_rank):
         "data": "synthetic (seeded; BASELINE.json length mix stands in for the Azure Conversation trace)",
         "config": {"workload": "configs[4]: LLaMA-2-70B TP=1 decode (B=256, 64q/8kv, D=128, 179 ctx in [128,1024] + 77 in "
                                "[4096,8192], page 16, 1 layer) + per-step ingest of 16x2048-token prompts (prefill TP=4 -> decode TP=1)",
+                   "step": "A1 host alloc/free + row upload, then ONE hx_decode_step(overlap_ingest=1) call",
                    "tokens_in_cache": int(st["lens"].sum()), "attention_kv_bytes": st["kv_bytes"],
                    "ingest_payload_bytes": st["ing_payload"], "l2": "inputs larger than L2 (2.3 GB KV read per step vs 126 MB)",
                    "sm_rate_tuning": "hx_tune_sm_rates once at set-up (outside the timed region)",
@@ -479,33 +523,39 @@ def run_hx(args, rank, world, local_rank):
                 "pull_mode_in_order_ms_per_step": e2e_pull_ms / args.steps,
                 "pull_mode_overlapped_ms_per_step": e2e_pull_ov_ms / args.steps},
         "gpu_launches": int(args.steps * LAUNCHES_PER_STEP),
-        "roofline": {"bound": "hbm", "kernel": "hx_decode_attention (attn_stream_kernel, in-kernel merge)",
+        "roofline": {"bound": "hbm", "kernel": "hx_decode_attention (attn_stream_kernel, in-kernel merge), timed inside the "
+                                               "step with the ingest kernel running beside it",
                      "achieved": att_gbs, "peak": peak, "unit": "GB/s", "frac": att_gbs / peak,
                      "peak_source": peak_src, "frac_of_nominal_8000": att_gbs / NOMINAL_HBM_GBS,
-                     "traffic": NCU_TRAFFIC_BYTES, "algorithmic_bytes": st["kv_bytes"],
-                     "ms": att_ms, "ms_min": att_min_ms},
+                     "traffic": traffic, "traffic_source": traffic_note, "algorithmic_bytes": st["kv_bytes"],
+                     "ms": att_ms, "ms_min": att_min_ms, "ms_alone_in_order_step": ser_att_ms},
         "attention": {"kv_GBps": att_gbs, "tokens_per_s_one_layer": B / (att_ms * 1e-3),
                       "tokens_per_s_80_layers": B / (att_ms * 1e-3 * 80), "ms": att_ms},
         "ingest": {"traffic_GBps": ing_gbs, "payload_GBps": ing_gbs / 2, "frac": ing_gbs / peak,
-                   "frac_of_nominal_8000": ing_gbs / NOMINAL_HBM_GBS, "ms": ing_ms},
+                   "frac_of_nominal_8000": ing_gbs / NOMINAL_HBM_GBS, "ms": ing_ms,
+                   "note": "timed on the library's side stream while the attention runs beside it"},
+        "in_order": {"ms_per_step": ser_ms / args.steps, "value": whole_job_value(step_bytes, args.steps, world, ser_ms), "unit": UNIT,
+                     "ingest_ms": ser_ing_ms, "attention_ms": ser_att_ms,
+                     "ingest_traffic_GBps": 2 * st["ing_payload"] / ser_ing_ms / 1e6,
+                     "ingest_frac_of_measured": 2 * st["ing_payload"] / ser_ing_ms / 1e6 / peak,
+                     "attention_kv_GBps": st["kv_bytes"] / ser_att_ms / 1e6,
+                     "note": "hx_decode_step(overlap_ingest=0): ingest then attention on one stream"},
         "overlapped_launch": {"ms_per_step": pdl_ms / args.steps, "value": whole_job_value(step_bytes, args.steps, world, pdl_ms),
                               "unit": UNIT, "note": "single stream; hx_decode_attention_overlapped starts under the ingest kernel "
                                                     "(programmatic dependent launch, disjoint pages)"},
         "cuda_graph": {"ms_per_step": graph_ms / args.steps, "value": whole_job_value(step_bytes, args.steps, world, graph_ms),
-                       "unit": UNIT, "note": "the single-stream step (row upload, ingest, attention) captured once and replayed"},
-        "two_stream": {"ms_per_step": two_ms / args.steps, "value": whole_job_value(step_bytes, args.steps, world, two_ms),
-                       "unit": UNIT, "note": "ingest on a side stream, attention on the main stream (disjoint pages)"},
+                       "unit": UNIT, "note": "the headline step (row upload + hx_decode_step with its fork/join) captured once and replayed"},
         "other_configs": extra,
     }
     if rank == 0:
         line["cpu_baseline"] = cpu_baseline(st) if world == 1 and not args.no_cpu else None
         print(json.dumps(line), flush=True)
+    hx.shutdown()
     if world > 1:
         dist.destroy_process_group()
 
 
-LAUNCHES_PER_STEP = 2          # ingest rows kernel + attention stream kernel (merge is in-kernel)
-NCU_TRAFFIC_BYTES = 2348367000  # dram read+write bytes per attention launch, ncu --set full (profiles/r01_launches_v6.md)
+LAUNCHES_PER_STEP = 2          # ingest kernel + attention stream kernel (merge is in-kernel)
 
 
 def time_kernel(torch, fn, iters=20, warm=5):
@@ -573,7 +623,7 @@ def other_configs(torch, hx, dev, peak):
         kvb = int(lens.astype(np.int64).sum()) * c.kv_heads * c.head_dim * 4
         res[name] = {"kv_bytes": kvb, "ms_back_to_back": b2b, "ms_median": med, "ms_min": mn, "kv_GBps": kvb / b2b / 1e6,
                      "frac_of_measured": kvb / b2b / 1e6 / peak, "frac_of_nominal_8000": kvb / b2b / 1e6 / NOMINAL_HBM_GBS,
-                     "kv_GBps_per_call_events": kvb / med / 1e6,
+                     "kv_GBps_per_call_events": kvb / med / 1e6, "frac_of_measured_per_call_events": kvb / med / 1e6 / peak,
                      "tokens_per_s_one_layer": c.batch / (b2b * 1e-3),
                      "timing": "kv_GBps from one CUDA-event pair around 40 back-to-back calls; ms_median from an event pair per call",
                      "l2": f"rotating over {copies} cache copies"}
@@ -670,6 +720,48 @@ def run_reference(args, rank):
     }), flush=True)
 
 
+def oracle_table(args):
+    """BASELINE.md section 5 / SURVEY section 8(d): the oracle as it stands, per config, at 1 thread and at all cores, on
+    this box's host cores.  Attention configs run a bounded sample of requests at 1 thread (stated); the whole config
+    at all cores.  configs[3] is one of its 80 layers (the oracle handles it one layer at a time)."""
+    import oracle
+    oracle.build()
+    rows = []
+    allc = oracle.max_threads()
+    for name in ("tiny", "opt30b_tp4", "llama70b_tp2", "llama70b_tp1"):
+        c = W.CONFIGS[name]
+        w = W.make_attention_inputs(c, spare=1.0)
+        for threads, frac in ((1, 1 if name == "tiny" else 8), (allc, 1)):
+            pick = np.arange(0, c.batch, frac)
+            t0 = time.perf_counter()
+            oracle.decode_attention(np.ascontiguousarray(w["q"][pick]), w["k"], w["v"], np.ascontiguousarray(w["block_table"][pick]),
+                                    np.ascontiguousarray(w["seq_lens"][pick]), threads=threads)
+            dt = time.perf_counter() - t0
+            nb = int(w["seq_lens"][pick].astype(np.int64).sum()) * c.kv_heads * c.head_dim * 4
+            rows.append({"config": name, "threads": threads, "requests": len(pick), "of": c.batch, "seconds": dt,
+                         "kv_GBps": nb / dt / 1e9, "tokens_per_s_one_layer": len(pick) / dt})
+    for name, kw in (("tiny_ingest", {}), ("llama70b_ingest", {"layers": 1}), ("llama70b_tp1_ingest", {"src_tp": 4})):
+        c = W.CONFIGS[name]
+        w = W.make_ingest_inputs(c, **kw)
+        for threads in (1, allc):
+            for q in range(w["dst_tp"]):
+                dk = np.zeros((w["layers"], w["num_pages"], w["heads"] // w["dst_tp"], 16, w["head_dim"]), dtype=np.uint16)
+                dv = np.zeros_like(dk)
+                t0 = time.perf_counter()
+                oracle.kv_ingest(w["src_k"], w["src_v"], dk, dv, heads=w["heads"], src_tp=w["src_tp"], dst_tp=w["dst_tp"], dst_rank=q,
+                                 block_table=w["block_table"], cu_seqlens=w["cu_seqlens"], seq_lens=w["seq_lens"], threads=threads)
+                dt = time.perf_counter() - t0
+                rows.append({"config": name, "threads": threads, "dst_rank": q, "layers": w["layers"], "seconds": dt,
+                             "traffic_GBps": 2 * w["payload_bytes"] / w["dst_tp"] / dt / 1e9})
+    print(json.dumps({"oracle_table": rows, "host_cores": os.cpu_count(), "oracle_max_threads": allc}), flush=True)
+
+
+def free_port() -> int:
+    with socket.socket() as s_:
+        s_.bind(("127.0.0.1", 0))
+        return s_.getsockname()[1]
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -678,13 +770,22 @@ def main():
     ap.add_argument("--impl", default="hx", choices=["hx", "reference"])
     ap.add_argument("--no-extra", action="store_true", help="skip the configs[1..3] kernel-only section")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--oracle-table", action="store_true", help="time the oracle per config at 1 thread and all cores, then exit")
     args = ap.parse_args()
+    if args.oracle_table:
+        oracle_table(args)
+        return
+    if args.impl == "reference":
+        run_reference(args, int(os.environ.get("RANK", "0")))     # rank 0 alone works; n_gpus echoes --gpus
+        return
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        # a bare `python bench.py --gpus N`: start the N ranks ourselves (one process per GPU, replicas only)
+        os.execv(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+                                  "--master-addr", "127.0.0.1", "--master-port", str(free_port()),
+                                  os.path.abspath(__file__), *sys.argv[1:]])
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
-        run_reference(args, rank)
-        return
     from paper_2502_07903_b200.build import build
     build()
     run_hx(args, rank, world, local_rank)

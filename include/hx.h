@@ -311,6 +311,9 @@ typedef struct {
   const int32_t* ing_cu_seqlens;  const int32_t* ing_seq_lens;      /* device */
   int32_t ing_batch, ing_total_tokens, ing_max_seq_len;
   int32_t overlap_ingest;
+  /* optional timing: cudaEvent_t handles (or NULL) recorded directly before / after the ingest kernel on the stream
+   * it runs on, and directly before / after the attention kernel on `stream` */
+  void* ev_ingest_begin; void* ev_ingest_end; void* ev_attention_begin; void* ev_attention_end;
 } hx_step_args;
 int hx_decode_step(const hx_step_args* args, void* stream);
 

@@ -63,6 +63,8 @@ class _CStepDevArgs(C.Structure):
         ("ing_cu_seqlens", C.c_void_p), ("ing_seq_lens", C.c_void_p),
         ("ing_batch", C.c_int32), ("ing_total_tokens", C.c_int32), ("ing_max_seq_len", C.c_int32),
         ("overlap_ingest", C.c_int32),
+        ("ev_ingest_begin", C.c_void_p), ("ev_ingest_end", C.c_void_p),
+        ("ev_attention_begin", C.c_void_p), ("ev_attention_end", C.c_void_p),
     ]
 
 
@@ -171,6 +173,8 @@ def _ptr(t) -> Optional[int]:
         return t
     if hasattr(t, "data_ptr"):
         return t.data_ptr()
+    if hasattr(t, "cuda_event"):               # torch.cuda.Event (already recorded once, so the handle exists)
+        return t.cuda_event
     return t.ctypes.data
 
 

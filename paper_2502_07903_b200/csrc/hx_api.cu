@@ -427,15 +427,20 @@ int step_impl(const char* who, const hx_step_args* a, const hx_step_host_args* h
       STEP_CUDA(cudaMemcpyAsync(const_cast<int32_t*>(a->ing_seq_lens), h->ing_seq_lens_host, (size_t)a->ing_batch * 4,
                                 cudaMemcpyHostToDevice, ing_stream));
     }
+    if (a->ev_ingest_begin) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_ingest_begin), ing_stream));
     if (rc == HX_OK && ce == cudaSuccess)
       rc = ingest_common(a->src_k, a->src_v, a->ing_layers, a->heads, a->cache->head_dim, a->src_tp, a->dst_tp, a->dst_rank,
                          a->cache, a->ing_block_table, a->ing_block_table_stride, a->ing_cu_seqlens, a->ing_seq_lens,
                          a->ing_batch, a->ing_total_tokens, a->ing_max_seq_len, static_cast<void*>(ing_stream), false, who, -1, 0, 0);
+    if (a->ev_ingest_end) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_ingest_end), ing_stream));
   }
   if (do_att && rc == HX_OK && ce == cudaSuccess) {
-    rc = attention_common(who, a->out, a->q, nullptr, nullptr, false, false, a->cache, a->layer, a->q_heads, a->block_table,
-                          a->block_table_stride, a->seq_lens, a->batch, a->max_seq_len, a->sm_scale, a->workspace,
-                          a->workspace_bytes, stream_);
+    if (a->ev_attention_begin) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_attention_begin), main_stream));
+    if (rc == HX_OK && ce == cudaSuccess)
+      rc = attention_common(who, a->out, a->q, nullptr, nullptr, false, false, a->cache, a->layer, a->q_heads, a->block_table,
+                            a->block_table_stride, a->seq_lens, a->batch, a->max_seq_len, a->sm_scale, a->workspace,
+                            a->workspace_bytes, stream_);
+    if (a->ev_attention_end) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_attention_end), main_stream));
     if (h) STEP_CUDA(cudaMemcpyAsync(h->out_host, a->out, qbytes, cudaMemcpyDeviceToHost, main_stream));
   }
 #undef STEP_CUDA

@@ -257,3 +257,49 @@ def test_attention_overlapped_validates_like_attention():
             hx.decode_attention_overlapped(0x6000, 0x7000, FakeCache(), **dict(kw, **over))
         assert e.value.status == status, str(e.value)
     hx.decode_attention_overlapped(0, 0, FakeCache(), **dict(kw, batch=0, block_table=0, seq_lens=0))   # HX_OK, no launch
+
+
+# ---------------------------------------------------------------- whole-step entry points
+def _step(**over):
+    kw = dict(out=0x6000, q=0x7000, cache=FakeCache(heads=4), layer=0, q_heads=4, block_table=0x3000, block_table_stride=4,
+              seq_lens=0x4000, batch=2, max_seq_len=64, sm_scale=0.0, workspace=0x5000, workspace_bytes=1 << 30,
+              src_k=[0x10000, 0x20000], src_v=[0x30000, 0x40000], ing_layers=2, heads=4, src_tp=2, dst_tp=1, dst_rank=0,
+              ing_block_table=0x8000, ing_block_table_stride=4, ing_cu_seqlens=0x9000, ing_seq_lens=0xA000, ing_batch=2,
+              ing_total_tokens=100, ing_max_seq_len=64, overlap_ingest=1, stream=0)
+    kw.update(over)
+    hx.decode_step(**kw)
+
+
+@pytest.mark.parametrize("over,status", [
+    # an error in EITHER half is found before anything is enqueued (no CUDA call is made: this runs without a GPU)
+    (dict(layer=2), B.HX_ERR_INVALID_ARG), (dict(q_heads=3), B.HX_ERR_INVALID_ARG), (dict(workspace=0), B.HX_ERR_WORKSPACE),
+    (dict(out=0), B.HX_ERR_INVALID_ARG), (dict(block_table_stride=3), B.HX_ERR_INVALID_ARG),
+    (dict(heads=5), B.HX_ERR_INVALID_ARG), (dict(dst_rank=1), B.HX_ERR_INVALID_ARG), (dict(ing_layers=3), B.HX_ERR_INVALID_ARG),
+    (dict(src_k=[0, 0x20000]), B.HX_ERR_INVALID_ARG), (dict(ing_cu_seqlens=0), B.HX_ERR_INVALID_ARG),
+    (dict(ing_max_seq_len=200), B.HX_ERR_INVALID_ARG), (dict(batch=-1), B.HX_ERR_INVALID_ARG), (dict(ing_batch=-1), B.HX_ERR_INVALID_ARG),
+])
+def test_decode_step_validates_both_halves_before_it_enqueues(over, status):
+    with pytest.raises(hx.HxError) as e:
+        _step(**over)
+    assert e.value.status == status, str(e.value)
+    assert hx.last_error()
+
+
+def test_decode_step_with_nothing_to_do_is_ok():
+    _step(batch=0, ing_batch=0)                                       # HX_OK, nothing enqueued
+
+
+def test_decode_step_host_validates_before_it_enqueues():
+    kw = dict(q_host=0x100, out_host=0x200, q_dev=0x7000, out_dev=0x6000, cache=FakeCache(heads=4), layer=0, q_heads=4,
+              block_table_dev=0x3000, block_table_stride=4, seq_lens_dev=0x4000, batch=2, max_seq_len=64, sm_scale=0.0,
+              workspace=0x5000, workspace_bytes=1 << 30, src_k_host=[0x10000, 0x20000], src_v_host=[0x30000, 0x40000],
+              src_k_dev=[0x50000, 0x60000], src_v_dev=[0x70000, 0x80000], ing_layers=2, heads=4, src_tp=2, dst_tp=1, dst_rank=0,
+              ing_block_table_host=0x300, ing_block_table_stride=4, ing_cu_seqlens_host=0x400, ing_seq_lens_host=0x500,
+              ing_block_table_dev=0x8000, ing_cu_seqlens_dev=0x9000, ing_seq_lens_dev=0xA000, ing_batch=2, ing_total_tokens=100,
+              ing_max_seq_len=64, pull_src=0, overlap_ingest=1, stream=0)
+    for over, status in [(dict(layer=5), B.HX_ERR_INVALID_ARG), (dict(q_host=0), B.HX_ERR_INVALID_ARG),
+                         (dict(ing_seq_lens_host=0), B.HX_ERR_INVALID_ARG), (dict(heads=3), B.HX_ERR_INVALID_ARG),
+                         (dict(workspace_bytes=16), B.HX_ERR_WORKSPACE), (dict(src_k_dev=[0, 0]), B.HX_ERR_INVALID_ARG)]:
+        with pytest.raises(hx.HxError) as e:
+            hx.decode_step_host(**dict(kw, **over))
+        assert e.value.status == status, (over, str(e.value))

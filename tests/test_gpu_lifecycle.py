@@ -1,0 +1,231 @@
+"""The decode-side cache life cycle driven through the library's OWN allocator (SURVEY.md section 3.5, rows A1 -> A3 ->
+A4-A8 -> free), and the ordering guarantees of the overlapped launches."""
+import numpy as np
+import pytest
+
+import workloads as W
+from helpers import MAX_ABS_TOL, REL_L2_TOL, attn_errors, dev_u16, to_dev
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device (no CPU fallback exists)")
+    import paper_2502_07903_b200 as hx
+    import oracle
+    oracle.build()
+    return hx, torch, oracle
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("overlap", [1, 0])
+def test_cache_life_cycle_through_the_page_pool(env, overlap):
+    """Five cfg5-shaped steps (64 q / 8 kv heads, D = 128, heavy-tailed contexts, new 2048-token prompts from a prefill
+    TP = 4 group).  Every step: hx_pool_free of the requests that retired, hx_pool_alloc_table for the new prompts (the
+    LIFO free list hands the retired pages straight back out: page REUSE), upload of their rows, hx_decode_step
+    (ingest of the new prompts + attention over the active batch), then the new prompts replace the retired requests
+    in the batch, so the NEXT step's attention reads what this step ingested.  After every step the whole cache equals
+    the oracle's bit for bit and every output row is within tolerance."""
+    hx, torch, oracle = env
+    Hq, Hkv, D, S = 64, 8, 128, 4
+    B, NEW, NLEN, STRIDE = 48, 4, 2048, 512
+    g = W.rng(5, 40, overlap)
+    lens = np.concatenate([g.integers(128, 1024, size=34, endpoint=True), g.integers(4096, 8192, size=14, endpoint=True)])
+    g.shuffle(lens)
+    lens = lens.astype(np.int32)
+    need = int(W.pages_for(lens).sum())
+    P = need + 2 * NEW * (NLEN // 16) + 64
+    pool = hx.PagePool(P, shuffle_seed=3)
+    bt_np = pool.alloc_table(lens, STRIDE)
+    k_np = W.draw_fp16_normal((1, P, Hkv, 16, D), 5, 41, overlap)
+    v_np = W.draw_fp16_normal((1, P, Hkv, 16, D), 5, 42, overlap)
+    ok, ov = k_np.view(np.uint16).copy(), v_np.view(np.uint16).copy()
+    cache = hx.PagedCache(to_dev(k_np, torch), to_dev(v_np, torch))
+    wsb = hx.decode_attention_workspace_bytes(B, Hq, Hkv, D, 8192)
+    ws = torch.zeros(wsb, dtype=torch.uint8, device="cuda")
+    ci = W.IngestConfig(5, "life", 1, Hkv, D, S, 1, NEW, "x")
+    ilens = np.full(NEW, NLEN, dtype=np.int32)
+    seen_pages = set(bt_np[bt_np >= 0].tolist())
+    reused = 0
+    for step in range(5):
+        # A1: the host allocator places the step's new prompts
+        ibt_np = pool.alloc_table(ilens, NLEN // 16)
+        new_pages = ibt_np[ibt_np >= 0]
+        reused += len(seen_pages & set(new_pages.tolist()))
+        seen_pages |= set(new_pages.tolist())
+        assert not (set(new_pages.tolist()) & set(bt_np[bt_np >= 0].tolist()))          # disjoint from the active batch
+        wi = W.make_ingest_inputs(ci, lens=ilens, src_tp=S, bits=(step % 2 == 0), seed_extra=100 * overlap + step)
+        q_np = W.draw_fp16_normal((B, Hq, D), 5, 43, overlap, step)
+        qd = to_dev(q_np, torch)
+        out = torch.full_like(qd, float("nan"))
+        hx.decode_step(out=out, q=qd, cache=cache, layer=0, q_heads=Hq, block_table=torch.from_numpy(bt_np).cuda(),
+                       block_table_stride=STRIDE, seq_lens=torch.from_numpy(lens).cuda(), batch=B, max_seq_len=int(lens.max()),
+                       sm_scale=0.0, workspace=ws, workspace_bytes=wsb,
+                       src_k=[to_dev(a, torch) for a in wi["src_k"]], src_v=[to_dev(a, torch) for a in wi["src_v"]],
+                       ing_layers=1, heads=Hkv, src_tp=S, dst_tp=1, dst_rank=0, ing_block_table=torch.from_numpy(ibt_np).cuda(),
+                       ing_block_table_stride=NLEN // 16, ing_cu_seqlens=torch.from_numpy(wi["cu_seqlens"]).cuda(),
+                       ing_seq_lens=torch.from_numpy(ilens).cuda(), ing_batch=NEW, ing_total_tokens=NEW * NLEN,
+                       ing_max_seq_len=NLEN, overlap_ingest=overlap)
+        k_after, v_after = cache.k.clone(), cache.v.clone()      # on the caller's stream: after the join
+        torch.cuda.synchronize()
+        # the oracle's step.  overlap = 1 asserts that the attention does not read the new pages, so the order of the
+        # two oracle calls does not matter; overlap = 0 is ingest first
+        oracle.kv_ingest(wi["src_k"], wi["src_v"], ok, ov, heads=Hkv, src_tp=S, dst_tp=1, dst_rank=0, block_table=ibt_np,
+                         cu_seqlens=wi["cu_seqlens"], seq_lens=ilens)
+        ref = oracle.decode_attention(q_np, ok.view(np.float16), ov.view(np.float16), bt_np, lens)
+        assert np.array_equal(dev_u16(k_after), ok) and np.array_equal(dev_u16(v_after), ov), step
+        got = out.cpu().numpy()
+        assert np.isfinite(got.astype(np.float32)).all(), step
+        max_abs, rel = attn_errors(got, ref)
+        assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (step, max_abs, rel)
+        # the NEW oldest requests retire; the new prompts take their batch slots
+        retire = np.arange(step * NEW, step * NEW + NEW) % B
+        for j, i in enumerate(retire):
+            pool.free(bt_np[i][bt_np[i] >= 0])
+            bt_np[i] = -1
+            bt_np[i, :NLEN // 16] = ibt_np[j]
+            lens[i] = NLEN
+    assert reused > 0, "the free list never handed a retired page back out"
+    assert pool.num_free == P - int(W.pages_for(lens).sum())
+
+
+def _long_ingest_setup(hx, torch, oracle, layers):
+    """A handoff of 16 x 2048-token prompts over `layers` layers (~45 us per layer) next to a tiny active batch."""
+    Hkv, D, Hq, S = 8, 128, 64, 4
+    ilens = np.full(16, 2048, dtype=np.int32)
+    T = int(ilens.sum())
+    alens = np.array([40, 100, 17, 300], dtype=np.int32)
+    P = 16 * 128 + int(W.pages_for(alens).sum()) + 32
+    pool = hx.PagePool(P, shuffle_seed=9)
+    abt = pool.alloc_table(alens, 32)
+    ibt = pool.alloc_table(ilens, 128)
+    g = torch.Generator(device="cuda")
+    g.manual_seed(17)
+    sk = [torch.randint(-32768, 32767, (layers, T, Hkv // S, D), dtype=torch.int16, device="cuda", generator=g) for _ in range(S)]
+    sv = [torch.randint(-32768, 32767, (layers, T, Hkv // S, D), dtype=torch.int16, device="cuda", generator=g) for _ in range(S)]
+    checked = (0, layers - 1)                                # the last layer's CTAs run last
+    host = {}
+    for l in checked:
+        hk = [W.draw_u16_bits((1, T, Hkv // S, D), 5, 44, r, l) for r in range(S)]
+        hv = [W.draw_u16_bits((1, T, Hkv // S, D), 5, 45, r, l) for r in range(S)]
+        for r in range(S):
+            sk[r][l].copy_(torch.from_numpy(hk[r][0].view(np.int16)))
+            sv[r][l].copy_(torch.from_numpy(hv[r][0].view(np.int16)))
+        host[l] = (hk, hv)
+    k0 = W.draw_fp16_normal((1, P, Hkv, 16, D), 5, 46)
+    v0 = W.draw_fp16_normal((1, P, Hkv, 16, D), 5, 47)
+    q = W.draw_fp16_normal((len(alens), Hq, D), 5, 48)
+    cu = np.zeros(17, dtype=np.int32)
+    np.cumsum(ilens, out=cu[1:])
+    expect = {}
+    for l in checked:
+        ek, ev = k0.view(np.uint16).copy(), v0.view(np.uint16).copy()
+        oracle.kv_ingest(host[l][0], host[l][1], ek, ev, heads=Hkv, src_tp=S, dst_tp=1, dst_rank=0, block_table=ibt,
+                         cu_seqlens=cu, seq_lens=ilens)
+        expect[l] = (ek[0], ev[0])
+    ref = oracle.decode_attention(q, k0, v0, abt, alens)     # the active batch lives in layer 0's pages, untouched
+    return dict(Hkv=Hkv, D=D, Hq=Hq, S=S, ilens=ilens, T=T, alens=alens, P=P, abt=abt, ibt=ibt, sk=sk, sv=sv, k0=k0, v0=v0,
+                q=q, cu=cu, expect=expect, ref=ref, checked=checked)
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("tuned", [False, True])
+def test_long_ingest_then_tiny_overlapped_attention_then_immediate_read(env, tuned):
+    """include/hx.h promises that work enqueued after hx_decode_attention_overlapped is ordered after BOTH kernels.
+    The hard case: an ingest that runs for more than a millisecond (32 layers, 4.3 GB of traffic), a tiny attention that
+    would be done in microseconds, and a copy of the ingested pages enqueued right behind it.  The copy must hold the
+    complete handoff (checked against the oracle on the first and the last layer, the last one being written last),
+    and the attention's own result must be right; several repetitions, equal ranges and tuned ranges."""
+    hx, torch, oracle = env
+    LAYERS = 32
+    s = _long_ingest_setup(hx, torch, oracle, LAYERS)
+    Hkv, D, Hq, S, P = s["Hkv"], s["D"], s["Hq"], s["S"], s["P"]
+    skh, svh = [t.view(torch.float16) for t in s["sk"]], [t.view(torch.float16) for t in s["sv"]]
+    ibt, cu, isl = torch.from_numpy(s["ibt"]).cuda(), torch.from_numpy(s["cu"]).cuda(), torch.from_numpy(s["ilens"]).cuda()
+    abt, asl = torch.from_numpy(s["abt"]).cuda(), torch.from_numpy(s["alens"]).cuda()
+    qd = to_dev(s["q"], torch)
+    wsb = hx.decode_attention_workspace_bytes(4, Hq, Hkv, D, 300)
+    ws = torch.zeros(wsb, dtype=torch.uint8, device="cuda")
+    base_k = to_dev(s["k0"], torch).expand(LAYERS, -1, -1, -1, -1)
+    base_v = to_dev(s["v0"], torch).expand(LAYERS, -1, -1, -1, -1)
+    if tuned:
+        hx.tune_sm_rates(torch.empty(320 << 20, dtype=torch.uint8, device="cuda"))
+    try:
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for rep in range(4):
+            cache = hx.PagedCache(base_k.contiguous(), base_v.contiguous())
+            out = torch.full_like(qd, float("nan"))
+            torch.cuda.synchronize()
+            t0.record()
+            hx.kv_ingest(skh, svh, layers=LAYERS, heads=Hkv, head_dim=D, src_tp=S, dst_tp=1, dst_rank=0, dst=cache,
+                         block_table=ibt, block_table_stride=128, cu_seqlens=cu, seq_lens=isl, batch=16,
+                         total_tokens=s["T"], max_seq_len=2048)
+            if rep == 0:
+                t1.record()      # only here, to show that the ingest is long: an event between the two launches takes
+                                 # away their kernel-to-kernel adjacency; repetitions 1-3 are back to back
+            hx.decode_attention_overlapped(out, qd, cache, layer=0, q_heads=Hq, block_table=abt, block_table_stride=32,
+                                           seq_lens=asl, batch=4, max_seq_len=300, workspace=ws, workspace_bytes=wsb)
+            k_after = {l: cache.k[l].clone() for l in s["checked"]}      # the immediate read
+            v_after = {l: cache.v[l].clone() for l in s["checked"]}
+            torch.cuda.synchronize()
+            if rep == 0:
+                assert t0.elapsed_time(t1) >= 1.0, "the ingest is meant to run for >= 1 ms"
+            for l in s["checked"]:
+                assert np.array_equal(dev_u16(k_after[l]), s["expect"][l][0]), (rep, l)
+                assert np.array_equal(dev_u16(v_after[l]), s["expect"][l][1]), (rep, l)
+            max_abs, rel = attn_errors(out.cpu().numpy(), s["ref"])
+            assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (rep, max_abs, rel)
+    finally:
+        if tuned:
+            hx.tune_sm_rates(None)
+
+
+@pytest.mark.parametrize("tuned", [False, True])
+def test_overlapped_attention_back_to_back_and_after_an_empty_ingest(env, tuned):
+    """The overlapped launch is a programmatic dependent ONLY directly behind an ingest kernel.  Behind another
+    attention (same workspace: counters and range claims) or behind an hx_kv_ingest that launched nothing
+    (batch == 0) it must behave exactly like hx_decode_attention."""
+    hx, torch, oracle = env
+    Hq, Hkv, D = 32, 4, 128
+    c = W.AttnConfig(88, "t", 24, Hq, Hkv, D, 256, "x")
+    lens = W.rng(88, 1).integers(1, 3000, size=24).astype(np.int32)
+    w = W.make_attention_inputs(c, lens=lens, layers=2)
+    refs = [oracle.decode_attention(w["q"], w["k"], w["v"], w["block_table"], lens, layer=l) for l in (0, 1)]
+    cache = hx.PagedCache(to_dev(w["k"], torch), to_dev(w["v"], torch))
+    qd = to_dev(w["q"], torch)
+    bt, sl = torch.from_numpy(w["block_table"]).cuda(), torch.from_numpy(lens).cuda()
+    mx = int(lens.max())
+    wsb = hx.decode_attention_workspace_bytes(24, Hq, Hkv, D, mx)
+    ws = torch.zeros(wsb, dtype=torch.uint8, device="cuda")
+    kw = dict(q_heads=Hq, block_table=bt, block_table_stride=bt.shape[1], seq_lens=sl, batch=24, max_seq_len=mx, workspace=ws,
+              workspace_bytes=wsb)
+    empty = torch.zeros(1, dtype=torch.int32, device="cuda")
+    if tuned:
+        hx.tune_sm_rates(torch.empty(320 << 20, dtype=torch.uint8, device="cuda"))
+    try:
+        outs = [torch.full_like(qd, float("nan")) for _ in range(6)]
+        for j in range(0, 6, 2):                             # six launches back to back, alternating layers
+            hx.decode_attention_overlapped(outs[j], qd, cache, layer=0, **kw)
+            hx.decode_attention_overlapped(outs[j + 1], qd, cache, layer=1, **kw)
+        torch.cuda.synchronize()
+        for j, o in enumerate(outs):
+            max_abs, rel = attn_errors(o.cpu().numpy(), refs[j % 2])
+            assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (j, max_abs, rel)
+        for j in range(2, 6):                                # same table, same inputs -> same bits
+            assert torch.equal(outs[j].view(torch.int16), outs[j % 2].view(torch.int16)), j
+        # an ingest of an empty batch launches nothing: the call behind it follows whatever ran before
+        out = torch.full_like(qd, float("nan"))
+        hx.decode_attention(outs[0], qd, cache, layer=1, **kw)
+        hx.kv_ingest([empty.view(torch.float16)] * 2, [empty.view(torch.float16)] * 2, layers=1, heads=Hkv, head_dim=D, src_tp=2,
+                     dst_tp=1, dst_rank=0, dst=cache, block_table=empty, block_table_stride=1, cu_seqlens=empty, seq_lens=empty,
+                     batch=0, total_tokens=0, max_seq_len=0)
+        hx.decode_attention_overlapped(out, qd, cache, layer=0, **kw)
+        torch.cuda.synchronize()
+        max_abs, rel = attn_errors(out.cpu().numpy(), refs[0])
+        assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (max_abs, rel)
+    finally:
+        if tuned:
+            hx.tune_sm_rates(None)
