@@ -262,7 +262,6 @@ def run_hx(args, rank, world, local_rank):
     sl = torch.from_numpy(st["lens"]).to(dev)
     ws_bytes = hx.decode_attention_workspace_bytes(B, Hq, Hkv, D, max_len)
     ws = torch.zeros(max(ws_bytes, 16), dtype=torch.uint8, device=dev)
-    hx.tune_sm_rates(cache.k)            # once per process: per-SM range sizes; reads the cache only
     # ingest sources resident in HBM (the prefill shards as they arrived)
     src_k = [torch.from_numpy(a.view(np.int16)).to(dev).view(torch.float16) for a in ing["src_k"]]
     src_v = [torch.from_numpy(a.view(np.int16)).to(dev).view(torch.float16) for a in ing["src_v"]]
@@ -511,7 +510,6 @@ def run_hx(args, rank, world, local_rank):
                    "step": "A1 host alloc/free + row upload, then ONE hx_decode_step(overlap_ingest=1) call",
                    "tokens_in_cache": int(st["lens"].sum()), "attention_kv_bytes": st["kv_bytes"],
                    "ingest_payload_bytes": st["ing_payload"], "l2": "inputs larger than L2 (2.3 GB KV read per step vs 126 MB)",
-                   "sm_rate_tuning": "hx_tune_sm_rates once at set-up (outside the timed region)",
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
         "clocks": clocks,
         "e2e": {"value": whole_job_value(step_bytes, args.steps, world, e2e_ms), "unit": UNIT,
@@ -618,14 +616,34 @@ def other_configs(torch, hx, dev, peak):
             hx.decode_attention(out, q, cache, layer=state["i"], q_heads=c.q_heads, block_table=bt,
                                 block_table_stride=bt.shape[1], seq_lens=sl, batch=c.batch, max_seq_len=mx,
                                 workspace=ws, workspace_bytes=wsb)
+        plan = torch.empty(hx.decode_plan_bytes(c.batch, c.kv_heads, mx), dtype=torch.uint8, device=dev)
+        hx.decode_plan(plan, cache, q_heads=c.q_heads, block_table=bt, block_table_stride=bt.shape[1], seq_lens=sl, batch=c.batch,
+                       max_seq_len=mx)
+
+        def fn_planned():
+            state["i"] = (state["i"] + 1) % copies
+            hx.decode_attention_planned(out, q, cache, layer=state["i"], q_heads=c.q_heads, plan=plan, batch=c.batch,
+                                        max_seq_len=mx, workspace=ws, workspace_bytes=wsb)
         med, mn = time_kernel(torch, fn, iters=40)               # one event pair per call (adds ~2 us of event work)
         b2b = time_back_to_back(torch, fn)                       # one event pair around 40 calls: the layer-loop rate
+        medp, mnp = time_kernel(torch, fn_planned, iters=40)
+        b2bp = time_back_to_back(torch, fn_planned)
+        plan_ms, _ = time_kernel(torch, lambda: hx.decode_plan(plan, cache, q_heads=c.q_heads, block_table=bt,
+                                                               block_table_stride=bt.shape[1], seq_lens=sl, batch=c.batch,
+                                                               max_seq_len=mx), iters=10)
         kvb = int(lens.astype(np.int64).sum()) * c.kv_heads * c.head_dim * 4
-        res[name] = {"kv_bytes": kvb, "ms_back_to_back": b2b, "ms_median": med, "ms_min": mn, "kv_GBps": kvb / b2b / 1e6,
-                     "frac_of_measured": kvb / b2b / 1e6 / peak, "frac_of_nominal_8000": kvb / b2b / 1e6 / NOMINAL_HBM_GBS,
-                     "kv_GBps_per_call_events": kvb / med / 1e6, "frac_of_measured_per_call_events": kvb / med / 1e6 / peak,
-                     "tokens_per_s_one_layer": c.batch / (b2b * 1e-3),
-                     "timing": "kv_GBps from one CUDA-event pair around 40 back-to-back calls; ms_median from an event pair per call",
+        res[name] = {"kv_bytes": kvb,
+                     "per_call_events": {"ms_median": med, "ms_min": mn, "kv_GBps": kvb / med / 1e6, "frac_of_measured": kvb / med / 1e6 / peak,
+                                         "frac_of_nominal_8000": kvb / med / 1e6 / NOMINAL_HBM_GBS},
+                     "back_to_back": {"ms": b2b, "kv_GBps": kvb / b2b / 1e6, "frac_of_measured": kvb / b2b / 1e6 / peak},
+                     "planned_per_call_events": {"ms_median": medp, "ms_min": mnp, "kv_GBps": kvb / medp / 1e6,
+                                                 "frac_of_measured": kvb / medp / 1e6 / peak,
+                                                 "frac_of_nominal_8000": kvb / medp / 1e6 / NOMINAL_HBM_GBS},
+                     "planned_back_to_back": {"ms": b2bp, "kv_GBps": kvb / b2bp / 1e6, "frac_of_measured": kvb / b2bp / 1e6 / peak},
+                     "plan_ms": plan_ms, "tokens_per_s_one_layer": c.batch / (medp * 1e-3),
+                     "timing": "per_call_events: one CUDA-event pair per call (SURVEY 8(d) protocol), median of 40; back_to_back: one event "
+                               "pair around 40 calls; planned_*: hx_decode_plan once (plan_ms), then hx_decode_attention_planned per call, "
+                               "as the layer loop of a decode step issues them",
                      "l2": f"rotating over {copies} cache copies"}
         del k, v, cache
     # configs[3]: 80-layer ingest, prefill TP=4 -> decode TP=2, both destination ranks

@@ -10,11 +10,11 @@
  * Conventions (all entry points)
  *  - Payload is IEEE fp16 (B_type = 2).  fp32 accumulation inside attention.
  *  - DEVICE pointers are marked "device"; everything else is host memory.  The caller owns all
- *    device memory, including the workspace.  The library allocates no device memory.  Its state:
- *    (1) the optional SM rate table of hx_tune_sm_rates (a static __device__ array); (2) per device, one
- *    side stream and two events, created by the first hx_decode_step / hx_decode_step_host call that
- *    asks for an overlapped handoff and destroyed by hx_shutdown(); (3) host-side caches of device
- *    properties and TMA descriptors.  hx_page_pool is the only heap object the caller owns (host).
+ *    device memory, including the workspace.  The library allocates no device memory and keeps no
+ *    state on the device.  Its host-side state: (1) per device, one side stream and two events, created
+ *    by the first hx_decode_step / hx_decode_step_host call that asks for an overlapped handoff and
+ *    destroyed by hx_shutdown(); (2) caches of device properties and TMA descriptors.  hx_page_pool is
+ *    the only heap object the caller owns (host).
  *  - Thread safety: every entry point may be called from several host threads (on different streams);
  *    hx_decode_step* serialise on one library mutex while they enqueue.  An hx_page_pool and an attention
  *    workspace each serve one caller at a time.
@@ -28,8 +28,9 @@
  *    page ids in [0, num_pages); row i of the block table holds ceil(n_i/page_size) valid
  *    entries; cu_seqlens is the exclusive prefix sum of seq_lens; ingest destinations are
  *    pairwise distinct.  Attention may read a page shared by several requests.
- *  - Determinism: same inputs -> same bits, run to run (no floating-point atomics; partial
- *    results are merged in a fixed order).
+ *  - Determinism: same inputs -> same bits, run to run, on a given GPU model (no floating-point
+ *    atomics; the work partition depends only on seq_lens and the SM count; partial results are
+ *    merged in a fixed order).
  *
  * Layouts (readings S4, S7, S8, S9)
  *  - Source shard r of a prefill TP group of degree S:  fp16 [layers][total_tokens][heads/S][head_dim]
@@ -53,7 +54,7 @@
 extern "C" {
 #endif
 
-#define HX_VERSION 130 /* 0.1.3.0: + hx_decode_step (device buffers), hx_shutdown; overlapped launch waits for the ingest */
+#define HX_VERSION 131 /* 0.1.3.1: + hx_decode_step (device buffers), hx_shutdown, per-step plan; - hx_tune_sm_rates */
 
 typedef enum {
   HX_OK = 0,
@@ -258,14 +259,36 @@ int hx_prefill_attention(void* out, const void* q,
                          int32_t batch, int32_t total_q_tokens, int32_t max_q_len, int32_t max_seq_len,
                          float sm_scale, void* stream);
 
-/* Optional, once per process and device: measure how fast each SM streams from HBM when all SMs
- * load at once, and size hx_decode_attention's per-SM ranges accordingly.  On B200 the SMs fall into
- * stable rate classes (about 1.19 / 1.00 / 0.88 of the mean), so equal ranges leave the fast SMs
- * idle at the end of the kernel.  `scratch` is any device buffer of >= 256 MiB
- * (e.g. the KV cache itself); it is only read.  Enqueues ~0.3 ms of probe kernels on `stream`.
- * The table is library state in device memory; scratch == NULL resets it to equal ranges.
- * Results stay deterministic for a given table: same inputs -> same bits until the next tune. */
-int hx_tune_sm_rates(const void* scratch, size_t scratch_bytes, void* stream);
+/* ---- (b') per-step plan for the layer calls of a decode step ------------------------------
+ * A model calls hx_decode_attention once per layer (80 times per step for LLaMA-2-70B), every time with the SAME
+ * seq_lens and block table (reading S9: one table serves every layer).  What the kernel derives from those two
+ * alone - the page-count prefix sums, the work partition (row A4) and, per (request, kv head, page) tile, the cache
+ * row to load - can be computed once per step: hx_decode_plan writes it into a caller-owned device buffer, and
+ * hx_decode_attention_planned is hx_decode_attention reading that buffer instead of seq_lens / block_table (its
+ * first K/V load is issued after one L2 round trip instead of a scan, a search and a table load).  Same work
+ * partition, same arithmetic: the result is bit-identical to hx_decode_attention's.
+ *
+ * plan        : device, 16-byte aligned, >= hx_decode_plan_bytes(batch, cache->kv_heads, max_seq_len, page_size)
+ *               bytes.  Valid for the (seq_lens, block_table, batch, q_heads, kv_heads) it was made from, on the
+ *               device it was made on, until one of them changes; any number of layer calls may read it.
+ * batch       : <= 2048 (HX_ERR_UNSUPPORTED above).
+ * Device-side contract: the plan passed to hx_decode_attention_planned was written by hx_decode_plan with the same
+ * batch and head counts (the kernel checks the plan's header and traps on a mismatch). */
+size_t hx_decode_plan_bytes(int32_t batch, int32_t kv_heads, int32_t max_seq_len, int32_t page_size);
+
+int hx_decode_plan(void* plan, size_t plan_bytes,
+                   const hx_paged_cache* cache, int32_t q_heads,
+                   const int32_t* block_table, int32_t block_table_stride,
+                   const int32_t* seq_lens,
+                   int32_t batch, int32_t max_seq_len,
+                   void* stream);
+
+int hx_decode_attention_planned(void* out, const void* q,
+                                const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
+                                const void* plan, size_t plan_bytes,
+                                int32_t batch, int32_t max_seq_len, float sm_scale,
+                                void* workspace, size_t workspace_bytes,
+                                void* stream);
 
 /* ---- host page allocator (paging by citation PAPER.md:L110, OOM
  * remark PAPER.md:L136).  A free list of page ids; alloc is all-or-nothing.  Not thread-safe. */

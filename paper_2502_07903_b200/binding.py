@@ -15,7 +15,8 @@ EXPORTS = [
     "hx_version", "hx_status_string", "hx_last_error", "hx_paged_cache_bytes", "hx_kv_ingest",
     "hx_kv_gather", "hx_decode_attention_workspace_bytes", "hx_decode_attention", "hx_pool_create",
     "hx_pool_shuffle", "hx_pool_alloc", "hx_pool_free", "hx_pool_num_free", "hx_pool_num_pages",
-    "hx_pool_alloc_table", "hx_pool_destroy", "hx_decode_step_host", "hx_tune_sm_rates",
+    "hx_pool_alloc_table", "hx_pool_destroy", "hx_decode_step_host", "hx_decode_plan_bytes", "hx_decode_plan",
+    "hx_decode_attention_planned",
     "hx_kv_ingest_stage", "hx_stage_overlap", "hx_kv_append", "hx_decode_attention_append",
     "hx_prefill_attention", "hx_decode_attention_overlapped", "hx_decode_step", "hx_shutdown",
 ]
@@ -114,8 +115,14 @@ def lib() -> C.CDLL:
         L.hx_pool_alloc_table.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32]
         L.hx_pool_destroy.restype = None
         L.hx_pool_destroy.argtypes = [C.c_void_p]
-        L.hx_tune_sm_rates.restype = C.c_int
-        L.hx_tune_sm_rates.argtypes = [C.c_void_p, C.c_size_t, C.c_void_p]
+        L.hx_decode_plan_bytes.restype = C.c_size_t
+        L.hx_decode_plan_bytes.argtypes = [C.c_int32] * 4
+        L.hx_decode_plan.restype = C.c_int
+        L.hx_decode_plan.argtypes = [C.c_void_p, C.c_size_t, C.POINTER(_CCache), C.c_int32, C.c_void_p, C.c_int32, C.c_void_p,
+                                     C.c_int32, C.c_int32, C.c_void_p]
+        L.hx_decode_attention_planned.restype = C.c_int
+        L.hx_decode_attention_planned.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CCache), C.c_int32, C.c_int32, C.c_void_p,
+                                                  C.c_size_t, C.c_int32, C.c_int32, C.c_float, C.c_void_p, C.c_size_t, C.c_void_p]
         L.hx_kv_ingest_stage.restype = C.c_int
         L.hx_kv_ingest_stage.argtypes = [C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)] + [C.c_int32] * 9 + [
             C.POINTER(_CCache), C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32,
@@ -309,14 +316,29 @@ def decode_attention_overlapped(out, q, cache: PagedCache, *, layer, q_heads, bl
                                                 _stream_ptr(stream)))
 
 
-def tune_sm_rates(scratch=None, scratch_bytes=None, stream=None):
-    """hx_tune_sm_rates: scratch is a device tensor of >= 256 MiB (only read); None resets."""
-    if scratch is None:
-        _check(lib().hx_tune_sm_rates(None, 0, _stream_ptr(stream)))
-        return
-    if scratch_bytes is None:
-        scratch_bytes = scratch.numel() * scratch.element_size()
-    _check(lib().hx_tune_sm_rates(_ptr(scratch), scratch_bytes, _stream_ptr(stream)))
+def decode_plan_bytes(batch, kv_heads, max_seq_len, page_size=16) -> int:
+    return int(lib().hx_decode_plan_bytes(batch, kv_heads, max_seq_len, page_size))
+
+
+def decode_plan(plan, cache: PagedCache, *, q_heads, block_table, block_table_stride, seq_lens, batch, max_seq_len,
+                plan_bytes=None, stream=None):
+    """hx_decode_plan (include/hx.h): once per decode step; `plan` is a device byte tensor of >= decode_plan_bytes()."""
+    if plan_bytes is None:
+        plan_bytes = plan.numel() * plan.element_size()
+    _check(lib().hx_decode_plan(_ptr(plan), plan_bytes, cache.ref, q_heads, _ptr(block_table), block_table_stride,
+                                _ptr(seq_lens), batch, max_seq_len, _stream_ptr(stream)))
+
+
+def decode_attention_planned(out, q, cache: PagedCache, *, layer, q_heads, plan, batch, max_seq_len, sm_scale=0.0,
+                             workspace=None, workspace_bytes=None, plan_bytes=None, stream=None):
+    """hx_decode_attention_planned: hx_decode_attention reading a plan instead of seq_lens / block_table."""
+    if workspace_bytes is None:
+        workspace_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    if plan_bytes is None:
+        plan_bytes = plan.numel() * plan.element_size()
+    _check(lib().hx_decode_attention_planned(_ptr(out), _ptr(q), cache.ref, layer, q_heads, _ptr(plan), plan_bytes, batch,
+                                             max_seq_len, C.c_float(sm_scale), _ptr(workspace), workspace_bytes,
+                                             _stream_ptr(stream)))
 
 
 def _fill_struct(a, kw):

@@ -2,17 +2,24 @@
 // FlashAttention and gives no kernel: the design below is ours, for sm_100a).
 //
 // Roofline: HBM.  Algorithmic bytes = sum_i n_i * kv_heads * head_dim * 2 tensors * 2 B; G flops
-// per byte (G = q heads per kv head), so the job is to keep ~50 KB of loads in flight per SM and
-// to spend as few issue slots as possible per 8 KiB (page, kv-head) K+V tile.
+// per byte (G = q heads per kv head), so the job is to keep HBM saturated from every SM and to
+// spend as few issue slots as possible per 8 KiB (page, kv-head) K+V tile.
 //
 // attn_stream_kernel — "stream-K over page tiles":
 //  * The work is the linear sequence of (request, kv head, page) tiles.  Every warp of a
 //    persistent grid (one CTA per SM, 8 warps) owns an equal contiguous range of that sequence
-//    (row A4: the cut depends only on seq_lens and the grid size, never on page placement, so the
-//    result is bit-identical under page permutation and from run to run).
-//  * Each warp runs its own 3-stage ring: lane 0 issues one TMA tensor-tile load per K tile and
-//    per V tile (cp.async.bulk.tensor, 128-byte swizzle, mbarrier complete_tx); block-table
-//    entries are fetched 32-64 tiles ahead, one per lane.  No CTA-wide barrier after setup.
+//    (row A4: the cut depends only on seq_lens and the grid size, never on page placement or on
+//    timing, so the result is bit-identical under page permutation and from run to run).
+//  * A tile is described by a 16-byte descriptor (cache row, first query row, context length, page
+//    index).  Lanes produce descriptors 32-64 tiles ahead: either by a binary search over the page
+//    prefix sums plus one block-table load (hx_decode_attention), or by one coalesced load from a
+//    per-step PLAN that hx_decode_plan wrote once for all the layer calls of a decode step
+//    (hx_decode_attention_planned: no prefix sums, no search, first TMA issued after one L2 hop).
+//  * Each warp runs its own 2-stage ring: lane 0 issues one TMA tensor-tile load per K tile and
+//    per V tile (cp.async.bulk.tensor, 128-byte swizzle, mbarrier complete_tx).  No CTA-wide
+//    barrier after setup.  Two stages x 8 warps = 128 KiB in flight per SM: enough to saturate HBM
+//    (7.4-8 TB/s of reads while all SMs stream), and the SMs share it far more evenly than with
+//    three.
 //  * Scores (row A5) and PV (row A7) run on mma.sync.m16n8k16 with the page as M (16 tokens) and
 //    the GQA group as N (8 heads): S^T = K Q^T and O^T += V^T P^T, so one K/V tile serves all G
 //    query heads from shared memory and nothing is padded along tokens.  Online softmax (row A6)
@@ -27,6 +34,7 @@
 #include <cuda.h>
 #include <cuda_fp16.h>
 
+#include <cstring>
 #include <mutex>
 
 #include "hx_internal.h"
@@ -39,10 +47,12 @@ constexpr int kBMax = 2048;        // requests per launch (prefix sums live in s
 constexpr int kMaxWorkers = 2048;  // workspace is sized for this many workers (>= SMs * kWarps)
 constexpr int kMaxSm = 256;        // CTAs (= SMs) per launch
 constexpr float kLog2e = 1.4426950408889634f;
+constexpr int kPlanMagic = 0x68785032;
+constexpr int kPlanHeaderInts = 16;
 
 template <int D, int NT>
 struct Cfg {
-  static constexpr int kStages = (NT == 1) ? 3 : 2;
+  static constexpr int kStages = 2;                  // 16 tiles (128 KiB) in flight per SM: see DESIGN.md 6.3
   static constexpr int kTile = 16 * D * 2;           // bytes of one (page, head) K or V tile
   static constexpr int kStage = 2 * kTile;           // K + V
   static constexpr int kQBytes = NT * 8 * D * 2;     // Q slot: NT*8 heads
@@ -50,8 +60,21 @@ struct Cfg {
   static constexpr int kMT = D / 16;                 // m-tiles of PV
   static constexpr int kSlotFloats = NT * (kMT * 128 + 16);   // partial: acc[NT][MT][32][4], m[NT][8], l[NT][8]
   static constexpr int kSmem = kWarps * kStages * kStage + kWarps * kQBytes + kWarps * (kStages + 1) * 8 +
-                               (kBMax + 1) * 4 + kBMax * 4 + (kMaxSm + 1) * 4 + 16;
+                               (kBMax + 1) * 4 + kBMax * 4 + 16;
 };
+
+// A per-step plan (hx_decode_plan), int32 words:
+//   [0, 16)                header: magic, B, Hkv, Hq, nC, N (tiles), n_empty
+//   [16, 16 + B)           indices of the requests with an empty context (n_empty of them)
+//   first[W][32] x int4    the first 32 descriptors of every worker's range (so that a warp needs ONE load)
+//   tiles[N] x int4        descriptor of every tile
+struct PlanView {
+  const int32_t* header;
+  const int32_t* empty;
+  const int4* first;
+  const int4* tiles;
+};
+__host__ __device__ inline size_t plan_first_offset_ints(int B) { return (size_t)((kPlanHeaderInts + B + 3) & ~3); }
 
 struct StreamParams {
   const __half* q;
@@ -60,7 +83,6 @@ struct StreamParams {
   const int32_t* lens;
   float* partials;        // [2 * W][kSlotFloats]
   int32_t* counters;      // [B * Hkv] arrival counters of split pairs; zero between calls
-  int32_t* claim;         // [kMaxSm] range-claim flags + [kMaxSm] finished-CTA counter; zero between calls
   int32_t B, Hq, Hkv, G, bt_stride;
   uint32_t layer_row0;    // first tensor-map row of the layer
   float scale_log2;
@@ -74,6 +96,7 @@ struct StreamParams {
   // reads nothing that kernel writes; every CTA executes griddepcontrol.wait before it exits, so completion of this
   // grid implies completion (and visibility) of the ingest
   int32_t pdl_wait_at_end;
+  const int32_t* plan;    // hx_decode_attention_planned
 };
 
 // ---------------------------------------------------------------------------- PTX helpers
@@ -137,122 +160,107 @@ __device__ __forceinline__ float ex2(float x) {
   return y;
 }
 
-struct Loc { int i, g, j, np; };
 
-// tile index k -> (request, kv head, page-in-request).  Tiles are ordered request-major, then kv
-// head, then page: request i owns [Hkv*cum[i], Hkv*cum[i+1]).
-__device__ __forceinline__ Loc locate(long long k, const int* cum, int B, int Hkv) {
+// ---------------------------------------------------------------------------- work partition (row A4)
+// Tiles are ordered request-major, then kv head, then page: request i owns [Hkv*cum[i], Hkv*cum[i+1]).
+// CTA-level range s of nC is [N*s/nC, N*(s+1)/nC); worker (s, j) owns the j-th of its 8 equal parts.
+__device__ __forceinline__ int cta_lo(int s, int N, int nC) { return (int)((long long)N * s / nC); }
+__device__ __forceinline__ int worker_lo(int ww, int N, int nC) {
+  const int s = ww >> 3, j = ww & 7;
+  const int lo = cta_lo(s, N, nC), hi = cta_lo(s + 1, N, nC);
+  return lo + (int)((long long)(hi - lo) * j >> 3);
+}
+__device__ __forceinline__ int owner_of(int k, int N, int nC) {          // worker whose range holds tile k
+  const int s = (int)((((long long)k + 1) * nC - 1) / N);               // largest s with cta_lo(s) <= k
+  const int lo = cta_lo(s, N, nC), len = cta_lo(s + 1, N, nC) - lo;
+  return s * 8 + (int)((((unsigned)(k - lo) + 1u) * 8u - 1u) / (unsigned)len);   // len < 2^28 (host check)
+}
+
+// descriptor of tile k: x = cache row of the tile's first token within a layer (page*Hkv*16 + g*16),
+// y = first query row (i*Hq + g*G), z = context length n_i, w = page index j within the request
+__device__ __forceinline__ int4 make_desc(long long k, const int* cum, const int* slen, int B, int Hkv, int Hq, int G,
+                                          const int32_t* bt, int bt_stride) {
   int lo = 0, hi = B;     // invariant: Hkv*cum[lo] <= k < Hkv*cum[hi]
   while (hi - lo > 1) {
     const int mid = (lo + hi) >> 1;
     if ((long long)Hkv * cum[mid] <= k) lo = mid; else hi = mid;
   }
-  Loc r;
-  r.i = lo;
-  r.np = cum[lo + 1] - cum[lo];
+  const int np = cum[lo + 1] - cum[lo];
   const int rem = (int)(k - (long long)Hkv * cum[lo]);
-  r.g = rem / r.np;
-  r.j = rem - r.g * r.np;
-  return r;
+  const int g = rem / np, j = rem - g * np;
+  const int page = __ldg(bt + (size_t)lo * bt_stride + j);
+  return make_int4(page * (Hkv * 16) + g * 16, lo * Hq + g * G, slen[lo], j);
+}
+
+// Page-count prefix sums of the batch in shared memory: slen[i] = max(n_i, 0), cum[i] = pages before request i.
+// Called by every thread of a 256-thread CTA; ends with a __syncthreads().
+__device__ __forceinline__ void prefix_pages(const int32_t* lens, int B, int* slen, int* cum) {
+  constexpr int PER = kBMax / (kWarps * 32);
+  constexpr uint32_t FULL = 0xffffffffu;
+  __shared__ int warp_tot[kWarps];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  int np[PER], sum = 0;
+#pragma unroll
+  for (int e = 0; e < PER; ++e) {
+    const int i = tid * PER + e;
+    const int n = (i < B) ? max(__ldg(lens + i), 0) : 0;
+    if (i < B) slen[i] = n;
+    np[e] = (n + 15) >> 4;
+    sum += np[e];
+  }
+  int incl = sum;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int t = __shfl_up_sync(FULL, incl, o);
+    if (lane >= o) incl += t;
+  }
+  if (lane == 31) warp_tot[warp] = incl;
+  __syncthreads();
+  int off = incl - sum;
+  for (int w = 0; w < warp; ++w) off += warp_tot[w];
+  if (tid == 0) cum[0] = 0;
+#pragma unroll
+  for (int e = 0; e < PER; ++e) {
+    const int i = tid * PER + e;
+    off += np[e];
+    if (i < B) cum[i + 1] = off;
+  }
+  __syncthreads();
 }
 
 // ------------------------------------------------------------------------------------------
-// SM streaming-rate table (hx_tune_sm_rates).  On B200 the SMs do not stream from HBM at the same
-// rate when all of them load at once: they fall into stable classes (about 1.19 / 1.00 / 0.88 of
-// the mean; TPC pairs alike), a property of the chip's fabric.  With equal ranges the kernel waits
-// for the slow class.  The table holds a per-SM weight in 1/256 of the median rate; range sizes
-// follow it.  g_sm_w_n == 0 means "not tuned": equal ranges.
-__device__ int g_sm_w[kMaxSm];
-__device__ int g_sm_w_n;
-__device__ unsigned int g_sm_cnt[kMaxSm];
-
-// Every SM streams 8 KiB bulk copies from `scratch` through the same per-warp rings as the
-// attention kernel for a fixed time window and counts what it got.
+// hx_decode_plan: everything of a decode step's attention that depends only on seq_lens and the block table,
+// computed once for all the layer calls of the step.  Same grid as the attention kernel.
 __global__ void __launch_bounds__(kWarps * 32, 1)
-sm_rate_probe_kernel(const uint8_t* scratch, unsigned long long chunks, unsigned int window_ns) {
-  extern __shared__ __align__(1024) uint8_t smem[];
-  constexpr int kStages = 3, kStage = 8192;
-  __shared__ uint64_t bars[kWarps * kStages];
-  __shared__ unsigned int warp_cnt[kWarps];
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  if (lane == 0) {
-    for (int s = 0; s < kStages; ++s) mbar_init(smem_u32(&bars[warp * kStages + s]), 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  __syncthreads();
-  unsigned int smid;
-  asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-  unsigned long long t0, t;
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
-  unsigned long long h = (unsigned long long)(smid * kWarps + warp) * 0x9E3779B97F4A7C15ull + 12345;
-  const uint32_t stage0 = smem_u32(smem + warp * kStages * kStage);
-  auto issue = [&](int n) {
-    h = h * 6364136223846793005ull + 1442695040888963407ull;
-    const unsigned long long c = (h >> 20) % chunks;
-    const uint32_t bar = smem_u32(&bars[warp * kStages + n % kStages]);
-    mbar_expect_tx(bar, kStage);
-    bulk_load(stage0 + (n % kStages) * kStage, scratch + c * kStage, kStage, bar);
-  };
-  unsigned int n = 0;
-  if (lane == 0) for (int s = 0; s < kStages; ++s) issue(s);
-  while (true) {
-    mbar_wait(smem_u32(&bars[warp * kStages + n % kStages]), (n / kStages) & 1);
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    if (t - t0 >= window_ns) break;
-    if (lane == 0) issue(n + kStages);
-    ++n;
-  }
-  // drain what is still in flight so that no bulk copy outlives the CTA
-  for (unsigned int e = n + 1; e < n + kStages; ++e) mbar_wait(smem_u32(&bars[warp * kStages + e % kStages]), (e / kStages) & 1);
-  if (lane == 0) warp_cnt[warp] = n;
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    unsigned int tot = 0;
-    for (int w2 = 0; w2 < kWarps; ++w2) tot += warp_cnt[w2];
-    if (smid < kMaxSm) atomicMax(&g_sm_cnt[smid], tot);
-  }
-}
-
-// One CTA: raw[s] = count[s] / median count; weight[s] = 256 * (1 + damp * (raw - 1)) rounded to a
-// multiple of 8 (3 %: keeps the table stable from run to run) and clamped to [192, 352].  damp < 1
-// because HBM is a shared, saturated pie: an SM that is given more work also runs longer against
-// fewer competitors, so the probe's rate spread overstates the spread that balances the kernel.
-// SMs that saw no probe CTA get the nominal 256.
-__global__ void sm_rate_finalize_kernel(int n_sm, int reset, int damp_256) {
-  __shared__ unsigned int cnt[kMaxSm];
-  __shared__ unsigned int median;
-  const int t = threadIdx.x;
-  if (reset) {
-    if (t < kMaxSm) { g_sm_w[t] = 256; g_sm_cnt[t] = 0; }
-    if (t == 0) g_sm_w_n = 0;
-    return;
-  }
-  if (t < kMaxSm) cnt[t] = t < n_sm ? g_sm_cnt[t] : 0;
-  if (t == 0) median = 0;
-  __syncthreads();
-  if (t < n_sm && cnt[t] > 0) {
-    int below = 0, valid = 0;
-    for (int u = 0; u < n_sm; ++u)
-      if (cnt[u] > 0) { ++valid; below += (cnt[u] < cnt[t]) || (cnt[u] == cnt[t] && u < t); }
-    if (below == valid / 2) median = cnt[t];
-  }
-  __syncthreads();
-  if (t < kMaxSm) {
-    int w = 256;
-    if (t < n_sm && cnt[t] > 0 && median > 0) {
-      const long long raw = (256ll * cnt[t]) / median;               // 1/256 units
-      long long d = 256 + ((raw - 256) * damp_256) / 256;
-      d = (d + 4) & ~7ll;
-      w = (int)(d < 192 ? 192 : (d > 352 ? 352 : d));
+plan_kernel(int32_t* plan, const int32_t* lens, const int32_t* bt, int B, int Hkv, int Hq, int bt_stride) {
+  __shared__ int cum[kBMax + 1];
+  __shared__ int slen[kBMax];
+  __shared__ int n_empty;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int nC = gridDim.x, G = Hq / Hkv;
+  if (tid == 0) n_empty = 0;
+  prefix_pages(lens, B, slen, cum);
+  const int N = Hkv * cum[B];
+  int4* first = reinterpret_cast<int4*>(plan + plan_first_offset_ints(B));
+  int4* tiles = first + (size_t)nC * kWarps * 32;
+  if (blockIdx.x == 0) {
+    for (int i = tid; i < B; i += kWarps * 32)
+      if (slen[i] == 0) plan[kPlanHeaderInts + atomicAdd(&n_empty, 1)] = i;       // (order is irrelevant: rows get zeros)
+    __syncthreads();
+    if (tid == 0) {
+      plan[0] = kPlanMagic; plan[1] = B; plan[2] = Hkv; plan[3] = Hq; plan[4] = nC; plan[5] = N; plan[6] = n_empty;
     }
-    g_sm_w[t] = w;
-    g_sm_cnt[t] = 0;
   }
-  if (t == 0) { __threadfence(); g_sm_w_n = n_sm; }
+  if (N == 0) return;
+  const int w = blockIdx.x * kWarps + warp;
+  const int k0 = worker_lo(w, N, nC), k1 = worker_lo(w + 1, N, nC);
+  first[(size_t)w * 32 + lane] = (k0 + lane < k1) ? make_desc(k0 + lane, cum, slen, B, Hkv, Hq, G, bt, bt_stride) : make_int4(0, 0, 0, 0);
+  for (long long k = (long long)blockIdx.x * (kWarps * 32) + tid; k < N; k += (long long)nC * (kWarps * 32))
+    tiles[k] = make_desc(k, cum, slen, B, Hkv, Hq, G, bt, bt_stride);
 }
 
 // ------------------------------------------------------------------------------------------
-template <int D, int NT, bool APPEND>
+template <int D, int NT, bool APPEND, bool PLANNED>
 __global__ void __launch_bounds__(kWarps * 32, 1)
 attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
                    const StreamParams p) {
@@ -262,10 +270,8 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
   extern __shared__ __align__(1024) uint8_t smem[];
   uint8_t* q_base = smem + kWarps * kStages * C::kStage;
   uint64_t* bars = reinterpret_cast<uint64_t*>(q_base + kWarps * C::kQBytes);
-  int* cum = reinterpret_cast<int*>(bars + kWarps * (kStages + 1));
+  int* cum = reinterpret_cast<int*>(bars + kWarps * (kStages + 1));    // (unplanned only)
   int* slen = cum + (kBMax + 1);
-  int* smlo = slen + kBMax;            // [nC + 1] first tile of each CTA-level range; then [nC+1] = my slot
-  int* my_slot = smlo + kMaxSm + 1;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int B = p.B, Hkv = p.Hkv, G = p.G;
@@ -275,71 +281,38 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tmK) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tmV) : "memory");
   }
-
-  // ---- which CTA-level range is mine.  Not tuned: range blockIdx.x.  Tuned (hx_tune_sm_rates):
-  // range sizes follow the per-SM rate table, so the range of SM s belongs to the CTA running on
-  // SM s; it is claimed with a flag, and a CTA that finds its SM's range taken (two CTAs landed on
-  // one SM) takes any free one, so every range is processed exactly once whatever the placement.
-  const bool tuned = (g_sm_w_n == nC);
-  const int my_w = (tid < nC) ? (tuned ? g_sm_w[tid] : 256) : 0;   // weight of CTA-level range `tid`
-  if (tid == 0) {
-    int slot = blockIdx.x;
-    if (tuned) {
-      unsigned int smid;
-      asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-      slot = (int)(smid % (unsigned)nC);
-      while (atomicCAS(p.claim + slot, 0, 1) != 0) slot = (slot + 1 == nC) ? 0 : slot + 1;
-    }
-    *my_slot = slot;
+  const int w = blockIdx.x * kWarps + warp;          // worker id
+  if (lane == 0) {
+    const uint32_t b0 = smem_u32(bars + warp * (kStages + 1));
+    for (int s = 0; s <= kStages; ++s) mbar_init(b0 + 8 * s, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
 
-  // ---- setup: page-count prefix sums (row A4) and barrier init; the only CTA-wide syncs
-  {
-    constexpr int PER = kBMax / (kWarps * 32);
-    __shared__ int warp_tot[kWarps], warp_tot_w[kWarps];
-    int np[PER], sum = 0;
-#pragma unroll
-    for (int e = 0; e < PER; ++e) {
-      const int i = tid * PER + e;
-      const int n = (i < B) ? max(__ldg(p.lens + i), 0) : 0;
-      if (i < B) slen[i] = n;
-      np[e] = (n + 15) >> 4;
-      sum += np[e];
+  // ---- setup (row A4).  Unplanned: page-count prefix sums in shared memory (the only CTA-wide syncs).
+  // Planned: the header and this worker's first 32 descriptors arrive with one round of loads; no CTA-wide sync.
+  int N;
+  PlanView pv = {nullptr, nullptr, nullptr, nullptr};
+  int4 d_cur = make_int4(0, 0, 0, 0), d_nxt = make_int4(0, 0, 0, 0);    // lane L of round r describes tile k0 + 32 r + L
+  if (PLANNED) {
+    pv.header = p.plan;
+    pv.empty = p.plan + kPlanHeaderInts;
+    pv.first = reinterpret_cast<const int4*>(p.plan + plan_first_offset_ints(B));
+    pv.tiles = pv.first + (size_t)nC * kWarps * 32;
+    d_cur = __ldg(pv.first + (size_t)w * 32 + lane);
+    const int hv = (lane < 8) ? __ldg(pv.header + lane) : 0;
+    N = __shfl_sync(FULL, hv, 5);
+    // a plan made for another batch, head layout or grid would send the warps to wrong tiles: stop loudly
+    if (__shfl_sync(FULL, hv, 0) != kPlanMagic || __shfl_sync(FULL, hv, 1) != B || __shfl_sync(FULL, hv, 2) != Hkv ||
+        __shfl_sync(FULL, hv, 3) != p.Hq || __shfl_sync(FULL, hv, 4) != nC) __trap();
+    const int n_empty = __shfl_sync(FULL, hv, 6);
+    for (int e = w; e < n_empty; e += nC * kWarps) {                     // reading S11: empty context -> zero row
+      int4* row = reinterpret_cast<int4*>(p.out + (size_t)__ldg(pv.empty + e) * p.Hq * D);
+      for (int x = lane; x < p.Hq * D / 8; x += 32) row[x] = make_int4(0, 0, 0, 0);
     }
-    int incl = sum, incl_w = my_w;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const int t = __shfl_up_sync(FULL, incl, o);
-      const int tw = __shfl_up_sync(FULL, incl_w, o);
-      if (lane >= o) { incl += t; incl_w += tw; }
-    }
-    if (lane == 31) { warp_tot[warp] = incl; warp_tot_w[warp] = incl_w; }
-    if (lane == 0) {
-      const uint32_t b0 = smem_u32(bars + warp * (kStages + 1));
-      for (int s = 0; s <= kStages; ++s) mbar_init(b0 + 8 * s, 1);
-      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncthreads();
-    int off = incl - sum;
-    for (int w = 0; w < warp; ++w) off += warp_tot[w];
-    if (tid == 0) cum[0] = 0;
-#pragma unroll
-    for (int e = 0; e < PER; ++e) {
-      const int i = tid * PER + e;
-      off += np[e];
-      if (i < B) cum[i + 1] = off;
-    }
-    __syncthreads();
-    {
-      // CTA-level range starts: smlo[s] = N * (weights before s) / (all weights)
-      int before = incl_w - my_w, all = 0;
-#pragma unroll
-      for (int w2 = 0; w2 < kWarps; ++w2) { if (w2 < warp) before += warp_tot_w[w2]; all += warp_tot_w[w2]; }
-      const long long Nt = (long long)Hkv * cum[B];
-      if (tid < nC) smlo[tid] = (int)(Nt * before / all);
-      if (tid == nC || (nC == kWarps * 32 && tid == 0)) smlo[nC] = (int)Nt;
-    }
-    __syncthreads();
+    __syncwarp();
+  } else {
+    prefix_pages(p.lens, B, slen, cum);
+    N = Hkv * cum[B];
     // reading S11: an empty context gives a zero output row (no tile ever touches it)
     for (int i = blockIdx.x * (kWarps * 32) + tid; i < B; i += gridDim.x * (kWarps * 32))
       if (slen[i] == 0) {
@@ -348,23 +321,9 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
       }
   }
 
-  // worker (slot s, warp j) owns [lo(s, j), lo(s, j + 1)): the CTA range cut in 8 equal parts
-  auto w_lo = [&](int ww) -> int {
-    const int s = ww >> 3, j = ww & 7;
-    return smlo[s] + (int)((long long)(smlo[s + 1] - smlo[s]) * j >> 3);
-  };
-  auto owner_of = [&](int k) -> int {                       // worker whose range holds tile k
-    int lo = 0, hi = nC;                                    // smlo[lo] <= k < smlo[hi]
-    while (hi - lo > 1) {
-      const int mid = (lo + hi) >> 1;
-      if (smlo[mid] <= k) lo = mid; else hi = mid;
-    }
-    const int len = smlo[lo + 1] - smlo[lo];
-    return lo * 8 + (int)((((unsigned)(k - smlo[lo]) + 1u) * 8u - 1u) / (unsigned)len);   // len < 2^28 (host check)
-  };
-  const int w = *my_slot * kWarps + warp;
-  const int k0 = w_lo(w), k1 = w_lo(w + 1);
   do {
+  if (N == 0) break;
+  const int k0 = worker_lo(w, N, nC), k1 = worker_lo(w + 1, N, nC);
   if (k0 >= k1) break;
 
   uint8_t* my_stage = smem + warp * kStages * C::kStage;
@@ -375,25 +334,20 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
   const uint32_t qbar = bar_u32 + 8 * kStages;
   const uint64_t kv_policy = policy_evict_first();
 
-  // ---- per-lane lookahead: lane L of round r describes tile k0 + 32 r + L
-  int page_cur = 0, gpart_cur = 0, meta_cur = 0, page_nxt = 0, gpart_nxt = 0, meta_nxt = 0;
-  auto load_round = [&](int r, int& page, int& gpart, int& meta) {
+  auto load_round = [&](int r) -> int4 {
     const long long k = k0 + 32ll * r + lane;
-    page = 0; gpart = 0; meta = 0;
-    if (k < k1) {
-      const Loc t = locate(k, cum, B, Hkv);
-      page = __ldg(p.bt + (size_t)t.i * p.bt_stride + t.j);
-      gpart = t.g * 16;
-      meta = ((t.i * p.Hq + t.g * G) << 1) | (t.j == 0 ? 1 : 0);
-    }
+    if (k >= k1) return make_int4(0, 0, 0, 0);
+    if (PLANNED) return __ldg(pv.tiles + k);
+    return make_desc(k, cum, slen, B, Hkv, p.Hq, G, p.bt, p.bt_stride);
   };
-  load_round(0, page_cur, gpart_cur, meta_cur);
-  load_round(1, page_nxt, gpart_nxt, meta_nxt);
+  if (!PLANNED) d_cur = load_round(0);
+  d_nxt = load_round(1);
   int cur_round = 0;
 
-  // ---- consumer cursor (warp-uniform)
-  Loc c = locate(k0, cum, B, Hkv);
-  int cn = slen[c.i];
+  // descriptor fields of the tile in each stage (warp-uniform), stashed when the tile is issued
+  int st_qrow[kStages], st_n[kStages], st_j[kStages], st_row[kStages];
+#pragma unroll
+  for (int s = 0; s < kStages; ++s) st_qrow[s] = st_n[s] = st_j[s] = st_row[s] = 0;
   int seg_j0 = 0, segs_started = 0;
   bool q_busy = false;
 
@@ -403,36 +357,41 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
   const int v_row = (lane & 7) + (lane >> 4) * 8;         // V (A, trans): token row
   const int v_csel = (lane >> 3) & 1;
   const int tok0 = lane >> 2;
+  const int gshift = 31 - __clz(G);
 
   uint32_t qb[NT][kKS][2];
   float o[NT][kMT][4];
   float m_run[NT][2], l_run[NT][2];
 
-  long long pk = k0, ck = k0;
+  int pk = k0, ck = k0;
   while (ck < k1) {
     // ------------------------------------------------ produce: keep kStages tiles in flight
     while (pk < k1 && pk - ck < kStages) {
-      const int idx = (int)(pk - k0);
+      const int idx = pk - k0;
       if ((idx >> 5) != cur_round) {
-        page_cur = page_nxt; gpart_cur = gpart_nxt; meta_cur = meta_nxt;
+        d_cur = d_nxt;
         ++cur_round;
-        load_round(cur_round + 1, page_nxt, gpart_nxt, meta_nxt);
+        d_nxt = load_round(cur_round + 1);
       }
       const int src = idx & 31;
-      const int meta = __shfl_sync(FULL, meta_cur, src);
-      const bool segstart = (idx == 0) || (meta & 1);
+      const int dj = __shfl_sync(FULL, d_cur.w, src);
+      const bool segstart = (idx == 0) || (dj == 0);
       if (segstart && q_busy) break;
-      const int page = __shfl_sync(FULL, page_cur, src);
-      const int gpart = __shfl_sync(FULL, gpart_cur, src);
+      const int drow = __shfl_sync(FULL, d_cur.x, src);
+      const int dq = __shfl_sync(FULL, d_cur.y, src);
+      const int dn = __shfl_sync(FULL, d_cur.z, src);
       const int stage = idx % kStages;
+#pragma unroll
+      for (int s = 0; s < kStages; ++s)
+        if (s == stage) { st_qrow[s] = dq; st_n[s] = dn; st_j[s] = dj; st_row[s] = drow; }
       if (lane == 0) {
         if (segstart) {
           mbar_expect_tx(qbar, (uint32_t)(G * D * 2));
-          bulk_load(q_u32, p.q + (size_t)(meta >> 1) * D, (uint32_t)(G * D * 2), qbar);
+          bulk_load(q_u32, p.q + (size_t)dq * D, (uint32_t)(G * D * 2), qbar);
         }
         const uint32_t full = bar_u32 + 8 * stage;
         const uint32_t dst = stage_u32 + stage * C::kStage;
-        const int row = (int)(p.layer_row0 + (uint32_t)page * (uint32_t)(Hkv * 16) + (uint32_t)gpart);
+        const int row = (int)(p.layer_row0 + (uint32_t)drow);
         mbar_expect_tx(full, 2 * kTile);
         tma_tile_3d(dst, &tmK, 0, row, 0, full, kv_policy);
         tma_tile_3d(dst + kTile, &tmV, 0, row, 0, full, kv_policy);
@@ -442,9 +401,14 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     }
 
     // ------------------------------------------------ consume tile ck
-    const int idx = (int)(ck - k0);
+    const int idx = ck - k0;
     const int stage = idx % kStages;
-    if (c.j == 0 || idx == 0) {                      // segment start: fetch Q fragments, reset state
+    int c_qrow = 0, c_n = 0, c_j = 0, c_row = 0;
+#pragma unroll
+    for (int s = 0; s < kStages; ++s)
+      if (s == stage) { c_qrow = st_qrow[s]; c_n = st_n[s]; c_j = st_j[s]; c_row = st_row[s]; }
+    const int c_np = (c_n + 15) >> 4;
+    if (c_j == 0 || idx == 0) {                      // segment start: fetch Q fragments, reset state
       mbar_wait(qbar, segs_started & 1);
       ++segs_started;
 #pragma unroll
@@ -465,21 +429,20 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
       }
       __syncwarp();
       q_busy = false;
-      seg_j0 = c.j;
+      seg_j0 = c_j;
     }
-    const bool last_page = (c.j == c.np - 1);
-    const int valid = last_page ? cn - 16 * (c.np - 1) : 16;
+    const bool last_page = (c_j == c_np - 1);
+    const int valid = last_page ? c_n - 16 * (c_np - 1) : 16;
+    const int pair = c_qrow >> gshift;               // request * Hkv + kv head (G is a power of two)
     // fused append (F1): token n-1 is the step's new token; its K/V row comes from k_new/v_new, not
     // from the page.  Fetch it (lanes [0,CH): K chunks, [CH,2CH): V chunks) while the tile lands.
     int4 new_row = make_int4(0, 0, 0, 0);
-    int new_page = 0;
     if (APPEND && last_page) {
       constexpr int CH = D / 8;
       if (lane < 2 * CH) {
-        const __half* src = (lane < CH ? p.k_new : p.v_new) + ((size_t)c.i * Hkv + c.g) * D + (lane % CH) * 8;
+        const __half* src = (lane < CH ? p.k_new : p.v_new) + (size_t)pair * D + (lane % CH) * 8;
         new_row = __ldg(reinterpret_cast<const int4*>(src));
       }
-      new_page = __ldg(p.bt + (size_t)c.i * p.bt_stride + c.j);
     }
     mbar_wait(bar_u32 + 8 * stage, (idx / kStages) & 1);
 
@@ -493,7 +456,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         const int x = lane >= CH ? 1 : 0, ch = lane - x * CH;
         *reinterpret_cast<int4*>(my_stage + stage * C::kStage + x * kTile + (ch >> 3) * 2048 + r * 128 +
                                  (((ch & 7) ^ (r & 7)) << 4)) = new_row;
-        __half* dstg = (x ? p.vc : p.kc) + (((size_t)new_page * Hkv + c.g) * 16 + r) * D + ch * 8;
+        __half* dstg = (x ? p.vc : p.kc) + ((size_t)c_row + r) * D + ch * 8;     // cache row of the tile's token r
         *reinterpret_cast<int4*>(dstg) = new_row;
       }
       __syncwarp();
@@ -605,52 +568,66 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
           }
         }
         // ---- last arriver merges (row A8).  Owners of this pair's tiles [a, b): workers wa..wb.
-        const int a = Hkv * cum[c.i] + c.g * c.np, b = a + c.np;
-        const int wa = owner_of(a), wb = owner_of(b - 1);
-        const bool dense = smlo[nC] >= 16 * nC;                // then every worker's range is non-empty
+        const int a = ck - c_j, b = a + c_np;
+        const int wa = owner_of(a, N, nC), wb = owner_of(b - 1, N, nC);
+        const bool dense = N >= 16 * nC;                       // then every worker's range is non-empty
         auto next_owner = [&](int ww) -> int {                 // next worker with a tile of the pair
           if (dense) return ww + 1;
-          const int kn = w_lo(ww + 1);                         // (workers with an empty range own none)
-          return kn >= b ? wb + 1 : owner_of(kn);
+          const int kn = worker_lo(ww + 1, N, nC);             // (workers with an empty range own none)
+          return kn >= b ? wb + 1 : owner_of(kn, N, nC);
         };
         int nseg = wb - wa + 1;
         if (!dense) { nseg = 0; for (int ww = wa; ww <= wb; ww = next_owner(ww)) ++nseg; }
-        int* counter = p.counters + c.i * Hkv + c.g;
-        __threadfence();
+        int* counter = p.counters + pair;
+        __threadfence();                                       // release: this warp's partial before its count-up
         __syncwarp();
         int old = 0;
         if (lane == 0) old = atomicAdd(counter, 1);
         old = __shfl_sync(FULL, old, 0);
         if (old == nseg - 1) {
-          if (lane == 0) *counter = 0;                           // leave the workspace clean for the next call
-          __threadfence();
-          const bool wa_first = (w_lo(wa) == a);
+          // Last arriver: every other owner's partial is in L2 (its fence precedes its count-up, and this warp saw
+          // all the count-ups).  The loads below bypass L1 (ld.global.cg) and are issued after the atomic returned,
+          // so no second fence is needed.  The counter goes back to zero with a plain store (flushed at kernel end).
+          if (lane == 0) *counter = 0;
+          const bool wa_first = (worker_lo(wa, N, nC) == a);
           auto slot_of = [&](int ww) -> const float* {
             return p.partials + (size_t)((ww == wa && !wa_first) ? 2 * ww + 1 : 2 * ww) * C::kSlotFloats;
           };
           const int hb = 2 * (lane & 3);
+          // Online merge in worker (= token) order, deterministic; two partials are fetched per round trip.
 #pragma unroll
           for (int nt = 0; nt < NT; ++nt) {
-            float mm0 = -INFINITY, mm1 = -INFINITY;
-            for (int ww = wa; ww <= wb; ww = next_owner(ww)) {
-              const float2 mv = __ldcg(reinterpret_cast<const float2*>(slot_of(ww) + NT * kMT * 128 + nt * 8 + hb));
-              mm0 = fmaxf(mm0, mv.x); mm1 = fmaxf(mm1, mv.y);
-            }
-            float l0 = 0.f, l1 = 0.f;
+            float mr0 = -INFINITY, mr1 = -INFINITY, l0 = 0.f, l1 = 0.f;
 #pragma unroll
             for (int mt = 0; mt < kMT; ++mt) o[nt][mt][0] = o[nt][mt][1] = o[nt][mt][2] = o[nt][mt][3] = 0.f;
-            for (int ww = wa; ww <= wb; ww = next_owner(ww)) {     // fixed (token) order: deterministic
-              const float* sl = slot_of(ww);
-              const float2 mv = __ldcg(reinterpret_cast<const float2*>(sl + NT * kMT * 128 + nt * 8 + hb));
-              const float2 lv = __ldcg(reinterpret_cast<const float2*>(sl + NT * kMT * 128 + NT * 8 + nt * 8 + hb));
-              const float c0 = ex2(mv.x - mm0), c1 = ex2(mv.y - mm1);
-              l0 += lv.x * c0; l1 += lv.y * c1;
+            auto fetch = [&](const float* sl, float4 (&v)[kMT], float2& mv, float2& lv) {
+              mv = __ldcg(reinterpret_cast<const float2*>(sl + NT * kMT * 128 + nt * 8 + hb));
+              lv = __ldcg(reinterpret_cast<const float2*>(sl + NT * kMT * 128 + NT * 8 + nt * 8 + hb));
+#pragma unroll
+              for (int mt = 0; mt < kMT; ++mt) v[mt] = __ldcg(reinterpret_cast<const float4*>(sl) + (nt * kMT + mt) * 32 + lane);
+            };
+            auto fold = [&](const float4 (&v)[kMT], const float2 mv, const float2 lv) {
+              const float n0 = fmaxf(mr0, mv.x), n1 = fmaxf(mr1, mv.y);
+              const float r0 = ex2(mr0 - n0), r1 = ex2(mr1 - n1);       // 0 for the first partial (-inf)
+              const float c0 = ex2(mv.x - n0), c1 = ex2(mv.y - n1);
+              mr0 = n0; mr1 = n1;
+              l0 = l0 * r0 + lv.x * c0; l1 = l1 * r1 + lv.y * c1;
 #pragma unroll
               for (int mt = 0; mt < kMT; ++mt) {
-                const float4 v = __ldcg(reinterpret_cast<const float4*>(sl) + (nt * kMT + mt) * 32 + lane);
-                o[nt][mt][0] += v.x * c0; o[nt][mt][1] += v.y * c1;
-                o[nt][mt][2] += v.z * c0; o[nt][mt][3] += v.w * c1;
+                o[nt][mt][0] = o[nt][mt][0] * r0 + v[mt].x * c0; o[nt][mt][1] = o[nt][mt][1] * r1 + v[mt].y * c1;
+                o[nt][mt][2] = o[nt][mt][2] * r0 + v[mt].z * c0; o[nt][mt][3] = o[nt][mt][3] * r1 + v[mt].w * c1;
               }
+            };
+            for (int ww = wa; ww <= wb;) {
+              const int ww2 = next_owner(ww);
+              const bool two = ww2 <= wb;
+              float4 va[kMT], vb2[kMT];
+              float2 ma, la, mb = make_float2(0.f, 0.f), lb = make_float2(0.f, 0.f);
+              fetch(slot_of(ww), va, ma, la);
+              if (two) fetch(slot_of(ww2), vb2, mb, lb);
+              fold(va, ma, la);
+              if (two) fold(vb2, mb, lb);
+              ww = two ? next_owner(ww2) : wb + 1;
             }
             l_run[nt][0] = l0; l_run[nt][1] = l1;
           }
@@ -674,7 +651,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
           }
         }
         __syncwarp();
-        int4* dst = reinterpret_cast<int4*>(p.out + ((size_t)c.i * p.Hq + (size_t)c.g * G) * D);
+        int4* dst = reinterpret_cast<int4*>(p.out + (size_t)c_qrow * D);
         const int4* srcv = reinterpret_cast<const int4*>(scratch);
         for (int e = lane; e < G * D / 8; e += 32) dst[e] = srcv[e];
         __syncwarp();
@@ -682,29 +659,10 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
       }
     }
     if (wrote_smem) { fence_proxy_async(); __syncwarp(); }   // generic writes before the TMA refill
-
-    // ------------------------------------------------ advance the cursor
     ++ck;
-    if (++c.j == c.np) {
-      c.j = 0;
-      if (++c.g == Hkv) {
-        c.g = 0;
-        do { ++c.i; } while (c.i < B && cum[c.i + 1] == cum[c.i]);
-        if (c.i < B) { c.np = cum[c.i + 1] - cum[c.i]; cn = slen[c.i]; }
-      }
-    }
   }
   } while (false);
   if (p.pdl_wait_at_end) asm volatile("griddepcontrol.wait;" ::: "memory");
-
-  // ---- tuned mode: the last CTA of the grid to finish clears the claim flags for the next call.
-  // No fences: every CTA's claim (an atomic whose result it consumed) precedes its own count-up, and
-  // the plain stores below are flushed by kernel completion.
-  if (tuned) {
-    __syncthreads();
-    if (tid == 0 && atomicAdd(p.claim + kMaxSm, 1) == nC - 1)
-      for (int s = 0; s <= kMaxSm; ++s) p.claim[s] = 0;
-  }
 }
 
 // ---------------------------------------------------------------------------- host side
@@ -771,7 +729,8 @@ int get_tile_maps(const void* k, const void* v, uint64_t rows, int D, CUtensorMa
   return HX_OK;
 }
 
-template <int D, int NT, bool APPEND>
+
+template <int D, int NT, bool APPEND, bool PLANNED>
 int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream) {
   using C = Cfg<D, NT>;
   {
@@ -780,7 +739,7 @@ int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream
     std::lock_guard<std::mutex> lock(mu);
     if (!attr_set[di.device]) {
       if (C::kSmem > di.max_smem_optin) HX_FAIL(HX_ERR_UNSUPPORTED, "device offers %d B shared memory per CTA, kernel needs %d", di.max_smem_optin, C::kSmem);
-      HX_CUDA_OK(cudaFuncSetAttribute(attn_stream_kernel<D, NT, APPEND>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmem));
+      HX_CUDA_OK(cudaFuncSetAttribute(attn_stream_kernel<D, NT, APPEND, PLANNED>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmem));
       attr_set[di.device] = true;
     }
   }
@@ -795,18 +754,18 @@ int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream
   if (grid > kMaxSm) grid = kMaxSm;
   char* ws = static_cast<char*>(a.workspace);
   const size_t partial_bytes = (size_t)2 * kMaxWorkers * C::kSlotFloats * sizeof(float);
-  const size_t counter_bytes = ((size_t)kBMax * a.kv_heads * sizeof(int32_t) + 15) & ~(size_t)15;
   if ((long long)kBMax * a.bt_stride * a.kv_heads >= (1ll << 28)) HX_FAIL(HX_ERR_UNSUPPORTED, "block_table_stride * kv_heads too large");
+  if (PLANNED && a.batch > kBMax) HX_FAIL(HX_ERR_UNSUPPORTED, "a plan covers at most %d requests (batch %d)", kBMax, a.batch);
   for (int b0 = 0; b0 < a.batch; b0 += kBMax) {
     StreamParams p;
+    memset(&p, 0, sizeof(p));
     p.B = (a.batch - b0 < kBMax) ? a.batch - b0 : kBMax;
     p.q = static_cast<const __half*>(a.q) + (size_t)b0 * a.q_heads * D;
     p.out = static_cast<__half*>(a.out) + (size_t)b0 * a.q_heads * D;
-    p.bt = a.block_table + (size_t)b0 * a.bt_stride;
-    p.lens = a.seq_lens + b0;
+    p.bt = a.block_table ? a.block_table + (size_t)b0 * a.bt_stride : nullptr;
+    p.lens = a.seq_lens ? a.seq_lens + b0 : nullptr;
     p.partials = reinterpret_cast<float*>(ws);
     p.counters = reinterpret_cast<int32_t*>(ws + partial_bytes);
-    p.claim = reinterpret_cast<int32_t*>(ws + partial_bytes + counter_bytes);
     p.Hq = a.q_heads; p.Hkv = a.kv_heads; p.G = a.q_heads / a.kv_heads; p.bt_stride = a.bt_stride;
     p.layer_row0 = (uint32_t)(rows_per_layer * a.layer);
     p.scale_log2 = a.sm_scale * kLog2e;
@@ -815,6 +774,7 @@ int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream
     p.v_new = APPEND ? static_cast<const __half*>(a.v_new) + (size_t)b0 * a.kv_heads * D : nullptr;
     p.kc = static_cast<__half*>(const_cast<void*>(a.k_base)) + layer_elems * a.layer;
     p.vc = static_cast<__half*>(const_cast<void*>(a.v_base)) + layer_elems * a.layer;
+    p.plan = PLANNED ? static_cast<const int32_t*>(a.plan) : nullptr;
     p.pdl_wait_at_end = (a.overlap_prev && b0 == 0) ? 1 : 0;
     if (p.pdl_wait_at_end) {
       // programmatic dependent launch: this grid may start while the ingest kernel enqueued just before it (which
@@ -827,9 +787,9 @@ int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream
       at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
       at[0].val.programmaticStreamSerializationAllowed = 1;
       cfg.attrs = at; cfg.numAttrs = 1;
-      HX_CUDA_OK(cudaLaunchKernelEx(&cfg, attn_stream_kernel<D, NT, APPEND>, tk, tv, p));
+      HX_CUDA_OK(cudaLaunchKernelEx(&cfg, attn_stream_kernel<D, NT, APPEND, PLANNED>, tk, tv, p));
     } else {
-      attn_stream_kernel<D, NT, APPEND><<<grid, kWarps * 32, C::kSmem, stream>>>(tk, tv, p);
+      attn_stream_kernel<D, NT, APPEND, PLANNED><<<grid, kWarps * 32, C::kSmem, stream>>>(tk, tv, p);
     }
     HX_CUDA_OK(cudaGetLastError());
   }
@@ -845,36 +805,24 @@ size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, in
   const int nt = G > 8 ? 2 : 1;
   const size_t slot = (size_t)nt * ((head_dim / 16) * 128 + 16) * sizeof(float);
   const size_t counter_bytes = ((size_t)kBMax * kv_heads * sizeof(int32_t) + 15) & ~(size_t)15;
-  return 2 * (size_t)kMaxWorkers * slot + counter_bytes + (size_t)(2 * kMaxSm) * sizeof(int32_t);
+  return 2 * (size_t)kMaxWorkers * slot + counter_bytes;
 }
 
-int tune_sm_rates(const void* scratch, size_t bytes, cudaStream_t stream) {
+// Upper bound of a plan's size: header + empty list + first[W][32] + one descriptor per possible tile.
+size_t attn_plan_bytes(int32_t batch, int32_t kv_heads, int32_t max_seq_len, int32_t page_size) {
+  const size_t tiles = (size_t)batch * kv_heads * ((max_seq_len + page_size - 1) / page_size);
+  return plan_first_offset_ints(batch) * 4 + (size_t)kMaxSm * kWarps * 32 * 16 + tiles * 16;
+}
+
+int launch_plan(const AttnParams& a, cudaStream_t stream) {
   DeviceInfo di;
   int rc = device_info(&di);
   if (rc) return rc;
+  if (a.batch > kBMax) HX_FAIL(HX_ERR_UNSUPPORTED, "a plan covers at most %d requests (batch %d)", kBMax, a.batch);
+  if ((long long)kBMax * a.bt_stride * a.kv_heads >= (1ll << 28)) HX_FAIL(HX_ERR_UNSUPPORTED, "block_table_stride * kv_heads too large");
   const int grid = di.sm_count < kMaxSm ? di.sm_count : kMaxSm;
-  if (!scratch || bytes == 0) {                              // back to equal ranges
-    sm_rate_finalize_kernel<<<1, kMaxSm, 0, stream>>>(grid, 1, 0);
-    HX_CUDA_OK(cudaGetLastError());
-    return HX_OK;
-  }
-  constexpr int kProbeSmem = kWarps * 3 * 8192;
-  {
-    static std::mutex mu;
-    static bool attr_set[64] = {false};
-    std::lock_guard<std::mutex> lock(mu);
-    if (!attr_set[di.device]) {
-      HX_CUDA_OK(cudaFuncSetAttribute(sm_rate_probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kProbeSmem));
-      attr_set[di.device] = true;
-    }
-  }
-  // three windows of 80 us: the counts of a window are max-merged per SM, which drops start-up noise
-  for (int rep = 0; rep < 3; ++rep) {
-    sm_rate_probe_kernel<<<grid, kWarps * 32, kProbeSmem, stream>>>(static_cast<const uint8_t*>(scratch), bytes / 8192, 80000u);
-    HX_CUDA_OK(cudaGetLastError());
-  }
-  const int damp = 176;                                     // 0.69 (B200 sweep: 160-192 best), see sm_rate_finalize_kernel
-  sm_rate_finalize_kernel<<<1, kMaxSm, 0, stream>>>(grid, 0, damp);
+  plan_kernel<<<grid, kWarps * 32, 0, stream>>>(static_cast<int32_t*>(a.plan), a.seq_lens, a.block_table, a.batch, a.kv_heads,
+                                               a.q_heads, a.bt_stride);
   HX_CUDA_OK(cudaGetLastError());
   return HX_OK;
 }
@@ -885,11 +833,15 @@ int launch_attention(const AttnParams& a, cudaStream_t stream) {
   if (rc) return rc;
   const int G = a.q_heads / a.kv_heads;
   if (a.k_new) {
-    if (a.head_dim == 128) return G > 8 ? launch_stream<128, 2, true>(a, di, stream) : launch_stream<128, 1, true>(a, di, stream);
-    return G > 8 ? launch_stream<64, 2, true>(a, di, stream) : launch_stream<64, 1, true>(a, di, stream);
+    if (a.head_dim == 128) return G > 8 ? launch_stream<128, 2, true, false>(a, di, stream) : launch_stream<128, 1, true, false>(a, di, stream);
+    return G > 8 ? launch_stream<64, 2, true, false>(a, di, stream) : launch_stream<64, 1, true, false>(a, di, stream);
   }
-  if (a.head_dim == 128) return G > 8 ? launch_stream<128, 2, false>(a, di, stream) : launch_stream<128, 1, false>(a, di, stream);
-  return G > 8 ? launch_stream<64, 2, false>(a, di, stream) : launch_stream<64, 1, false>(a, di, stream);
+  if (a.plan) {
+    if (a.head_dim == 128) return G > 8 ? launch_stream<128, 2, false, true>(a, di, stream) : launch_stream<128, 1, false, true>(a, di, stream);
+    return G > 8 ? launch_stream<64, 2, false, true>(a, di, stream) : launch_stream<64, 1, false, true>(a, di, stream);
+  }
+  if (a.head_dim == 128) return G > 8 ? launch_stream<128, 2, false, false>(a, di, stream) : launch_stream<128, 1, false, false>(a, di, stream);
+  return G > 8 ? launch_stream<64, 2, false, false>(a, di, stream) : launch_stream<64, 1, false, false>(a, di, stream);
 }
 
 }  // namespace hx

@@ -186,11 +186,13 @@ size_t hx_decode_attention_workspace_bytes(int32_t batch, int32_t q_heads, int32
   return hx::attn_workspace_bytes(batch, q_heads, kv_heads, head_dim, max_seq_len, page_size);
 }
 
+// mode: 0 = hx_decode_attention (and _append / _overlapped), 1 = hx_decode_plan (writes `plan`), 2 = hx_decode_attention_planned
 static int attention_common(const char* who, void* out, const void* q, const void* k_new, const void* v_new, bool append, bool overlap,
                             const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
                             const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
                             int32_t batch, int32_t max_seq_len, float sm_scale, void* workspace,
-                            size_t workspace_bytes, void* stream, bool dry_run = false) {
+                            size_t workspace_bytes, void* stream, bool dry_run = false, int mode = 0,
+                            void* plan = nullptr, size_t plan_bytes = 0) {
   using namespace hx;
   clear_error();
   if (batch < 0 || max_seq_len < 0) HX_FAIL(HX_ERR_INVALID_ARG, "%s: negative size (batch=%d max_seq_len=%d)", who, batch, max_seq_len);
@@ -202,16 +204,23 @@ static int attention_common(const char* who, void* out, const void* q, const voi
   if (G != 1 && G != 2 && G != 4 && G != 8 && G != 16) HX_FAIL(HX_ERR_UNSUPPORTED, "%s: group size %d not in {1,2,4,8,16}", who, G);
   if (!(sm_scale == sm_scale) || sm_scale > 1e30f) HX_FAIL(HX_ERR_INVALID_ARG, "%s: sm_scale is NaN or too large", who);
   if (batch == 0) return HX_OK;
-  if (!out || !q) HX_FAIL(HX_ERR_INVALID_ARG, "%s: out/q is NULL", who);
-  if (!aligned16(out) || !aligned16(q)) HX_FAIL(HX_ERR_INVALID_ARG, "%s: out/q must be 16-byte aligned", who);
-  if (!block_table || !seq_lens) HX_FAIL(HX_ERR_INVALID_ARG, "%s: block_table/seq_lens is NULL", who);
+  if (mode != 1) {
+    if (!out || !q) HX_FAIL(HX_ERR_INVALID_ARG, "%s: out/q is NULL", who);
+    if (!aligned16(out) || !aligned16(q)) HX_FAIL(HX_ERR_INVALID_ARG, "%s: out/q must be 16-byte aligned", who);
+  }
+  if (mode != 2 && (!block_table || !seq_lens)) HX_FAIL(HX_ERR_INVALID_ARG, "%s: block_table/seq_lens is NULL", who);
+  if (mode != 0) {
+    if (!plan || !aligned16(plan)) HX_FAIL(HX_ERR_INVALID_ARG, "%s: plan is NULL or not 16-byte aligned", who);
+    const size_t pneed = attn_plan_bytes(batch, cache->kv_heads, max_seq_len, cache->page_size);
+    if (plan_bytes < pneed) HX_FAIL(HX_ERR_WORKSPACE, "%s: plan buffer %zu bytes < required %zu", who, plan_bytes, pneed);
+  }
   if (append) {
     if (!k_new || !v_new) HX_FAIL(HX_ERR_INVALID_ARG, "%s: k_new/v_new is NULL", who);
     if (!aligned16(k_new) || !aligned16(v_new)) HX_FAIL(HX_ERR_INVALID_ARG, "%s: k_new/v_new must be 16-byte aligned", who);
   }
   if ((int64_t)block_table_stride * cache->page_size < (int64_t)max_seq_len)
     HX_FAIL(HX_ERR_INVALID_ARG, "%s: block_table_stride %d < ceil(max_seq_len %d / %d)", who, block_table_stride, max_seq_len, cache->page_size);
-  const size_t need = attn_workspace_bytes(batch, q_heads, cache->kv_heads, cache->head_dim, max_seq_len, cache->page_size);
+  const size_t need = mode == 1 ? 0 : attn_workspace_bytes(batch, q_heads, cache->kv_heads, cache->head_dim, max_seq_len, cache->page_size);
   if (need > 0 && (!workspace || workspace_bytes < need)) HX_FAIL(HX_ERR_WORKSPACE, "%s: workspace %zu bytes < required %zu (or NULL)", who, workspace_bytes, need);
   if (need > 0 && !aligned16(workspace)) HX_FAIL(HX_ERR_INVALID_ARG, "%s: workspace must be 16-byte aligned", who);
   if (sm_scale <= 0.f) sm_scale = 1.0f / sqrtf((float)cache->head_dim);
@@ -228,8 +237,9 @@ static int attention_common(const char* who, void* out, const void* q, const voi
   p.k_new = append ? k_new : nullptr; p.v_new = append ? v_new : nullptr;
   // a programmatic dependent launch only directly behind an ingest kernel this thread enqueued on this stream
   p.overlap_prev = (overlap && g_last.kind == kLaunchIngest && g_last.stream == stream) ? 1 : 0;
+  p.plan = mode != 0 ? plan : nullptr;
   if (dry_run) return HX_OK;
-  rc = launch_attention(p, static_cast<cudaStream_t>(stream));
+  rc = mode == 1 ? launch_plan(p, static_cast<cudaStream_t>(stream)) : launch_attention(p, static_cast<cudaStream_t>(stream));
   if (rc == HX_OK) note_launch(stream, kLaunchOther);
   return rc;
 }
@@ -326,16 +336,24 @@ int hx_prefill_attention(void* out, const void* q, const hx_paged_cache* cache, 
   return rc;
 }
 
-int hx_tune_sm_rates(const void* scratch, size_t scratch_bytes, void* stream) {
-  using namespace hx;
-  clear_error();
-  if (scratch && scratch_bytes > 0) {
-    if (!aligned16(scratch)) HX_FAIL(HX_ERR_INVALID_ARG, "hx_tune_sm_rates: scratch must be 16-byte aligned");
-    if (scratch_bytes < ((size_t)256 << 20)) HX_FAIL(HX_ERR_UNSUPPORTED, "hx_tune_sm_rates: scratch of %zu bytes is too small to be HBM-bound (need >= 256 MiB)", scratch_bytes);
-  }
-  const int rc = tune_sm_rates(scratch, scratch_bytes, static_cast<cudaStream_t>(stream));
-  if (rc == HX_OK) note_launch(stream, kLaunchOther);
-  return rc;
+size_t hx_decode_plan_bytes(int32_t batch, int32_t kv_heads, int32_t max_seq_len, int32_t page_size) {
+  if (batch < 0 || kv_heads <= 0 || max_seq_len < 0 || page_size <= 0) return 0;
+  return hx::attn_plan_bytes(batch, kv_heads, max_seq_len, page_size);
+}
+
+int hx_decode_plan(void* plan, size_t plan_bytes, const hx_paged_cache* cache, int32_t q_heads, const int32_t* block_table,
+                   int32_t block_table_stride, const int32_t* seq_lens, int32_t batch, int32_t max_seq_len, void* stream) {
+  return attention_common("hx_decode_plan", nullptr, nullptr, nullptr, nullptr, false, false, cache, 0, q_heads, block_table,
+                          block_table_stride, seq_lens, batch, max_seq_len, 0.f, nullptr, 0, stream, false, 1, plan, plan_bytes);
+}
+
+int hx_decode_attention_planned(void* out, const void* q, const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
+                                const void* plan, size_t plan_bytes, int32_t batch, int32_t max_seq_len, float sm_scale,
+                                void* workspace, size_t workspace_bytes, void* stream) {
+  const int32_t ps = (cache && cache->page_size > 0) ? cache->page_size : 16;
+  return attention_common("hx_decode_attention_planned", out, q, nullptr, nullptr, false, false, cache, layer, q_heads, nullptr,
+                          (max_seq_len + ps - 1) / ps, nullptr, batch, max_seq_len, sm_scale, workspace, workspace_bytes, stream,
+                          false, 2, const_cast<void*>(plan), plan_bytes);
 }
 
 // ---- whole decode step (row A9): library-owned side stream per device for the overlapped handoff ----

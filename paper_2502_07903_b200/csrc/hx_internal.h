@@ -66,11 +66,13 @@ struct AttnParams {
   const void* k_new;              // fused append (hx_decode_attention_append); NULL otherwise
   const void* v_new;
   int32_t overlap_prev;           // launch as a programmatic dependent of the preceding kernel (hx_decode_attention_overlapped)
+  void* plan;                     // hx_decode_plan's output (written by launch_plan, read by a planned launch); NULL otherwise
 };
 size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, int32_t head_dim,
                             int32_t max_seq_len, int32_t page_size);
+size_t attn_plan_bytes(int32_t batch, int32_t kv_heads, int32_t max_seq_len, int32_t page_size);
 int launch_attention(const AttnParams& p, cudaStream_t stream);
-int tune_sm_rates(const void* scratch, size_t bytes, cudaStream_t stream);
+int launch_plan(const AttnParams& p, cudaStream_t stream);      // uses seq_lens, block_table, batch, heads, bt_stride, plan
 
 struct PrefillArgs {
   void* out;

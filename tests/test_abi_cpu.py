@@ -22,7 +22,7 @@ def test_library_exports_every_declared_symbol():
     L = hx.lib()
     for name in declared:
         assert hasattr(L, name), name
-    assert hx.version() == 130
+    assert hx.version() == 131
     assert hx.status_string(0) == "HX_OK" and hx.status_string(5) == "HX_ERR_NO_PAGES"
     assert hx.status_string(77) == "HX_ERR_UNKNOWN"
 
@@ -303,3 +303,29 @@ def test_decode_step_host_validates_before_it_enqueues():
         with pytest.raises(hx.HxError) as e:
             hx.decode_step_host(**dict(kw, **over))
         assert e.value.status == status, (over, str(e.value))
+
+
+# ---------------------------------------------------------------- per-step plan
+def test_plan_entry_points_reject_invalid_arguments_without_launching():
+    need = hx.decode_plan_bytes(2, 2, 64)
+    assert need > 0 and hx.decode_plan_bytes(-1, 2, 64) == 0
+    pk = dict(q_heads=4, block_table=0x3000, block_table_stride=4, seq_lens=0x4000, batch=2, max_seq_len=64, plan_bytes=need, stream=0)
+    for over, status in [(dict(plan_bytes=need - 1), B.HX_ERR_WORKSPACE), (dict(q_heads=3), B.HX_ERR_INVALID_ARG),
+                         (dict(block_table=0), B.HX_ERR_INVALID_ARG), (dict(seq_lens=0), B.HX_ERR_INVALID_ARG),
+                         (dict(block_table_stride=3), B.HX_ERR_INVALID_ARG), (dict(batch=-1), B.HX_ERR_INVALID_ARG)]:
+        with pytest.raises(hx.HxError) as e:
+            hx.decode_plan(0x9000, FakeCache(), **dict(pk, **over))
+        assert e.value.status == status, (over, str(e.value))
+    with pytest.raises(hx.HxError) as e:
+        hx.decode_plan(0, FakeCache(), **pk)
+    assert e.value.status == B.HX_ERR_INVALID_ARG
+    hx.decode_plan(0, FakeCache(), **dict(pk, batch=0))                 # HX_OK, nothing launched
+    ak = dict(layer=0, q_heads=4, plan=0x9000, plan_bytes=need, batch=2, max_seq_len=64, sm_scale=0.0, workspace=0x5000,
+              workspace_bytes=1 << 30, stream=0)
+    for over, status in [(dict(plan=0), B.HX_ERR_INVALID_ARG), (dict(plan=0x9004), B.HX_ERR_INVALID_ARG),
+                         (dict(plan_bytes=16), B.HX_ERR_WORKSPACE), (dict(layer=2), B.HX_ERR_INVALID_ARG),
+                         (dict(workspace=0), B.HX_ERR_WORKSPACE), (dict(q_heads=6), B.HX_ERR_UNSUPPORTED)]:
+        with pytest.raises(hx.HxError) as e:
+            hx.decode_attention_planned(0x6000, 0x7000, FakeCache(), **dict(ak, **over))
+        assert e.value.status == status, (over, str(e.value))
+    hx.decode_attention_planned(0, 0, FakeCache(), **dict(ak, batch=0))  # HX_OK, nothing launched

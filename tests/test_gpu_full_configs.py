@@ -1,7 +1,7 @@
 """Full-size BASELINE.json configs on the GPU, in the launch configuration bench.py times.
-Attention: EVERY output row of configs[1], [2] and [4] against the float64 oracle, with equal ranges (untuned) and
-after hx_tune_sm_rates (the configuration bench.py times); configs[4] also through hx_decode_step with the step's
-handoff overlapped, as bench.py runs it.  Ingest: the whole 80-layer configs[3] call for both destination ranks,
+Attention: EVERY output row of configs[1], [2] and [4] against the float64 oracle, through hx_decode_attention and
+through hx_decode_plan + hx_decode_attention_planned (bit-identical to each other); configs[4] also through
+hx_decode_step with the step's handoff overlapped, as bench.py runs it.  Ingest: the whole 80-layer configs[3] call for both destination ranks,
 layers 0 / 40 / 79 bit for bit against the oracle (element offsets past 2^31), every layer through the on-device
 gather round trip, unowned pages intact."""
 import numpy as np
@@ -34,7 +34,7 @@ def _check_all_rows(name, got, ref, label):
 
 
 @pytest.mark.parametrize("name", ["opt30b_tp4", "llama70b_tp2", "llama70b_tp1"])
-def test_attention_full_config_every_row_untuned_and_tuned(env, name):
+def test_attention_full_config_every_row_unplanned_and_planned(env, name):
     hx, torch, oracle = env
     c = W.CONFIGS[name]
     w = W.make_attention_inputs(c)
@@ -47,26 +47,27 @@ def test_attention_full_config_every_row_untuned_and_tuned(env, name):
     mx = int(w["seq_lens"].max())
     wsb = hx.decode_attention_workspace_bytes(B, Hq, c.kv_heads, D, mx)
     ws = torch.zeros(wsb, dtype=torch.uint8, device="cuda")
-    scratch = torch.empty(320 << 20, dtype=torch.uint8, device="cuda")
-    try:
-        outs = {}
-        for label in ("untuned", "tuned", "tuned again"):
-            if label == "tuned":
-                hx.tune_sm_rates(scratch)
-            out = torch.full_like(qd, float("nan"))
+    plan = torch.empty(hx.decode_plan_bytes(B, c.kv_heads, mx), dtype=torch.uint8, device="cuda")
+    hx.decode_plan(plan, cache, q_heads=Hq, block_table=bt, block_table_stride=bt.shape[1], seq_lens=sl, batch=B, max_seq_len=mx)
+    outs = {}
+    for label in ("unplanned", "planned", "planned again", "unplanned again"):
+        out = torch.full_like(qd, float("nan"))
+        if label.startswith("planned"):
+            hx.decode_attention_planned(out, qd, cache, layer=0, q_heads=Hq, plan=plan, batch=B, max_seq_len=mx, workspace=ws,
+                                        workspace_bytes=wsb)
+        else:
             hx.decode_attention(out, qd, cache, layer=0, q_heads=Hq, block_table=bt, block_table_stride=bt.shape[1],
                                 seq_lens=sl, batch=B, max_seq_len=mx, workspace=ws, workspace_bytes=wsb)
-            torch.cuda.synchronize()
-            outs[label] = out.cpu().numpy()
-            _check_all_rows(name, outs[label], ref, label)
-        # for a given rate table the result is the same bits run to run
-        assert np.array_equal(outs["tuned"].view(np.uint16), outs["tuned again"].view(np.uint16))
-    finally:
-        hx.tune_sm_rates(None)
+        torch.cuda.synchronize()
+        outs[label] = out.cpu().numpy()
+        _check_all_rows(name, outs[label], ref, label)
+    # same work partition, same arithmetic: the same bits with and without the plan, run to run
+    for label in ("planned", "planned again", "unplanned again"):
+        assert np.array_equal(outs[label].view(np.uint16), outs["unplanned"].view(np.uint16)), label
 
 
 def test_config5_step_as_bench_runs_it(env):
-    """configs[4] through hx_decode_step(overlap_ingest=1) after hx_tune_sm_rates — bench.py's timed call: the 16
+    """configs[4] through hx_decode_step(overlap_ingest=1) — bench.py's timed call: the 16
     new 2048-token prompts land (prefill TP=4 -> decode TP=1) in pages the host allocator hands out while the
     attention runs over the 256-request batch.  Every output row and every page of the cache against the oracle."""
     hx, torch, oracle = env
@@ -93,8 +94,7 @@ def test_config5_step_as_bench_runs_it(env):
     ws = torch.zeros(wsb, dtype=torch.uint8, device="cuda")
     sk = [to_dev(a, torch) for a in wi["src_k"]]
     sv = [to_dev(a, torch) for a in wi["src_v"]]
-    try:
-        hx.tune_sm_rates(cache.k)
+    if True:
         hx.decode_step(out=out, q=qd, cache=cache, layer=0, q_heads=ca.q_heads, block_table=torch.from_numpy(bt_np).cuda(),
                        block_table_stride=bt_np.shape[1], seq_lens=torch.from_numpy(lens).cuda(), batch=ca.batch,
                        max_seq_len=mx, sm_scale=0.0, workspace=ws, workspace_bytes=wsb, src_k=sk, src_v=sv, ing_layers=1,
@@ -104,10 +104,8 @@ def test_config5_step_as_bench_runs_it(env):
                        ing_total_tokens=wi["total_tokens"], ing_max_seq_len=2048, overlap_ingest=1)
         k_after = cache.k.clone()                       # enqueued on the caller's stream: ordered after BOTH kernels
         torch.cuda.synchronize()
-    finally:
-        hx.tune_sm_rates(None)
     assert np.array_equal(dev_u16(k_after), ok) and np.array_equal(dev_u16(cache.v), ov)
-    _check_all_rows("llama70b_tp1", out.cpu().numpy(), ref, "hx_decode_step, tuned, overlapped handoff")
+    _check_all_rows("llama70b_tp1", out.cpu().numpy(), ref, "hx_decode_step, overlapped handoff")
 
 
 def test_ingest_config4_all_80_layers_both_ranks(env):

@@ -57,7 +57,7 @@ def test_cache_life_cycle_through_the_page_pool(env, overlap):
         reused += len(seen_pages & set(new_pages.tolist()))
         seen_pages |= set(new_pages.tolist())
         assert not (set(new_pages.tolist()) & set(bt_np[bt_np >= 0].tolist()))          # disjoint from the active batch
-        wi = W.make_ingest_inputs(ci, lens=ilens, src_tp=S, bits=(step % 2 == 0), seed_extra=100 * overlap + step)
+        wi = W.make_ingest_inputs(ci, lens=ilens, src_tp=S, seed_extra=100 * overlap + step)
         q_np = W.draw_fp16_normal((B, Hq, D), 5, 43, overlap, step)
         qd = to_dev(q_np, torch)
         out = torch.full_like(qd, float("nan"))
@@ -132,13 +132,12 @@ def _long_ingest_setup(hx, torch, oracle, layers):
 
 
 @pytest.mark.slow
-@pytest.mark.parametrize("tuned", [False, True])
-def test_long_ingest_then_tiny_overlapped_attention_then_immediate_read(env, tuned):
+def test_long_ingest_then_tiny_overlapped_attention_then_immediate_read(env):
     """include/hx.h promises that work enqueued after hx_decode_attention_overlapped is ordered after BOTH kernels.
     The hard case: an ingest that runs for more than a millisecond (32 layers, 4.3 GB of traffic), a tiny attention that
     would be done in microseconds, and a copy of the ingested pages enqueued right behind it.  The copy must hold the
     complete handoff (checked against the oracle on the first and the last layer, the last one being written last),
-    and the attention's own result must be right; several repetitions, equal ranges and tuned ranges."""
+    and the attention's own result must be right; several repetitions."""
     hx, torch, oracle = env
     LAYERS = 32
     s = _long_ingest_setup(hx, torch, oracle, LAYERS)
@@ -151,9 +150,7 @@ def test_long_ingest_then_tiny_overlapped_attention_then_immediate_read(env, tun
     ws = torch.zeros(wsb, dtype=torch.uint8, device="cuda")
     base_k = to_dev(s["k0"], torch).expand(LAYERS, -1, -1, -1, -1)
     base_v = to_dev(s["v0"], torch).expand(LAYERS, -1, -1, -1, -1)
-    if tuned:
-        hx.tune_sm_rates(torch.empty(320 << 20, dtype=torch.uint8, device="cuda"))
-    try:
+    if True:
         t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         for rep in range(4):
             cache = hx.PagedCache(base_k.contiguous(), base_v.contiguous())
@@ -178,15 +175,11 @@ def test_long_ingest_then_tiny_overlapped_attention_then_immediate_read(env, tun
                 assert np.array_equal(dev_u16(v_after[l]), s["expect"][l][1]), (rep, l)
             max_abs, rel = attn_errors(out.cpu().numpy(), s["ref"])
             assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (rep, max_abs, rel)
-    finally:
-        if tuned:
-            hx.tune_sm_rates(None)
 
 
-@pytest.mark.parametrize("tuned", [False, True])
-def test_overlapped_attention_back_to_back_and_after_an_empty_ingest(env, tuned):
+def test_overlapped_attention_back_to_back_and_after_an_empty_ingest(env):
     """The overlapped launch is a programmatic dependent ONLY directly behind an ingest kernel.  Behind another
-    attention (same workspace: counters and range claims) or behind an hx_kv_ingest that launched nothing
+    attention (same workspace: partial slots and arrival counters) or behind an hx_kv_ingest that launched nothing
     (batch == 0) it must behave exactly like hx_decode_attention."""
     hx, torch, oracle = env
     Hq, Hkv, D = 32, 4, 128
@@ -203,9 +196,7 @@ def test_overlapped_attention_back_to_back_and_after_an_empty_ingest(env, tuned)
     kw = dict(q_heads=Hq, block_table=bt, block_table_stride=bt.shape[1], seq_lens=sl, batch=24, max_seq_len=mx, workspace=ws,
               workspace_bytes=wsb)
     empty = torch.zeros(1, dtype=torch.int32, device="cuda")
-    if tuned:
-        hx.tune_sm_rates(torch.empty(320 << 20, dtype=torch.uint8, device="cuda"))
-    try:
+    if True:
         outs = [torch.full_like(qd, float("nan")) for _ in range(6)]
         for j in range(0, 6, 2):                             # six launches back to back, alternating layers
             hx.decode_attention_overlapped(outs[j], qd, cache, layer=0, **kw)
@@ -226,6 +217,3 @@ def test_overlapped_attention_back_to_back_and_after_an_empty_ingest(env, tuned)
         torch.cuda.synchronize()
         max_abs, rel = attn_errors(out.cpu().numpy(), refs[0])
         assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (max_abs, rel)
-    finally:
-        if tuned:
-            hx.tune_sm_rates(None)

@@ -188,28 +188,71 @@ def test_ingest_then_attention_end_to_end_tiny(env):
     check_attn(env, wa, "tiny e2e")
 
 
-def test_attention_with_tuned_sm_rates(env):
-    """hx_tune_sm_rates changes only how the tile sequence is cut: results stay inside the tolerance,
-    stay bit-identical from run to run and under page permutation, and reset restores equal ranges."""
+def _planned(hx, torch, w, *, layer=0, sm_scale=0.0):
+    """hx_decode_plan + hx_decode_attention_planned on a workload dict; returns fp16 numpy [B][Hq][D]."""
+    B, Hq, D = w["q"].shape
+    cache = hx.PagedCache(to_dev(w["k"], torch), to_dev(w["v"], torch))
+    Hkv = cache.k.shape[2]
+    qd = to_dev(w["q"], torch)
+    out = torch.full_like(qd, float("nan"))
+    bt = torch.from_numpy(w["block_table"]).cuda()
+    sl = torch.from_numpy(np.ascontiguousarray(w["seq_lens"], dtype=np.int32)).cuda()
+    mx = int(w["seq_lens"].max(initial=0))
+    wsb = hx.decode_attention_workspace_bytes(B, Hq, Hkv, D, mx)
+    ws = torch.zeros(max(wsb, 16), dtype=torch.uint8, device="cuda")
+    plan = torch.full((max(hx.decode_plan_bytes(B, Hkv, mx), 16),), 0xAB, dtype=torch.uint8, device="cuda")
+    hx.decode_plan(plan, cache, q_heads=Hq, block_table=bt, block_table_stride=bt.shape[1], seq_lens=sl, batch=B, max_seq_len=mx)
+    bt.fill_(-7)                                    # the planned call must not need the table or the lengths any more
+    sl.fill_(-7)
+    hx.decode_attention_planned(out, qd, cache, layer=layer, q_heads=Hq, plan=plan, batch=B, max_seq_len=mx, sm_scale=sm_scale,
+                                workspace=ws, workspace_bytes=wsb)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+@pytest.mark.parametrize("G,Hkv,D", [(1, 4, 64), (8, 2, 128), (16, 1, 128), (1, 14, 128), (4, 2, 64), (8, 4, 128)])
+def test_planned_attention_equals_unplanned_bit_for_bit(env, G, Hkv, D):
+    """hx_decode_plan hoists what depends only on seq_lens and the block table out of the layer calls; the planned
+    kernel uses the same work partition and arithmetic, so its output is the unplanned call's, bit for bit — page
+    boundaries, empty contexts, a context of one token, two layers, custom scale."""
     hx, torch, oracle = env
-    c = W.AttnConfig(77, "tuned", 12, 32, 4, 128, 256, "x")
-    w = W.make_attention_inputs(c, lens=np.array([1, 17, 64, 100, 255, 256, 700, 1000, 2000, 3000, 4000, 33], dtype=np.int32))
-    base = run_gpu_attention(hx, torch, w)
-    scratch = torch.empty(320 << 20, dtype=torch.uint8, device="cuda")
-    scratch.random_()
-    try:
-        hx.tune_sm_rates(scratch)
-        torch.cuda.synchronize()
-        got, _ = check_attn(env, w, "tuned")
-        again = run_gpu_attention(hx, torch, w)
-        assert np.array_equal(got.view(np.uint16), again.view(np.uint16))
-        check_attn(env, W.make_attention_inputs(W.CONFIGS["tiny"]), "tuned tiny")
-        with pytest.raises(hx.HxError):
-            hx.tune_sm_rates(scratch[: 1 << 20])                      # too small to be HBM-bound
-    finally:
-        hx.tune_sm_rates(None)
-        torch.cuda.synchronize()
-    assert np.array_equal(base.view(np.uint16), run_gpu_attention(hx, torch, w).view(np.uint16))
+    lens = np.array([1, 15, 16, 17, 0, 31, 32, 33, 255, 256, 257, 1000, 2, 0, 3000], dtype=np.int32)
+    c = W.AttnConfig(78, "plan", len(lens), G * Hkv, Hkv, D, 256, "x")
+    w = W.make_attention_inputs(c, lens=lens, layers=2, seed_extra=G * 100 + Hkv)
+    for layer, scale in ((0, 0.0), (1, 0.07)):
+        base = run_gpu_attention(hx, torch, w, layer=layer, sm_scale=scale)
+        got = _planned(hx, torch, w, layer=layer, sm_scale=scale)
+        assert np.array_equal(base.view(np.uint16), got.view(np.uint16)), (G, Hkv, D, layer)
+        ref = oracle.decode_attention(w["q"], w["k"], w["v"], w["block_table"], lens, layer=layer, sm_scale=scale or None)
+        max_abs, rel = attn_errors(got, ref)
+        assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (G, Hkv, D, layer, max_abs, rel)
+        assert (got[4] == 0).all() and (got[13] == 0).all()               # reading S11 through the plan's empty list
+
+
+def test_one_plan_serves_every_layer_of_a_step(env):
+    """The use the plan is for: one hx_decode_plan, then one planned call per layer, all against the oracle."""
+    hx, torch, oracle = env
+    lens = W.rng(79, 0).integers(1, 1500, size=40).astype(np.int32)
+    c = W.AttnConfig(79, "plan", 40, 32, 4, 128, 128, "x")
+    L = 5
+    w = W.make_attention_inputs(c, lens=lens, layers=L)
+    cache = hx.PagedCache(to_dev(w["k"], torch), to_dev(w["v"], torch))
+    bt, sl = torch.from_numpy(w["block_table"]).cuda(), torch.from_numpy(lens).cuda()
+    mx = int(lens.max())
+    wsb = hx.decode_attention_workspace_bytes(40, 32, 4, 128, mx)
+    ws = torch.zeros(wsb, dtype=torch.uint8, device="cuda")
+    plan = torch.empty(hx.decode_plan_bytes(40, 4, mx), dtype=torch.uint8, device="cuda")
+    hx.decode_plan(plan, cache, q_heads=32, block_table=bt, block_table_stride=bt.shape[1], seq_lens=sl, batch=40, max_seq_len=mx)
+    qs = [W.draw_fp16_normal((40, 32, 128), 79, 5, l) for l in range(L)]
+    outs = [torch.full((40, 32, 128), float("nan"), dtype=torch.float16, device="cuda") for _ in range(L)]
+    for l in range(L):                                   # back to back, as a model's layer loop issues them
+        hx.decode_attention_planned(outs[l], to_dev(qs[l], torch), cache, layer=l, q_heads=32, plan=plan, batch=40, max_seq_len=mx,
+                                    workspace=ws, workspace_bytes=wsb)
+    torch.cuda.synchronize()
+    for l in range(L):
+        ref = oracle.decode_attention(qs[l], w["k"], w["v"], w["block_table"], lens, layer=l)
+        max_abs, rel = attn_errors(outs[l].cpu().numpy(), ref)
+        assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (l, max_abs, rel)
 
 
 def test_attention_batch_larger_than_one_launch(env):
