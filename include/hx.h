@@ -12,8 +12,8 @@
  *  - DEVICE pointers are marked "device"; everything else is host memory.  The caller owns all
  *    device memory, including the workspace.  The library allocates no device memory and keeps no
  *    state on the device.  Its host-side state: (1) per device, one side stream and two events, created
- *    by the first hx_decode_step / hx_decode_step_host call that asks for an overlapped handoff and
- *    destroyed by hx_shutdown(); (2) caches of device properties and TMA descriptors.  hx_page_pool is
+ *    by the first hx_decode_step_host call that asks for an overlapped handoff and destroyed by
+ *    hx_shutdown(); (2) caches of device properties and TMA descriptors.  hx_page_pool is
  *    the only heap object the caller owns (host).
  *  - Thread safety: every entry point may be called from several host threads (on different streams);
  *    hx_decode_step* serialise on one library mutex while they enqueue.  An hx_page_pool and an attention
@@ -309,13 +309,19 @@ void    hx_pool_destroy(hx_page_pool* pool);
  * KV cache communication is asynchronous "to enable overlapping between computation and
  * communication".  One call = hx_kv_ingest of the step's new prompts (ing_* arguments; skipped when
  * ing_batch == 0) + hx_decode_attention over the active batch (skipped when batch == 0).  Every argument means
- * what it means in those two calls.  overlap_ingest != 0: the caller asserts that the attention does NOT read
- * the pages this step ingests (the new prompts join the batch in a later step); the ingest then runs on a
- * library-owned side stream, forked from `stream` at entry (so it sees everything enqueued on `stream` so
- * far, e.g. the upload of ing_block_table) and joined to `stream` before return, on every path: work enqueued
- * on `stream` afterwards is ordered after both kernels.  overlap_ingest == 0: both in order on `stream`.
+ * what it means in those two calls.
+ * overlap_ingest == 0: ingest, then attention, in order on `stream` (the attention may read the new pages).
+ * overlap_ingest != 0: the caller asserts that the attention does NOT read the pages this step ingests (the new
+ * prompts join the batch in a later step).  Both kernels are HBM-bound, so running them side by side would only
+ * slow the attention down by what the handoff moves; instead the attention kernel is enqueued first and the
+ * handoff kernel follows on the same stream as its programmatic dependent: the attention's CTAs release it at
+ * once, but its CTAs ask for more shared memory than an attention CTA leaves free on an SM, so each is placed only
+ * where the attention has already finished.  The handoff thus runs in the attention kernel's tail, on the SMs
+ * that finished early, and each of its CTAs waits for the attention grid before it exits: work enqueued on
+ * `stream` afterwards is ordered after BOTH kernels.  Uses the last 16 bytes of `workspace` (two counters that
+ * every call leaves at zero).
  * Every host-side check of both calls runs first; nothing is enqueued unless all pass.  Capturable in a CUDA
- * graph (the fork/join is the standard event pattern). */
+ * graph. */
 typedef struct {
   /* attention over the active batch (hx_decode_attention) */
   void*       out;               /* device fp16 [batch][q_heads][head_dim] */
@@ -334,14 +340,16 @@ typedef struct {
   const int32_t* ing_cu_seqlens;  const int32_t* ing_seq_lens;      /* device */
   int32_t ing_batch, ing_total_tokens, ing_max_seq_len;
   int32_t overlap_ingest;
-  /* optional timing: cudaEvent_t handles (or NULL) recorded directly before / after the ingest kernel on the stream
-   * it runs on, and directly before / after the attention kernel on `stream` */
+  /* optional timing: cudaEvent_t handles (or NULL) recorded directly before / after the ingest kernel and directly
+   * before / after the attention kernel.  With overlap_ingest != 0 nothing may sit between the two launches, so both
+   * "begin" events are recorded before the pair and both "end" events after it. */
   void* ev_ingest_begin; void* ev_ingest_end; void* ev_attention_begin; void* ev_attention_end;
 } hx_step_args;
 int hx_decode_step(const hx_step_args* args, void* stream);
 
-/* Destroys the library-owned side streams and events of every device (after synchronising them).  Optional:
- * call when no hx_decode_step* call is in flight; a later call re-creates them. */
+/* Destroys the library-owned side streams and events of every device (after synchronising them; only
+ * hx_decode_step_host with overlap_ingest creates them).  Optional: call when no such call is in flight; a later
+ * call re-creates them. */
 int hx_shutdown(void);
 
 /* ---- whole decode step with HOST inputs (bench.py "e2e") --------

@@ -281,6 +281,9 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tmK) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tmV) : "memory");
   }
+  // a kernel launched as a programmatic dependent of this one (hx_decode_step's handoff) may be scheduled from now
+  // on: it gets an SM only where this grid has left one; without such a launch this is a no-op
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const int w = blockIdx.x * kWarps + warp;          // worker id
   if (lane == 0) {
     const uint32_t b0 = smem_u32(bars + warp * (kStages + 1));
@@ -805,7 +808,17 @@ size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, in
   const int nt = G > 8 ? 2 : 1;
   const size_t slot = (size_t)nt * ((head_dim / 16) * 128 + 16) * sizeof(float);
   const size_t counter_bytes = ((size_t)kBMax * kv_heads * sizeof(int32_t) + 15) & ~(size_t)15;
-  return 2 * (size_t)kMaxWorkers * slot + counter_bytes;
+  return 2 * (size_t)kMaxWorkers * slot + counter_bytes + 16;     // + the overlapped step's two claim counters
+}
+
+size_t attn_workspace_claim_offset(int32_t q_heads, int32_t kv_heads, int32_t head_dim) {
+  return attn_workspace_bytes(0, q_heads, kv_heads, head_dim, 0, 16) - 16;
+}
+
+int attn_smem_bytes(int32_t head_dim, int32_t q_heads, int32_t kv_heads) {
+  const bool nt2 = q_heads / kv_heads > 8;
+  if (head_dim == 128) return (nt2 ? Cfg<128, 2>::kSmem : Cfg<128, 1>::kSmem) + 1024;      // + the static part
+  return (nt2 ? Cfg<64, 2>::kSmem : Cfg<64, 1>::kSmem) + 1024;
 }
 
 // Upper bound of a plan's size: header + empty list + first[W][32] + one descriptor per possible tile.

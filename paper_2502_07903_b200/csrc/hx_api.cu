@@ -60,7 +60,7 @@ static int ingest_common(const void* const* src_k, const void* const* src_v, int
                          const int32_t* cu_seqlens, const int32_t* seq_lens, int32_t batch,
                          int32_t total_tokens, int32_t max_seq_len, void* stream, bool gather,
                          const char* who, int32_t src_layers, int32_t src_layer0, int32_t dst_layer0,
-                         bool dry_run = false) {
+                         bool dry_run = false, int32_t tail_smem = 0, int32_t* tail_claim = nullptr) {
   clear_error();
   if (layers < 0 || batch < 0 || total_tokens < 0 || max_seq_len < 0)
     HX_FAIL(HX_ERR_INVALID_ARG, "%s: negative size (layers=%d batch=%d total_tokens=%d max_seq_len=%d)", who, layers, batch, total_tokens, max_seq_len);
@@ -101,6 +101,11 @@ static int ingest_common(const void* const* src_k, const void* const* src_v, int
   p.src_layer0 = src_layer0; p.dst_layer0 = dst_layer0;
   p.head_dim = head_dim; p.page_size = ps; p.num_pages = dst->num_pages; p.bt_stride = stride;
   if (dry_run) return HX_OK;                                   // checks only (hx_decode_step validates before it enqueues)
+  if (tail_claim) {                                            // hx_decode_step: dependent of the attention kernel before it
+    rc = launch_ingest_tail(p, tail_smem, tail_claim, static_cast<cudaStream_t>(stream));
+    if (rc == HX_OK) note_launch(stream, kLaunchOther);
+    return rc;
+  }
   rc = launch_ingest(p, gather, static_cast<cudaStream_t>(stream));
   if (rc == HX_OK) note_launch(stream, gather ? kLaunchOther : kLaunchIngest);
   return rc;
@@ -411,10 +416,16 @@ int step_impl(const char* who, const hx_step_args* a, const hx_step_host_args* h
     }
   }
 
-  // ---- enqueue.  overlap_ingest: the handoff goes to the side stream, forked from and joined to the caller's
-  // stream; once forked, every exit path joins, so the caller's stream always covers whatever was enqueued.
+  // ---- enqueue.
+  // overlap_ingest, device buffers: ONE stream.  The attention kernel goes first; the handoff follows as its programmatic
+  // dependent ("tail filler", ingest.cu): its CTAs get an SM only where the attention has left one, and each waits for
+  // the attention grid before it exits, so whatever is enqueued afterwards is ordered after both kernels.
+  // overlap_ingest, host buffers (hx_decode_step_host): the shards must cross PCIe first; copies + ingest go to the
+  // library's side stream, forked from and joined to the caller's stream; once forked, every exit path joins.
   std::lock_guard<std::mutex> lock(g_step_mu);
-  const bool fork = a->overlap_ingest != 0 && do_ing && do_att;
+  const bool overlap = a->overlap_ingest != 0 && do_ing && do_att;
+  const bool tail = overlap && !h;
+  const bool fork = overlap && h;
   SideStream* ss = nullptr;
   cudaStream_t ing_stream = main_stream;
   int dev = 0;
@@ -431,35 +442,62 @@ int step_impl(const char* who, const hx_step_args* a, const hx_step_host_args* h
 #define STEP_CUDA(expr) do { if (rc == HX_OK && ce == cudaSuccess) { ce = (expr); if (ce != cudaSuccess) what = #expr; } } while (0)
   // the attention's small q upload goes first on the caller's stream so that it is not queued behind the shards
   if (h && do_att) STEP_CUDA(cudaMemcpyAsync(const_cast<void*>(a->q), h->q_host, qbytes, cudaMemcpyHostToDevice, main_stream));
-  if (do_ing) {
-    if (h) {
-      for (int r = 0; r < a->src_tp && !h->pull_src; ++r) {
-        if (!h->src_k_host[r] || !h->src_k_dev[r]) continue;   // shard not needed by this rank
-        STEP_CUDA(cudaMemcpyAsync(h->src_k_dev[r], h->src_k_host[r], shard, cudaMemcpyHostToDevice, ing_stream));
-        STEP_CUDA(cudaMemcpyAsync(h->src_v_dev[r], h->src_v_host[r], shard, cudaMemcpyHostToDevice, ing_stream));
-      }
-      STEP_CUDA(cudaMemcpyAsync(const_cast<int32_t*>(a->ing_block_table), h->ing_block_table_host,
-                                (size_t)a->ing_batch * a->ing_block_table_stride * 4, cudaMemcpyHostToDevice, ing_stream));
-      STEP_CUDA(cudaMemcpyAsync(const_cast<int32_t*>(a->ing_cu_seqlens), h->ing_cu_seqlens_host, (size_t)(a->ing_batch + 1) * 4,
-                                cudaMemcpyHostToDevice, ing_stream));
-      STEP_CUDA(cudaMemcpyAsync(const_cast<int32_t*>(a->ing_seq_lens), h->ing_seq_lens_host, (size_t)a->ing_batch * 4,
-                                cudaMemcpyHostToDevice, ing_stream));
-    }
-    if (a->ev_ingest_begin) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_ingest_begin), ing_stream));
-    if (rc == HX_OK && ce == cudaSuccess)
-      rc = ingest_common(a->src_k, a->src_v, a->ing_layers, a->heads, a->cache->head_dim, a->src_tp, a->dst_tp, a->dst_rank,
-                         a->cache, a->ing_block_table, a->ing_block_table_stride, a->ing_cu_seqlens, a->ing_seq_lens,
-                         a->ing_batch, a->ing_total_tokens, a->ing_max_seq_len, static_cast<void*>(ing_stream), false, who, -1, 0, 0);
-    if (a->ev_ingest_end) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_ingest_end), ing_stream));
-  }
-  if (do_att && rc == HX_OK && ce == cudaSuccess) {
-    if (a->ev_attention_begin) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_attention_begin), main_stream));
+  auto enqueue_attention = [&]() {
     if (rc == HX_OK && ce == cudaSuccess)
       rc = attention_common(who, a->out, a->q, nullptr, nullptr, false, false, a->cache, a->layer, a->q_heads, a->block_table,
                             a->block_table_stride, a->seq_lens, a->batch, a->max_seq_len, a->sm_scale, a->workspace,
                             a->workspace_bytes, stream_);
+  };
+  auto enqueue_ingest = [&](int32_t tail_smem, int32_t* tail_claim) {
+    if (rc == HX_OK && ce == cudaSuccess)
+      rc = ingest_common(a->src_k, a->src_v, a->ing_layers, a->heads, a->cache->head_dim, a->src_tp, a->dst_tp, a->dst_rank,
+                         a->cache, a->ing_block_table, a->ing_block_table_stride, a->ing_cu_seqlens, a->ing_seq_lens,
+                         a->ing_batch, a->ing_total_tokens, a->ing_max_seq_len, static_cast<void*>(ing_stream), false, who, -1, 0, 0,
+                         false, tail_smem, tail_claim);
+  };
+  if (tail) {
+    // nothing may sit between the two launches (an event record would take away their kernel-to-kernel adjacency): the
+    // optional timing events bracket the PAIR
+    if (a->ev_ingest_begin) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_ingest_begin), main_stream));
+    if (a->ev_attention_begin) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_attention_begin), main_stream));
+    enqueue_attention();
+    DeviceInfo di;
+    if (rc == HX_OK && ce == cudaSuccess) rc = device_info(&di);
+    if (rc == HX_OK && ce == cudaSuccess) {
+      // one byte more than an attention CTA leaves free on an SM (each CTA also costs the SM 1 KiB of bookkeeping)
+      const int32_t sm_total = di.max_smem_optin + 1024;
+      const int32_t req = sm_total - (attn_smem_bytes(a->cache->head_dim, a->q_heads, a->cache->kv_heads) + 1024) - 1024 + 256;
+      int32_t* claim = reinterpret_cast<int32_t*>(static_cast<char*>(a->workspace) +
+                                                  attn_workspace_claim_offset(a->q_heads, a->cache->kv_heads, a->cache->head_dim));
+      enqueue_ingest(req, claim);
+    }
     if (a->ev_attention_end) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_attention_end), main_stream));
-    if (h) STEP_CUDA(cudaMemcpyAsync(h->out_host, a->out, qbytes, cudaMemcpyDeviceToHost, main_stream));
+    if (a->ev_ingest_end) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_ingest_end), main_stream));
+  } else {
+    if (do_ing) {
+      if (h) {
+        for (int r = 0; r < a->src_tp && !h->pull_src; ++r) {
+          if (!h->src_k_host[r] || !h->src_k_dev[r]) continue;   // shard not needed by this rank
+          STEP_CUDA(cudaMemcpyAsync(h->src_k_dev[r], h->src_k_host[r], shard, cudaMemcpyHostToDevice, ing_stream));
+          STEP_CUDA(cudaMemcpyAsync(h->src_v_dev[r], h->src_v_host[r], shard, cudaMemcpyHostToDevice, ing_stream));
+        }
+        STEP_CUDA(cudaMemcpyAsync(const_cast<int32_t*>(a->ing_block_table), h->ing_block_table_host,
+                                  (size_t)a->ing_batch * a->ing_block_table_stride * 4, cudaMemcpyHostToDevice, ing_stream));
+        STEP_CUDA(cudaMemcpyAsync(const_cast<int32_t*>(a->ing_cu_seqlens), h->ing_cu_seqlens_host, (size_t)(a->ing_batch + 1) * 4,
+                                  cudaMemcpyHostToDevice, ing_stream));
+        STEP_CUDA(cudaMemcpyAsync(const_cast<int32_t*>(a->ing_seq_lens), h->ing_seq_lens_host, (size_t)a->ing_batch * 4,
+                                  cudaMemcpyHostToDevice, ing_stream));
+      }
+      if (a->ev_ingest_begin) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_ingest_begin), ing_stream));
+      enqueue_ingest(0, nullptr);
+      if (a->ev_ingest_end) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_ingest_end), ing_stream));
+    }
+    if (do_att) {
+      if (a->ev_attention_begin) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_attention_begin), main_stream));
+      enqueue_attention();
+      if (a->ev_attention_end) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_attention_end), main_stream));
+      if (h) STEP_CUDA(cudaMemcpyAsync(h->out_host, a->out, qbytes, cudaMemcpyDeviceToHost, main_stream));
+    }
   }
 #undef STEP_CUDA
   if (fork) {                                                   // join on every path, error or not

@@ -50,6 +50,9 @@ struct IngestParams {
   int32_t head_dim, page_size, num_pages, bt_stride;
 };
 int launch_ingest(const IngestParams& p, bool gather, cudaStream_t stream);
+// the handoff as a programmatic dependent of the attention kernel enqueued just before it (hx_decode_step); `claim` = two
+// zeroed ints of device memory that the kernel leaves at zero
+int launch_ingest_tail(const IngestParams& p, int32_t smem_request, int32_t* claim, cudaStream_t stream);
 
 struct AttnParams {
   void* out;
@@ -72,7 +75,11 @@ size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, in
                             int32_t max_seq_len, int32_t page_size);
 size_t attn_plan_bytes(int32_t batch, int32_t kv_heads, int32_t max_seq_len, int32_t page_size);
 int launch_attention(const AttnParams& p, cudaStream_t stream);
-int launch_plan(const AttnParams& p, cudaStream_t stream);      // uses seq_lens, block_table, batch, heads, bt_stride, plan
+int launch_plan(const AttnParams& p, cudaStream_t stream);
+// shared memory one CTA of the attention kernel occupies for this head layout, and where the two claim counters of the
+// overlapped step live in the attention workspace (hx_decode_step)
+int attn_smem_bytes(int32_t head_dim, int32_t q_heads, int32_t kv_heads);
+size_t attn_workspace_claim_offset(int32_t q_heads, int32_t kv_heads, int32_t head_dim);      // uses seq_lens, block_table, batch, heads, bt_stride, plan
 
 struct PrefillArgs {
   void* out;

@@ -12,6 +12,8 @@
 // the 16 tokens of a CTA tile that share a page write one contiguous 4 KiB (page, head) run.
 #include <cuda_fp16.h>
 
+#include <mutex>
+
 #include "hx_internal.h"
 
 namespace hx {
@@ -37,15 +39,13 @@ __device__ __forceinline__ void st_stream(int4* p, const int4& v) {
                :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
+// One CTA tile: TOK packed tokens starting at token tile `tile`, layers l0, l0 + lstep, ... of the call.
 template <int D, bool GATHER>
-__global__ void __launch_bounds__(kThreads, kMinCtas) ingest_rows_kernel(const __grid_constant__ IngestParams p, int layer_splits) {
+__device__ __forceinline__ void move_token_tile(const IngestParams& p, int tile, int l0, int lstep) {
   constexpr int CH = D / 8;                 // 16-byte chunks per row
   constexpr int TOK = kThreads / CH;        // packed tokens per CTA tile
-  // a kernel launched as a programmatic dependent of this one (hx_decode_attention_overlapped) may start now;
-  // without such a launch this is a no-op
-  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const int dc = threadIdx.x % CH;
-  const int tk = blockIdx.x * TOK + threadIdx.x / CH;
+  const int tk = tile * TOK + threadIdx.x / CH;
   if (tk >= p.total_tokens) return;
 
   // request i with cu[i] <= tk < cu[i+1] (largest i whose start is <= tk; empty requests skipped)
@@ -66,7 +66,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) ingest_rows_kernel(const _
   const size_t src_tok = ((size_t)tk * p.hs) * D + dc * 8;
   const size_t dst_tok = ((size_t)page * p.hd * ps + slot) * D + dc * 8;
 
-  for (int l = blockIdx.y; l < p.layers; l += layer_splits) {
+  for (int l = l0; l < p.layers; l += lstep) {
     for (int base = 0; base < nitems; base += kBatch) {
       int4 val[kBatch];
       int4* wr[kBatch];
@@ -93,6 +93,39 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) ingest_rows_kernel(const _
         if (base + u < nitems) st_stream(wr[u], val[u]);
     }
   }
+}
+
+template <int D, bool GATHER>
+__global__ void __launch_bounds__(kThreads, kMinCtas) ingest_rows_kernel(const __grid_constant__ IngestParams p, int layer_splits) {
+  // a kernel launched as a programmatic dependent of this one (hx_decode_attention_overlapped) may start now;
+  // without such a launch this is a no-op
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  move_token_tile<D, GATHER>(p, blockIdx.x, blockIdx.y, layer_splits);
+}
+
+// The handoff as a TAIL FILLER (hx_decode_step, overlap_ingest): launched as a programmatic dependent of the attention
+// kernel, whose CTAs release their dependents as soon as they start.  Every CTA of this grid REQUESTS more shared
+// memory than an attention CTA leaves free (it uses none), so it is placed on an SM only when that SM's attention CTA
+// has left: the handoff runs in the attention kernel's tail, on the SMs that finished early, instead of taking
+// bandwidth from its main phase (both kernels are HBM-bound).  CTAs start at different times, so (token tile, layer)
+// units are claimed from a counter; a bit copy does not care who moves what.  Each CTA waits for the attention grid
+// before it exits: completion of this grid implies completion of both.
+template <int D>
+__global__ void __launch_bounds__(kThreads, 3) ingest_rows_tail_kernel(const __grid_constant__ IngestParams p, int tiles, int* claim) {
+  __shared__ int unit[2];
+  const int units = tiles * p.layers;
+  if (threadIdx.x == 0) unit[0] = atomicAdd(claim, 1);
+  __syncthreads();
+  for (int it = 0;; ++it) {
+    const int u = unit[it & 1];
+    if (u >= units) break;
+    if (threadIdx.x == 0) unit[(it + 1) & 1] = atomicAdd(claim, 1);      // next claim rides under this unit's copies
+    move_token_tile<D, false>(p, u % tiles, u / tiles, p.layers);         // unit = one token tile of one layer
+    __syncthreads();
+  }
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  // the last CTA out leaves the two counters at zero for the next call (plain stores, flushed at kernel end)
+  if (threadIdx.x == 0 && atomicAdd(claim + 1, 1) == (int)gridDim.x - 1) { claim[0] = 0; claim[1] = 0; }
 }
 
 // hx_kv_append: one thread per 16-byte chunk of one
@@ -125,6 +158,39 @@ int launch_append(const AppendParams& p, cudaStream_t stream) {
   if (p.head_dim == 128) append_kernel<128><<<grid, kThreads, 0, stream>>>(p);
   else                   append_kernel<64><<<grid, kThreads, 0, stream>>>(p);
   HX_CUDA_OK(cudaGetLastError());
+  return HX_OK;
+}
+
+int launch_ingest_tail(const IngestParams& p, int32_t smem_request, int32_t* claim, cudaStream_t stream) {
+  DeviceInfo di;
+  int rc = device_info(&di);
+  if (rc) return rc;
+  const int tok = kThreads / (p.head_dim / 8);
+  const int tiles = (p.total_tokens + tok - 1) / tok;
+  if ((long long)tiles * p.layers >= (1ll << 30)) HX_FAIL(HX_ERR_UNSUPPORTED, "handoff too large for the overlapped step");
+  const int max_dyn = di.max_smem_optin - 1024;               // (the kernel has a few bytes of static shared memory)
+  if (smem_request > max_dyn) smem_request = max_dyn;
+  if (smem_request < 0) smem_request = 0;
+  {
+    static std::mutex mu;
+    static bool attr_set[64] = {false};
+    std::lock_guard<std::mutex> lock(mu);
+    if (!attr_set[di.device]) {
+      HX_CUDA_OK(cudaFuncSetAttribute(ingest_rows_tail_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn));
+      HX_CUDA_OK(cudaFuncSetAttribute(ingest_rows_tail_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn));
+      attr_set[di.device] = true;
+    }
+  }
+  long long grid = (long long)di.sm_count * 3;                 // what fits once every SM is free
+  if (grid > (long long)tiles * p.layers) grid = (long long)tiles * p.layers;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = (size_t)smem_request; cfg.stream = stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  if (p.head_dim == 128) HX_CUDA_OK(cudaLaunchKernelEx(&cfg, ingest_rows_tail_kernel<128>, p, tiles, claim));
+  else                   HX_CUDA_OK(cudaLaunchKernelEx(&cfg, ingest_rows_tail_kernel<64>, p, tiles, claim));
   return HX_OK;
 }
 
