@@ -618,11 +618,14 @@ def time_back_to_back(torch, fn, calls=40, reps=5, warm=5):
     return float(np.median(ts))
 
 
-def other_configs(torch, hx, dev, peak):
+def other_configs(torch, hx, dev, peak, only=None):
     """Kernel-only numbers for configs[1], [2] (attention) and [3] (80-layer ingest), outside the
-    timed step.  Cold L2: each timed call reads a different one of several cache copies."""
+    timed step.  Cold L2: each timed call reads a different one of several cache copies.
+    `only` (--kernel-only) restricts the run to one of them: a short command to put under ncu."""
     res = {}
-    for name in ("opt30b_tp4", "llama70b_tp2"):
+    for name in ("opt30b_tp4", "llama70b_tp2", "llama70b_tp1"):
+        if name != only and (only is not None or name == "llama70b_tp1"):
+            continue
         c = W.CONFIGS[name]
         lens = W.attn_lengths(c)
         need = int(W.pages_for(lens).sum())
@@ -676,6 +679,8 @@ def other_configs(torch, hx, dev, peak):
                                "as the layer loop of a decode step issues them",
                      "l2": f"rotating over {copies} cache copies"}
         del k, v, cache
+    if only not in (None, "llama70b_ingest"):
+        return res
     # configs[3]: 80-layer ingest, prefill TP=4 -> decode TP=2, both destination ranks
     c = W.CONFIGS["llama70b_ingest"]
     w1 = W.make_ingest_inputs(c, layers=1)
@@ -819,6 +824,8 @@ def main():
     ap.add_argument("--no-extra", action="store_true", help="skip the configs[1..3] kernel-only section")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--oracle-table", action="store_true", help="time the oracle per config at 1 thread and all cores, then exit")
+    ap.add_argument("--kernel-only", default=None, choices=["opt30b_tp4", "llama70b_tp2", "llama70b_tp1", "llama70b_ingest", "prefill"],
+                    help="time only this config's kernel (no step, no extras) and print a small JSON line: the command to profile")
     args = ap.parse_args()
     if args.oracle_table:
         oracle_table(args)
@@ -836,6 +843,16 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     from paper_2502_07903_b200.build import build
     build()
+    if args.kernel_only:
+        import torch
+        import paper_2502_07903_b200 as hx
+        torch.cuda.set_device(local_rank)
+        torch.manual_seed(1234)
+        dev = torch.device("cuda", local_rank)
+        peak, _ = measured_peak()
+        res = prefill_extra(torch, hx, dev) if args.kernel_only == "prefill" else other_configs(torch, hx, dev, peak, only=args.kernel_only)
+        print(json.dumps({"kernel_only": args.kernel_only, "result": res}), flush=True)
+        return
     run_hx(args, rank, world, local_rank)
 
 
