@@ -657,10 +657,18 @@ def other_configs(torch, hx, dev, peak, only=None):
             state["i"] = (state["i"] + 1) % copies
             hx.decode_attention_planned(out, q, cache, layer=state["i"], q_heads=c.q_heads, plan=plan, batch=c.batch,
                                         max_seq_len=mx, workspace=ws, workspace_bytes=wsb)
+        def fn_chained(ready):
+            def f():
+                state["i"] = (state["i"] + 1) % copies
+                hx.decode_attention_chained(out, q, cache, layer=state["i"], q_heads=c.q_heads, plan=plan, batch=c.batch,
+                                            max_seq_len=mx, workspace=ws, workspace_bytes=wsb, inputs_ready=ready)
+            return f
         med, mn = time_kernel(torch, fn, iters=40)               # one event pair per call (adds ~2 us of event work)
         b2b = time_back_to_back(torch, fn)                       # one event pair around 40 calls: the layer-loop rate
         medp, mnp = time_kernel(torch, fn_planned, iters=40)
         b2bp = time_back_to_back(torch, fn_planned)
+        b2bc1 = time_back_to_back(torch, fn_chained(1))          # layer calls as programmatic dependents of one another
+        b2bc0 = time_back_to_back(torch, fn_chained(0))
         plan_ms, _ = time_kernel(torch, lambda: hx.decode_plan(plan, cache, q_heads=c.q_heads, block_table=bt,
                                                                block_table_stride=bt.shape[1], seq_lens=sl, batch=c.batch,
                                                                max_seq_len=mx), iters=10)
@@ -673,6 +681,12 @@ def other_configs(torch, hx, dev, peak, only=None):
                                                  "frac_of_measured": kvb / medp / 1e6 / peak,
                                                  "frac_of_nominal_8000": kvb / medp / 1e6 / NOMINAL_HBM_GBS},
                      "planned_back_to_back": {"ms": b2bp, "kv_GBps": kvb / b2bp / 1e6, "frac_of_measured": kvb / b2bp / 1e6 / peak},
+                     "chained_back_to_back": {"ms": b2bc1, "kv_GBps": kvb / b2bc1 / 1e6, "frac_of_measured": kvb / b2bc1 / 1e6 / peak,
+                                              "frac_of_nominal_8000": kvb / b2bc1 / 1e6 / NOMINAL_HBM_GBS,
+                                              "inputs_ready_0_ms": b2bc0,
+                                              "note": "hx_decode_attention_chained: each call a programmatic dependent of the one "
+                                                      "before it (inputs_ready=1: streams under its predecessor's tail, writes wait; "
+                                                      "inputs_ready=0: only launch + set-up overlap)"},
                      "plan_ms": plan_ms, "tokens_per_s_one_layer": c.batch / (medp * 1e-3),
                      "timing": "per_call_events: one CUDA-event pair per call (SURVEY 8(d) protocol), median of 40; back_to_back: one event "
                                "pair around 40 calls; planned_*: hx_decode_plan once (plan_ms), then hx_decode_attention_planned per call, "

@@ -54,7 +54,7 @@
 extern "C" {
 #endif
 
-#define HX_VERSION 131 /* 0.1.3.1: + hx_decode_step (device buffers), hx_shutdown, per-step plan; - hx_tune_sm_rates */
+#define HX_VERSION 132 /* 0.1.3.2: + hx_decode_attention_chained */
 
 typedef enum {
   HX_OK = 0,
@@ -289,6 +289,29 @@ int hx_decode_attention_planned(void* out, const void* q,
                                 int32_t batch, int32_t max_seq_len, float sm_scale,
                                 void* workspace, size_t workspace_bytes,
                                 void* stream);
+
+/* hx_decode_attention_planned launched as a PROGRAMMATIC DEPENDENT of whatever kernel precedes it on `stream`
+ * ("asynchronous ... to enable overlapping"; a model issues one attention call per layer, and a call of
+ * configs[2]'s size is so short that its launch latency, set-up and the tail in which its last warps finish are a fifth
+ * of it).  Same arguments and bit-identical result.  The grid may be placed on an SM as soon as the preceding kernel
+ * has left it (this library's kernels release their dependents as soon as they start; any other kernel does when it
+ * exits, which makes this a plain launch), and
+ *   inputs_ready == 0: it reads nothing from device memory until the preceding kernel has completed and its writes are
+ *                      visible (griddepcontrol.wait): safe behind ANY kernel, e.g. the projection that produced q and
+ *                      the append that wrote this token's K/V; launch latency and barrier/descriptor set-up overlap.
+ *   inputs_ready != 0: the CALLER asserts that nothing this call reads (q, the plan, this layer's K/V) is written by the
+ *                      kernel directly before it on `stream`.  The grid then streams its first K/V ranges under that
+ *                      kernel's tail; every global write (out, workspace) still waits for that kernel's completion, so
+ *                      consecutive calls may share `workspace` and `out`.
+ * In both modes every CTA waits for the preceding kernel before it exits: work enqueued after this call is ordered
+ * after both.  Nothing may be enqueued on `stream` between the preceding kernel and this call for the overlap to
+ * happen (an event record in between turns it into a plain launch; the result is the same). */
+int hx_decode_attention_chained(void* out, const void* q,
+                                const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
+                                const void* plan, size_t plan_bytes,
+                                int32_t batch, int32_t max_seq_len, float sm_scale,
+                                void* workspace, size_t workspace_bytes,
+                                int32_t inputs_ready, void* stream);
 
 /* ---- host page allocator (paging by citation PAPER.md:L110, OOM
  * remark PAPER.md:L136).  A free list of page ids; alloc is all-or-nothing.  Not thread-safe. */

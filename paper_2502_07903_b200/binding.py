@@ -16,7 +16,7 @@ EXPORTS = [
     "hx_kv_gather", "hx_decode_attention_workspace_bytes", "hx_decode_attention", "hx_pool_create",
     "hx_pool_shuffle", "hx_pool_alloc", "hx_pool_free", "hx_pool_num_free", "hx_pool_num_pages",
     "hx_pool_alloc_table", "hx_pool_destroy", "hx_decode_step_host", "hx_decode_plan_bytes", "hx_decode_plan",
-    "hx_decode_attention_planned",
+    "hx_decode_attention_planned", "hx_decode_attention_chained",
     "hx_kv_ingest_stage", "hx_stage_overlap", "hx_kv_append", "hx_decode_attention_append",
     "hx_prefill_attention", "hx_decode_attention_overlapped", "hx_decode_step", "hx_shutdown",
 ]
@@ -123,6 +123,10 @@ def lib() -> C.CDLL:
         L.hx_decode_attention_planned.restype = C.c_int
         L.hx_decode_attention_planned.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CCache), C.c_int32, C.c_int32, C.c_void_p,
                                                   C.c_size_t, C.c_int32, C.c_int32, C.c_float, C.c_void_p, C.c_size_t, C.c_void_p]
+        L.hx_decode_attention_chained.restype = C.c_int
+        L.hx_decode_attention_chained.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CCache), C.c_int32, C.c_int32, C.c_void_p,
+                                                  C.c_size_t, C.c_int32, C.c_int32, C.c_float, C.c_void_p, C.c_size_t, C.c_int32,
+                                                  C.c_void_p]
         L.hx_kv_ingest_stage.restype = C.c_int
         L.hx_kv_ingest_stage.argtypes = [C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)] + [C.c_int32] * 9 + [
             C.POINTER(_CCache), C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32,
@@ -339,6 +343,18 @@ def decode_attention_planned(out, q, cache: PagedCache, *, layer, q_heads, plan,
     _check(lib().hx_decode_attention_planned(_ptr(out), _ptr(q), cache.ref, layer, q_heads, _ptr(plan), plan_bytes, batch,
                                              max_seq_len, C.c_float(sm_scale), _ptr(workspace), workspace_bytes,
                                              _stream_ptr(stream)))
+
+
+def decode_attention_chained(out, q, cache: PagedCache, *, layer, q_heads, plan, batch, max_seq_len, inputs_ready, sm_scale=0.0,
+                             workspace=None, workspace_bytes=None, plan_bytes=None, stream=None):
+    """hx_decode_attention_chained: hx_decode_attention_planned as a programmatic dependent of the preceding kernel."""
+    if workspace_bytes is None:
+        workspace_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    if plan_bytes is None:
+        plan_bytes = plan.numel() * plan.element_size()
+    _check(lib().hx_decode_attention_chained(_ptr(out), _ptr(q), cache.ref, layer, q_heads, _ptr(plan), plan_bytes, batch,
+                                             max_seq_len, C.c_float(sm_scale), _ptr(workspace), workspace_bytes,
+                                             int(inputs_ready), _stream_ptr(stream)))
 
 
 def _fill_struct(a, kw):

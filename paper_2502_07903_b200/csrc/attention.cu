@@ -49,6 +49,7 @@ constexpr int kMaxSm = 256;        // CTAs (= SMs) per launch
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr int kPlanMagic = 0x68785032;
 constexpr int kPlanHeaderInts = 16;
+enum PdlMode { kPdlNone = 0, kPdlInputs = 1, kPdlWrites = 2, kPdlEnd = 3 };
 
 template <int D, int NT>
 struct Cfg {
@@ -92,10 +93,17 @@ struct StreamParams {
   const __half* v_new;
   __half* kc;
   __half* vc;
-  // hx_decode_attention_overlapped: this grid was launched as a programmatic dependent of the ingest kernel and
-  // reads nothing that kernel writes; every CTA executes griddepcontrol.wait before it exits, so completion of this
-  // grid implies completion (and visibility) of the ingest
-  int32_t pdl_wait_at_end;
+  // Programmatic dependent launch: this grid may start while the kernel enqueued before it on the stream still runs.
+  // Every CTA executes griddepcontrol.wait before it exits in every mode, so completion of this grid implies completion
+  // (and visibility) of its predecessor; the mode says what else must wait:
+  //   kPdlInputs (hx_decode_attention_chained, inputs_ready = 0): nothing is read from global memory before the wait;
+  //              only the launch latency, the barrier set-up and the descriptor prefetch run under the predecessor.
+  //   kPdlWrites (hx_decode_attention_chained, inputs_ready = 1): the caller asserts that nothing this grid READS is
+  //              written by the predecessor; every global WRITE (out, partials, counters) comes after the wait, so the
+  //              grid streams its first ranges under the predecessor's tail and may share its workspace and `out`.
+  //   kPdlEnd    (hx_decode_attention_overlapped behind hx_kv_ingest): reads nothing and writes nothing the ingest
+  //              touches; only the exit waits.
+  int32_t pdl_mode;
   const int32_t* plan;    // hx_decode_attention_planned
 };
 
@@ -290,6 +298,11 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     for (int s = 0; s <= kStages; ++s) mbar_init(b0 + 8 * s, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  if (p.pdl_mode == kPdlInputs) asm volatile("griddepcontrol.wait;" ::: "memory");
+  bool pdl_pending = (p.pdl_mode == kPdlWrites);         // this thread has not yet waited for the preceding grid
+  auto pdl_before_write = [&]() {
+    if (pdl_pending) { asm volatile("griddepcontrol.wait;" ::: "memory"); pdl_pending = false; }
+  };
 
   // ---- setup (row A4).  Unplanned: page-count prefix sums in shared memory (the only CTA-wide syncs).
   // Planned: the header and this worker's first 32 descriptors arrive with one round of loads; no CTA-wide sync.
@@ -308,6 +321,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     if (__shfl_sync(FULL, hv, 0) != kPlanMagic || __shfl_sync(FULL, hv, 1) != B || __shfl_sync(FULL, hv, 2) != Hkv ||
         __shfl_sync(FULL, hv, 3) != p.Hq || __shfl_sync(FULL, hv, 4) != nC) __trap();
     const int n_empty = __shfl_sync(FULL, hv, 6);
+    if (n_empty > 0) pdl_before_write();
     for (int e = w; e < n_empty; e += nC * kWarps) {                     // reading S11: empty context -> zero row
       int4* row = reinterpret_cast<int4*>(p.out + (size_t)__ldg(pv.empty + e) * p.Hq * D);
       for (int x = lane; x < p.Hq * D / 8; x += 32) row[x] = make_int4(0, 0, 0, 0);
@@ -319,6 +333,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     // reading S11: an empty context gives a zero output row (no tile ever touches it)
     for (int i = blockIdx.x * (kWarps * 32) + tid; i < B; i += gridDim.x * (kWarps * 32))
       if (slen[i] == 0) {
+        pdl_before_write();
         int4* row = reinterpret_cast<int4*>(p.out + (size_t)i * p.Hq * D);
         for (int e = 0; e < p.Hq * D / 8; ++e) row[e] = make_int4(0, 0, 0, 0);
       }
@@ -455,6 +470,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
       // the page: cache and output both equal hx_kv_append followed by hx_decode_attention
       constexpr int CH = D / 8;
       const int r = valid - 1;
+      pdl_before_write();
       if (lane < 2 * CH) {
         const int x = lane >= CH ? 1 : 0, ch = lane - x * CH;
         *reinterpret_cast<int4*>(my_stage + stage * C::kStage + x * kTile + (ch >> 3) * 2048 + r * 128 +
@@ -543,6 +559,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     const bool seg_end = last_page || (ck == k1 - 1);
     bool wrote_smem = valid < 16 || (APPEND && last_page);
     if (seg_end) {
+      pdl_before_write();
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
@@ -665,7 +682,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     ++ck;
   }
   } while (false);
-  if (p.pdl_wait_at_end) asm volatile("griddepcontrol.wait;" ::: "memory");
+  if (p.pdl_mode != kPdlNone) asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 // ---------------------------------------------------------------------------- host side
@@ -778,12 +795,11 @@ int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream
     p.kc = static_cast<__half*>(const_cast<void*>(a.k_base)) + layer_elems * a.layer;
     p.vc = static_cast<__half*>(const_cast<void*>(a.v_base)) + layer_elems * a.layer;
     p.plan = PLANNED ? static_cast<const int32_t*>(a.plan) : nullptr;
-    p.pdl_wait_at_end = (a.overlap_prev && b0 == 0) ? 1 : 0;
-    if (p.pdl_wait_at_end) {
-      // programmatic dependent launch: this grid may start while the ingest kernel enqueued just before it (which
-      // executes griddepcontrol.launch_dependents at once) is still running.  The caller asserted that it reads
-      // nothing that kernel writes; each CTA waits for the ingest's completion before it exits, so that whatever is
-      // ordered after this grid is ordered after the ingest too.
+    p.pdl_mode = (b0 == 0) ? a.overlap_prev : kPdlNone;
+    if (p.pdl_mode != kPdlNone) {
+      // programmatic dependent launch: this grid may start while the kernel enqueued just before it is still running
+      // (at once if that kernel executes griddepcontrol.launch_dependents early, as the ingest and attention kernels
+      // do; when it exits otherwise).  StreamParams::pdl_mode says what waits for that kernel's completion.
       cudaLaunchConfig_t cfg = {};
       cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kWarps * 32); cfg.dynamicSmemBytes = C::kSmem; cfg.stream = stream;
       cudaLaunchAttribute at[1];

@@ -192,7 +192,9 @@ size_t hx_decode_attention_workspace_bytes(int32_t batch, int32_t q_heads, int32
 }
 
 // mode: 0 = hx_decode_attention (and _append / _overlapped), 1 = hx_decode_plan (writes `plan`), 2 = hx_decode_attention_planned
-static int attention_common(const char* who, void* out, const void* q, const void* k_new, const void* v_new, bool append, bool overlap,
+// pdl: 0 = plain launch; 3 = hx_decode_attention_overlapped (programmatic dependent only directly behind an ingest);
+//      1 / 2 = hx_decode_attention_chained (inputs_ready = 0 / 1)
+static int attention_common(const char* who, void* out, const void* q, const void* k_new, const void* v_new, bool append, int pdl,
                             const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
                             const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
                             int32_t batch, int32_t max_seq_len, float sm_scale, void* workspace,
@@ -240,8 +242,9 @@ static int attention_common(const char* who, void* out, const void* q, const voi
   p.page_size = cache->page_size; p.num_pages = cache->num_pages; p.bt_stride = block_table_stride;
   p.max_seq_len = max_seq_len; p.sm_scale = sm_scale;
   p.k_new = append ? k_new : nullptr; p.v_new = append ? v_new : nullptr;
-  // a programmatic dependent launch only directly behind an ingest kernel this thread enqueued on this stream
-  p.overlap_prev = (overlap && g_last.kind == kLaunchIngest && g_last.stream == stream) ? 1 : 0;
+  // hx_decode_attention_overlapped: a programmatic dependent launch only directly behind an ingest kernel this thread
+  // enqueued on this stream; hx_decode_attention_chained: behind whatever precedes it
+  p.overlap_prev = pdl == 3 ? ((g_last.kind == kLaunchIngest && g_last.stream == stream) ? 3 : 0) : pdl;
   p.plan = mode != 0 ? plan : nullptr;
   if (dry_run) return HX_OK;
   rc = mode == 1 ? launch_plan(p, static_cast<cudaStream_t>(stream)) : launch_attention(p, static_cast<cudaStream_t>(stream));
@@ -253,7 +256,7 @@ int hx_decode_attention(void* out, const void* q, const hx_paged_cache* cache, i
                         const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
                         int32_t batch, int32_t max_seq_len, float sm_scale, void* workspace,
                         size_t workspace_bytes, void* stream) {
-  return attention_common("hx_decode_attention", out, q, nullptr, nullptr, false, false, cache, layer, q_heads, block_table,
+  return attention_common("hx_decode_attention", out, q, nullptr, nullptr, false, 0, cache, layer, q_heads, block_table,
                           block_table_stride, seq_lens, batch, max_seq_len, sm_scale, workspace, workspace_bytes, stream);
 }
 
@@ -262,7 +265,7 @@ int hx_decode_attention_append(void* out, const void* q, const void* k_new, cons
                                const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
                                int32_t batch, int32_t max_seq_len, float sm_scale, void* workspace,
                                size_t workspace_bytes, void* stream) {
-  return attention_common("hx_decode_attention_append", out, q, k_new, v_new, true, false, cache, layer, q_heads, block_table,
+  return attention_common("hx_decode_attention_append", out, q, k_new, v_new, true, 0, cache, layer, q_heads, block_table,
                           block_table_stride, seq_lens, batch, max_seq_len, sm_scale, workspace, workspace_bytes, stream);
 }
 
@@ -270,7 +273,7 @@ int hx_decode_attention_overlapped(void* out, const void* q, const hx_paged_cach
                                    const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
                                    int32_t batch, int32_t max_seq_len, float sm_scale, void* workspace,
                                    size_t workspace_bytes, void* stream) {
-  return attention_common("hx_decode_attention_overlapped", out, q, nullptr, nullptr, false, true, cache, layer, q_heads,
+  return attention_common("hx_decode_attention_overlapped", out, q, nullptr, nullptr, false, 3, cache, layer, q_heads,
                           block_table, block_table_stride, seq_lens, batch, max_seq_len, sm_scale, workspace,
                           workspace_bytes, stream);
 }
@@ -348,7 +351,7 @@ size_t hx_decode_plan_bytes(int32_t batch, int32_t kv_heads, int32_t max_seq_len
 
 int hx_decode_plan(void* plan, size_t plan_bytes, const hx_paged_cache* cache, int32_t q_heads, const int32_t* block_table,
                    int32_t block_table_stride, const int32_t* seq_lens, int32_t batch, int32_t max_seq_len, void* stream) {
-  return attention_common("hx_decode_plan", nullptr, nullptr, nullptr, nullptr, false, false, cache, 0, q_heads, block_table,
+  return attention_common("hx_decode_plan", nullptr, nullptr, nullptr, nullptr, false, 0, cache, 0, q_heads, block_table,
                           block_table_stride, seq_lens, batch, max_seq_len, 0.f, nullptr, 0, stream, false, 1, plan, plan_bytes);
 }
 
@@ -356,9 +359,18 @@ int hx_decode_attention_planned(void* out, const void* q, const hx_paged_cache* 
                                 const void* plan, size_t plan_bytes, int32_t batch, int32_t max_seq_len, float sm_scale,
                                 void* workspace, size_t workspace_bytes, void* stream) {
   const int32_t ps = (cache && cache->page_size > 0) ? cache->page_size : 16;
-  return attention_common("hx_decode_attention_planned", out, q, nullptr, nullptr, false, false, cache, layer, q_heads, nullptr,
+  return attention_common("hx_decode_attention_planned", out, q, nullptr, nullptr, false, 0, cache, layer, q_heads, nullptr,
                           (max_seq_len + ps - 1) / ps, nullptr, batch, max_seq_len, sm_scale, workspace, workspace_bytes, stream,
                           false, 2, const_cast<void*>(plan), plan_bytes);
+}
+
+int hx_decode_attention_chained(void* out, const void* q, const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
+                                const void* plan, size_t plan_bytes, int32_t batch, int32_t max_seq_len, float sm_scale,
+                                void* workspace, size_t workspace_bytes, int32_t inputs_ready, void* stream) {
+  const int32_t ps = (cache && cache->page_size > 0) ? cache->page_size : 16;
+  return attention_common("hx_decode_attention_chained", out, q, nullptr, nullptr, false, inputs_ready ? 2 : 1, cache, layer, q_heads,
+                          nullptr, (max_seq_len + ps - 1) / ps, nullptr, batch, max_seq_len, sm_scale, workspace, workspace_bytes,
+                          stream, false, 2, const_cast<void*>(plan), plan_bytes);
 }
 
 // ---- whole decode step (row A9): library-owned side stream per device for the overlapped handoff ----
@@ -399,7 +411,7 @@ int step_impl(const char* who, const hx_step_args* a, const hx_step_host_args* h
     if (rc) return rc;
   }
   if (do_att) {
-    rc = attention_common(who, a->out, a->q, nullptr, nullptr, false, false, a->cache, a->layer, a->q_heads, a->block_table,
+    rc = attention_common(who, a->out, a->q, nullptr, nullptr, false, 0, a->cache, a->layer, a->q_heads, a->block_table,
                           a->block_table_stride, a->seq_lens, a->batch, a->max_seq_len, a->sm_scale, a->workspace,
                           a->workspace_bytes, stream_, /*dry_run=*/true);
     if (rc) return rc;
@@ -444,7 +456,7 @@ int step_impl(const char* who, const hx_step_args* a, const hx_step_host_args* h
   if (h && do_att) STEP_CUDA(cudaMemcpyAsync(const_cast<void*>(a->q), h->q_host, qbytes, cudaMemcpyHostToDevice, main_stream));
   auto enqueue_attention = [&]() {
     if (rc == HX_OK && ce == cudaSuccess)
-      rc = attention_common(who, a->out, a->q, nullptr, nullptr, false, false, a->cache, a->layer, a->q_heads, a->block_table,
+      rc = attention_common(who, a->out, a->q, nullptr, nullptr, false, 0, a->cache, a->layer, a->q_heads, a->block_table,
                             a->block_table_stride, a->seq_lens, a->batch, a->max_seq_len, a->sm_scale, a->workspace,
                             a->workspace_bytes, stream_);
   };

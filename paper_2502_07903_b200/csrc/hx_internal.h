@@ -68,7 +68,9 @@ struct AttnParams {
   float sm_scale;
   const void* k_new;              // fused append (hx_decode_attention_append); NULL otherwise
   const void* v_new;
-  int32_t overlap_prev;           // launch as a programmatic dependent of the preceding kernel (hx_decode_attention_overlapped)
+  int32_t overlap_prev;           // 0, or launch as a programmatic dependent of the preceding kernel: 1 = wait before any read,
+                                  // 2 = wait before the first global write (hx_decode_attention_chained), 3 = wait at exit only
+                                  // (hx_decode_attention_overlapped); attention.cu PdlMode
   void* plan;                     // hx_decode_plan's output (written by launch_plan, read by a planned launch); NULL otherwise
 };
 size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, int32_t head_dim,

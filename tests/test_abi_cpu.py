@@ -22,7 +22,7 @@ def test_library_exports_every_declared_symbol():
     L = hx.lib()
     for name in declared:
         assert hasattr(L, name), name
-    assert hx.version() == 131
+    assert hx.version() == 132
     assert hx.status_string(0) == "HX_OK" and hx.status_string(5) == "HX_ERR_NO_PAGES"
     assert hx.status_string(77) == "HX_ERR_UNKNOWN"
 
@@ -329,3 +329,10 @@ def test_plan_entry_points_reject_invalid_arguments_without_launching():
             hx.decode_attention_planned(0x6000, 0x7000, FakeCache(), **dict(ak, **over))
         assert e.value.status == status, (over, str(e.value))
     hx.decode_attention_planned(0, 0, FakeCache(), **dict(ak, batch=0))  # HX_OK, nothing launched
+    for ready in (0, 1):                                                 # the chained launch validates like the planned one
+        for over, status in [(dict(plan=0), B.HX_ERR_INVALID_ARG), (dict(plan_bytes=16), B.HX_ERR_WORKSPACE),
+                             (dict(layer=2), B.HX_ERR_INVALID_ARG), (dict(workspace=0), B.HX_ERR_WORKSPACE)]:
+            with pytest.raises(hx.HxError) as e:
+                hx.decode_attention_chained(0x6000, 0x7000, FakeCache(), inputs_ready=ready, **dict(ak, **over))
+            assert e.value.status == status, (ready, over, str(e.value))
+        hx.decode_attention_chained(0, 0, FakeCache(), inputs_ready=ready, **dict(ak, batch=0))

@@ -217,3 +217,86 @@ def test_overlapped_attention_back_to_back_and_after_an_empty_ingest(env):
         torch.cuda.synchronize()
         max_abs, rel = attn_errors(out.cpu().numpy(), refs[0])
         assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (max_abs, rel)
+
+
+def _chain_setup(hx, torch, oracle, cfg_id, B, Hq, Hkv, D, L, hi):
+    lens = W.rng(cfg_id, 1).integers(1, hi, size=B).astype(np.int32)
+    lens[3] = 0                                                  # an empty context in the chain (reading S11)
+    c = W.AttnConfig(cfg_id, "chain", B, Hq, Hkv, D, (hi + 15) // 16, "x")
+    w = W.make_attention_inputs(c, lens=lens, layers=L)
+    cache = hx.PagedCache(to_dev(w["k"], torch), to_dev(w["v"], torch))
+    bt, sl = torch.from_numpy(w["block_table"]).cuda(), torch.from_numpy(lens).cuda()
+    mx = int(lens.max())
+    wsb = hx.decode_attention_workspace_bytes(B, Hq, Hkv, D, mx)
+    ws = torch.zeros(wsb, dtype=torch.uint8, device="cuda")
+    plan = torch.empty(hx.decode_plan_bytes(B, Hkv, mx), dtype=torch.uint8, device="cuda")
+    hx.decode_plan(plan, cache, q_heads=Hq, block_table=bt, block_table_stride=bt.shape[1], seq_lens=sl, batch=B, max_seq_len=mx)
+    qs = [W.draw_fp16_normal((B, Hq, D), cfg_id, 5, l) for l in range(L)]
+    kw = dict(q_heads=Hq, plan=plan, batch=B, max_seq_len=mx, workspace=ws, workspace_bytes=wsb)
+    return w, lens, cache, qs, kw
+
+
+@pytest.mark.parametrize("ready", [1, 0])
+def test_chained_layer_calls_equal_plain_planned_calls_bit_for_bit(env, ready):
+    """hx_decode_attention_chained: the layer calls of a step launched as programmatic dependents of one another,
+    sharing ONE workspace (partial slots, arrival counters).  inputs_ready = 1 lets call n+1 stream its first ranges
+    while call n's last warps still merge, so every write of n+1 must wait for n: each layer's output must equal the
+    plain planned call's bit for bit and the oracle within tolerance, over several repetitions of a 12-call chain."""
+    hx, torch, oracle = env
+    B, Hq, Hkv, D, L = 48, 32, 4, 128, 6
+    w, lens, cache, qs, kw = _chain_setup(hx, torch, oracle, 91, B, Hq, Hkv, D, L, 2500)
+    qd = [to_dev(q, torch) for q in qs]
+    base = []
+    for l in range(L):
+        o = torch.full_like(qd[l], float("nan"))
+        hx.decode_attention_planned(o, qd[l], cache, layer=l, **kw)
+        torch.cuda.synchronize()
+        base.append(o)
+        ref = oracle.decode_attention(qs[l], w["k"], w["v"], w["block_table"], lens, layer=l)
+        max_abs, rel = attn_errors(o.cpu().numpy(), ref)
+        assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (l, max_abs, rel)
+        assert (o[3] == 0).all()
+    for rep in range(5):
+        outs = [torch.full_like(qd[0], float("nan")) for _ in range(2 * L)]
+        torch.cuda.synchronize()
+        for j in range(2 * L):                               # nothing between the launches: they chain
+            hx.decode_attention_chained(outs[j], qd[j % L], cache, layer=j % L, inputs_ready=ready, **kw)
+        torch.cuda.synchronize()
+        for j in range(2 * L):
+            assert torch.equal(outs[j].view(torch.int16), base[j % L].view(torch.int16)), (ready, rep, j)
+
+
+def test_chained_calls_sharing_one_output_buffer_and_behind_a_producer_kernel(env):
+    """(a) inputs_ready = 1 with every call writing the SAME `out`: call n's late rows must not land over call n+1's, so
+    after the chain `out` holds the last call's result exactly.  (b) inputs_ready = 0 directly behind the kernel that
+    PRODUCES q (a device copy into q's buffer): the call must see the new q, whatever it overlapped."""
+    hx, torch, oracle = env
+    B, Hq, Hkv, D, L = 64, 16, 2, 128, 4
+    w, lens, cache, qs, kw = _chain_setup(hx, torch, oracle, 92, B, Hq, Hkv, D, L, 1200)
+    qd = [to_dev(q, torch) for q in qs]
+    base = []
+    for l in range(L):
+        o = torch.full_like(qd[l], float("nan"))
+        hx.decode_attention_planned(o, qd[l], cache, layer=l, **kw)
+        base.append(o)
+    torch.cuda.synchronize()
+    for rep in range(5):
+        out = torch.full_like(qd[0], float("nan"))
+        n = 9 + rep
+        for j in range(n):
+            hx.decode_attention_chained(out, qd[j % L], cache, layer=j % L, inputs_ready=1, **kw)
+        torch.cuda.synchronize()
+        assert torch.equal(out.view(torch.int16), base[(n - 1) % L].view(torch.int16)), rep
+    # (b): q arrives by a kernel enqueued directly before the call
+    big = [q.repeat(64, 1, 1) for q in qd]                   # a copy long enough to still run when the next launch is ready
+    qbuf = torch.zeros_like(big[0])
+    for rep in range(3):
+        outs = []
+        for l in range(L):
+            qbuf.copy_(big[l])                               # producer kernel (writes the q the next call reads)
+            o = torch.full_like(qd[0], float("nan"))
+            hx.decode_attention_chained(o, qbuf, cache, layer=l, inputs_ready=0, **kw)
+            outs.append(o)
+        torch.cuda.synchronize()
+        for l in range(L):
+            assert torch.equal(outs[l].view(torch.int16), base[l].view(torch.int16)), (rep, l)
