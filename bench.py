@@ -4,10 +4,11 @@
 A "step" = the whole hot path over one batch: the host page
 allocator frees last step's 16 prompts and allocates 16 new ones (2048 tokens each), their
 block-table rows are uploaded, and ONE C-ABI call, hx_decode_step(overlap_ingest=1), lands their KV
-(hx_kv_ingest: prefill TP=4 -> decode TP=1, one layer, on the library's side stream) while
-hx_decode_attention runs over the fixed 256-request heavy-tailed batch (64 q / 8 kv heads,
-head_dim 128); the new prompts' pages are disjoint from the batch's (the handoff
-is asynchronous "to enable overlapping").  Inputs are seeded synthetic data (workloads/).
+(the hx_kv_ingest copy: prefill TP=4 -> decode TP=1, one layer) inside the SAME kernel that runs
+hx_decode_attention over the fixed 256-request heavy-tailed batch (64 q / 8 kv heads, head_dim 128):
+warps that have finished their attention range move the handoff's tiles with the copy engines.  The new
+prompts' pages are disjoint from the batch's (the handoff is asynchronous "to enable
+overlapping").  Inputs are seeded synthetic data (workloads/).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl hx|reference] [--oracle-table]
 
@@ -316,7 +317,7 @@ def run_hx(args, rank, world, local_rank):
                    src_k=src_k, src_v=src_v, ing_layers=1, heads=ci.heads, src_tp=4, dst_tp=1, dst_rank=0,
                    ing_block_table=ing_bt_dev, ing_block_table_stride=ing_stride, ing_cu_seqlens=ing_cu, ing_seq_lens=ing_sl,
                    ing_batch=nI, ing_total_tokens=TI, ing_max_seq_len=2048)
-    # the headline step: ONE hx_decode_step call, the handoff overlapped on the library's side stream
+    # the headline step: ONE hx_decode_step call = one kernel (attention carrying the handoff)
     stepper = [hx.DecodeStep(overlap_ingest=1, **dict(step_kw, ing_block_table=b)) for b in ing_bt_devs]
     stepper_in_order = [hx.DecodeStep(overlap_ingest=0, **dict(step_kw, ing_block_table=b)) for b in ing_bt_devs]
     EV = ("ev_ingest_begin", "ev_ingest_end", "ev_attention_begin", "ev_attention_end")
@@ -362,9 +363,8 @@ def run_hx(args, rank, world, local_rank):
         att = [e[2].elapsed_time(e[3]) for e in ev]
         return max_over_ranks(t0.elapsed_time(t1), world, dev), float(np.mean(ing)), float(np.mean(att)), float(np.min(att))
 
-    # headline: in the overlapped step the two kernels are a programmatic pair (nothing may sit between their launches),
-    # so the library's timing events could only bracket the PAIR.  The headline K steps carry no per-step events at all;
-    # the pair is timed in a second pass of K steps.
+    # headline: in the overlapped step attention and handoff are ONE kernel, so the library's timing events bracket both.
+    # The headline K steps carry no per-step events at all; the kernel is timed in a second pass of K steps.
     total_ms, _, _, _ = timed_steps(stepper, with_events=False)
     _, _, pair_ms, pair_min_ms = timed_steps(stepper)
     step_bytes = st["kv_bytes"] + 2 * st["ing_payload"]
@@ -399,7 +399,7 @@ def run_hx(args, rank, world, local_rank):
     barrier()
     pdl_ms = max_over_ranks(p0.elapsed_time(p1), world, dev)
 
-    # ---- extra: the headline step captured once in a CUDA graph (row upload + hx_decode_step: the programmatic pair
+    # ---- extra: the headline step captured once in a CUDA graph (row upload + hx_decode_step: the fused kernel
     # becomes a graph edge) and replayed; two graphs alternate so that the host can stage step n+1's rows while step n runs
     main = torch.cuda.current_stream(dev)
     graphs = []
@@ -532,8 +532,8 @@ def run_hx(args, rank, world, local_rank):
         "data": "synthetic (seeded; BASELINE.json length mix stands in for the Azure Conversation trace)",
         "config": {"workload": "configs[4]: LLaMA-2-70B TP=1 decode (B=256, 64q/8kv, D=128, 179 ctx in [128,1024] + 77 in "
                                "[4096,8192], page 16, 1 layer) + per-step ingest of 16x2048-token prompts (prefill TP=4 -> decode TP=1)",
-                   "step": "A1 host alloc/free + row upload, then ONE hx_decode_step(overlap_ingest=1) call: attention kernel, then "
-                           "the handoff kernel as its programmatic dependent, filling the attention's tail (one stream)",
+                   "step": "A1 host alloc/free + row upload, then ONE hx_decode_step(overlap_ingest=1) call = ONE kernel: decode "
+                           "attention whose warps, once their range is done, move the handoff's (page, head) tiles (TMA load + bulk store)",
                    "tokens_in_cache": int(st["lens"].sum()), "attention_kv_bytes": st["kv_bytes"],
                    "ingest_payload_bytes": st["ing_payload"], "l2": "inputs larger than L2 (2.3 GB KV read per step vs 126 MB)",
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
@@ -548,14 +548,14 @@ def run_hx(args, rank, world, local_rank):
                 "pull_mode_overlapped_ms_per_step": e2e_pull_ov_ms / args.steps},
         "gpu_launches": int(args.steps * LAUNCHES_PER_STEP),
         "roofline": {"bound": "hbm", "kernel": "hx_decode_attention (attn_stream_kernel, in-kernel merge): CUDA events around the "
-                                               "kernel inside K timed in-order steps (in the headline step the two kernels are "
-                                               "a programmatic pair and cannot be timed apart; see step_pair)",
+                                               "kernel inside K timed in-order steps (in the headline step attention and handoff "
+                                               "are one kernel and cannot be timed apart; see step_pair)",
                      "achieved": att_gbs, "peak": peak, "unit": "GB/s", "frac": att_gbs / peak,
                      "peak_source": peak_src, "frac_of_nominal_8000": att_gbs / NOMINAL_HBM_GBS,
                      "traffic": traffic, "traffic_source": traffic_note, "algorithmic_bytes": st["kv_bytes"],
                      "ms": att_ms, "ms_min": att_min_ms},
         "step_pair": {"ms": pair_ms, "ms_min": pair_min_ms, "GBps": step_bytes / pair_ms / 1e6, "frac_of_measured": step_bytes / pair_ms / 1e6 / peak,
-                      "note": "attention kernel + handoff kernel of the headline step, first launch to last completion (CUDA events); "
+                      "note": "the ONE kernel of the headline step (attention + handoff), CUDA events around it; "
                               "bytes = attention KV read + ingest read + write"},
         "attention": {"kv_GBps": att_gbs, "tokens_per_s_one_layer": B / (att_ms * 1e-3),
                       "tokens_per_s_80_layers": B / (att_ms * 1e-3 * 80), "ms": att_ms},
@@ -583,7 +583,7 @@ def run_hx(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
-LAUNCHES_PER_STEP = 2          # ingest kernel + attention stream kernel (merge is in-kernel)
+LAUNCHES_PER_STEP = 1          # hx_decode_step(overlap_ingest=1): the attention kernel carries the handoff (merge is in-kernel too)
 
 
 def time_kernel(torch, fn, iters=20, warm=5):

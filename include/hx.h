@@ -54,7 +54,7 @@
 extern "C" {
 #endif
 
-#define HX_VERSION 132 /* 0.1.3.2: + hx_decode_attention_chained */
+#define HX_VERSION 133 /* 0.1.3.3: + hx_decode_attention_chained; hx_decode_step(overlap_ingest) is one fused kernel */
 
 typedef enum {
   HX_OK = 0,
@@ -335,14 +335,17 @@ void    hx_pool_destroy(hx_page_pool* pool);
  * what it means in those two calls.
  * overlap_ingest == 0: ingest, then attention, in order on `stream` (the attention may read the new pages).
  * overlap_ingest != 0: the caller asserts that the attention does NOT read the pages this step ingests (the new
- * prompts join the batch in a later step).  Both kernels are HBM-bound, so running them side by side would only
- * slow the attention down by what the handoff moves; instead the attention kernel is enqueued first and the
- * handoff kernel follows on the same stream as its programmatic dependent: the attention's CTAs release it at
- * once, but its CTAs ask for more shared memory than an attention CTA leaves free on an SM, so each is placed only
- * where the attention has already finished.  The handoff thus runs in the attention kernel's tail, on the SMs
- * that finished early, and each of its CTAs waits for the attention grid before it exits: work enqueued on
- * `stream` afterwards is ordered after BOTH kernels.  Uses the last 16 bytes of `workspace` (two counters that
- * every call leaves at zero).
+ * prompts join the batch in a later step).  Both parts are HBM-bound, so side by side they would only share the
+ * bandwidth; what CAN be won is the slack of the attention's uneven finish (its warps end up to tens of microseconds
+ * apart).  The step is therefore ONE kernel: the attention kernel carries the handoff, and every warp that has
+ * finished its attention range moves (page, head) tiles of the new prompts with the copy engines (one TMA tensor load
+ * of the tile's 16 token rows into the warp's shared-memory ring, one bulk store into the page), claiming units from
+ * a counter until none are left.  Work enqueued on `stream` afterwards is ordered after both parts.  Uses the last 16
+ * bytes of `workspace` (two counters that every call leaves at zero).  The fused kernel is used when batch <= 2048,
+ * at most 8 source shards hold this rank's heads and they are in this device's memory; otherwise (e.g. shards in
+ * pinned host or peer memory) the two kernels run in order, which is always allowed.
+ * block-table rows of the handoff: entries [ceil(n_i/page_size), ceil(ing_max_seq_len/page_size)) of a row may be
+ * READ by the fused kernel (they lie inside the row) but are never used.
  * Every host-side check of both calls runs first; nothing is enqueued unless all pass.  Capturable in a CUDA
  * graph. */
 typedef struct {

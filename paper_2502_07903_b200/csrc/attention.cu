@@ -37,6 +37,7 @@
 #include <cstring>
 #include <mutex>
 
+#include "handoff_tiles.cuh"
 #include "hx_internal.h"
 
 namespace hx {
@@ -60,8 +61,9 @@ struct Cfg {
   static constexpr int kKS = D / 16;                 // k-steps of QK^T
   static constexpr int kMT = D / 16;                 // m-tiles of PV
   static constexpr int kSlotFloats = NT * (kMT * 128 + 16);   // partial: acc[NT][MT][32][4], m[NT][8], l[NT][8]
-  static constexpr int kSmem = kWarps * kStages * kStage + kWarps * kQBytes + kWarps * (kStages + 1) * 8 +
+  static constexpr int kSmem = kWarps * kStages * kStage + kWarps * kQBytes + kWarps * (kStages + 1 + tiles::kBufs) * 8 +
                                (kBMax + 1) * 4 + kBMax * 4 + 16;
+  static_assert(kStages * kStage == tiles::kBufs * kTile, "a warp's ring doubles as the tile mover's four buffers");
 };
 
 // A per-step plan (hx_decode_plan), int32 words:
@@ -105,6 +107,11 @@ struct StreamParams {
   //              touches; only the exit waits.
   int32_t pdl_mode;
   const int32_t* plan;    // hx_decode_attention_planned
+  // HANDOFF (hx_decode_step, overlap_ingest): the step's KV handoff, moved by the warps that have finished their attention
+  // range (handoff_tiles.cuh); claim[0] hands out units, claim[1] counts the warps that are done (both left at zero)
+  IngestParams ing;
+  TileUnits ing_units;
+  int32_t* claim;
 };
 
 // ---------------------------------------------------------------------------- PTX helpers
@@ -268,17 +275,17 @@ plan_kernel(int32_t* plan, const int32_t* lens, const int32_t* bt, int B, int Hk
 }
 
 // ------------------------------------------------------------------------------------------
-template <int D, int NT, bool APPEND, bool PLANNED>
-__global__ void __launch_bounds__(kWarps * 32, 1)
-attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
-                   const StreamParams p) {
+template <int D, int NT, bool APPEND, bool PLANNED, bool HANDOFF>
+__device__ __forceinline__ void attn_stream_body(const CUtensorMap& tmK, const CUtensorMap& tmV, const StreamParams& p,
+                                                 const TileMaps* hmaps) {
   using C = Cfg<D, NT>;
   constexpr int kStages = C::kStages, kTile = C::kTile, kKS = C::kKS, kMT = C::kMT;
   constexpr uint32_t FULL = 0xffffffffu;
   extern __shared__ __align__(1024) uint8_t smem[];
   uint8_t* q_base = smem + kWarps * kStages * C::kStage;
   uint64_t* bars = reinterpret_cast<uint64_t*>(q_base + kWarps * C::kQBytes);
-  int* cum = reinterpret_cast<int*>(bars + kWarps * (kStages + 1));    // (unplanned only)
+  uint64_t* hbars = bars + kWarps * (kStages + 1);                      // (HANDOFF only)
+  int* cum = reinterpret_cast<int*>(hbars + kWarps * tiles::kBufs);    // (unplanned only)
   int* slen = cum + (kBMax + 1);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -296,6 +303,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
   if (lane == 0) {
     const uint32_t b0 = smem_u32(bars + warp * (kStages + 1));
     for (int s = 0; s <= kStages; ++s) mbar_init(b0 + 8 * s, 1);
+    if (HANDOFF) for (int s = 0; s < tiles::kBufs; ++s) mbar_init(smem_u32(hbars + warp * tiles::kBufs) + 8 * s, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (p.pdl_mode == kPdlInputs) asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -682,29 +690,39 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     ++ck;
   }
   } while (false);
+  if (HANDOFF) {
+    // This warp's attention range is done (its partials stored, its merges written): it now moves tiles of the step's
+    // KV handoff through its ring, claiming units from a global counter, until none are left.  The handoff writes pages
+    // that this grid's attention does not read (the caller's assertion, include/hx.h), so no ordering between the two
+    // is needed inside the kernel.
+    __syncwarp();
+    fence_proxy_async();                               // this warp's generic accesses to its ring precede the copy engines'
+    __syncwarp();
+    int32_t* claim = p.claim;
+    tiles::move_tiles<D, tiles::kBufs, tiles::kAhead>(p.ing, p.ing_units, *hmaps, smem_u32(smem + warp * kStages * C::kStage), smem_u32(hbars + warp * tiles::kBufs),
+                         [&]() -> long long { return lane == 0 ? (long long)atomicAdd(claim, 1) : 0ll; });
+    // the last warp out leaves both counters at zero for the next call (plain stores, flushed at kernel end)
+    if (lane == 0 && atomicAdd(claim + 1, 1) == (int)(gridDim.x * kWarps) - 1) { claim[0] = 0; claim[1] = 0; }
+  }
   if (p.pdl_mode != kPdlNone) asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
-// ---------------------------------------------------------------------------- host side
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-int get_encode_fn(EncodeTiledFn* out) {
-  static EncodeTiledFn fn = nullptr;
-  static std::mutex mu;
-  std::lock_guard<std::mutex> lock(mu);
-  if (!fn) {
-    void* ptr = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    HX_CUDA_OK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres));
-    if (qres != cudaDriverEntryPointSuccess || !ptr) HX_FAIL(HX_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
-    fn = reinterpret_cast<EncodeTiledFn>(ptr);
-  }
-  *out = fn;
-  return HX_OK;
+template <int D, int NT, bool APPEND, bool PLANNED>
+__global__ void __launch_bounds__(kWarps * 32, 1)
+attn_stream_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
+                   const __grid_constant__ StreamParams p) {
+  attn_stream_body<D, NT, APPEND, PLANNED, false>(tmK, tmV, p, nullptr);
 }
 
+// hx_decode_step(overlap_ingest): the attention kernel that also carries the step's KV handoff
+template <int D, int NT>
+__global__ void __launch_bounds__(kWarps * 32, 1)
+attn_handoff_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
+                    const __grid_constant__ StreamParams p, const __grid_constant__ TileMaps hmaps) {
+  attn_stream_body<D, NT, false, false, true>(tmK, tmV, p, &hmaps);
+}
+
+// ---------------------------------------------------------------------------- host side
 // Tensor map over a whole K or V cache viewed as [D/64 halves][rows][64] with rows = layers*P*Hkv*16:
 // box {64, 16, D/64} = one (page, head) tile, landing in shared memory as [half][16 tok][128 B] with
 // the 128-byte swizzle (conflict-free ldmatrix).
@@ -750,7 +768,7 @@ int get_tile_maps(const void* k, const void* v, uint64_t rows, int D, CUtensorMa
 }
 
 
-template <int D, int NT, bool APPEND, bool PLANNED>
+template <int D, int NT, bool APPEND, bool PLANNED, bool HANDOFF = false>
 int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream) {
   using C = Cfg<D, NT>;
   {
@@ -759,7 +777,8 @@ int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream
     std::lock_guard<std::mutex> lock(mu);
     if (!attr_set[di.device]) {
       if (C::kSmem > di.max_smem_optin) HX_FAIL(HX_ERR_UNSUPPORTED, "device offers %d B shared memory per CTA, kernel needs %d", di.max_smem_optin, C::kSmem);
-      HX_CUDA_OK(cudaFuncSetAttribute(attn_stream_kernel<D, NT, APPEND, PLANNED>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmem));
+      if constexpr (HANDOFF) HX_CUDA_OK(cudaFuncSetAttribute(attn_handoff_kernel<D, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmem));
+      else HX_CUDA_OK(cudaFuncSetAttribute(attn_stream_kernel<D, NT, APPEND, PLANNED>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmem));
       attr_set[di.device] = true;
     }
   }
@@ -795,8 +814,17 @@ int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream
     p.kc = static_cast<__half*>(const_cast<void*>(a.k_base)) + layer_elems * a.layer;
     p.vc = static_cast<__half*>(const_cast<void*>(a.v_base)) + layer_elems * a.layer;
     p.plan = PLANNED ? static_cast<const int32_t*>(a.plan) : nullptr;
+    if (HANDOFF) {
+      if (a.batch > kBMax) HX_FAIL(HX_ERR_UNSUPPORTED, "the fused step covers at most %d requests (batch %d)", kBMax, a.batch);
+      p.ing = *a.handoff;
+      p.ing_units = tile_units(p.ing, a.handoff_max_seq_len, (long long)grid * kWarps);
+      if (p.ing_units.units >= (1ll << 30)) HX_FAIL(HX_ERR_UNSUPPORTED, "handoff too large for the fused step");
+      p.claim = reinterpret_cast<int32_t*>(ws + attn_workspace_claim_offset(a.q_heads, a.kv_heads, a.head_dim));
+    }
     p.pdl_mode = (b0 == 0) ? a.overlap_prev : kPdlNone;
-    if (p.pdl_mode != kPdlNone) {
+    if constexpr (HANDOFF) {
+      attn_handoff_kernel<D, NT><<<grid, kWarps * 32, C::kSmem, stream>>>(tk, tv, p, *a.handoff_maps);
+    } else if (p.pdl_mode != kPdlNone) {
       // programmatic dependent launch: this grid may start while the kernel enqueued just before it is still running
       // (at once if that kernel executes griddepcontrol.launch_dependents early, as the ingest and attention kernels
       // do; when it exits otherwise).  StreamParams::pdl_mode says what waits for that kernel's completion.
@@ -817,6 +845,21 @@ int launch_stream(const AttnParams& a, const DeviceInfo& di, cudaStream_t stream
 
 }  // namespace
 
+int get_encode_fn(EncodeTiledFn* out) {
+  static EncodeTiledFn fn = nullptr;
+  static std::mutex mu;
+  std::lock_guard<std::mutex> lock(mu);
+  if (!fn) {
+    void* ptr = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    HX_CUDA_OK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres));
+    if (qres != cudaDriverEntryPointSuccess || !ptr) HX_FAIL(HX_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
+    fn = reinterpret_cast<EncodeTiledFn>(ptr);
+  }
+  *out = fn;
+  return HX_OK;
+}
+
 size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, int32_t head_dim,
                             int32_t max_seq_len, int32_t page_size) {
   (void)batch; (void)max_seq_len; (void)page_size;
@@ -829,12 +872,6 @@ size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, in
 
 size_t attn_workspace_claim_offset(int32_t q_heads, int32_t kv_heads, int32_t head_dim) {
   return attn_workspace_bytes(0, q_heads, kv_heads, head_dim, 0, 16) - 16;
-}
-
-int attn_smem_bytes(int32_t head_dim, int32_t q_heads, int32_t kv_heads) {
-  const bool nt2 = q_heads / kv_heads > 8;
-  if (head_dim == 128) return (nt2 ? Cfg<128, 2>::kSmem : Cfg<128, 1>::kSmem) + 1024;      // + the static part
-  return (nt2 ? Cfg<64, 2>::kSmem : Cfg<64, 1>::kSmem) + 1024;
 }
 
 // Upper bound of a plan's size: header + empty list + first[W][32] + one descriptor per possible tile.
@@ -864,6 +901,10 @@ int launch_attention(const AttnParams& a, cudaStream_t stream) {
   if (a.k_new) {
     if (a.head_dim == 128) return G > 8 ? launch_stream<128, 2, true, false>(a, di, stream) : launch_stream<128, 1, true, false>(a, di, stream);
     return G > 8 ? launch_stream<64, 2, true, false>(a, di, stream) : launch_stream<64, 1, true, false>(a, di, stream);
+  }
+  if (a.handoff) {
+    if (a.head_dim == 128) return G > 8 ? launch_stream<128, 2, false, false, true>(a, di, stream) : launch_stream<128, 1, false, false, true>(a, di, stream);
+    return G > 8 ? launch_stream<64, 2, false, false, true>(a, di, stream) : launch_stream<64, 1, false, false, true>(a, di, stream);
   }
   if (a.plan) {
     if (a.head_dim == 128) return G > 8 ? launch_stream<128, 2, false, true>(a, di, stream) : launch_stream<128, 1, false, true>(a, di, stream);

@@ -4,6 +4,7 @@
 #include <cstring>
 #include <mutex>
 
+#include "handoff_tiles.cuh"
 #include "hx_internal.h"
 
 namespace hx {
@@ -60,7 +61,7 @@ static int ingest_common(const void* const* src_k, const void* const* src_v, int
                          const int32_t* cu_seqlens, const int32_t* seq_lens, int32_t batch,
                          int32_t total_tokens, int32_t max_seq_len, void* stream, bool gather,
                          const char* who, int32_t src_layers, int32_t src_layer0, int32_t dst_layer0,
-                         bool dry_run = false, int32_t tail_smem = 0, int32_t* tail_claim = nullptr) {
+                         bool dry_run = false, IngestParams* params_out = nullptr) {
   clear_error();
   if (layers < 0 || batch < 0 || total_tokens < 0 || max_seq_len < 0)
     HX_FAIL(HX_ERR_INVALID_ARG, "%s: negative size (layers=%d batch=%d total_tokens=%d max_seq_len=%d)", who, layers, batch, total_tokens, max_seq_len);
@@ -98,14 +99,10 @@ static int ingest_common(const void* const* src_k, const void* const* src_v, int
   p.dst_k = dst->k; p.dst_v = dst->v;
   p.block_table = block_table; p.cu_seqlens = cu_seqlens; p.seq_lens = seq_lens;
   p.layers = layers; p.total_tokens = total_tokens; p.batch = batch;
-  p.src_layer0 = src_layer0; p.dst_layer0 = dst_layer0;
+  p.src_layer0 = src_layer0; p.dst_layer0 = dst_layer0; p.src_layers = src_layers;
   p.head_dim = head_dim; p.page_size = ps; p.num_pages = dst->num_pages; p.bt_stride = stride;
+  if (params_out) *params_out = p;                             // hx_decode_step(overlap_ingest): moved inside the attention kernel
   if (dry_run) return HX_OK;                                   // checks only (hx_decode_step validates before it enqueues)
-  if (tail_claim) {                                            // hx_decode_step: dependent of the attention kernel before it
-    rc = launch_ingest_tail(p, tail_smem, tail_claim, static_cast<cudaStream_t>(stream));
-    if (rc == HX_OK) note_launch(stream, kLaunchOther);
-    return rc;
-  }
   rc = launch_ingest(p, gather, static_cast<cudaStream_t>(stream));
   if (rc == HX_OK) note_launch(stream, gather ? kLaunchOther : kLaunchIngest);
   return rc;
@@ -199,7 +196,8 @@ static int attention_common(const char* who, void* out, const void* q, const voi
                             const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
                             int32_t batch, int32_t max_seq_len, float sm_scale, void* workspace,
                             size_t workspace_bytes, void* stream, bool dry_run = false, int mode = 0,
-                            void* plan = nullptr, size_t plan_bytes = 0) {
+                            void* plan = nullptr, size_t plan_bytes = 0, const hx::IngestParams* handoff = nullptr,
+                            int32_t handoff_max_seq_len = 0, const hx::TileMaps* handoff_maps = nullptr) {
   using namespace hx;
   clear_error();
   if (batch < 0 || max_seq_len < 0) HX_FAIL(HX_ERR_INVALID_ARG, "%s: negative size (batch=%d max_seq_len=%d)", who, batch, max_seq_len);
@@ -246,6 +244,7 @@ static int attention_common(const char* who, void* out, const void* q, const voi
   // enqueued on this stream; hx_decode_attention_chained: behind whatever precedes it
   p.overlap_prev = pdl == 3 ? ((g_last.kind == kLaunchIngest && g_last.stream == stream) ? 3 : 0) : pdl;
   p.plan = mode != 0 ? plan : nullptr;
+  p.handoff = handoff; p.handoff_max_seq_len = handoff_max_seq_len; p.handoff_maps = handoff_maps;
   if (dry_run) return HX_OK;
   rc = mode == 1 ? launch_plan(p, static_cast<cudaStream_t>(stream)) : launch_attention(p, static_cast<cudaStream_t>(stream));
   if (rc == HX_OK) note_launch(stream, kLaunchOther);
@@ -429,14 +428,24 @@ int step_impl(const char* who, const hx_step_args* a, const hx_step_host_args* h
   }
 
   // ---- enqueue.
-  // overlap_ingest, device buffers: ONE stream.  The attention kernel goes first; the handoff follows as its programmatic
-  // dependent ("tail filler", ingest.cu): its CTAs get an SM only where the attention has left one, and each waits for
-  // the attention grid before it exits, so whatever is enqueued afterwards is ordered after both kernels.
+  // overlap_ingest, device buffers: ONE kernel.  The attention kernel carries the handoff: every warp that has finished
+  // its attention range moves (page, head) tiles of the new prompts with the copy engines (handoff_tiles.cuh) until none
+  // are left, so the handoff runs in the slack the attention's uneven finish leaves, at warp granularity.
   // overlap_ingest, host buffers (hx_decode_step_host): the shards must cross PCIe first; copies + ingest go to the
   // library's side stream, forked from and joined to the caller's stream; once forked, every exit path joins.
   std::lock_guard<std::mutex> lock(g_step_mu);
   const bool overlap = a->overlap_ingest != 0 && do_ing && do_att;
-  const bool tail = overlap && !h;
+  bool fused = overlap && !h && a->batch <= 2048 && (int64_t)a->ing_layers * a->ing_batch * ((a->ing_max_seq_len + 15) / 16) * a->heads < ((int64_t)1 << 28);
+  IngestParams ip;
+  TileMaps ip_maps;
+  if (fused) {                       // the handoff's parameters and the tensor maps of its source shards (no launch yet)
+    rc = ingest_common(a->src_k, a->src_v, a->ing_layers, a->heads, a->cache->head_dim, a->src_tp, a->dst_tp, a->dst_rank,
+                       a->cache, a->ing_block_table, a->ing_block_table_stride, a->ing_cu_seqlens, a->ing_seq_lens,
+                       a->ing_batch, a->ing_total_tokens, a->ing_max_seq_len, stream_, false, who, -1, 0, 0, /*dry_run=*/true, &ip);
+    if (rc) return rc;
+    rc = tile_maps(ip, &ip_maps, &fused);   // shards the copy engines cannot take (pull mode, > 8 shards): in order instead
+    if (rc) return rc;
+  }
   const bool fork = overlap && h;
   SideStream* ss = nullptr;
   cudaStream_t ing_stream = main_stream;
@@ -460,29 +469,20 @@ int step_impl(const char* who, const hx_step_args* a, const hx_step_host_args* h
                             a->block_table_stride, a->seq_lens, a->batch, a->max_seq_len, a->sm_scale, a->workspace,
                             a->workspace_bytes, stream_);
   };
-  auto enqueue_ingest = [&](int32_t tail_smem, int32_t* tail_claim) {
+  auto enqueue_ingest = [&]() {
     if (rc == HX_OK && ce == cudaSuccess)
       rc = ingest_common(a->src_k, a->src_v, a->ing_layers, a->heads, a->cache->head_dim, a->src_tp, a->dst_tp, a->dst_rank,
                          a->cache, a->ing_block_table, a->ing_block_table_stride, a->ing_cu_seqlens, a->ing_seq_lens,
-                         a->ing_batch, a->ing_total_tokens, a->ing_max_seq_len, static_cast<void*>(ing_stream), false, who, -1, 0, 0,
-                         false, tail_smem, tail_claim);
+                         a->ing_batch, a->ing_total_tokens, a->ing_max_seq_len, static_cast<void*>(ing_stream), false, who, -1, 0, 0);
   };
-  if (tail) {
-    // nothing may sit between the two launches (an event record would take away their kernel-to-kernel adjacency): the
-    // optional timing events bracket the PAIR
+  if (fused) {
+    // one launch: the timing events (optional) bracket it
     if (a->ev_ingest_begin) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_ingest_begin), main_stream));
     if (a->ev_attention_begin) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_attention_begin), main_stream));
-    enqueue_attention();
-    DeviceInfo di;
-    if (rc == HX_OK && ce == cudaSuccess) rc = device_info(&di);
-    if (rc == HX_OK && ce == cudaSuccess) {
-      // one byte more than an attention CTA leaves free on an SM (each CTA also costs the SM 1 KiB of bookkeeping)
-      const int32_t sm_total = di.max_smem_optin + 1024;
-      const int32_t req = sm_total - (attn_smem_bytes(a->cache->head_dim, a->q_heads, a->cache->kv_heads) + 1024) - 1024 + 256;
-      int32_t* claim = reinterpret_cast<int32_t*>(static_cast<char*>(a->workspace) +
-                                                  attn_workspace_claim_offset(a->q_heads, a->cache->kv_heads, a->cache->head_dim));
-      enqueue_ingest(req, claim);
-    }
+    if (rc == HX_OK && ce == cudaSuccess)
+      rc = attention_common(who, a->out, a->q, nullptr, nullptr, false, 0, a->cache, a->layer, a->q_heads, a->block_table,
+                            a->block_table_stride, a->seq_lens, a->batch, a->max_seq_len, a->sm_scale, a->workspace,
+                            a->workspace_bytes, stream_, false, 0, nullptr, 0, &ip, a->ing_max_seq_len, &ip_maps);
     if (a->ev_attention_end) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_attention_end), main_stream));
     if (a->ev_ingest_end) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_ingest_end), main_stream));
   } else {
@@ -501,7 +501,7 @@ int step_impl(const char* who, const hx_step_args* a, const hx_step_host_args* h
                                   cudaMemcpyHostToDevice, ing_stream));
       }
       if (a->ev_ingest_begin) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_ingest_begin), ing_stream));
-      enqueue_ingest(0, nullptr);
+      enqueue_ingest();
       if (a->ev_ingest_end) STEP_CUDA(cudaEventRecord(static_cast<cudaEvent_t>(a->ev_ingest_end), ing_stream));
     }
     if (do_att) {

@@ -1,5 +1,6 @@
 // Internal helpers shared by the libhx translation units (not part of the ABI).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <cstdarg>
 #include <cstdint>
@@ -36,6 +37,8 @@ struct DeviceInfo {
 int device_info(DeviceInfo* out);
 
 // ---- launchers implemented in ingest.cu / attention.cu (arguments already validated) ----
+struct TileUnits;
+struct TileMaps;
 struct IngestParams {
   const void* src_k[16];
   const void* src_v[16];
@@ -46,13 +49,21 @@ struct IngestParams {
   const int32_t* seq_lens;
   int32_t layers, total_tokens, batch;
   int32_t src_layer0, dst_layer0;  // first source / cache layer of the call (pipeline-stage ingest)
+  int32_t src_layers;              // layers the source buffers hold
   int32_t hs, hd, head0;          // heads per source shard, per dest rank, first owned global head
   int32_t head_dim, page_size, num_pages, bt_stride;
 };
 int launch_ingest(const IngestParams& p, bool gather, cudaStream_t stream);
-// the handoff as a programmatic dependent of the attention kernel enqueued just before it (hx_decode_step); `claim` = two
-// zeroed ints of device memory that the kernel leaves at zero
-int launch_ingest_tail(const IngestParams& p, int32_t smem_request, int32_t* claim, cudaStream_t stream);
+// The tile mover (handoff_tiles.cuh): how it cuts a handoff into units for `workers` warps, and the tensor maps of the
+// source shards.  tile_maps sets *ok = false (and returns HX_OK) when the call must use the rows kernel instead: more
+// than kMaxTileShards source shards, a shard outside this device's memory (pull mode), or a shard too large for a map.
+TileUnits tile_units(const IngestParams& p, int32_t max_seq_len, long long workers);
+int tile_maps(const IngestParams& p, TileMaps* maps, bool* ok);
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+int get_encode_fn(EncodeTiledFn* out);      // cuTensorMapEncodeTiled through the runtime's driver entry point (attention.cu)
 
 struct AttnParams {
   void* out;
@@ -72,16 +83,17 @@ struct AttnParams {
                                   // 2 = wait before the first global write (hx_decode_attention_chained), 3 = wait at exit only
                                   // (hx_decode_attention_overlapped); attention.cu PdlMode
   void* plan;                     // hx_decode_plan's output (written by launch_plan, read by a planned launch); NULL otherwise
+  const IngestParams* handoff;    // hx_decode_step(overlap_ingest): the step's handoff, moved inside the attention kernel; NULL otherwise
+  int32_t handoff_max_seq_len;
+  const struct TileMaps* handoff_maps;
 };
 size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, int32_t head_dim,
                             int32_t max_seq_len, int32_t page_size);
 size_t attn_plan_bytes(int32_t batch, int32_t kv_heads, int32_t max_seq_len, int32_t page_size);
 int launch_attention(const AttnParams& p, cudaStream_t stream);
 int launch_plan(const AttnParams& p, cudaStream_t stream);
-// shared memory one CTA of the attention kernel occupies for this head layout, and where the two claim counters of the
-// overlapped step live in the attention workspace (hx_decode_step)
-int attn_smem_bytes(int32_t head_dim, int32_t q_heads, int32_t kv_heads);
-size_t attn_workspace_claim_offset(int32_t q_heads, int32_t kv_heads, int32_t head_dim);      // uses seq_lens, block_table, batch, heads, bt_stride, plan
+// where the two counters of the fused step's handoff live in the attention workspace (hx_decode_step)
+size_t attn_workspace_claim_offset(int32_t q_heads, int32_t kv_heads, int32_t head_dim);
 
 struct PrefillArgs {
   void* out;

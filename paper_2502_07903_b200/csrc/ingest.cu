@@ -10,10 +10,16 @@
 // 16-byte loads are issued before the 4 stores (64 B in flight per thread).  A half-warp
 // (D=128) covers one 256-byte row: reads and writes are both full 32-byte-sector runs, and
 // the 16 tokens of a CTA tile that share a page write one contiguous 4 KiB (page, head) run.
+//
+// The same copy as a warp-level TILE MOVER on the copy engines lives in handoff_tiles.cuh; the decode-attention kernel
+// runs it in its slack (hx_decode_step, overlap_ingest).  As a kernel of its own it was measured at 0.94-0.95 of this
+// kernel's rate on configs[3] and equal on a one-layer handoff, so hx_kv_ingest stays here; this file only builds the
+// mover's units and tensor maps (tile_units, tile_maps).
 #include <cuda_fp16.h>
 
 #include <mutex>
 
+#include "handoff_tiles.cuh"
 #include "hx_internal.h"
 
 namespace hx {
@@ -103,31 +109,6 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) ingest_rows_kernel(const _
   move_token_tile<D, GATHER>(p, blockIdx.x, blockIdx.y, layer_splits);
 }
 
-// The handoff as a TAIL FILLER (hx_decode_step, overlap_ingest): launched as a programmatic dependent of the attention
-// kernel, whose CTAs release their dependents as soon as they start.  Every CTA of this grid REQUESTS more shared
-// memory than an attention CTA leaves free (it uses none), so it is placed on an SM only when that SM's attention CTA
-// has left: the handoff runs in the attention kernel's tail, on the SMs that finished early, instead of taking
-// bandwidth from its main phase (both kernels are HBM-bound).  CTAs start at different times, so (token tile, layer)
-// units are claimed from a counter; a bit copy does not care who moves what.  Each CTA waits for the attention grid
-// before it exits: completion of this grid implies completion of both.
-template <int D>
-__global__ void __launch_bounds__(kThreads, 3) ingest_rows_tail_kernel(const __grid_constant__ IngestParams p, int tiles, int* claim) {
-  __shared__ int unit[2];
-  const int units = tiles * p.layers;
-  if (threadIdx.x == 0) unit[0] = atomicAdd(claim, 1);
-  __syncthreads();
-  for (int it = 0;; ++it) {
-    const int u = unit[it & 1];
-    if (u >= units) break;
-    if (threadIdx.x == 0) unit[(it + 1) & 1] = atomicAdd(claim, 1);      // next claim rides under this unit's copies
-    move_token_tile<D, false>(p, u % tiles, u / tiles, p.layers);         // unit = one token tile of one layer
-    __syncthreads();
-  }
-  asm volatile("griddepcontrol.wait;" ::: "memory");
-  // the last CTA out leaves the two counters at zero for the next call (plain stores, flushed at kernel end)
-  if (threadIdx.x == 0 && atomicAdd(claim + 1, 1) == (int)gridDim.x - 1) { claim[0] = 0; claim[1] = 0; }
-}
-
 // hx_kv_append: one thread per 16-byte chunk of one
 // (request, K|V, kv head) row of the step's new token; B * 2 * Hkv * D/8 threads in all.
 template <int D>
@@ -161,36 +142,63 @@ int launch_append(const AppendParams& p, cudaStream_t stream) {
   return HX_OK;
 }
 
-int launch_ingest_tail(const IngestParams& p, int32_t smem_request, int32_t* claim, cudaStream_t stream) {
-  DeviceInfo di;
-  int rc = device_info(&di);
+// Units of the tile mover (handoff_tiles.cuh) for this handoff: split the owned heads into groups until there are enough units to balance
+// `workers` warps (a unit is what one warp takes at a time).
+TileUnits tile_units(const IngestParams& p, int32_t max_seq_len, long long workers) {
+  TileUnits u;
+  u.pages_per_req = (max_seq_len + 15) / 16;
+  u.hg = p.hd;
+  const long long slots = (long long)p.layers * 2 * p.batch * u.pages_per_req;
+  while (u.hg % 2 == 0 && slots * (p.hd / u.hg) < 16 * workers) u.hg /= 2;
+  u.units = slots * (p.hd / u.hg);
+  return u;
+}
+
+// Tensor maps over the source shards, viewed as [src_layers * total_tokens][hs][D]: box {D, 1, 16} = the 16 token rows of
+// one head, landing contiguously (no swizzle) — the layout of a (page, head) tile.  Maps are cached by (pointer, shape).
+int tile_maps(const IngestParams& p, TileMaps* maps, bool* ok) {
+  struct Entry { const void* ptr; uint64_t rows; int hs, D; CUtensorMap tm; };
+  static std::mutex mu;
+  static Entry cache[64];
+  static int n = 0, next = 0;
+  *ok = false;
+  const int r_lo = p.head0 / p.hs, r_hi = (p.head0 + p.hd - 1) / p.hs;
+  const uint64_t rows = (uint64_t)p.src_layers * p.total_tokens;
+  if (r_hi - r_lo + 1 > kMaxTileShards || rows >= (1ull << 31)) return HX_OK;
+  int dev = 0;
+  HX_CUDA_OK(cudaGetDevice(&dev));
+  EncodeTiledFn enc;
+  int rc = get_encode_fn(&enc);
   if (rc) return rc;
-  const int tok = kThreads / (p.head_dim / 8);
-  const int tiles = (p.total_tokens + tok - 1) / tok;
-  if ((long long)tiles * p.layers >= (1ll << 30)) HX_FAIL(HX_ERR_UNSUPPORTED, "handoff too large for the overlapped step");
-  const int max_dyn = di.max_smem_optin - 1024;               // (the kernel has a few bytes of static shared memory)
-  if (smem_request > max_dyn) smem_request = max_dyn;
-  if (smem_request < 0) smem_request = 0;
-  {
-    static std::mutex mu;
-    static bool attr_set[64] = {false};
-    std::lock_guard<std::mutex> lock(mu);
-    if (!attr_set[di.device]) {
-      HX_CUDA_OK(cudaFuncSetAttribute(ingest_rows_tail_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn));
-      HX_CUDA_OK(cudaFuncSetAttribute(ingest_rows_tail_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn));
-      attr_set[di.device] = true;
+  std::lock_guard<std::mutex> lock(mu);
+  for (int r = r_lo; r <= r_hi; ++r)
+    for (int x = 0; x < 2; ++x) {
+      const void* ptr = x ? p.src_v[r] : p.src_k[r];
+      cudaPointerAttributes at;
+      if (cudaPointerGetAttributes(&at, ptr) != cudaSuccess) { cudaGetLastError(); return HX_OK; }
+      if (at.type != cudaMemoryTypeDevice || at.device != dev) return HX_OK;      // pinned host / peer memory: rows kernel
+      CUtensorMap* out = x ? &maps->v[r - r_lo] : &maps->k[r - r_lo];
+      bool hit = false;
+      for (int e = 0; e < n && !hit; ++e)
+        if (cache[e].ptr == ptr && cache[e].rows == rows && cache[e].hs == p.hs && cache[e].D == p.head_dim) { *out = cache[e].tm; hit = true; }
+      if (hit) continue;
+      Entry ent;
+      ent.ptr = ptr; ent.rows = rows; ent.hs = p.hs; ent.D = p.head_dim;
+      cuuint64_t dims[3] = {(cuuint64_t)p.head_dim, (cuuint64_t)p.hs, rows};
+      cuuint64_t strides[2] = {(cuuint64_t)p.head_dim * 2, (cuuint64_t)p.hs * p.head_dim * 2};
+      cuuint32_t box[3] = {(cuuint32_t)p.head_dim, 1, 16};
+      cuuint32_t es[3] = {1, 1, 1};
+      CUresult cr = enc(&ent.tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, const_cast<void*>(ptr), dims, strides, box, es,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      if (cr != CUDA_SUCCESS) HX_FAIL(HX_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d) for source shard %d (%p, %llu rows)", (int)cr, r, ptr,
+                                      (unsigned long long)rows);
+      cache[next] = ent;
+      next = (next + 1) % 64;
+      if (n < 64) ++n;
+      *out = ent.tm;
     }
-  }
-  long long grid = (long long)di.sm_count * 3;                 // what fits once every SM is free
-  if (grid > (long long)tiles * p.layers) grid = (long long)tiles * p.layers;
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = (size_t)smem_request; cfg.stream = stream;
-  cudaLaunchAttribute at[1];
-  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  at[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = at; cfg.numAttrs = 1;
-  if (p.head_dim == 128) HX_CUDA_OK(cudaLaunchKernelEx(&cfg, ingest_rows_tail_kernel<128>, p, tiles, claim));
-  else                   HX_CUDA_OK(cudaLaunchKernelEx(&cfg, ingest_rows_tail_kernel<64>, p, tiles, claim));
+  *ok = true;
   return HX_OK;
 }
 

@@ -300,3 +300,73 @@ def test_chained_calls_sharing_one_output_buffer_and_behind_a_producer_kernel(en
         torch.cuda.synchronize()
         for l in range(L):
             assert torch.equal(outs[l].view(torch.int16), base[l].view(torch.int16)), (rep, l)
+
+
+def _fused_step_case(env, heads, S, R, q_rank, D, ilens, layers, seed, alens=(33, 100, 1, 700, 16)):
+    """One hx_decode_step(overlap_ingest=1): the handoff (tile mover inside the attention kernel, handoff_tiles.cuh) lands
+    in pages [0, P) of a sentinel-filled cache while the attention reads an active batch living in pages [P, P + Pa).
+    Cache bit-exact against the oracle's ingest (sentinels intact), attention within tolerance."""
+    hx, torch, oracle = env
+    hd = heads // R
+    G = 2
+    c = W.IngestConfig(93, "fused", layers, heads, D, S, R, len(ilens), "x")
+    w = W.make_ingest_inputs(c, lens=np.asarray(ilens, dtype=np.int32), bits=True, seed_extra=seed)
+    P = w["num_pages"]
+    alens = np.asarray(alens, dtype=np.int32)
+    apages = W.pages_for(alens)
+    Pa = int(apages.sum())
+    abt = np.full((len(alens), int(apages.max())), -1, dtype=np.int32)
+    perm = P + W.rng(93, 7, seed).permutation(Pa).astype(np.int32)
+    o = 0
+    for i, n in enumerate(apages):
+        abt[i, :n] = perm[o:o + n]
+        o += n
+    k0 = np.full((layers, P + Pa, hd, 16, D), 0xDEAD, dtype=np.uint16)
+    v0 = np.full_like(k0, 0xDEAD)
+    k0[:, P:] = W.draw_fp16_normal((layers, Pa, hd, 16, D), 93, 8, seed).view(np.uint16)
+    v0[:, P:] = W.draw_fp16_normal((layers, Pa, hd, 16, D), 93, 9, seed).view(np.uint16)
+    q = W.draw_fp16_normal((len(alens), hd * G, D), 93, 10, seed)
+    layer_a = layers - 1
+    ref = oracle.decode_attention(q, k0.view(np.float16), v0.view(np.float16), abt, alens, layer=layer_a)
+    ek, ev = k0.copy(), v0.copy()
+    oracle.kv_ingest(w["src_k"], w["src_v"], ek, ev, heads=heads, src_tp=S, dst_tp=R, dst_rank=q_rank, block_table=w["block_table"],
+                     cu_seqlens=w["cu_seqlens"], seq_lens=w["seq_lens"])
+    cache = hx.PagedCache(to_dev(k0, torch), to_dev(v0, torch))
+    qd = to_dev(q, torch)
+    out = torch.full_like(qd, float("nan"))
+    mx = int(alens.max())
+    wsb = hx.decode_attention_workspace_bytes(len(alens), hd * G, hd, D, mx)
+    ws = torch.zeros(wsb, dtype=torch.uint8, device="cuda")
+    ibt = torch.from_numpy(w["block_table"]).cuda()
+    for rep in range(2):                                   # twice: the kernel must leave its counters at zero
+        hx.decode_step(out=out, q=qd, cache=cache, layer=layer_a, q_heads=hd * G, block_table=torch.from_numpy(abt).cuda(),
+                       block_table_stride=abt.shape[1], seq_lens=torch.from_numpy(alens).cuda(), batch=len(alens), max_seq_len=mx,
+                       sm_scale=0.0, workspace=ws, workspace_bytes=wsb, src_k=[to_dev(a, torch) for a in w["src_k"]],
+                       src_v=[to_dev(a, torch) for a in w["src_v"]], ing_layers=layers, heads=heads, src_tp=S, dst_tp=R,
+                       dst_rank=q_rank, ing_block_table=ibt, ing_block_table_stride=ibt.shape[1],
+                       ing_cu_seqlens=torch.from_numpy(w["cu_seqlens"]).cuda(), ing_seq_lens=torch.from_numpy(w["seq_lens"]).cuda(),
+                       ing_batch=len(ilens), ing_total_tokens=w["total_tokens"], ing_max_seq_len=int(max(ilens)), overlap_ingest=1)
+        k_after, v_after = cache.k.clone(), cache.v.clone()     # ordered after the one kernel that did both
+        torch.cuda.synchronize()
+        assert np.array_equal(dev_u16(k_after), ek), (heads, S, R, q_rank, D, rep)
+        assert np.array_equal(dev_u16(v_after), ev), (heads, S, R, q_rank, D, rep)
+        max_abs, rel = attn_errors(out.cpu().numpy(), ref)
+        assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (heads, S, R, q_rank, D, rep, max_abs, rel)
+    assert int(ws.view(torch.int32)[-4:].abs().sum()) == 0          # the two handoff counters are back at zero
+
+
+@pytest.mark.parametrize("S", [1, 2, 4, 8])
+@pytest.mark.parametrize("R", [1, 2, 4, 8])
+@pytest.mark.parametrize("D", [64, 128])
+def test_fused_step_handoff_tp_sweep_bit_exact(env, S, R, D):
+    """Rows A2 + A3 as the fused step performs them (TMA tensor load of 16 token rows -> one bulk store per (page, head)
+    tile): every (source TP, destination TP) pair, both head sizes, page-boundary prompt lengths, an empty prompt."""
+    ilens = [1, 15, 16, 17, 31, 32, 33, 255, 256, 257, 0, 5]
+    for q_rank in sorted({0, R - 1}):
+        _fused_step_case(env, 8, S, R, q_rank, D, ilens, layers=3, seed=S * 100 + R * 10 + D + q_rank)
+
+
+def test_fused_step_handoff_odd_heads_and_one_big_prompt(env):
+    for heads, S, R in [(14, 2, 7), (56, 4, 4), (6, 3, 2), (12, 4, 2)]:
+        _fused_step_case(env, heads, S, R, R - 1, 128, [40, 3, 129], layers=2, seed=heads)
+    _fused_step_case(env, 8, 4, 1, 0, 128, [4099], layers=1, seed=5, alens=(900, 2000, 64, 3100, 31, 500, 7, 2048))
