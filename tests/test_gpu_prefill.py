@@ -105,3 +105,19 @@ def test_prefill_head_dim_64(env, G, Hkv):
     lens = [17, 64, 100, 255, 129, 300]
     run_prefill(env, 80 + G, G * Hkv, Hkv, lens, lens, D=64)
     run_prefill(env, 84 + G, G * Hkv, Hkv, [300, 64, 200], [44, 1, 200], D=64, poison=True)
+
+
+@pytest.mark.parametrize("G,Hkv,D", [(1, 4, 128), (8, 2, 128), (2, 3, 64)])
+def test_prefill_many_items_per_cta(env, G, Hkv, D):
+    """The kernel is persistent: one CTA per SM walks (row-tile pair, request, kv head) items without draining between
+    them, two row tiles in lockstep, their output tiles sharing one staged buffer.  Far more items than SMs, with
+    everything that changes from one item to the next: prompts shorter than one row tile, requests with no query rows
+    (skipped items), a second row tile that exists in one item and not in the next, partial last row tiles (stored row
+    by row) between full ones (stored by TMA), chunked prefills, a context that ends inside a kv tile."""
+    g = W.rng(90 + G, 3)
+    lens = g.integers(1, 1500, size=44).astype(np.int32)
+    qlens = lens.copy()
+    qlens[::5] = np.minimum(lens[::5], g.integers(0, 200, size=len(lens[::5])))     # chunked / decode-like / empty
+    qlens[3], lens[7], qlens[7] = 0, 128, 128
+    lens[11], qlens[11] = 1, 1
+    run_prefill(env, 90 + G, G * Hkv, Hkv, lens, qlens, poison=True, D=D)
