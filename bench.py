@@ -193,14 +193,14 @@ NCU_TRAFFIC_FILE = os.path.join(ROOT, "profiles", "ncu_traffic.json")
 def kernel_source_hash() -> str:
     """sha256 over the CUDA sources of the two hot kernels: ties an ncu capture to the tree it was taken on."""
     h = hashlib.sha256()
-    for f in ("attention.cu", "ingest.cu"):
+    for f in ("attention.cu", "handoff_tiles.cuh", "ingest.cu"):
         with open(os.path.join(ROOT, "paper_2502_07903_b200", "csrc", f), "rb") as fh:
             h.update(fh.read())
     return h.hexdigest()
 
 
 def ncu_traffic():
-    """dram read+write bytes per attention launch from the committed ncu --set full capture — only if that capture
+    """dram read+write bytes per launch of the headline step's kernel from the committed ncu --set full capture — only if that capture
     was taken on THIS tree's kernels (profiles/ncu_traffic.json stores their source hash); else null, loudly."""
     try:
         with open(NCU_TRAFFIC_FILE) as f:
@@ -211,7 +211,7 @@ def ncu_traffic():
         print("bench.py: WARNING: profiles/ncu_traffic.json was captured on other kernel sources; roofline.traffic = null",
               file=sys.stderr, flush=True)
         return None, "stale: profiles/ncu_traffic.json was captured on other kernel sources"
-    return int(d["attn_dram_bytes_per_launch"]), f"ncu --set full capture {d.get('capture')} (same kernel sources, not measured in this run)"
+    return int(d["step_kernel_dram_bytes_per_launch"]), f"ncu --set full capture {d.get('capture')} (same kernel sources, not measured in this run)"
 
 
 # ----------------------------------------------------------------------------------------------
@@ -547,13 +547,18 @@ def run_hx(args, rank, world, local_rank):
                 "pull_mode_in_order_ms_per_step": e2e_pull_ms / args.steps,
                 "pull_mode_overlapped_ms_per_step": e2e_pull_ov_ms / args.steps},
         "gpu_launches": int(args.steps * LAUNCHES_PER_STEP),
-        "roofline": {"bound": "hbm", "kernel": "hx_decode_attention (attn_stream_kernel, in-kernel merge): CUDA events around the "
-                                               "kernel inside K timed in-order steps (in the headline step attention and handoff "
-                                               "are one kernel and cannot be timed apart; see step_pair)",
-                     "achieved": att_gbs, "peak": peak, "unit": "GB/s", "frac": att_gbs / peak,
-                     "peak_source": peak_src, "frac_of_nominal_8000": att_gbs / NOMINAL_HBM_GBS,
-                     "traffic": traffic, "traffic_source": traffic_note, "algorithmic_bytes": st["kv_bytes"],
-                     "ms": att_ms, "ms_min": att_min_ms},
+        "roofline": {"bound": "hbm", "kernel": "attn_handoff_kernel: THE kernel of the timed headline step (hx_decode_step, overlap_ingest=1): "
+                                               "decode attention (in-kernel merge) whose warps also move the step's KV handoff; CUDA events "
+                                               "around the kernel in a second pass of K steps (the headline K steps carry no events)",
+                     "achieved": step_bytes / pair_ms / 1e6, "peak": peak, "unit": "GB/s", "frac": step_bytes / pair_ms / 1e6 / peak,
+                     "peak_source": peak_src, "frac_of_nominal_8000": step_bytes / pair_ms / 1e6 / NOMINAL_HBM_GBS,
+                     "traffic": traffic, "traffic_source": traffic_note, "algorithmic_bytes": step_bytes,
+                     "algorithmic_bytes_note": "attention: sum n_i * 8 kv heads * 128 * 4 B read; handoff: payload read once + written once "
+                                               "(DESIGN.md 6.1, 6.2)",
+                     "ms": pair_ms, "ms_min": pair_min_ms,
+                     "attention_alone_in_order_step": {"achieved": att_gbs, "frac": att_gbs / peak, "ms": att_ms, "ms_min": att_min_ms,
+                                                       "algorithmic_bytes": st["kv_bytes"],
+                                                       "note": "attn_stream_kernel behind the ingest kernel in hx_decode_step(overlap_ingest=0)"}},
         "step_pair": {"ms": pair_ms, "ms_min": pair_min_ms, "GBps": step_bytes / pair_ms / 1e6, "frac_of_measured": step_bytes / pair_ms / 1e6 / peak,
                       "note": "the ONE kernel of the headline step (attention + handoff), CUDA events around it; "
                               "bytes = attention KV read + ingest read + write"},

@@ -99,8 +99,8 @@ def test_ncu_traffic_is_reported_only_for_the_tree_it_was_captured_on(tmp_path, 
     f = tmp_path / "ncu_traffic.json"
     monkeypatch.setattr(bench, "NCU_TRAFFIC_FILE", str(f))
     assert bench.ncu_traffic()[0] is None                                  # no file
-    f.write_text(json.dumps({"kernel_source_sha256": bench.kernel_source_hash(), "attn_dram_bytes_per_launch": 123, "capture": "x"}))
+    f.write_text(json.dumps({"kernel_source_sha256": bench.kernel_source_hash(), "step_kernel_dram_bytes_per_launch": 123, "capture": "x"}))
     assert bench.ncu_traffic()[0] == 123
-    f.write_text(json.dumps({"kernel_source_sha256": "0" * 64, "attn_dram_bytes_per_launch": 123, "capture": "x"}))
+    f.write_text(json.dumps({"kernel_source_sha256": "0" * 64, "step_kernel_dram_bytes_per_launch": 123, "capture": "x"}))
     val, note = bench.ncu_traffic()
     assert val is None and "stale" in note
