@@ -171,6 +171,7 @@ constexpr uint32_t kIdescS = (1u << 4) | ((uint32_t)(kKvTile >> 3) << 17) | ((ui
 // Tensor memory (all 512 columns): S_A | S_B | O_A | O_B, 128 columns each; P overwrites the first 64 of its S.
 constexpr int kPpThreads = 352;          // warps 0-3 softmax A, 4-7 softmax B, 8 MMA issuer, 9 TMA loader, 10 TMA storer
 constexpr int kPpIssuer = 8, kPpLoader = 9, kPpStorer = 10;
+constexpr int kPpBlock = 32;             // (request, kv head) pairs whose row tiles are in flight together
 template <int D>
 struct PpCfg {
   static constexpr int kHalves = D / 64;
@@ -232,13 +233,28 @@ prefill_pp_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   tc_fence_after();
   const uint32_t tmem = *tmem_slot;
 
-  // item k -> (qp, i, g): late (heavy) row-tile pairs first; within a pair index, requests and kv heads.  The three
-  // global loads of an item are issued one item ahead (load_raw) and only consumed when the item starts (make_item).
+  // item k -> (qp, i, g).  The (request, kv head) pairs are taken in blocks of kPpBlock; inside a block late (heavy)
+  // row-tile pairs come first, then the block's pairs.  The CTAs of a wave thus work on a few (request, kv head)
+  // pairs at a time, whose K/V stay in L2 for all their row tiles (ordering ALL pairs under each row-tile index
+  // re-read K/V from DRAM for every index: 3.2 GB instead of 0.7 GB per launch), while the heavy-first order inside a
+  // block still deals every CTA a similar sum.  The three global loads of an item are issued one item ahead (load_raw)
+  // and only consumed when the item starts (make_item).
   const long long per_qp = (long long)p.B * Hkv;
+  const long long per_block = (long long)kPpBlock * qpairs;
+  auto item_coords = [&](long long k, int* qp, int* ig) {
+    const long long blk = k / per_block;
+    const int r = (int)(k - blk * per_block);
+    const long long ig0 = blk * kPpBlock;
+    const int pb = (int)(per_qp - ig0 < kPpBlock ? per_qp - ig0 : kPpBlock);      // pairs in this block
+    *qp = qpairs - 1 - r / pb;
+    *ig = (int)ig0 + r % pb;
+  };
   auto load_raw = [&](long long k) -> PpRaw {
     PpRaw r = {0, 0, 0};
     if (k >= items) return r;
-    const int i = (int)((unsigned)(k % per_qp) / (unsigned)Hkv);
+    int qp, ig;
+    item_coords(k, &qp, &ig);
+    const int i = ig / Hkv;
     r.n = __ldg(p.lens + i); r.m = __ldg(p.qlens + i); r.cu = __ldg(p.cuq + i);
     return r;
   };
@@ -248,8 +264,8 @@ prefill_pp_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     it.act[0] = it.act[1] = it.full[0] = it.full[1] = false;
     it.row_tok0[0] = it.row_tok0[1] = 0; it.pos0[0] = it.pos0[1] = 0; it.r0[0] = it.r0[1] = 0;
     if (k >= items) return it;
-    const int qp = qpairs - 1 - (int)(k / per_qp);
-    const int rem = (int)(k % per_qp);
+    int qp, rem;
+    item_coords(k, &qp, &rem);
     it.i = rem / Hkv; it.g = rem - it.i * Hkv;
     it.n = max(r.n, 0);
     it.m = min(r.m, it.n);
