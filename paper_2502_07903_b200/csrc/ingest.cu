@@ -26,9 +26,10 @@ namespace hx {
 namespace {
 
 constexpr int kThreads = 256;
-// 4 loads in flight per thread and at most 51 registers (46 used): five or more CTAs per SM by themselves, and one
-// CTA still fits beside a decode-attention CTA (51 K of the SM's 64 K registers), so an ingest on a side stream
-// or under hx_decode_attention_overlapped keeps moving while attention runs.  cfg4: 6 511 -> 6 592 GB/s.
+// 4 loads in flight per thread and at most 51 registers (48 used): five or more CTAs per SM.  (Eight loads in flight
+// and 78 registers moved less: cfg4 6 511 -> 6 592 GB/s.)  A decode-attention CTA takes 236 registers x 256 threads and
+// 165 KiB of shared memory, so an ingest CTA does NOT fit beside one: an ingest on a side stream or under
+// hx_decode_attention_overlapped shares the GPU with the attention SM by SM, as attention CTAs leave or before they arrive.
 constexpr int kBatch = 4;     // independent 16-byte loads in flight per thread
 constexpr int kMinCtas = 5;   // __launch_bounds__ occupancy target (register cap)
 
