@@ -345,7 +345,8 @@ void    hx_pool_destroy(hx_page_pool* pool);
  * at most 8 source shards hold this rank's heads and they are in this device's memory; otherwise (e.g. shards in
  * pinned host or peer memory) the two kernels run in order, which is always allowed.
  * block-table rows of the handoff: entries [ceil(n_i/page_size), ceil(ing_max_seq_len/page_size)) of a row may be
- * READ by the fused kernel (they lie inside the row) but are never used.
+ * READ by the fused kernel (they lie inside the row) but are never used.  ing_max_seq_len must not be smaller than
+ * any ing_seq_lens[i] (device-side contract): the fused kernel enumerates a prompt's pages up to it.
  * Every host-side check of both calls runs first; nothing is enqueued unless all pass.  Capturable in a CUDA
  * graph. */
 typedef struct {
