@@ -22,7 +22,8 @@ Beside the contract keys (roofline, e2e, cpu_baseline, clocks, gpu_launches) the
 `overlapped_launch` (one stream, programmatic dependent launch), `cuda_graph` (the headline step replayed as a
 CUDA graph), `e2e.*` (hx_decode_step_host from pinned host buffers) and `other_configs`: configs[1], [2]
 (attention) and [3] (80-layer ingest) kernel-only, `prefill` (hx_prefill_attention against the tensor roofline),
-`append_cfg5` (fused append + attention) and `stream_peaks` (read-only / write-only HBM rates of the run).
+`append_cfg5` (fused append + attention), `step_src_tp1` (the headline step with the handoff from a prefill TP=1 replica) and
+`stream_peaks` (read-only / write-only HBM rates of the run).
 `--oracle-table` prints the oracle's time per config at 1 thread and at all cores instead.
 """
 from __future__ import annotations
@@ -519,6 +520,16 @@ def run_hx(args, rank, world, local_rank):
         extra["attention_cfg5_alone"] = {"ms_median": m0, "ms_min": m0min, "kv_GBps": st["kv_bytes"] / m0 / 1e6,
                                          "frac_of_measured": st["kv_bytes"] / m0 / 1e6 / peak,
                                          "timing": "one CUDA-event pair per call, nothing else on the GPU"}
+        # SURVEY 8(d) reading (ii): the same step with the new prompts arriving from a prefill replica of TP = 1
+        # (one shard holding all 8 kv heads) instead of TP = 4
+        ing1 = W.make_ingest_inputs(ci, src_tp=1)
+        sk1 = [torch.from_numpy(a.view(np.int16)).to(dev).view(torch.float16) for a in ing1["src_k"]]
+        sv1 = [torch.from_numpy(a.view(np.int16)).to(dev).view(torch.float16) for a in ing1["src_v"]]
+        stepper_s1 = [hx.DecodeStep(overlap_ingest=1, **dict(step_kw, src_k=sk1, src_v=sv1, src_tp=1, ing_block_table=b)) for b in ing_bt_devs]
+        s1_ms, _, _, _ = timed_steps(stepper_s1, with_events=False)
+        extra["step_src_tp1"] = {"ms_per_step": s1_ms / args.steps, "value": whole_job_value(step_bytes, args.steps, 1, s1_ms), "unit": UNIT,
+                                 "note": "the headline step with the handoff from a prefill TP=1 replica (S=1 -> R=1) instead of TP=4"}
+        del sk1, sv1, stepper_s1
         extra["prefill"] = prefill_extra(torch, hx, dev)
         extra["stream_peaks"] = stream_peaks(torch, dev)
         extra["append_cfg5"] = {"append_then_attention_ms": m2, "fused_append_attention_ms": m1,
