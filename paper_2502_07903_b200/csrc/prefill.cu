@@ -541,7 +541,7 @@ prefill_pp_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
           }
           // Pass 2: weights -> fp16 -> P over the first 64 columns of this row's S (the TMEM A operand of P V).  Chunk c's
           // 16 packed columns land on columns [16c, 16c + 16), all of which lie in score chunks <= c, already read.
-          float rs4[4] = {0.f, 0.f, 0.f, 0.f};
+          unsigned long long rs2[2] = {0ull, 0ull};           // two packed pairs of fp32 partial row sums
 #pragma unroll 1
           for (int c = 0; c < 4; ++c) {
             uint32_t sc[32];
@@ -552,37 +552,42 @@ prefill_pp_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
               for (int e = 0; e < 32; ++e)
                 if (t0 + c * 32 + e > my_pos) sc[e] = 0xff800000u;              // -inf -> weight 0
             }
-            // One warp per scheduler works on this tile, and the MUFU pipe takes a warp's ex2 only every 8 cycles, so the
+
             // other instructions should sit between the ex2's.  The source is written in that software-pipelined order
             // (each ex2 followed by the FMA of a later pair and the conversion / row-sum adds of an earlier one); ptxas
             // still reschedules, but from this starting point it interleaves better (-3 % cycles, measured).
+            // Packed fp32 arithmetic (fma.rn.f32x2 / add.f32x2: two scores per instruction) for the scale-and-subtract and the
+            // row sum: the warp scheduler, not a pipe, is what this loop saturates, so instructions are what to save.
             uint32_t pk[16];
-            float ta[16], tb[16], wa[16], wb[16];
-            auto fma_pair = [&](int i) {
-              asm volatile("fma.rn.f32 %0, %1, %2, %3;" : "=f"(ta[i]) : "f"(__uint_as_float(sc[2 * i])), "f"(p.scale_log2), "f"(-m_used));
-              asm volatile("fma.rn.f32 %0, %1, %2, %3;" : "=f"(tb[i]) : "f"(__uint_as_float(sc[2 * i + 1])), "f"(p.scale_log2), "f"(-m_used));
-            };
-#pragma unroll
-            for (int i = 0; i < 2; ++i) fma_pair(i);
+            unsigned long long sc2, nm2, t2[16];
+            asm("mov.b64 %0, {%1, %1};" : "=l"(sc2) : "f"(p.scale_log2));
+            asm("mov.b64 %0, {%1, %1};" : "=l"(nm2) : "f"(-m_used));
 #pragma unroll
             for (int i = 0; i < 16; ++i) {
-              asm volatile("ex2.approx.ftz.f32 %0, %1;" : "=f"(wa[i]) : "f"(ta[i]));
-              if (i + 2 < 16) asm volatile("fma.rn.f32 %0, %1, %2, %3;" : "=f"(ta[i + 2]) : "f"(__uint_as_float(sc[2 * i + 4])), "f"(p.scale_log2), "f"(-m_used));
-              if (i > 0) asm volatile("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(pk[i - 1]) : "f"(wb[i - 1]), "f"(wa[i - 1]));
-              asm volatile("ex2.approx.ftz.f32 %0, %1;" : "=f"(wb[i]) : "f"(tb[i]));
-              if (i + 2 < 16) asm volatile("fma.rn.f32 %0, %1, %2, %3;" : "=f"(tb[i + 2]) : "f"(__uint_as_float(sc[2 * i + 5])), "f"(p.scale_log2), "f"(-m_used));
-              if (i > 0) {
-                asm volatile("add.f32 %0, %0, %1;" : "+f"(rs4[(i - 1) & 1]) : "f"(wa[i - 1]));
-                asm volatile("add.f32 %0, %0, %1;" : "+f"(rs4[2 + ((i - 1) & 1)]) : "f"(wb[i - 1]));
-              }
+              unsigned long long s2;
+              asm("mov.b64 %0, {%1, %2};" : "=l"(s2) : "r"(sc[2 * i]), "r"(sc[2 * i + 1]));
+              asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(t2[i]) : "l"(s2), "l"(sc2), "l"(nm2));
             }
-            asm volatile("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(pk[15]) : "f"(wb[15]), "f"(wa[15]));
-            asm volatile("add.f32 %0, %0, %1;" : "+f"(rs4[1]) : "f"(wa[15]));
-            asm volatile("add.f32 %0, %0, %1;" : "+f"(rs4[3]) : "f"(wb[15]));
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+              float ta, tb, wa, wb;
+              asm("mov.b64 {%0, %1}, %2;" : "=f"(ta), "=f"(tb) : "l"(t2[i]));
+              asm volatile("ex2.approx.ftz.f32 %0, %1;" : "=f"(wa) : "f"(ta));
+              asm volatile("ex2.approx.ftz.f32 %0, %1;" : "=f"(wb) : "f"(tb));
+              asm volatile("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(pk[i]) : "f"(wb), "f"(wa));
+              unsigned long long w2;
+              asm("mov.b64 %0, {%1, %2};" : "=l"(w2) : "f"(wa), "f"(wb));
+              asm volatile("add.f32x2 %0, %0, %1;" : "+l"(rs2[i & 1]) : "l"(w2));
+            }
             tmem_st16(tS + c * 16, pk);
           }
           asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-          l_run += (rs4[0] + rs4[1]) + (rs4[2] + rs4[3]);
+          {
+            float r0, r1, r2, r3;
+            asm("mov.b64 {%0, %1}, %2;" : "=f"(r0), "=f"(r1) : "l"(rs2[0]));
+            asm("mov.b64 {%0, %1}, %2;" : "=f"(r2), "=f"(r3) : "l"(rs2[1]));
+            l_run += (r0 + r1) + (r2 + r3);
+          }
           if (t0 + kKvTile > it.n) {
             // V rows of slots past the context end / of pages that were not loaded must be zero (0 * Inf = NaN in P V;
             // reading S10).  Both row tiles' warps write the same zeros; each does so before ITS barrier arrival.
