@@ -552,10 +552,6 @@ prefill_pp_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
               for (int e = 0; e < 32; ++e)
                 if (t0 + c * 32 + e > my_pos) sc[e] = 0xff800000u;              // -inf -> weight 0
             }
-
-            // other instructions should sit between the ex2's.  The source is written in that software-pipelined order
-            // (each ex2 followed by the FMA of a later pair and the conversion / row-sum adds of an earlier one); ptxas
-            // still reschedules, but from this starting point it interleaves better (-3 % cycles, measured).
             // Packed fp32 arithmetic (fma.rn.f32x2 / add.f32x2: two scores per instruction) for the scale-and-subtract and the
             // row sum: the warp scheduler, not a pipe, is what this loop saturates, so instructions are what to save.
             uint32_t pk[16];
