@@ -126,12 +126,12 @@ def test_fuzz_fused_decode_step(env, seed):
     assert int(ws.view(torch.int32)[-4:].abs().sum()) == 0, tag
 
 
-@pytest.mark.parametrize("seed", range(8))
+@pytest.mark.parametrize("seed", range(6))
 def test_fuzz_prefill(env, seed):
     hx, torch, oracle = env
     g = W.rng(97, seed)
     G = int(g.choice([1, 2, 4, 8, 16])); Hkv = int(g.integers(1, 5)); D = int(g.choice([64, 128]))
-    B = int(g.choice([1, 5, 30])); hi = int(g.choice([60, 500, 1800]))
+    B = int(g.choice([1, 5, 20])); hi = int(g.choice([60, 500, 1200]))      # (the float64 oracle sets the size)
     lens = np.maximum(_draw_lens(g, B, hi), 1)
     mode = g.integers(0, 3)
     qlens = lens.copy() if mode == 0 else np.minimum(lens, g.integers(0, 300, size=B)).astype(np.int32) if mode == 1 else \
