@@ -370,3 +370,42 @@ def test_fused_step_handoff_odd_heads_and_one_big_prompt(env):
     for heads, S, R in [(14, 2, 7), (56, 4, 4), (6, 3, 2), (12, 4, 2)]:
         _fused_step_case(env, heads, S, R, R - 1, 128, [40, 3, 129], layers=2, seed=heads)
     _fused_step_case(env, 8, 4, 1, 0, 128, [4099], layers=1, seed=5, alens=(900, 2000, 64, 3100, 31, 500, 7, 2048))
+
+
+def test_layer_loop_of_chained_calls_in_a_cuda_graph(env):
+    """A decode step's layer loop — one hx_decode_plan, then one hx_decode_attention_chained per layer — captured once in
+    a CUDA graph (the programmatic launches become graph edges) and replayed with new queries: every layer of every
+    replay must equal the plain planned call bit for bit."""
+    hx, torch, oracle = env
+    B, Hq, Hkv, D, L = 32, 32, 4, 128, 4
+    w, lens, cache, qs, kw = _chain_setup(hx, torch, oracle, 94, B, Hq, Hkv, D, L, 1500)
+    qbuf = [torch.empty((B, Hq, D), dtype=torch.float16, device="cuda") for _ in range(L)]
+    outs = [torch.empty((B, Hq, D), dtype=torch.float16, device="cuda") for _ in range(L)]
+
+    def loop():
+        for l in range(L):
+            hx.decode_attention_chained(outs[l], qbuf[l], cache, layer=l, inputs_ready=1, **kw)
+
+    for l in range(L):
+        qbuf[l].copy_(to_dev(qs[l], torch))
+    loop()                                              # warm-up outside capture (function attributes, tensor maps)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        loop()
+    for rep in range(3):
+        qrep = [W.draw_fp16_normal((B, Hq, D), 94, 20 + rep, l) for l in range(L)]
+        for l in range(L):
+            qbuf[l].copy_(to_dev(qrep[l], torch))
+            outs[l].fill_(float("nan"))
+        g.replay()
+        torch.cuda.synchronize()
+        for l in range(L):
+            base = torch.full_like(outs[l], float("nan"))
+            hx.decode_attention_planned(base, qbuf[l], cache, layer=l, **kw)
+            torch.cuda.synchronize()
+            assert torch.equal(outs[l].view(torch.int16), base.view(torch.int16)), (rep, l)
+            if rep == 0:
+                ref = oracle.decode_attention(qrep[l], w["k"], w["v"], w["block_table"], lens, layer=l)
+                max_abs, rel = attn_errors(outs[l].cpu().numpy(), ref)
+                assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (l, max_abs, rel)
