@@ -191,8 +191,9 @@ int hx_kv_append(const void* k_new, const void* v_new,
  * sm_scale    : <= 0 means 1/sqrt(head_dim) rounded to fp32.
  * workspace   : device, 16-byte aligned, >= hx_decode_attention_workspace_bytes(...) bytes.
  *               It must be ZERO-FILLED once before its first use (cudaMemsetAsync) and then only
- *               be passed to hx_decode_attention: every call leaves its arrival counters at zero
- *               again.  One workspace serves one call at a time (calls on one stream are fine). */
+ *               be passed to hx_decode_attention* / hx_decode_step: every call leaves its counters at zero
+ *               again (zero it again after a launch that failed with a CUDA error: an aborted kernel
+ *               may leave them set).  One workspace serves one call at a time (calls on one stream are fine). */
 size_t hx_decode_attention_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads,
                                            int32_t head_dim, int32_t max_seq_len, int32_t page_size);
 
