@@ -848,7 +848,7 @@ def free_port() -> int:
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="hx", choices=["hx", "reference"])
     ap.add_argument("--no-extra", action="store_true", help="skip the configs[1..3] kernel-only section")
