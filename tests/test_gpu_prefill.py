@@ -121,3 +121,38 @@ def test_prefill_many_items_per_cta(env, G, Hkv, D):
     qlens[3], lens[7], qlens[7] = 0, 128, 128
     lens[11], qlens[11] = 1, 1
     run_prefill(env, 90 + G, G * Hkv, Hkv, lens, qlens, poison=True, D=D)
+
+
+def test_prefill_degenerate_calls_do_not_hang(env):
+    """No query rows at all (every item of the persistent walk is skipped), a single one-token request, and q_lens above
+    seq_lens (a contract violation that the kernel clamps): each must return, and the valid ones must be right."""
+    hx, torch, oracle = env
+    lens = np.array([100, 33, 1], dtype=np.int32)
+    c = W.AttnConfig(98, "t", 3, 8, 1, 128, 8, "x")
+    w = W.make_attention_inputs(c, lens=lens)
+    cache = hx.PagedCache(to_dev(w["k"], torch), to_dev(w["v"], torch))
+    bt = torch.from_numpy(w["block_table"]).cuda()
+    q = W.draw_fp16_normal((141, 8, 128), 98, 40)              # room for the rows of every call below
+    qd = to_dev(q, torch)
+
+    def call(qlens, max_q):
+        qlens = np.asarray(qlens, dtype=np.int32)
+        cu = np.zeros(4, dtype=np.int32)
+        np.cumsum(qlens, out=cu[1:])
+        out = torch.full_like(qd, float("nan"))
+        hx.prefill_attention(out, qd, cache, layer=0, q_heads=8, block_table=bt, block_table_stride=bt.shape[1],
+                             seq_lens=torch.from_numpy(lens).cuda(), q_lens=torch.from_numpy(qlens).cuda(),
+                             cu_q_lens=torch.from_numpy(cu).cuda(), batch=3, total_q_tokens=141, max_q_len=max_q, max_seq_len=100)
+        torch.cuda.synchronize()
+        return out.cpu().numpy(), cu
+
+    got, _ = call([0, 0, 0], 1)                                   # nothing to do: nothing written
+    assert np.isnan(got.astype(np.float32)).all()
+    got, cu = call([0, 0, 1], 1)                                  # one row, one token of context: returns v_0
+    ref = oracle.prefill_attention(q[:1], w["k"], w["v"], w["block_table"], lens, np.array([0, 0, 1], dtype=np.int32))
+    assert attn_errors(got[:1], ref)[0] <= MAX_ABS_TOL
+    got, cu = call([100, 40, 1], 100)                             # q_lens[1] = 40 > seq_lens[1] = 33: clamped to 33 rows, no hang
+    ref = oracle.prefill_attention(np.concatenate([q[:100], q[100:133], q[140:141]]), w["k"], w["v"], w["block_table"], lens,
+                                   np.array([100, 33, 1], dtype=np.int32))
+    max_abs, rel = attn_errors(got[:100], ref[:100])              # request 0 is untouched by the violation
+    assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (max_abs, rel)
