@@ -31,6 +31,12 @@
 //  * APPEND (hx_decode_attention_append): the warp that streams the
 //    last page of a (request, kv head) overlays the step's new K/V row on the tile in shared memory
 //    and stores it to the page, so the decode step needs no separate append launch.
+//  * Chained launches (hx_decode_attention_chained, row A9): the kernel can be launched as a programmatic dependent of
+//    the kernel before it and then waits for that kernel either before its first global read or only before its first
+//    global write (StreamParams::pdl_mode), so a layer loop's calls run in one another's tails.
+//  * HANDOFF (attn_handoff_kernel, hx_decode_step with overlap_ingest, rows A2 + A3 + A9): warps that have finished their
+//    attention range move (page, head) tiles of the step's KV handoff with the copy engines (handoff_tiles.cuh), so one
+//    kernel does the whole decode step and the handoff fills the slack the attention's uneven finish leaves.
 #include <cuda.h>
 #include <cuda_fp16.h>
 
