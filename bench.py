@@ -122,13 +122,21 @@ def prefill_extra(torch, hx, dev):
                      "roofline": {"bound": "tensor", "achieved": flops / med / 1e9, "peak": peak, "unit": "TFLOP/s",
                                   "frac": flops / med / 1e9 / peak, "peak_source": src}}
         if name == "llama70b_tp1_16x2048":
-            # the same kernel in a 0.5 s back-to-back loop, against the SUSTAINED cuBLAS figure (both sag with the clocks)
-            calls = 400
-            sus = time_back_to_back(torch, fn, calls=calls, reps=1, warm=1)
-            speak, ssrc = measured_tensor_peak_sustained()
-            res[name]["sustained"] = {"ms": sus, "TFLOPs": flops / sus / 1e9, "calls_back_to_back": calls, "peak": speak,
-                                      "frac": flops / sus / 1e9 / speak, "peak_source": ssrc}
+            def fn_keep(out=out, q=q, cache=cache, bt=bt, lens=lens, cu=cu, B=B, n=n, Hq=Hq):     # (bound now: the loop rebinds the names)
+                hx.prefill_attention(out, q, cache, layer=0, q_heads=Hq, block_table=bt, block_table_stride=bt.shape[1],
+                                     seq_lens=lens, q_lens=lens, cu_q_lens=cu, batch=B, total_q_tokens=B * n, max_q_len=n,
+                                     max_seq_len=n)
+            keep = (fn_keep, flops)                               # for the sustained loop below (after the burst figures)
         del k, v, cache, q, out
+    # the LLaMA-2-70B prefill again in a 0.5 s back-to-back loop, against the SUSTAINED cuBLAS figure (both sag with the clocks);
+    # last, so that the heat it leaves does not sit in the burst figures above
+    fn, flops = keep[0], keep[1]
+    calls = 400
+    sus = time_back_to_back(torch, fn, calls=calls, reps=1, warm=1)
+    speak, ssrc = measured_tensor_peak_sustained()
+    res["llama70b_tp1_16x2048"]["sustained"] = {"ms": sus, "TFLOPs": flops / sus / 1e9, "calls_back_to_back": calls, "peak": speak,
+                                                "frac": flops / sus / 1e9 / speak, "peak_source": ssrc}
+    del keep
     return res
 
 
