@@ -11,7 +11,8 @@
  *  - Payload is IEEE fp16 (B_type = 2).  fp32 accumulation inside attention.
  *  - DEVICE pointers are marked "device"; everything else is host memory.  The caller owns all
  *    device memory, including the workspace.  The library allocates no device memory and keeps no
- *    state on the device.  Its host-side state: (1) per device, one side stream and two events, created
+ *    state on the device (one exception, part of the library's image rather than an allocation: the
+ *    fixed scratch array behind hx_decode_attention_noalloc).  Its host-side state: (1) per device, one side stream and two events, created
  *    by the first hx_decode_step_host call that asks for an overlapped handoff and destroyed by
  *    hx_shutdown(); (2) caches of device properties and TMA descriptors.  hx_page_pool is
  *    the only heap object the caller owns (host).
@@ -54,7 +55,7 @@
 extern "C" {
 #endif
 
-#define HX_VERSION 133 /* 0.1.3.3: + hx_decode_attention_chained; hx_decode_step(overlap_ingest) is one fused kernel */
+#define HX_VERSION 134 /* 0.1.3.4: + hx_decode_attention_noalloc (built-in scratch, no workspace argument) */
 
 typedef enum {
   HX_OK = 0,
@@ -222,6 +223,44 @@ int hx_decode_attention_overlapped(void* out, const void* q,
                                    int32_t batch, int32_t max_seq_len, float sm_scale,
                                    void* workspace, size_t workspace_bytes,
                                    void* stream);
+
+/* ---- (b'') decode attention for callers that have no device memory to give ---------------------
+ * Same operation, same kernel and same result as hx_decode_attention (definition above), without the
+ * workspace argument: the partial results and counters live in an array that is part of libhx's device image.
+ *
+ * Who this is for.  hx_decode_attention needs ~17 MB of scratch from the caller.  Some callers have none and cannot get
+ * any: a decode replica sizes its paged KV cache to fill the GPU at start-up (PAPER.md:L136 names out-of-memory as
+ * what an overloaded replica dies of, so every spare byte becomes pages), which leaves a later cudaMalloc to fail; an attention backend plugged
+ * into someone else's serving engine is handed tensors but no allocator, and a raw cudaMalloc from inside the engine's
+ * step loop would also synchronise the whole device in the middle of a step; and code that runs while another
+ * thread's stream capture is open must not call cudaMalloc at all.  For them the scratch is paid for once, when the
+ * library's image is loaded onto a GPU, and this call allocates nothing: no cudaMalloc / cudaFree, no
+ * stream-ordered allocation, no library routine that allocates behind the caller's back.
+ *
+ * The price and the limits.
+ *  - Every GPU on which this process uses libhx holds HX_NOALLOC_SCRATCH_BYTES (20 MiB) of device memory from the
+ *    moment the image is loaded there until the process exits, whether or not this call is ever made.
+ *  - Shapes whose hx_decode_attention_workspace_bytes() exceeds HX_NOALLOC_SCRATCH_BYTES are refused with
+ *    HX_ERR_WORKSPACE and a message naming both sizes (today: group size 16 at head_dim 128, or more than ~470 local
+ *    kv heads); nothing is enqueued.  Those shapes need hx_decode_attention and a caller-owned workspace.
+ *  - ONE array per GPU serves every call from every thread and stream.  Calls are safe one after another on one
+ *    stream (or otherwise ordered so that one finishes before the next starts); two calls that can run on the GPU at
+ *    the same time - different streams, different threads - write the same scratch and corrupt each other's result.
+ *    The library does not detect this.
+ *  - The array keeps whatever the previous call left in it, and where the counters sit depends on the shape, so
+ *    each call first clears the counters it is about to use (one small cudaMemsetAsync on `stream`, ahead of the
+ *    kernel).  Nothing needs zero-filling by the caller, also not after a launch that failed.
+ *  - First call on each GPU: the library looks up the array's device address (cudaGetSymbolAddress, with that GPU
+ *    current; this may load the library's device image) and remembers it per device.  Make that first call outside
+ *    any stream capture, e.g. once at start-up on each GPU; later calls do no such look-up.
+ * Arguments and errors otherwise exactly as hx_decode_attention.  Size checks run on the host before any CUDA call. */
+#define HX_NOALLOC_SCRATCH_BYTES ((size_t)20 * 1024 * 1024)
+int hx_decode_attention_noalloc(void* out, const void* q,
+                                const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
+                                const int32_t* block_table, int32_t block_table_stride,
+                                const int32_t* seq_lens,
+                                int32_t batch, int32_t max_seq_len, float sm_scale,
+                                void* stream);
 
 /* Fused append-then-attend (F1): the same result, bit for bit, in the cache AND in `out`, as
  * hx_kv_append(k_new, v_new, ...) followed by hx_decode_attention(...), in ONE launch: the warp

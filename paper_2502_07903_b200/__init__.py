@@ -11,4 +11,5 @@ from .binding import (  # noqa: F401
     paged_cache_bytes, kv_ingest, kv_gather, decode_attention, decode_attention_workspace_bytes,
     decode_step_host, decode_plan_bytes, decode_plan, decode_attention_planned, decode_attention_chained, EXPORTS, kv_ingest_stage, stage_overlap, kv_append,
     decode_attention_append, prefill_attention, decode_attention_overlapped, decode_step, DecodeStep, shutdown,
+    decode_attention_noalloc, NOALLOC_SCRATCH_BYTES,
 )

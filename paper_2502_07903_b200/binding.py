@@ -19,7 +19,10 @@ EXPORTS = [
     "hx_decode_attention_planned", "hx_decode_attention_chained",
     "hx_kv_ingest_stage", "hx_stage_overlap", "hx_kv_append", "hx_decode_attention_append",
     "hx_prefill_attention", "hx_decode_attention_overlapped", "hx_decode_step", "hx_shutdown",
+    "hx_decode_attention_noalloc",
 ]
+
+NOALLOC_SCRATCH_BYTES = 20 * 1024 * 1024      # HX_NOALLOC_SCRATCH_BYTES (include/hx.h)
 
 
 class HxError(RuntimeError):
@@ -146,6 +149,10 @@ def lib() -> C.CDLL:
                                            C.c_int32, C.c_int32, C.c_int32, C.c_float, C.c_void_p]
         L.hx_decode_attention_overlapped.restype = C.c_int
         L.hx_decode_attention_overlapped.argtypes = L.hx_decode_attention.argtypes
+        L.hx_decode_attention_noalloc.restype = C.c_int
+        L.hx_decode_attention_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CCache), C.c_int32, C.c_int32,
+                                                  C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_int32, C.c_float,
+                                                  C.c_void_p]
         L.hx_decode_step_host.restype = C.c_int
         L.hx_decode_step_host.argtypes = [C.POINTER(_CStepArgs), C.c_void_p]
         L.hx_decode_step.restype = C.c_int
@@ -307,6 +314,19 @@ def decode_attention(out, q, cache: PagedCache, *, layer, q_heads, block_table, 
     _check(lib().hx_decode_attention(_ptr(out), _ptr(q), cache.ref, layer, q_heads, _ptr(block_table),
                                      block_table_stride, _ptr(seq_lens), batch, max_seq_len,
                                      C.c_float(sm_scale), _ptr(workspace), workspace_bytes, _stream_ptr(stream)))
+
+
+def decode_attention_noalloc(out, q, cache: PagedCache, *, layer, q_heads, block_table, block_table_stride, seq_lens,
+                             batch, max_seq_len, sm_scale=0.0, stream=None):
+    """hx_decode_attention_noalloc (include/hx.h): decode_attention for a caller that has no device memory to spare
+    for a workspace and no way to allocate one (a GPU already filled with KV pages, a plug-in without the host
+    engine's allocator, a thread that must not cudaMalloc while a capture is open).  The scratch is a fixed
+    NOALLOC_SCRATCH_BYTES array inside libhx, shared by every call on that GPU: calls must not overlap on the device,
+    shapes that need more are refused (HxError, HX_ERR_WORKSPACE), and the first call on each GPU should happen at
+    start-up, outside any stream capture.  Same result as decode_attention."""
+    _check(lib().hx_decode_attention_noalloc(_ptr(out), _ptr(q), cache.ref, layer, q_heads, _ptr(block_table),
+                                             block_table_stride, _ptr(seq_lens), batch, max_seq_len,
+                                             C.c_float(sm_scale), _stream_ptr(stream)))
 
 
 def decode_attention_overlapped(out, q, cache: PagedCache, *, layer, q_heads, block_table, block_table_stride, seq_lens,

@@ -880,6 +880,16 @@ size_t attn_workspace_claim_offset(int32_t q_heads, int32_t kv_heads, int32_t he
   return attn_workspace_bytes(0, q_heads, kv_heads, head_dim, 0, 16) - 16;
 }
 
+// The bytes of a workspace a launch expects to find at zero: the split pairs' arrival counters and, behind them, the two
+// claim counters.  They sit BEHIND the partials, so their offset moves with (group size, head_dim); the partials
+// themselves are written before they are read and need no clearing.  (hx_decode_attention_noalloc clears this span.)
+void attn_workspace_zero_span(int32_t q_heads, int32_t kv_heads, int32_t head_dim, size_t* offset, size_t* bytes) {
+  const size_t total = attn_workspace_bytes(0, q_heads, kv_heads, head_dim, 0, 16);
+  const size_t counter_bytes = ((size_t)kBMax * kv_heads * sizeof(int32_t) + 15) & ~(size_t)15;
+  *offset = total - counter_bytes - 16;
+  *bytes = counter_bytes + 16;
+}
+
 // Upper bound of a plan's size: header + empty list + first[W][32] + one descriptor per possible tile.
 size_t attn_plan_bytes(int32_t batch, int32_t kv_heads, int32_t max_seq_len, int32_t page_size) {
   const size_t tiles = (size_t)batch * kv_heads * ((max_seq_len + page_size - 1) / page_size);

@@ -277,6 +277,74 @@ int hx_decode_attention_overlapped(void* out, const void* q, const hx_paged_cach
                           workspace_bytes, stream);
 }
 
+// ---- hx_decode_attention_noalloc: the attention workspace for callers that cannot allocate one (include/hx.h) ----
+// The scratch is a file-scope device array: it is part of this translation unit's device image, so the driver places it
+// on every GPU that loads the image and releases it when the process exits; nobody calls cudaMalloc for it.
+// Its zero-initialisation at load time only helps the very first call; after that it holds the last call's partials and
+// counters, which is why every call clears the counter span of ITS shape first (the span's offset depends on the shape).
+//
+// g_noalloc_scratch is usable by name in device code only.  On the host the name is a stand-in symbol whose address is
+// NOT a device address (passing it to a kernel faults, or silently reads host memory where the GPU can reach it), so
+// host code asks the runtime for the real address once per device, with that device current, and caches it.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[HX_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+std::mutex g_noalloc_mu;
+void* g_noalloc_ptr[64] = {nullptr};   // device address of g_noalloc_scratch on device d; filled by the first call there
+
+// Device address of the built-in scratch on the CURRENT device.  The first call per device does the look-up (it may
+// load this module onto the device, so it belongs outside any stream capture); later calls only read the table.
+int noalloc_scratch(void** out) {
+  using namespace hx;
+  int dev = 0;
+  HX_CUDA_OK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) HX_FAIL(HX_ERR_CUDA, "device id %d out of range", dev);
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  if (!g_noalloc_ptr[dev]) {
+    void* ptr = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);
+    if (e != cudaSuccess || !ptr)
+      HX_FAIL(HX_ERR_CUDA, "hx_decode_attention_noalloc: cudaGetSymbolAddress(built-in scratch) on device %d: %s", dev,
+              e != cudaSuccess ? cudaGetErrorString(e) : "returned a NULL address");
+    g_noalloc_ptr[dev] = ptr;
+  }
+  *out = g_noalloc_ptr[dev];
+  return HX_OK;
+}
+}  // namespace
+
+int hx_decode_attention_noalloc(void* out, const void* q, const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
+                                const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
+                                int32_t batch, int32_t max_seq_len, float sm_scale, void* stream) {
+  using namespace hx;
+  const char* who = "hx_decode_attention_noalloc";
+  // 1. every argument check of hx_decode_attention, without touching CUDA (a placeholder stands in for the workspace:
+  //    a dry run reads neither the pointer's target nor the device)
+  void* const placeholder = reinterpret_cast<void*>(static_cast<uintptr_t>(256));
+  int rc = attention_common(who, out, q, nullptr, nullptr, false, 0, cache, layer, q_heads, block_table, block_table_stride,
+                            seq_lens, batch, max_seq_len, sm_scale, placeholder, ~(size_t)0, stream, /*dry_run=*/true);
+  if (rc) return rc;
+  if (batch == 0) return HX_OK;                                 // nothing to do, as in hx_decode_attention
+  // 2. does this shape fit the built-in array?
+  const size_t need = attn_workspace_bytes(batch, q_heads, cache->kv_heads, cache->head_dim, max_seq_len, cache->page_size);
+  if (need > HX_NOALLOC_SCRATCH_BYTES)
+    HX_FAIL(HX_ERR_WORKSPACE, "%s: q_heads=%d kv_heads=%d head_dim=%d needs %zu bytes of scratch, the built-in array holds "
+            "%zu (HX_NOALLOC_SCRATCH_BYTES); call hx_decode_attention with a workspace of your own for this shape",
+            who, q_heads, cache->kv_heads, cache->head_dim, need, (size_t)HX_NOALLOC_SCRATCH_BYTES);
+  // 3. the array's address on this device (looked up once per device)
+  void* scratch = nullptr;
+  rc = noalloc_scratch(&scratch);
+  if (rc) return rc;
+  // 4. the array still holds the previous call's contents, and for another shape the counters lie where that call kept
+  //    partial results: clear this shape's counters, on the caller's stream, directly ahead of the kernel
+  size_t zoff = 0, zbytes = 0;
+  attn_workspace_zero_span(q_heads, cache->kv_heads, cache->head_dim, &zoff, &zbytes);
+  HX_CUDA_OK(cudaMemsetAsync(static_cast<char*>(scratch) + zoff, 0, zbytes, static_cast<cudaStream_t>(stream)));
+  // 5. the unchanged hx_decode_attention path, with the built-in array as its workspace
+  return attention_common(who, out, q, nullptr, nullptr, false, 0, cache, layer, q_heads, block_table, block_table_stride,
+                          seq_lens, batch, max_seq_len, sm_scale, scratch, HX_NOALLOC_SCRATCH_BYTES, stream);
+}
+
 int hx_kv_append(const void* k_new, const void* v_new, const hx_paged_cache* cache, int32_t layer,
                  const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens, int32_t batch,
                  int32_t max_seq_len, void* stream) {

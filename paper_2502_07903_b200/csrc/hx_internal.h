@@ -94,6 +94,8 @@ int launch_attention(const AttnParams& p, cudaStream_t stream);
 int launch_plan(const AttnParams& p, cudaStream_t stream);
 // where the two counters of the fused step's handoff live in the attention workspace (hx_decode_step)
 size_t attn_workspace_claim_offset(int32_t q_heads, int32_t kv_heads, int32_t head_dim);
+// which bytes of a workspace must be zero when a launch starts (the counters behind the partials)
+void attn_workspace_zero_span(int32_t q_heads, int32_t kv_heads, int32_t head_dim, size_t* offset, size_t* bytes);
 
 struct PrefillArgs {
   void* out;

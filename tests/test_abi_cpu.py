@@ -22,7 +22,7 @@ def test_library_exports_every_declared_symbol():
     L = hx.lib()
     for name in declared:
         assert hasattr(L, name), name
-    assert hx.version() == 133
+    assert hx.version() == 134
     assert hx.status_string(0) == "HX_OK" and hx.status_string(5) == "HX_ERR_NO_PAGES"
     assert hx.status_string(77) == "HX_ERR_UNKNOWN"
 
