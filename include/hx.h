@@ -387,8 +387,9 @@ void    hx_pool_destroy(hx_page_pool* pool);
  * block-table rows of the handoff: entries [ceil(n_i/page_size), ceil(ing_max_seq_len/page_size)) of a row may be
  * READ by the fused kernel (they lie inside the row) but are never used.  ing_max_seq_len must not be smaller than
  * any ing_seq_lens[i] (device-side contract): the fused kernel enumerates a prompt's pages up to it.
- * Every host-side check of both calls runs first; nothing is enqueued unless all pass.  Capturable in a CUDA
- * graph. */
+ * Every host-side check of both calls runs first, size limits of the launches included; nothing is enqueued unless
+ * all pass.  (The one check that needs the device - that it offers the shared memory per CTA the kernels use - runs
+ * when the first kernel of a kind is launched on that device; it cannot fail on sm_100.)  Capturable in a CUDA graph. */
 typedef struct {
   /* attention over the active batch (hx_decode_attention) */
   void*       out;               /* device fp16 [batch][q_heads][head_dim] */

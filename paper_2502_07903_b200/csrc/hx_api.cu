@@ -225,6 +225,15 @@ static int attention_common(const char* who, void* out, const void* q, const voi
   }
   if ((int64_t)block_table_stride * cache->page_size < (int64_t)max_seq_len)
     HX_FAIL(HX_ERR_INVALID_ARG, "%s: block_table_stride %d < ceil(max_seq_len %d / %d)", who, block_table_stride, max_seq_len, cache->page_size);
+  // size limits of the launch itself, checked here so that a dry run (hx_decode_step validates the whole step before it
+  // enqueues anything) sees them too; launch_stream / launch_plan repeat them
+  if (mode != 1 && (uint64_t)cache->num_pages * cache->kv_heads * 16 * cache->layers >= (1ull << 31))
+    HX_FAIL(HX_ERR_UNSUPPORTED, "%s: cache too large for one tensor map (%llu rows)", who,
+            (unsigned long long)((uint64_t)cache->num_pages * cache->kv_heads * 16 * cache->layers));
+  if ((long long)kAttnBatchPerLaunch * block_table_stride * cache->kv_heads >= (1ll << 28))
+    HX_FAIL(HX_ERR_UNSUPPORTED, "%s: block_table_stride * kv_heads too large", who);
+  if (mode != 0 && batch > kAttnBatchPerLaunch)
+    HX_FAIL(HX_ERR_UNSUPPORTED, "%s: a plan covers at most %d requests (batch %d)", who, kAttnBatchPerLaunch, batch);
   const size_t need = mode == 1 ? 0 : attn_workspace_bytes(batch, q_heads, cache->kv_heads, cache->head_dim, max_seq_len, cache->page_size);
   if (need > 0 && (!workspace || workspace_bytes < need)) HX_FAIL(HX_ERR_WORKSPACE, "%s: workspace %zu bytes < required %zu (or NULL)", who, workspace_bytes, need);
   if (need > 0 && !aligned16(workspace)) HX_FAIL(HX_ERR_INVALID_ARG, "%s: workspace must be 16-byte aligned", who);
@@ -453,9 +462,18 @@ int side_stream(int* dev_out, SideStream** out) {
   if (dev < 0 || dev >= 64) HX_FAIL(HX_ERR_CUDA, "device id %d out of range", dev);
   SideStream& s = g_side[dev];
   if (!s.stream) {
-    HX_CUDA_OK(cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking));
-    HX_CUDA_OK(cudaEventCreateWithFlags(&s.fork, cudaEventDisableTiming));
-    HX_CUDA_OK(cudaEventCreateWithFlags(&s.join, cudaEventDisableTiming));
+    // all three or none: a half-made set would be skipped by every later call and fail in cudaEventRecord for good
+    SideStream made;
+    cudaError_t e = cudaStreamCreateWithFlags(&made.stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&made.fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&made.join, cudaEventDisableTiming);
+    if (e != cudaSuccess) {
+      if (made.join) cudaEventDestroy(made.join);
+      if (made.fork) cudaEventDestroy(made.fork);
+      if (made.stream) cudaStreamDestroy(made.stream);
+      HX_FAIL(HX_ERR_CUDA, "side stream / events for the overlapped handoff on device %d: %s", dev, cudaGetErrorString(e));
+    }
+    s = made;
   }
   *dev_out = dev; *out = &s;
   return HX_OK;
@@ -503,8 +521,12 @@ int step_impl(const char* who, const hx_step_args* a, const hx_step_host_args* h
   // library's side stream, forked from and joined to the caller's stream; once forked, every exit path joins.
   std::lock_guard<std::mutex> lock(g_step_mu);
   const bool overlap = a->overlap_ingest != 0 && do_ing && do_att;
-  bool fused = overlap && !h && a->batch <= 2048 && (int64_t)a->ing_layers * a->ing_batch * ((a->ing_max_seq_len + 15) / 16) * a->heads < ((int64_t)1 << 28);
-  IngestParams ip;
+  // an EMPTY handoff (every new prompt of length 0, or no layers) is a valid no-op for hx_kv_ingest; ingest_common then
+  // returns before it fills `ip`, so such a step takes the in-order path (whose ingest half launches nothing)
+  const bool handoff_empty = a->ing_total_tokens == 0 || a->ing_layers == 0;
+  bool fused = overlap && !h && !handoff_empty && a->batch <= 2048 &&
+               (int64_t)a->ing_layers * a->ing_batch * ((a->ing_max_seq_len + 15) / 16) * a->heads < ((int64_t)1 << 28);
+  IngestParams ip{};
   TileMaps ip_maps;
   if (fused) {                       // the handoff's parameters and the tensor maps of its source shards (no launch yet)
     rc = ingest_common(a->src_k, a->src_v, a->ing_layers, a->heads, a->cache->head_dim, a->src_tp, a->dst_tp, a->dst_rank,

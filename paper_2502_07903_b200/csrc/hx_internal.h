@@ -87,6 +87,7 @@ struct AttnParams {
   int32_t handoff_max_seq_len;
   const struct TileMaps* handoff_maps;
 };
+constexpr int kAttnBatchPerLaunch = 2048;   // requests one attention launch covers (attention.cu kBMax; larger batches are cut)
 size_t attn_workspace_bytes(int32_t batch, int32_t q_heads, int32_t kv_heads, int32_t head_dim,
                             int32_t max_seq_len, int32_t page_size);
 size_t attn_plan_bytes(int32_t batch, int32_t kv_heads, int32_t max_seq_len, int32_t page_size);

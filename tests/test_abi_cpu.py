@@ -277,6 +277,10 @@ def _step(**over):
     (dict(heads=5), B.HX_ERR_INVALID_ARG), (dict(dst_rank=1), B.HX_ERR_INVALID_ARG), (dict(ing_layers=3), B.HX_ERR_INVALID_ARG),
     (dict(src_k=[0, 0x20000]), B.HX_ERR_INVALID_ARG), (dict(ing_cu_seqlens=0), B.HX_ERR_INVALID_ARG),
     (dict(ing_max_seq_len=200), B.HX_ERR_INVALID_ARG), (dict(batch=-1), B.HX_ERR_INVALID_ARG), (dict(ing_batch=-1), B.HX_ERR_INVALID_ARG),
+    # size limits of the attention launch are part of the dry run too (they used to surface only at launch time,
+    # after the ingest half of an in-order step had been enqueued)
+    (dict(cache=FakeCache(layers=80, pages=1 << 20, heads=4), overlap_ingest=0), B.HX_ERR_UNSUPPORTED),   # >= 2^31 cache rows
+    (dict(block_table_stride=1 << 16, overlap_ingest=0), B.HX_ERR_UNSUPPORTED),                          # 2048 * stride * heads >= 2^28
 ])
 def test_decode_step_validates_both_halves_before_it_enqueues(over, status):
     with pytest.raises(hx.HxError) as e:

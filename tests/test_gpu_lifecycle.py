@@ -302,7 +302,7 @@ def test_chained_calls_sharing_one_output_buffer_and_behind_a_producer_kernel(en
             assert torch.equal(outs[l].view(torch.int16), base[l].view(torch.int16)), (rep, l)
 
 
-def _fused_step_case(env, heads, S, R, q_rank, D, ilens, layers, seed, alens=(33, 100, 1, 700, 16)):
+def _fused_step_case(env, heads, S, R, q_rank, D, ilens, layers, seed, alens=(33, 100, 1, 700, 16), ing_layers=None):
     """One hx_decode_step(overlap_ingest=1): the handoff (tile mover inside the attention kernel, handoff_tiles.cuh) lands
     in pages [0, P) of a sentinel-filled cache while the attention reads an active batch living in pages [P, P + Pa).
     Cache bit-exact against the oracle's ingest (sentinels intact), attention within tolerance."""
@@ -329,8 +329,11 @@ def _fused_step_case(env, heads, S, R, q_rank, D, ilens, layers, seed, alens=(33
     layer_a = layers - 1
     ref = oracle.decode_attention(q, k0.view(np.float16), v0.view(np.float16), abt, alens, layer=layer_a)
     ek, ev = k0.copy(), v0.copy()
-    oracle.kv_ingest(w["src_k"], w["src_v"], ek, ev, heads=heads, src_tp=S, dst_tp=R, dst_rank=q_rank, block_table=w["block_table"],
-                     cu_seqlens=w["cu_seqlens"], seq_lens=w["seq_lens"])
+    if ing_layers is None:
+        ing_layers = layers
+    if ing_layers > 0:                                     # ing_layers == 0: a handoff of no layers changes nothing
+        oracle.kv_ingest(w["src_k"], w["src_v"], ek, ev, heads=heads, src_tp=S, dst_tp=R, dst_rank=q_rank, block_table=w["block_table"],
+                         cu_seqlens=w["cu_seqlens"], seq_lens=w["seq_lens"])
     cache = hx.PagedCache(to_dev(k0, torch), to_dev(v0, torch))
     qd = to_dev(q, torch)
     out = torch.full_like(qd, float("nan"))
@@ -342,7 +345,7 @@ def _fused_step_case(env, heads, S, R, q_rank, D, ilens, layers, seed, alens=(33
         hx.decode_step(out=out, q=qd, cache=cache, layer=layer_a, q_heads=hd * G, block_table=torch.from_numpy(abt).cuda(),
                        block_table_stride=abt.shape[1], seq_lens=torch.from_numpy(alens).cuda(), batch=len(alens), max_seq_len=mx,
                        sm_scale=0.0, workspace=ws, workspace_bytes=wsb, src_k=[to_dev(a, torch) for a in w["src_k"]],
-                       src_v=[to_dev(a, torch) for a in w["src_v"]], ing_layers=layers, heads=heads, src_tp=S, dst_tp=R,
+                       src_v=[to_dev(a, torch) for a in w["src_v"]], ing_layers=ing_layers, heads=heads, src_tp=S, dst_tp=R,
                        dst_rank=q_rank, ing_block_table=ibt, ing_block_table_stride=ibt.shape[1],
                        ing_cu_seqlens=torch.from_numpy(w["cu_seqlens"]).cuda(), ing_seq_lens=torch.from_numpy(w["seq_lens"]).cuda(),
                        ing_batch=len(ilens), ing_total_tokens=w["total_tokens"], ing_max_seq_len=int(max(ilens)), overlap_ingest=1)
@@ -370,6 +373,14 @@ def test_fused_step_handoff_odd_heads_and_one_big_prompt(env):
     for heads, S, R in [(14, 2, 7), (56, 4, 4), (6, 3, 2), (12, 4, 2)]:
         _fused_step_case(env, heads, S, R, R - 1, 128, [40, 3, 129], layers=2, seed=heads)
     _fused_step_case(env, 8, 4, 1, 0, 128, [4099], layers=1, seed=5, alens=(900, 2000, 64, 3100, 31, 500, 7, 2048))
+
+
+def test_fused_step_with_an_empty_handoff(env):
+    """hx_decode_step(overlap_ingest=1) whose handoff moves nothing - every new prompt empty, or zero layers - is valid
+    (hx_kv_ingest accepts both as no-ops): the cache keeps every bit, the attention result is unaffected."""
+    _fused_step_case(env, 8, 2, 2, 1, 128, [0, 0, 0], layers=2, seed=11)
+    _fused_step_case(env, 8, 4, 1, 0, 64, [0], layers=1, seed=12)
+    _fused_step_case(env, 8, 2, 4, 3, 128, [40, 3, 129], layers=2, seed=13, ing_layers=0)
 
 
 def test_layer_loop_of_chained_calls_in_a_cuda_graph(env):
