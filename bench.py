@@ -724,9 +724,15 @@ def other_configs(torch, hx, dev, peak, only=None):
                      "chained_back_to_back": {"ms": b2bc1, "kv_GBps": kvb / b2bc1 / 1e6, "frac_of_measured": kvb / b2bc1 / 1e6 / peak,
                                               "frac_of_nominal_8000": kvb / b2bc1 / 1e6 / NOMINAL_HBM_GBS,
                                               "inputs_ready_0_ms": b2bc0,
+                                              "layer_loop": {"ms": b2bc0, "kv_GBps": kvb / b2bc0 / 1e6, "frac_of_measured": kvb / b2bc0 / 1e6 / peak,
+                                                             "frac_of_nominal_8000": kvb / b2bc0 / 1e6 / NOMINAL_HBM_GBS,
+                                                             "note": "inputs_ready=0: the only mode that is legal behind a kernel that writes q / this "
+                                                                     "layer's K/V, i.e. in a real model's layer loop; THIS is the layer-loop figure"},
                                               "note": "hx_decode_attention_chained: each call a programmatic dependent of the one "
-                                                      "before it (inputs_ready=1: streams under its predecessor's tail, writes wait; "
-                                                      "inputs_ready=0: only launch + set-up overlap)"},
+                                                      "before it.  ms / kv_GBps / frac_* at this level are inputs_ready=1 (streams under its "
+                                                      "predecessor's tail, writes wait; the same q is reused and nothing runs between the calls): an "
+                                                      "UPPER BOUND that needs PDL-aware producer kernels.  layer_loop = inputs_ready=0 (only launch + "
+                                                      "set-up overlap)"},
                      "plan_ms": plan_ms, "tokens_per_s_one_layer": c.batch / (medp * 1e-3),
                      "timing": "per_call_events: one CUDA-event pair per call (SURVEY 8(d) protocol), median of 40; back_to_back: one event "
                                "pair around 40 calls; planned_*: hx_decode_plan once (plan_ms), then hx_decode_attention_planned per call, "

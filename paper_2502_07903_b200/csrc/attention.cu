@@ -18,7 +18,7 @@
 //  * Each warp runs its own 2-stage ring: lane 0 issues one TMA tensor-tile load per K tile and
 //    per V tile (cp.async.bulk.tensor, 128-byte swizzle, mbarrier complete_tx).  No CTA-wide
 //    barrier after setup.  Two stages x 8 warps = 128 KiB in flight per SM: enough to saturate HBM
-//    (7.4-8 TB/s of reads while all SMs stream), and the SMs share it far more evenly than with
+//    (6.9-7.4 TB/s of reads while all SMs stream), and the SMs share it far more evenly than with
 //    three.
 //  * Scores (row A5) and PV (row A7) run on mma.sync.m16n8k16 with the page as M (16 tokens) and
 //    the GQA group as N (8 heads): S^T = K Q^T and O^T += V^T P^T, so one K/V tile serves all G
@@ -50,7 +50,7 @@ namespace hx {
 namespace {
 
 constexpr int kWarps = 8;          // warps (= independent workers) per CTA
-constexpr int kBMax = 2048;        // requests per launch (prefix sums live in shared memory)
+constexpr int kBMax = kAttnBatchPerLaunch;   // 2048 requests per launch (prefix sums live in shared memory)
 constexpr int kMaxWorkers = 2048;  // workspace is sized for this many workers (>= SMs * kWarps)
 constexpr int kMaxSm = 256;        // CTAs (= SMs) per launch
 constexpr float kLog2e = 1.4426950408889634f;
