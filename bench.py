@@ -407,7 +407,8 @@ def run_hx(args, rank, world, local_rank):
                      dst=cache, block_table=ing_bt_devs[i], block_table_stride=ing_stride, cu_seqlens=ing_cu,
                      seq_lens=ing_sl, batch=nI, total_tokens=TI, max_seq_len=2048)
         hx.decode_attention_overlapped(out, q, cache, layer=0, q_heads=Hq, block_table=bt, block_table_stride=bt.shape[1],
-                                       seq_lens=sl, batch=B, max_seq_len=max_len, workspace=ws, workspace_bytes=ws_bytes)
+                                       seq_lens=sl, batch=B, max_seq_len=max_len, workspace=ws, workspace_bytes=ws_bytes,
+                                       behind_ingest=1)
         ev = buf_free[i] or torch.cuda.Event()
         ev.record()
         buf_free[i] = ev

@@ -16,6 +16,8 @@
  *    by the first hx_decode_step_host call that asks for an overlapped handoff and destroyed by
  *    hx_shutdown(); (2) caches of device properties and TMA descriptors.  hx_page_pool is
  *    the only heap object the caller owns (host).
+ *  - No call's behaviour depends on which library calls came before it: what a launch may overlap is always an
+ *    explicit argument (inputs_ready, behind_ingest, overlap_ingest).
  *  - Thread safety: every entry point may be called from several host threads (on different streams);
  *    hx_decode_step* serialise on one library mutex while they enqueue.  An hx_page_pool and an attention
  *    workspace each serve one caller at a time.
@@ -55,7 +57,8 @@
 extern "C" {
 #endif
 
-#define HX_VERSION 134 /* 0.1.3.4: + hx_decode_attention_noalloc (built-in scratch, no workspace argument) */
+#define HX_VERSION 135 /* 0.1.3.5: hx_decode_attention_overlapped takes an explicit behind_ingest (no inferred state);
+                          0.1.3.4: + hx_decode_attention_noalloc (built-in scratch, no workspace argument) */
 
 typedef enum {
   HX_OK = 0,
@@ -208,21 +211,27 @@ int hx_decode_attention(void* out, const void* q,
 
 /* hx_decode_attention that may OVERLAP the hx_kv_ingest enqueued just before it on `stream` (SURVEY.md §8(a) row
  * A9; "asynchronous ... to enable overlapping between computation and communication").  Same
- * arguments and result as hx_decode_attention.  When the LAST library call of this host thread was a launching
- * hx_kv_ingest / hx_kv_ingest_stage on the same `stream`, and the caller enqueued nothing on `stream` in between
- * (precondition), the grid is launched as a programmatic dependent of the ingest kernel (which signals its
- * dependents at once) and starts while the handoff is still landing; every CTA executes griddepcontrol.wait before
- * it exits, so the grid completes only after the ingest has completed and its writes are visible: work enqueued
- * after this call is ordered after BOTH kernels.  In every other case (ingest of an empty batch, another call in
- * between, another thread or stream) this is exactly hx_decode_attention.  The CALLER asserts that this call
- * reads nothing the ingest writes: the step's new prompts live in pages disjoint from the active batch's. */
+ * arguments and result as hx_decode_attention, plus one explicit statement by the caller (the library keeps no
+ * record of earlier calls and infers nothing):
+ *   behind_ingest == 0: exactly hx_decode_attention.
+ *   behind_ingest != 0: the CALLER asserts that (1) the kernel directly before this call on `stream` is the one an
+ *                       hx_kv_ingest / hx_kv_ingest_stage call LAUNCHED (a call that returned without launching -
+ *                       empty batch, no tokens, no layers - does not count), with nothing enqueued on `stream` in
+ *                       between, and (2) this call reads nothing that ingest writes: the step's new prompts live in
+ *                       pages disjoint from the active batch's.  The grid is then launched as a programmatic dependent
+ *                       of the ingest kernel (which signals its dependents at once) and starts while the handoff is
+ *                       still landing; every CTA executes griddepcontrol.wait before it exits, so the grid completes
+ *                       only after the ingest has completed and its writes are visible: work enqueued after this
+ *                       call is ordered after BOTH kernels.  If (1) is false because the predecessor is another kernel
+ *                       of this library sharing `workspace` or `out`, the two race (undefined result); behind a kernel
+ *                       of another library the call degrades to a plain launch. */
 int hx_decode_attention_overlapped(void* out, const void* q,
                                    const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
                                    const int32_t* block_table, int32_t block_table_stride,
                                    const int32_t* seq_lens,
                                    int32_t batch, int32_t max_seq_len, float sm_scale,
                                    void* workspace, size_t workspace_bytes,
-                                   void* stream);
+                                   int32_t behind_ingest, void* stream);
 
 /* ---- (b'') decode attention for callers that have no device memory to give ---------------------
  * Same operation, same kernel and same result as hx_decode_attention (definition above), without the
@@ -381,9 +390,11 @@ void    hx_pool_destroy(hx_page_pool* pool);
  * finished its attention range moves (page, head) tiles of the new prompts with the copy engines (one TMA tensor load
  * of the tile's 16 token rows into the warp's shared-memory ring, one bulk store into the page), claiming units from
  * a counter until none are left.  Work enqueued on `stream` afterwards is ordered after both parts.  Uses the last 16
- * bytes of `workspace` (two counters that every call leaves at zero).  The fused kernel is used when batch <= 2048,
- * at most 8 source shards hold this rank's heads and they are in this device's memory; otherwise (e.g. shards in
- * pinned host or peer memory) the two kernels run in order, which is always allowed.
+ * bytes of `workspace` (two counters that every call leaves at zero).  The fused kernel is used when batch <= 2048, the
+ * handoff is not empty and at most 8 source shards hold this rank's heads; otherwise the two kernels run in order, which is
+ * always allowed (hx_decode_step_is_fused tells which).  The shards may be in this device's memory, in pinned host memory
+ * or in a peer GPU's memory with peer access enabled: in the last two cases the fused step is a PULL-mode handoff (F2;
+ * PAPER.md:L110), the copy engines fetch each tile over the link straight into its page.
  * block-table rows of the handoff: entries [ceil(n_i/page_size), ceil(ing_max_seq_len/page_size)) of a row may be
  * READ by the fused kernel (they lie inside the row) but are never used.  ing_max_seq_len must not be smaller than
  * any ing_seq_lens[i] (device-side contract): the fused kernel enumerates a prompt's pages up to it.
@@ -414,6 +425,11 @@ typedef struct {
   void* ev_ingest_begin; void* ev_ingest_end; void* ev_attention_begin; void* ev_attention_end;
 } hx_step_args;
 int hx_decode_step(const hx_step_args* args, void* stream);
+
+/* Would hx_decode_step(args) run as the ONE fused kernel?  Runs the same checks and the same decision as the call itself
+ * and enqueues nothing: *fused = 1 when overlap_ingest != 0, both halves have work and the copy engines can take the
+ * handoff (see above), else 0 (the step then runs its two kernels in order).  Errors as hx_decode_step. */
+int hx_decode_step_is_fused(const hx_step_args* args, int32_t* fused);
 
 /* Destroys the library-owned side streams and events of every device (after synchronising them; only
  * hx_decode_step_host with overlap_ingest creates them).  Optional: call when no such call is in flight; a later

@@ -19,7 +19,7 @@ EXPORTS = [
     "hx_decode_attention_planned", "hx_decode_attention_chained",
     "hx_kv_ingest_stage", "hx_stage_overlap", "hx_kv_append", "hx_decode_attention_append",
     "hx_prefill_attention", "hx_decode_attention_overlapped", "hx_decode_step", "hx_shutdown",
-    "hx_decode_attention_noalloc",
+    "hx_decode_attention_noalloc", "hx_decode_step_is_fused",
 ]
 
 NOALLOC_SCRATCH_BYTES = 20 * 1024 * 1024      # HX_NOALLOC_SCRATCH_BYTES (include/hx.h)
@@ -148,7 +148,7 @@ def lib() -> C.CDLL:
                                            C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
                                            C.c_int32, C.c_int32, C.c_int32, C.c_float, C.c_void_p]
         L.hx_decode_attention_overlapped.restype = C.c_int
-        L.hx_decode_attention_overlapped.argtypes = L.hx_decode_attention.argtypes
+        L.hx_decode_attention_overlapped.argtypes = L.hx_decode_attention.argtypes[:-1] + [C.c_int32, C.c_void_p]
         L.hx_decode_attention_noalloc.restype = C.c_int
         L.hx_decode_attention_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CCache), C.c_int32, C.c_int32,
                                                   C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_int32, C.c_float,
@@ -157,6 +157,8 @@ def lib() -> C.CDLL:
         L.hx_decode_step_host.argtypes = [C.POINTER(_CStepArgs), C.c_void_p]
         L.hx_decode_step.restype = C.c_int
         L.hx_decode_step.argtypes = [C.POINTER(_CStepDevArgs), C.c_void_p]
+        L.hx_decode_step_is_fused.restype = C.c_int
+        L.hx_decode_step_is_fused.argtypes = [C.POINTER(_CStepDevArgs), C.POINTER(C.c_int32)]
         L.hx_shutdown.restype = C.c_int
         _lib = L
     return _lib
@@ -330,14 +332,17 @@ def decode_attention_noalloc(out, q, cache: PagedCache, *, layer, q_heads, block
 
 
 def decode_attention_overlapped(out, q, cache: PagedCache, *, layer, q_heads, block_table, block_table_stride, seq_lens,
-                                batch, max_seq_len, sm_scale=0.0, workspace=None, workspace_bytes=None, stream=None):
-    """hx_decode_attention_overlapped: may overlap the kernel enqueued just before it (see include/hx.h)."""
+                                batch, max_seq_len, behind_ingest, sm_scale=0.0, workspace=None, workspace_bytes=None,
+                                stream=None):
+    """hx_decode_attention_overlapped: with behind_ingest != 0 the caller states that the kernel directly before it on the
+    stream is a launched hx_kv_ingest whose pages this call does not read; the attention then starts under it
+    (see include/hx.h).  behind_ingest == 0: exactly decode_attention."""
     if workspace_bytes is None:
         workspace_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
     _check(lib().hx_decode_attention_overlapped(_ptr(out), _ptr(q), cache.ref, layer, q_heads, _ptr(block_table),
                                                 block_table_stride, _ptr(seq_lens), batch, max_seq_len,
                                                 C.c_float(sm_scale), _ptr(workspace), workspace_bytes,
-                                                _stream_ptr(stream)))
+                                                int(behind_ingest), _stream_ptr(stream)))
 
 
 def decode_plan_bytes(batch, kv_heads, max_seq_len, page_size=16) -> int:
@@ -418,6 +423,12 @@ class DecodeStep:
 
     def __call__(self, stream=None):
         _check(lib().hx_decode_step(C.byref(self.a), _stream_ptr(stream)))
+
+    def is_fused(self) -> bool:
+        """hx_decode_step_is_fused: would this step run as the one fused kernel?  Enqueues nothing."""
+        f = C.c_int32(0)
+        _check(lib().hx_decode_step_is_fused(C.byref(self.a), C.byref(f)))
+        return bool(f.value)
 
 
 def decode_step(stream=None, **kw):

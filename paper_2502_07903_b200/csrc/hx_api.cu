@@ -19,12 +19,6 @@ void set_error(const char* fmt, ...) {
 }
 void clear_error() { g_err[0] = 0; }
 
-// What this host thread enqueued last through the library, and where.  hx_decode_attention_overlapped launches as a
-// programmatic dependent only when that was an ingest kernel on the same stream (include/hx.h).
-enum LaunchKind { kLaunchNone = 0, kLaunchIngest = 1, kLaunchOther = 2 };
-static thread_local struct { void* stream; int kind; } g_last = {nullptr, kLaunchNone};
-static void note_launch(void* stream, int kind) { g_last.stream = stream; g_last.kind = kind; }
-
 int device_info(DeviceInfo* out) {
   static std::mutex mu;
   static DeviceInfo cache[64];
@@ -103,9 +97,7 @@ static int ingest_common(const void* const* src_k, const void* const* src_v, int
   p.head_dim = head_dim; p.page_size = ps; p.num_pages = dst->num_pages; p.bt_stride = stride;
   if (params_out) *params_out = p;                             // hx_decode_step(overlap_ingest): moved inside the attention kernel
   if (dry_run) return HX_OK;                                   // checks only (hx_decode_step validates before it enqueues)
-  rc = launch_ingest(p, gather, static_cast<cudaStream_t>(stream));
-  if (rc == HX_OK) note_launch(stream, gather ? kLaunchOther : kLaunchIngest);
-  return rc;
+  return launch_ingest(p, gather, static_cast<cudaStream_t>(stream));
 }
 
 }  // namespace hx
@@ -189,8 +181,8 @@ size_t hx_decode_attention_workspace_bytes(int32_t batch, int32_t q_heads, int32
 }
 
 // mode: 0 = hx_decode_attention (and _append / _overlapped), 1 = hx_decode_plan (writes `plan`), 2 = hx_decode_attention_planned
-// pdl: 0 = plain launch; 3 = hx_decode_attention_overlapped (programmatic dependent only directly behind an ingest);
-//      1 / 2 = hx_decode_attention_chained (inputs_ready = 0 / 1)
+// pdl: 0 = plain launch; 3 = hx_decode_attention_overlapped(behind_ingest != 0): programmatic dependent of the ingest kernel
+//      the caller says is directly before it; 1 / 2 = hx_decode_attention_chained (inputs_ready = 0 / 1)
 static int attention_common(const char* who, void* out, const void* q, const void* k_new, const void* v_new, bool append, int pdl,
                             const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
                             const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
@@ -249,15 +241,11 @@ static int attention_common(const char* who, void* out, const void* q, const voi
   p.page_size = cache->page_size; p.num_pages = cache->num_pages; p.bt_stride = block_table_stride;
   p.max_seq_len = max_seq_len; p.sm_scale = sm_scale;
   p.k_new = append ? k_new : nullptr; p.v_new = append ? v_new : nullptr;
-  // hx_decode_attention_overlapped: a programmatic dependent launch only directly behind an ingest kernel this thread
-  // enqueued on this stream; hx_decode_attention_chained: behind whatever precedes it
-  p.overlap_prev = pdl == 3 ? ((g_last.kind == kLaunchIngest && g_last.stream == stream) ? 3 : 0) : pdl;
+  p.overlap_prev = pdl;            // what the launch may overlap is the caller's explicit statement, never inferred
   p.plan = mode != 0 ? plan : nullptr;
   p.handoff = handoff; p.handoff_max_seq_len = handoff_max_seq_len; p.handoff_maps = handoff_maps;
   if (dry_run) return HX_OK;
-  rc = mode == 1 ? launch_plan(p, static_cast<cudaStream_t>(stream)) : launch_attention(p, static_cast<cudaStream_t>(stream));
-  if (rc == HX_OK) note_launch(stream, kLaunchOther);
-  return rc;
+  return mode == 1 ? launch_plan(p, static_cast<cudaStream_t>(stream)) : launch_attention(p, static_cast<cudaStream_t>(stream));
 }
 
 int hx_decode_attention(void* out, const void* q, const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
@@ -280,8 +268,8 @@ int hx_decode_attention_append(void* out, const void* q, const void* k_new, cons
 int hx_decode_attention_overlapped(void* out, const void* q, const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
                                    const int32_t* block_table, int32_t block_table_stride, const int32_t* seq_lens,
                                    int32_t batch, int32_t max_seq_len, float sm_scale, void* workspace,
-                                   size_t workspace_bytes, void* stream) {
-  return attention_common("hx_decode_attention_overlapped", out, q, nullptr, nullptr, false, 3, cache, layer, q_heads,
+                                   size_t workspace_bytes, int32_t behind_ingest, void* stream) {
+  return attention_common("hx_decode_attention_overlapped", out, q, nullptr, nullptr, false, behind_ingest ? 3 : 0, cache, layer, q_heads,
                           block_table, block_table_stride, seq_lens, batch, max_seq_len, sm_scale, workspace,
                           workspace_bytes, stream);
 }
@@ -379,9 +367,7 @@ int hx_kv_append(const void* k_new, const void* v_new, const hx_paged_cache* cac
   p.block_table = block_table; p.seq_lens = seq_lens;
   p.batch = batch; p.kv_heads = cache->kv_heads; p.head_dim = cache->head_dim; p.page_size = cache->page_size;
   p.bt_stride = block_table_stride;
-  rc = launch_append(p, static_cast<cudaStream_t>(stream));
-  if (rc == HX_OK) note_launch(stream, kLaunchOther);
-  return rc;
+  return launch_append(p, static_cast<cudaStream_t>(stream));
 }
 
 int hx_prefill_attention(void* out, const void* q, const hx_paged_cache* cache, int32_t layer, int32_t q_heads,
@@ -415,9 +401,7 @@ int hx_prefill_attention(void* out, const void* q, const hx_paged_cache* cache, 
   a.batch = batch; a.q_heads = q_heads; a.kv_heads = cache->kv_heads; a.head_dim = cache->head_dim;
   a.num_pages = cache->num_pages; a.bt_stride = block_table_stride; a.layer = layer; a.layers = cache->layers;
   a.total_q = total_q_tokens; a.max_q_len = max_q_len; a.sm_scale = sm_scale;
-  rc = launch_prefill(a, static_cast<cudaStream_t>(stream));
-  if (rc == HX_OK) note_launch(stream, kLaunchOther);
-  return rc;
+  return launch_prefill(a, static_cast<cudaStream_t>(stream));
 }
 
 size_t hx_decode_plan_bytes(int32_t batch, int32_t kv_heads, int32_t max_seq_len, int32_t page_size) {
@@ -480,7 +464,8 @@ int side_stream(int* dev_out, SideStream** out) {
 }
 
 // The step on device buffers.  `h` (optional) adds the host<->device copies of hx_decode_step_host.
-int step_impl(const char* who, const hx_step_args* a, const hx_step_host_args* h, void* stream_) {
+// query_fused != NULL: validate, decide whether the step would run as one fused kernel, report it and enqueue nothing.
+int step_impl(const char* who, const hx_step_args* a, const hx_step_host_args* h, void* stream_, int32_t* query_fused = nullptr) {
   using namespace hx;
   cudaStream_t main_stream = static_cast<cudaStream_t>(stream_);
   const bool do_ing = a->ing_batch > 0, do_att = a->batch > 0;
@@ -533,9 +518,10 @@ int step_impl(const char* who, const hx_step_args* a, const hx_step_host_args* h
                        a->cache, a->ing_block_table, a->ing_block_table_stride, a->ing_cu_seqlens, a->ing_seq_lens,
                        a->ing_batch, a->ing_total_tokens, a->ing_max_seq_len, stream_, false, who, -1, 0, 0, /*dry_run=*/true, &ip);
     if (rc) return rc;
-    rc = tile_maps(ip, &ip_maps, &fused);   // shards the copy engines cannot take (pull mode, > 8 shards): in order instead
+    rc = tile_maps(ip, &ip_maps, &fused);   // shards the copy engines cannot take (managed memory, > 8 shards): in order instead
     if (rc) return rc;
   }
+  if (query_fused) { *query_fused = fused ? 1 : 0; return HX_OK; }
   const bool fork = overlap && h;
   SideStream* ss = nullptr;
   cudaStream_t ing_stream = main_stream;
@@ -618,6 +604,14 @@ int hx_decode_step(const hx_step_args* a, void* stream) {
   clear_error();
   if (!a) HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step: args is NULL");
   return step_impl("hx_decode_step", a, nullptr, stream);
+}
+
+int hx_decode_step_is_fused(const hx_step_args* a, int32_t* fused) {
+  using namespace hx;
+  clear_error();
+  if (!a || !fused) HX_FAIL(HX_ERR_INVALID_ARG, "hx_decode_step_is_fused: args / fused is NULL");
+  *fused = 0;
+  return step_impl("hx_decode_step_is_fused", a, nullptr, nullptr, fused);
 }
 
 int hx_decode_step_host(const hx_step_host_args* h, void* stream) {

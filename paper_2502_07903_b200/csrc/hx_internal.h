@@ -56,7 +56,8 @@ struct IngestParams {
 int launch_ingest(const IngestParams& p, bool gather, cudaStream_t stream);
 // The tile mover (handoff_tiles.cuh): how it cuts a handoff into units for `workers` warps, and the tensor maps of the
 // source shards.  tile_maps sets *ok = false (and returns HX_OK) when the call must use the rows kernel instead: more
-// than kMaxTileShards source shards, a shard outside this device's memory (pull mode), or a shard too large for a map.
+// than kMaxTileShards source shards, a shard in managed or unregistered memory, or a shard too large for a map.  Shards in
+// pinned host memory or in a peer GPU's memory are fine: the copy engines pull them over the link (F2).
 TileUnits tile_units(const IngestParams& p, int32_t max_seq_len, long long workers);
 int tile_maps(const IngestParams& p, TileMaps* maps, bool* ok);
 

@@ -177,7 +177,11 @@ int tile_maps(const IngestParams& p, TileMaps* maps, bool* ok) {
       const void* ptr = x ? p.src_v[r] : p.src_k[r];
       cudaPointerAttributes at;
       if (cudaPointerGetAttributes(&at, ptr) != cudaSuccess) { cudaGetLastError(); return HX_OK; }
-      if (at.type != cudaMemoryTypeDevice || at.device != dev) return HX_OK;      // pinned host / peer memory: rows kernel
+      // What the copy engines can load from is any address the GPU can: this device's HBM, pinned host memory (UVA) and a
+      // peer GPU's memory with peer access enabled - the last two make the fused step a PULL-mode handoff (F2): each tile
+      // crosses the link once, straight into its page.  Managed or unregistered memory: rows kernel.
+      (void)dev;
+      if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeHost) return HX_OK;
       CUtensorMap* out = x ? &maps->v[r - r_lo] : &maps->k[r - r_lo];
       bool hit = false;
       for (int e = 0; e < n && !hit; ++e)

@@ -22,7 +22,7 @@ def test_library_exports_every_declared_symbol():
     L = hx.lib()
     for name in declared:
         assert hasattr(L, name), name
-    assert hx.version() == 134
+    assert hx.version() == 135
     assert hx.status_string(0) == "HX_OK" and hx.status_string(5) == "HX_ERR_NO_PAGES"
     assert hx.status_string(77) == "HX_ERR_UNKNOWN"
 
@@ -250,9 +250,10 @@ def test_prefill_rejects_invalid_arguments_without_launching(over, status):
 
 def test_attention_overlapped_validates_like_attention():
     kw = dict(layer=0, q_heads=4, block_table=0x3000, block_table_stride=4, seq_lens=0x4000, batch=2,
-              max_seq_len=64, sm_scale=0.0, workspace=0x5000, workspace_bytes=1 << 30, stream=0)
+              max_seq_len=64, sm_scale=0.0, workspace=0x5000, workspace_bytes=1 << 30, behind_ingest=1, stream=0)
     for over, status in [(dict(layer=2), B.HX_ERR_INVALID_ARG), (dict(q_heads=6), B.HX_ERR_UNSUPPORTED),
-                         (dict(workspace=0), B.HX_ERR_WORKSPACE), (dict(block_table_stride=3), B.HX_ERR_INVALID_ARG)]:
+                         (dict(workspace=0), B.HX_ERR_WORKSPACE), (dict(block_table_stride=3), B.HX_ERR_INVALID_ARG),
+                         (dict(behind_ingest=0, layer=2), B.HX_ERR_INVALID_ARG)]:
         with pytest.raises(hx.HxError) as e:
             hx.decode_attention_overlapped(0x6000, 0x7000, FakeCache(), **dict(kw, **over))
         assert e.value.status == status, str(e.value)

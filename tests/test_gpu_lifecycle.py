@@ -164,7 +164,8 @@ def test_long_ingest_then_tiny_overlapped_attention_then_immediate_read(env):
                 t1.record()      # only here, to show that the ingest is long: an event between the two launches takes
                                  # away their kernel-to-kernel adjacency; repetitions 1-3 are back to back
             hx.decode_attention_overlapped(out, qd, cache, layer=0, q_heads=Hq, block_table=abt, block_table_stride=32,
-                                           seq_lens=asl, batch=4, max_seq_len=300, workspace=ws, workspace_bytes=wsb)
+                                           seq_lens=asl, batch=4, max_seq_len=300, workspace=ws, workspace_bytes=wsb,
+                                           behind_ingest=1)
             k_after = {l: cache.k[l].clone() for l in s["checked"]}      # the immediate read
             v_after = {l: cache.v[l].clone() for l in s["checked"]}
             torch.cuda.synchronize()
@@ -178,9 +179,10 @@ def test_long_ingest_then_tiny_overlapped_attention_then_immediate_read(env):
 
 
 def test_overlapped_attention_back_to_back_and_after_an_empty_ingest(env):
-    """The overlapped launch is a programmatic dependent ONLY directly behind an ingest kernel.  Behind another
-    attention (same workspace: partial slots and arrival counters) or behind an hx_kv_ingest that launched nothing
-    (batch == 0) it must behave exactly like hx_decode_attention."""
+    """The overlapped launch may be a programmatic dependent ONLY directly behind a launched ingest kernel, and the caller
+    says so explicitly (behind_ingest).  Behind another attention (same workspace: partial slots and arrival counters) or
+    behind an hx_kv_ingest that launched nothing (batch == 0) the caller passes behind_ingest=0, and the call must behave
+    exactly like hx_decode_attention - the library keeps no record of earlier calls that could say otherwise."""
     hx, torch, oracle = env
     Hq, Hkv, D = 32, 4, 128
     c = W.AttnConfig(88, "t", 24, Hq, Hkv, D, 256, "x")
@@ -195,12 +197,13 @@ def test_overlapped_attention_back_to_back_and_after_an_empty_ingest(env):
     ws = torch.zeros(wsb, dtype=torch.uint8, device="cuda")
     kw = dict(q_heads=Hq, block_table=bt, block_table_stride=bt.shape[1], seq_lens=sl, batch=24, max_seq_len=mx, workspace=ws,
               workspace_bytes=wsb)
+    okw = dict(kw, behind_ingest=0)
     empty = torch.zeros(1, dtype=torch.int32, device="cuda")
     if True:
         outs = [torch.full_like(qd, float("nan")) for _ in range(6)]
         for j in range(0, 6, 2):                             # six launches back to back, alternating layers
-            hx.decode_attention_overlapped(outs[j], qd, cache, layer=0, **kw)
-            hx.decode_attention_overlapped(outs[j + 1], qd, cache, layer=1, **kw)
+            hx.decode_attention_overlapped(outs[j], qd, cache, layer=0, **okw)
+            hx.decode_attention_overlapped(outs[j + 1], qd, cache, layer=1, **okw)
         torch.cuda.synchronize()
         for j, o in enumerate(outs):
             max_abs, rel = attn_errors(o.cpu().numpy(), refs[j % 2])
@@ -213,7 +216,7 @@ def test_overlapped_attention_back_to_back_and_after_an_empty_ingest(env):
         hx.kv_ingest([empty.view(torch.float16)] * 2, [empty.view(torch.float16)] * 2, layers=1, heads=Hkv, head_dim=D, src_tp=2,
                      dst_tp=1, dst_rank=0, dst=cache, block_table=empty, block_table_stride=1, cu_seqlens=empty, seq_lens=empty,
                      batch=0, total_tokens=0, max_seq_len=0)
-        hx.decode_attention_overlapped(out, qd, cache, layer=0, **kw)
+        hx.decode_attention_overlapped(out, qd, cache, layer=0, **okw)
         torch.cuda.synchronize()
         max_abs, rel = attn_errors(out.cpu().numpy(), refs[0])
         assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, (max_abs, rel)
@@ -302,7 +305,8 @@ def test_chained_calls_sharing_one_output_buffer_and_behind_a_producer_kernel(en
             assert torch.equal(outs[l].view(torch.int16), base[l].view(torch.int16)), (rep, l)
 
 
-def _fused_step_case(env, heads, S, R, q_rank, D, ilens, layers, seed, alens=(33, 100, 1, 700, 16), ing_layers=None):
+def _fused_step_case(env, heads, S, R, q_rank, D, ilens, layers, seed, alens=(33, 100, 1, 700, 16), ing_layers=None,
+                     pinned_src=False, expect_fused=None):
     """One hx_decode_step(overlap_ingest=1): the handoff (tile mover inside the attention kernel, handoff_tiles.cuh) lands
     in pages [0, P) of a sentinel-filled cache while the attention reads an active batch living in pages [P, P + Pa).
     Cache bit-exact against the oracle's ingest (sentinels intact), attention within tolerance."""
@@ -341,14 +345,21 @@ def _fused_step_case(env, heads, S, R, q_rank, D, ilens, layers, seed, alens=(33
     wsb = hx.decode_attention_workspace_bytes(len(alens), hd * G, hd, D, mx)
     ws = torch.zeros(wsb, dtype=torch.uint8, device="cuda")
     ibt = torch.from_numpy(w["block_table"]).cuda()
+    if pinned_src:       # pull mode (F2): the shards stay in pinned host memory, the GPU fetches them over the link
+        place = lambda a: torch.from_numpy(a.view(np.int16)).pin_memory()
+    else:
+        place = lambda a: to_dev(a, torch)
+    step = hx.DecodeStep(out=out, q=qd, cache=cache, layer=layer_a, q_heads=hd * G, block_table=torch.from_numpy(abt).cuda(),
+                         block_table_stride=abt.shape[1], seq_lens=torch.from_numpy(alens).cuda(), batch=len(alens), max_seq_len=mx,
+                         sm_scale=0.0, workspace=ws, workspace_bytes=wsb, src_k=[place(a) for a in w["src_k"]],
+                         src_v=[place(a) for a in w["src_v"]], ing_layers=ing_layers, heads=heads, src_tp=S, dst_tp=R,
+                         dst_rank=q_rank, ing_block_table=ibt, ing_block_table_stride=ibt.shape[1],
+                         ing_cu_seqlens=torch.from_numpy(w["cu_seqlens"]).cuda(), ing_seq_lens=torch.from_numpy(w["seq_lens"]).cuda(),
+                         ing_batch=len(ilens), ing_total_tokens=w["total_tokens"], ing_max_seq_len=int(max(ilens)), overlap_ingest=1)
+    if expect_fused is not None:
+        assert step.is_fused() == expect_fused, (heads, S, R, q_rank, D)
     for rep in range(2):                                   # twice: the kernel must leave its counters at zero
-        hx.decode_step(out=out, q=qd, cache=cache, layer=layer_a, q_heads=hd * G, block_table=torch.from_numpy(abt).cuda(),
-                       block_table_stride=abt.shape[1], seq_lens=torch.from_numpy(alens).cuda(), batch=len(alens), max_seq_len=mx,
-                       sm_scale=0.0, workspace=ws, workspace_bytes=wsb, src_k=[to_dev(a, torch) for a in w["src_k"]],
-                       src_v=[to_dev(a, torch) for a in w["src_v"]], ing_layers=ing_layers, heads=heads, src_tp=S, dst_tp=R,
-                       dst_rank=q_rank, ing_block_table=ibt, ing_block_table_stride=ibt.shape[1],
-                       ing_cu_seqlens=torch.from_numpy(w["cu_seqlens"]).cuda(), ing_seq_lens=torch.from_numpy(w["seq_lens"]).cuda(),
-                       ing_batch=len(ilens), ing_total_tokens=w["total_tokens"], ing_max_seq_len=int(max(ilens)), overlap_ingest=1)
+        step()
         k_after, v_after = cache.k.clone(), cache.v.clone()     # ordered after the one kernel that did both
         torch.cuda.synchronize()
         assert np.array_equal(dev_u16(k_after), ek), (heads, S, R, q_rank, D, rep)
@@ -380,7 +391,29 @@ def test_fused_step_with_an_empty_handoff(env):
     (hx_kv_ingest accepts both as no-ops): the cache keeps every bit, the attention result is unaffected."""
     _fused_step_case(env, 8, 2, 2, 1, 128, [0, 0, 0], layers=2, seed=11)
     _fused_step_case(env, 8, 4, 1, 0, 64, [0], layers=1, seed=12)
-    _fused_step_case(env, 8, 2, 4, 3, 128, [40, 3, 129], layers=2, seed=13, ing_layers=0)
+    _fused_step_case(env, 8, 2, 4, 3, 128, [40, 3, 129], layers=2, seed=13, ing_layers=0, expect_fused=False)
+
+
+def test_fused_step_pulls_the_handoff_from_pinned_host_memory(env):
+    """F2 inside the fused step: the source shards are NOT in this GPU's HBM (pinned host memory here, reached over PCIe;
+    a peer GPU's memory is reached the same way over NVLink, tests/test_gpu_peer.py).  The step must still be the ONE
+    fused kernel - the copy engines load each (page, head) tile through a tensor map over the remote shard and store it
+    into its page - with the cache bit-exact and the attention within tolerance."""
+    ilens = [1, 15, 16, 17, 31, 32, 33, 255, 256, 257, 0, 5]
+    _fused_step_case(env, 8, 4, 2, 1, 128, ilens, layers=3, seed=31, pinned_src=True, expect_fused=True)
+    _fused_step_case(env, 8, 1, 1, 0, 64, ilens, layers=2, seed=32, pinned_src=True, expect_fused=True)
+    _fused_step_case(env, 8, 2, 8, 5, 128, [40, 3, 129], layers=2, seed=33, pinned_src=True, expect_fused=True)
+    # and the ordinary case reports itself as fused, the 2100-request one (below) as not
+    _fused_step_case(env, 8, 2, 2, 0, 128, [40, 3, 129], layers=2, seed=34, expect_fused=True)
+
+
+def test_step_with_more_than_2048_requests_runs_in_order(env):
+    """hx_decode_step(overlap_ingest=1) with an active batch above what one attention launch covers (2048): the fused
+    kernel cannot take it, the library runs ingest then attention (two launches for the 2100 requests) in order.  Same
+    checks as the fused case: cache bit-exact against the oracle's ingest, attention within tolerance."""
+    alens = W.rng(93, 21).integers(0, 80, size=2100).astype(np.int32)
+    alens[[0, 2047, 2048, 2099]] = [1, 79, 33, 16]
+    _fused_step_case(env, 8, 2, 2, 1, 128, [40, 3, 129, 0, 16], layers=2, seed=21, alens=alens, expect_fused=False)
 
 
 def test_layer_loop_of_chained_calls_in_a_cuda_graph(env):

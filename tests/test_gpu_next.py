@@ -380,7 +380,7 @@ def test_attention_overlapped_with_the_ingest_before_it(env):
                      block_table_stride=128, cu_seqlens=cu_i, seq_lens=sl_i, batch=3, total_tokens=int(ilens.sum()),
                      max_seq_len=2000)
         hx.decode_attention_overlapped(out, qd, cache, layer=0, q_heads=Hq, block_table=abt, block_table_stride=abt.shape[1],
-                                       seq_lens=asl, batch=8, max_seq_len=3000, workspace=ws)
+                                       seq_lens=asl, batch=8, max_seq_len=3000, workspace=ws, behind_ingest=1)
         k_after = cache.k.clone()                    # stream-ordered after BOTH kernels
         torch.cuda.synchronize()
         assert np.array_equal(dev_u16(k_after), ok) and np.array_equal(dev_u16(cache.v), ov), rep
